@@ -1,0 +1,90 @@
+"""CPU oracle for the Wilson Dslash operator -- TEST INFRASTRUCTURE ONLY.
+
+ctypes front-end of oracle/dslash_oracle.c (the plain-definition fp64 operator, PAPER.md:47-54,
+Eq. 1).  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+may import this package; the product (paper_2301_03636_b200/) never does, and this package never
+imports the product.
+
+Arrays are NumPy, canonical layout:
+    spinor  float64 [T, Z, Y, X, 4, 3, 2]      (s = x + L_X*(y + L_Y*(z + L_Z*t)), x fastest)
+    gauge   float64 [T, Z, Y, X, 4, 3, 3, 2]   ([mu][row i][col j][re/im])
+dims is always (L_X, L_Y, L_Z, L_T).
+"""
+import ctypes
+import os
+
+import numpy as np
+
+from . import build as _build
+
+_LIB = None
+
+
+def _lib():
+    global _LIB
+    if _LIB is None:
+        path = _build.build()
+        lib = ctypes.CDLL(path)
+        dbl_p = ctypes.POINTER(ctypes.c_double)
+        int_p = ctypes.POINTER(ctypes.c_int)
+        lib.oracle_gamma.argtypes = [ctypes.c_int, dbl_p]
+        lib.oracle_gamma.restype = None
+        lib.oracle_dslash.argtypes = [dbl_p, dbl_p, dbl_p, int_p, ctypes.c_int]
+        lib.oracle_dslash.restype = ctypes.c_int
+        lib.oracle_dslash_sites.argtypes = [dbl_p, dbl_p, dbl_p, int_p, ctypes.POINTER(ctypes.c_int64),
+                                            ctypes.c_int64, ctypes.c_int]
+        lib.oracle_dslash_sites.restype = ctypes.c_int
+        lib.oracle_max_threads.argtypes = []
+        lib.oracle_max_threads.restype = ctypes.c_int
+        _LIB = lib
+    return _LIB
+
+
+def _dp(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def _check(psi, gauge, dims):
+    lx, ly, lz, lt = (int(d) for d in dims)
+    v = lx * ly * lz * lt
+    if psi.dtype != np.float64 or gauge.dtype != np.float64:
+        raise TypeError("oracle takes float64 arrays")
+    if psi.size != v * 24 or gauge.size != v * 72:
+        raise ValueError("array sizes do not match dims")
+    psi = np.ascontiguousarray(psi)
+    gauge = np.ascontiguousarray(gauge)
+    cdims = (ctypes.c_int * 4)(lx, ly, lz, lt)
+    return psi, gauge, cdims, (lx, ly, lz, lt), v
+
+
+def gamma(mu: int) -> np.ndarray:
+    """gamma_mu as a complex128 [4, 4] array (DeGrand-Rossi, DESIGN.md Reading R4)."""
+    out = np.zeros((4, 4, 2), dtype=np.float64)
+    _lib().oracle_gamma(int(mu), _dp(out))
+    return out[..., 0] + 1j * out[..., 1]
+
+
+def dslash(psi: np.ndarray, gauge: np.ndarray, dims, nthreads: int = 0) -> np.ndarray:
+    """out = D[gauge] psi on the whole lattice (Eq. 1).  nthreads <= 0: all cores."""
+    psi, gauge, cdims, (lx, ly, lz, lt), _ = _check(psi, gauge, dims)
+    out = np.empty((lt, lz, ly, lx, 4, 3, 2), dtype=np.float64)
+    rc = _lib().oracle_dslash(_dp(out), _dp(psi), _dp(gauge), cdims, int(nthreads))
+    if rc != 0:
+        raise RuntimeError("oracle_dslash failed: %d" % rc)
+    return out
+
+
+def dslash_sites(psi: np.ndarray, gauge: np.ndarray, dims, sites, nthreads: int = 0) -> np.ndarray:
+    """(D psi)(s) for the linear site indices `sites`; returns float64 [n, 4, 3, 2]."""
+    psi, gauge, cdims, _, _ = _check(psi, gauge, dims)
+    sites = np.ascontiguousarray(np.asarray(sites, dtype=np.int64))
+    out = np.empty((sites.size, 4, 3, 2), dtype=np.float64)
+    rc = _lib().oracle_dslash_sites(_dp(out), _dp(psi), _dp(gauge), cdims,
+                                    sites.ctypes.data_as(ctypes.POINTER(ctypes.c_int64)), sites.size, int(nthreads))
+    if rc != 0:
+        raise RuntimeError("oracle_dslash_sites failed: %d" % rc)
+    return out
+
+
+def max_threads() -> int:
+    return int(_lib().oracle_max_threads())
