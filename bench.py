@@ -1,0 +1,411 @@
+#!/usr/bin/env python
+"""bench.py -- Wilson Dslash throughput on B200 (BASELINE.json metric), one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W]            # the CUDA library (default config 3)
+    python bench.py --impl reference [--steps K] [--warmup W]       # the CPU oracle, same metric/config
+    python bench.py --sweep [--sweep-csv PATH]                      # config 5: 120 variants, top-10
+
+A "step" is one application of D (one dslash_apply = one kernel launch covering SURVEY.md section 8(a)
+steps a1-a7) to one seeded synthetic lattice that is already resident in HBM in the native layout.
+`value` = 1320 flop/site * sites of all ranks / max-over-ranks device time (CUDA events on the
+launching stream).  `e2e` = the same through dslash_apply_host with pinned HOST buffers (H2D copy of
+gauge and spinor, pack, apply, unpack, D2H copy of the result inside the timed region).
+Multi-GPU: the path has no exchange step in this build ("replicas only"): under torchrun
+every rank runs its own lattice; value is the sum (weak scaling).
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "Dslash GFLOP/s (1320 flop/site) & HBM GB/s vs peak, 32^3x64 FP64, 1 B200"
+FLOP_PER_SITE = 1320
+SEED = 230103636
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
+
+# BASELINE.json configs (index = position in `configs`); bytes/site = compulsory traffic:
+# spinor in once + 4 links once + spinor out once.
+CONFIGS = {
+    "1": dict(dims=(4, 4, 4, 4), precision="f64", recon12=False, name="configs[0]: 4^4 FP64"),
+    "2": dict(dims=(16, 16, 16, 16), precision="f64", recon12=False, name="configs[1]: 16^4 FP64 (L2-resident)"),
+    "3": dict(dims=(32, 32, 32, 64), precision="f64", recon12=False, name="configs[2]: 32^3x64 FP64, 18-real links"),
+    "3r": dict(dims=(32, 32, 32, 64), precision="f64", recon12=True, name="configs[2]: 32^3x64 FP64, 12-real links"),
+    "4": dict(dims=(48, 48, 48, 96), precision="f32", recon12=False, name="configs[3]: 48^3x96 FP32"),
+    "5": dict(dims=(24, 24, 24, 24), precision="f64", recon12=False, name="configs[4]: 24^4 FP64 (sweep lattice)"),
+}
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+# `ncu --set full` capture (profiles/); None until captured for that workload.
+NCU_TRAFFIC_BYTES = {}
+
+
+def bytes_per_site(precision, recon12):
+    real = 8 if precision == "f64" else 4
+    return (24 + 4 * (12 if recon12 else 18) + 24) * real
+
+
+def hbm_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# ------------------------------------------------------------------ clocks during the timed region (NVML)
+class ClockSampler:
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown"}
+
+    def __init__(self, index):
+        self.samples, self.reasons, self.max_mhz, self.ok = [], set(), None, False
+        self._stop = threading.Event()
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for bit, name in self.REASONS.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.002)
+
+    def __enter__(self):
+        if self.ok:
+            self.t = threading.Thread(target=self._run, daemon=True)
+            self.t.start()
+        return self
+
+    def __exit__(self, *exc):
+        if self.ok:
+            self._stop.set()
+            self.t.join()
+
+    def summary(self):
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": 0}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------ CPU oracle legs
+def oracle_timing(dims, g64, p64, nsites, steps, warmup):
+    """Time the oracle as it stands on `nsites` seeded sample sites per step; returns (GFLOP/s, s/step, cores)."""
+    import oracle
+    from paper_2301_03636_b200 import inputs
+    v = inputs.volume(dims)
+    cores = oracle.max_threads()
+    if nsites >= v:
+        fn = lambda: oracle.dslash(p64, g64, dims)
+        n = v
+    else:
+        sites = np.sort(np.random.default_rng([SEED, 77]).choice(v, size=nsites, replace=False)).astype(np.int64)
+        fn = lambda: oracle.dslash_sites(p64, g64, dims, sites)
+        n = nsites
+    for _ in range(warmup):
+        fn()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        fn()
+    dt = (time.perf_counter() - t0) / max(steps, 1)
+    return FLOP_PER_SITE * n / dt / 1e9, dt, cores, n
+
+
+def run_reference(args, cfg):
+    """--impl reference: the oracle (oracle/dslash_oracle.c, unmodified) on the host cores."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_2301_03636_b200 import inputs
+    dims = cfg["dims"]
+    g, p = inputs.fields(dims, SEED + 3, cfg["precision"], check=False)
+    g64, p64 = inputs.promote(g), inputs.promote(p)
+    nsites = min(inputs.volume(dims), args.ref_sites)
+    gflops, dt, cores, n = oracle_timing(dims, g64, p64, nsites, args.steps, args.warmup)
+    sample = "%d seeded sample sites of the %s lattice per step (oracle_dslash_sites)" % (n, "x".join(map(str, dims)))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": gflops, "unit": "GFLOP/s", "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg["name"], "dims": list(dims), "sample": sample},
+        "cpu_baseline": {"value": gflops, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": gflops, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------ the CUDA arm
+def time_applies(torch, lat, out, inp, gauge, steps, warmup, dist, sampler_index):
+    for _ in range(warmup):
+        lat.apply(out, inp, gauge)
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(sampler_index) as cs:
+        e0.record()
+        for _ in range(steps):
+            lat.apply(out, inp, gauge)
+        e1.record()
+        torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    ms = e0.elapsed_time(e1)
+    if dist is not None:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    return ms, cs.summary()
+
+
+def run_cuda(args, cfg):
+    import torch
+    from paper_2301_03636_b200 import binding as B
+    from paper_2301_03636_b200 import device, inputs
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA library has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_
+        dist_.init_process_group("nccl", device_id=torch.device("cuda", local))
+        dist = dist_
+    dims, prec = cfg["dims"], cfg["precision"]
+    v = inputs.volume(dims)
+    g, p = inputs.fields(dims, SEED + 3 + 1000 * rank, prec, check=False)  # every rank its own replica
+
+    results = {}
+    clocks = None
+    launches = 0
+    for tag, recon12 in (("main", cfg["recon12"]), ("other_recon", not cfg["recon12"])):
+        if tag == "other_recon" and not args.both_recon:
+            continue
+        with device.Lattice(dims, prec, args.layout, recon12, device="cuda:%d" % local) as lat:
+            if args.tile:
+                lat.set_tile(args.tile)
+            gd, pd, od = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
+            n0 = B.dslash_launch_count(lat.ctx)
+            ms, ck = time_applies(torch, lat, od, pd, gd, args.steps, args.warmup, dist, local)
+            n1 = B.dslash_launch_count(lat.ctx)
+            bps = bytes_per_site(prec, recon12)
+            results[tag] = dict(ms=ms, ms_per_step=ms / args.steps, gflops=FLOP_PER_SITE * v * world / (ms / args.steps) / 1e6,
+                                gbs=bps * v / (ms / args.steps) / 1e6, bps=bps, recon12=recon12,
+                                tile=list(B.dslash_get_tile(lat.ctx)))
+            if tag == "main":
+                clocks, launches = ck, n1 - n0 - args.warmup
+            del gd, pd, od
+
+    main = results["main"]
+    peak, peak_src = hbm_peak()
+    key = "%s_%s_%s_r%d" % ("x".join(map(str, dims)), prec, args.layout, 12 if main["recon12"] else 18)
+    roofline = {"bound": "hbm", "achieved": main["gbs"], "peak": peak, "unit": "GB/s", "frac": main["gbs"] / peak,
+                "traffic": NCU_TRAFFIC_BYTES.get(key), "peak_source": peak_src, "kernel": "dslash_tuned_kernel",
+                "algorithmic_bytes_per_site": main["bps"], "algorithmic_bytes_per_launch": main["bps"] * v,
+                "frac_of_nominal_8TBs": main["gbs"] / 8000.0}
+
+    # end to end through the C ABI with pinned HOST buffers (H2D + pack + apply + unpack + D2H per step)
+    e2e = None
+    if not args.no_e2e:
+        with device.Lattice(dims, prec, args.layout, cfg["recon12"], device="cuda:%d" % local) as lat:
+            gh = torch.from_numpy(np.ascontiguousarray(g)).pin_memory()
+            ph = torch.from_numpy(np.ascontiguousarray(p)).pin_memory()
+            oh = torch.empty(ph.shape, dtype=ph.dtype).pin_memory()
+            stream = lat.stream()
+            n_e2e = max(1, min(args.steps, args.e2e_steps))
+            for _ in range(2):
+                h2d, d2h = B.dslash_apply_host(lat.ctx, oh.data_ptr(), ph.data_ptr(), gh.data_ptr(), B.DSLASH_MAP_MINIMAL, stream)
+            torch.cuda.synchronize()
+            if dist is not None:
+                dist.barrier()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(n_e2e):
+                B.dslash_apply_host(lat.ctx, oh.data_ptr(), ph.data_ptr(), gh.data_ptr(), B.DSLASH_MAP_MINIMAL, stream)
+            e1.record()
+            torch.cuda.synchronize()
+            ms_e = e0.elapsed_time(e1)
+            if dist is not None:
+                t = torch.tensor([ms_e], dtype=torch.float64, device="cuda")
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                ms_e = float(t.item())
+            e2e = {"value": FLOP_PER_SITE * v * world / (ms_e / n_e2e) / 1e6, "unit": "GFLOP/s", "h2d_bytes_per_step": int(h2d),
+                   "d2h_bytes_per_step": int(d2h), "ms_per_step": ms_e / n_e2e, "steps": n_e2e,
+                   "path": "dslash_apply_host(DSLASH_MAP_MINIMAL), pinned host buffers, canonical layout"}
+            del gh, ph, oh
+
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        g64, p64 = inputs.promote(g), inputs.promote(p)
+        gf, dt, cores, n = oracle_timing(dims, g64, p64, min(v, args.cpu_sites), 1, 0)
+        cpu_baseline = {"value": gf, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "seconds": dt,
+                        "sample": "1 application to %d of %d sites (%s)" % (n, v, "whole lattice" if n == v else "seeded sample")}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": main["gflops"], "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": main["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": prec, "data": "synthetic",
+            "config": {"workload": cfg["name"], "dims": list(dims), "layout": args.layout, "recon": 12 if main["recon12"] else 18,
+                       "tile": main["tile"], "sites": v, "parallelism": "replicas x%d" % world,
+                       "l2": "inputs larger than L2: %.2f GB working set per apply vs 126 MB L2, no flush needed"
+                             % (main["bps"] * v / 1e9)},
+            "hbm_gbs": main["gbs"], "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "clocks": clocks,
+            "gpu_launches": int(launches),
+        }
+        if "other_recon" in results:
+            o = results["other_recon"]
+            line["also"] = {"recon": 12 if o["recon12"] else 18, "value": o["gflops"], "ms_per_step": o["ms_per_step"],
+                            "hbm_gbs": o["gbs"], "roofline_frac": o["gbs"] / peak}
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+# ------------------------------------------------------------------ config 5: the Advisor-style sweep
+def run_sweep(args):
+    import torch
+    import oracle
+    from paper_2301_03636_b200 import binding as B
+    from paper_2301_03636_b200 import checks, device, inputs
+    cfg = CONFIGS["5"]
+    dims = cfg["dims"]
+    v = inputs.volume(dims)
+    g, p = inputs.fields(dims, SEED + 5, "f64", check=False)
+    ref = oracle.dslash(p, g, dims)
+    ref_t = torch.from_numpy(np.ascontiguousarray(ref)).cuda()
+    ref_c = torch.view_as_complex(ref_t)
+    den = torch.maximum(ref_c.abs(), torch.sqrt(torch.mean(ref_c.abs() ** 2)))
+    lats = {}
+    for lay in ("aos", "soa"):
+        lat = device.Lattice(dims, "f64", lay, False)
+        lats[lay] = (lat, lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor(),
+                     lat._bytes(B.dslash_canonical_spinor_bytes(lat.ctx)))
+    rows = []
+    for i in range(B.dslash_variant_count()):
+        depth, tpb, spt, layout = B.dslash_variant_at(i)
+        lay = "aos" if layout == B.DSLASH_AOS else "soa"
+        lat, gd, pd, od, can = lats[lay]
+        lat.set_variant(depth, tpb, spt)
+        od.zero_()
+        lat.apply(od, pd, gd)
+        B.dslash_unpack_spinor(lat.ctx, can.data_ptr(), od.data_ptr(), lat.stream())
+        got_c = torch.view_as_complex(can.view(torch.float64).view(ref_t.shape))
+        err = float(((got_c - ref_c).abs() / den).max())
+        # 3 warm-ups, then min(100, as many as fit in 0.5 s, >= 3) timed applies, each with its own event pair
+        times = []
+        for _ in range(3):
+            lat.apply(od, pd, gd)
+        torch.cuda.synchronize()
+        budget, n = 0.5, 0
+        while n < 100 and (n < 3 or budget > 0):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            lat.apply(od, pd, gd)
+            e1.record()
+            e1.synchronize()
+            ms = e0.elapsed_time(e1)
+            times.append(ms)
+            budget -= ms / 1e3
+            n += 1
+        med = float(np.median(times))
+        rows.append(dict(index=i, layout=lay, collapse=depth, tpb=tpb, spt=spt, median_ms=med, min_ms=float(min(times)),
+                         n=n, gflops=FLOP_PER_SITE * v / med / 1e6, parity=err, ok=bool(err <= 1e-12)))
+    # the tuned kernel, same protocol, for reference
+    lat, gd, pd, od, can = lats["soa"]
+    lat.set_variant(B.DSLASH_VARIANT_TUNED)
+    for _ in range(3):
+        lat.apply(od, pd, gd)
+    torch.cuda.synchronize()
+    tt = []
+    for _ in range(100):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        lat.apply(od, pd, gd)
+        e1.record()
+        e1.synchronize()
+        tt.append(e0.elapsed_time(e1))
+    tuned_ms = float(np.median(tt))
+    for lat, *_ in lats.values():
+        lat.close()
+    rows.sort(key=lambda r: r["median_ms"])
+    for k, r in enumerate(rows):
+        r["rank"] = k + 1
+    if args.sweep_csv:
+        os.makedirs(os.path.dirname(os.path.abspath(args.sweep_csv)), exist_ok=True)
+        with open(args.sweep_csv, "w") as f:
+            cols = ["rank", "index", "layout", "collapse", "tpb", "spt", "median_ms", "min_ms", "n", "gflops", "parity", "ok"]
+            f.write(",".join(cols) + "\n")
+            for r in rows:
+                f.write(",".join(str(r[c]) for c in cols) + "\n")
+    line = {"sweep": cfg["name"], "variants": len(rows), "all_parity_ok": all(r["ok"] for r in rows),
+            "worst_parity": max(r["parity"] for r in rows), "top10": rows[:10], "slowest": rows[-1],
+            "spread_ms": rows[-1]["median_ms"] - rows[0]["median_ms"],
+            "tuned_kernel": {"median_ms": tuned_ms, "gflops": FLOP_PER_SITE * v / tuned_ms / 1e6}}
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=500)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
+    ap.add_argument("--config", choices=sorted(CONFIGS), default="3")
+    ap.add_argument("--layout", choices=["soa", "aos"], default="soa")
+    ap.add_argument("--tile", type=int, nargs=4, default=None, help="tile of the tuned kernel (x y z t)")
+    ap.add_argument("--both-recon", action="store_true", default=True, help="also time the other link compression")
+    ap.add_argument("--one-recon", dest="both_recon", action="store_false")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=10)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-sites", type=int, default=1 << 21, help="sites the cpu_baseline oracle run covers")
+    ap.add_argument("--ref-sites", type=int, default=1 << 14, help="sample sites per step of --impl reference")
+    ap.add_argument("--sweep", action="store_true")
+    ap.add_argument("--sweep-csv", default=os.path.join(ROOT, "gpurun_out", "sweep_24x24x24x24.csv"))
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "cuda" and not args.sweep:
+        args.warmup = 3  # timing rule: at least 3 warm-up steps
+    if args.sweep:
+        return run_sweep(args)
+    cfg = CONFIGS[args.config]
+    if args.impl == "reference":
+        return run_reference(args, cfg)
+    return run_cuda(args, cfg)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

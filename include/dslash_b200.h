@@ -1,0 +1,195 @@
+/*
+ * dslash_b200.h -- C ABI of the B200-native Wilson Dslash library (libdslash_b200.so, sm_100a).
+ *
+ * The operator (section 1.1, Eq. 1; backward link argument corrected to x-mu^ as in
+ * BASELINE.json's north_star -- DESIGN.md Reading R1):
+ *
+ *   out(x) = sum_{mu=0..3} [ (1 - gamma_mu) U_mu(x) in(x+mu^)  +  (1 + gamma_mu) U_mu(x-mu^)^dagger in(x-mu^) ]
+ *
+ * on a periodic 4-D lattice dims = {L_X, L_Y, L_Z, L_T}; U_mu(x) in SU(3) acts on the colour index
+ * (COLORS = 3), gamma_mu (DeGrand-Rossi basis, DESIGN.md Reading R4) on the spin index (SPINS = 4)
+ * (PAPER.md:52).  mu = 0,1,2,3 <-> x,y,z,t.  No mass term, no factor 1/2.
+ *
+ * Conventions common to every call
+ *   - Every function returns an int status: DSLASH_OK (0) or a negative DSLASH_ERR_* code.  Nothing
+ *     throws, aborts or prints.  dslash_error_string() names a code.
+ *   - "device pointer" = CUDA global memory on the device that was current at dslash_create();
+ *     "host pointer" = ordinary or pinned host memory.  The library never takes ownership of a
+ *     caller's buffer, never frees it and never keeps it beyond the call (asynchronous work on
+ *     `stream` excepted: buffers must stay alive until that work has finished).
+ *   - stream: a cudaStream_t passed as an opaque pointer (NULL = the legacy default stream).  All
+ *     device work of a call is enqueued on it; no call except dslash_apply_host() and
+ *     dslash_destroy() synchronises.
+ *   - A ctx may be used from one host thread at a time; distinct ctxs are independent.
+ *   - There is no CPU fallback: without a CUDA device dslash_create() returns DSLASH_ERR_CUDA.
+ *
+ * Canonical layout ("array of structures", the flat arrays of PAPER.md:52 with the loop order of
+ * PAPER.md:54; x fastest):   site s = x + L_X*(y + L_Y*(z + L_Z*t)),  V = L_X*L_Y*L_Z*L_T
+ *     spinor  real[ ((s*4 + spin)*3 + colour)*2 + ri ]                      24 reals per site
+ *     gauge   real[ (((s*4 + mu)*3 + row)*3 + col)*2 + ri ]                 72 reals per site
+ *   ri = 0 real part, 1 imaginary part; (U v)[row] = sum_col U[row][col] v[col].
+ *   real = double for DSLASH_FP64 contexts, float for DSLASH_FP32 contexts.
+ *
+ * Native layouts (what dslash_apply() reads and writes; sizes from dslash_*_bytes()):
+ *   DSLASH_AOS                  the canonical layout itself (18 reals per link).
+ *   DSLASH_AOS|DSLASH_RECON12   spinor canonical; gauge keeps rows 0,1 only:
+ *                                 real[ (((s*4 + mu)*2 + row)*3 + col)*2 + ri ]
+ *   DSLASH_SOA  ("structure of arrays", one 16-byte vector per site and component, unit stride in s)
+ *       FP64 spinor  double2[ k*V + s ]           k = spin*3 + colour = 0..11      (re, im)
+ *       FP32 spinor  float4 [ q*V + s ]           q = 0..5: components k = 2q, 2q+1 (re,im,re,im)
+ *       FP64 gauge   double2[ (mu*R + e)*V + s ]  e = row*3 + col; R = 9, or 6 with DSLASH_RECON12
+ *       FP32 gauge   float2 [ (mu*R + e)*V + s ]
+ *   With DSLASH_RECON12 row 2 of every link is rebuilt in registers as conj(row0 x row1), which is
+ *   exact for SU(3) input (DESIGN.md Reading R14).
+ */
+#ifndef DSLASH_B200_H
+#define DSLASH_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dslash_ctx dslash_ctx;
+typedef void *dslash_stream_t; /* a cudaStream_t */
+
+#if defined(__GNUC__)
+#define DSLASH_API __attribute__((visibility("default")))
+#else
+#define DSLASH_API
+#endif
+
+/* precision */
+#define DSLASH_FP64 0
+#define DSLASH_FP32 1
+/* layout: base value, optionally OR-ed with DSLASH_RECON12 */
+#define DSLASH_AOS 0
+#define DSLASH_SOA 1
+#define DSLASH_RECON12 16
+
+/* status codes */
+#define DSLASH_OK 0
+#define DSLASH_ERR_NULL (-1)        /* a required pointer argument is NULL */
+#define DSLASH_ERR_DIMS (-2)        /* an extent < 1, or the lattice exceeds the 32-bit indexing limit */
+#define DSLASH_ERR_PRECISION (-3)   /* precision is not DSLASH_FP64 / DSLASH_FP32 */
+#define DSLASH_ERR_LAYOUT (-4)      /* layout is not (AOS|SOA) [| RECON12] */
+#define DSLASH_ERR_ALIGN (-5)       /* a field pointer is not 16-byte aligned */
+#define DSLASH_ERR_ALIAS (-6)       /* out overlaps in */
+#define DSLASH_ERR_UNSUPPORTED (-7) /* variant / tuning parameters outside the supported set */
+#define DSLASH_ERR_CUDA (-8)        /* a CUDA runtime call failed; see dslash_last_cuda_error() */
+#define DSLASH_ERR_NOMEM (-9)       /* host or device allocation failed */
+
+/* variant selection: collapse_depth DSLASH_VARIANT_TUNED selects the library's tuned kernel */
+#define DSLASH_VARIANT_TUNED 0
+
+/* host<->device mapping modes of dslash_apply_host() (section 4.1.2) */
+#define DSLASH_MAP_MINIMAL 0 /* to: gauge, in;  from: out            (after the Advisor's data analysis) */
+#define DSLASH_MAP_TOFROM 1  /* tofrom: gauge, in, out                (no data analysis)                  */
+
+/*
+ * Create a context for one lattice, precision and native layout on the current CUDA device.
+ *   ctx        out: receives the new context (library-owned; release with dslash_destroy).
+ *   dims       host pointer to {L_X, L_Y, L_Z, L_T}; every extent >= 1 (even or odd; L = 1 and 2 wrap
+ *              onto the site itself / the same neighbour, as the modulo in Eq. 1's deltas says);
+ *              36*V must be < 2^31 (32-bit vector indices; V <= 59 652 323 sites).
+ *   precision  DSLASH_FP64 or DSLASH_FP32: storage and arithmetic type of all three fields.
+ *   layout     DSLASH_AOS or DSLASH_SOA, optionally | DSLASH_RECON12.
+ * The context starts with the tuned kernel selected (DSLASH_VARIANT_TUNED).
+ * Errors: NULL, DIMS, PRECISION, LAYOUT, CUDA (no device), NOMEM.
+ */
+DSLASH_API int dslash_create(dslash_ctx **ctx, const int dims[4], int precision, int layout);
+
+/* Free a context and any staging buffers it owns (synchronises the device if it owns any).
+ * NULL is a no-op returning DSLASH_OK. */
+DSLASH_API int dslash_destroy(dslash_ctx *ctx);
+
+/*
+ * out = D[gauge] in -- one application of Eq. 1, asynchronous on `stream`.
+ *   out, in   device pointers, native spinor layout of the ctx, dslash_spinor_bytes() each,
+ *             16-byte aligned, must not overlap.
+ *   gauge     device pointer, native gauge layout, dslash_gauge_bytes(), 16-byte aligned.
+ * Exactly one kernel launch; no allocation, copy or synchronisation.
+ * Errors: NULL, ALIGN, ALIAS, CUDA (launch failure, also stored in the ctx).
+ */
+DSLASH_API int dslash_apply(dslash_ctx *ctx, void *out, const void *in, const void *gauge, dslash_stream_t stream);
+
+/* Bytes of one spinor / of the gauge field in the ctx's native layout (0 if ctx is NULL). */
+DSLASH_API size_t dslash_spinor_bytes(const dslash_ctx *ctx);
+DSLASH_API size_t dslash_gauge_bytes(const dslash_ctx *ctx);
+/* Bytes of the same fields in the canonical layout at the ctx's precision. */
+DSLASH_API size_t dslash_canonical_spinor_bytes(const dslash_ctx *ctx);
+DSLASH_API size_t dslash_canonical_gauge_bytes(const dslash_ctx *ctx);
+
+/*
+ * Layout module (north_star subsystem (1)): canonical <-> native, device to device, asynchronous
+ * on `stream`, one kernel launch each.  src and dst must not overlap.  pack_gauge drops row 2 when
+ * the ctx has DSLASH_RECON12.  For DSLASH_AOS without RECON12 these are plain copies.
+ * Errors: NULL, ALIGN, CUDA.
+ */
+DSLASH_API int dslash_pack_spinor(dslash_ctx *ctx, void *dst_native, const void *src_canonical, dslash_stream_t stream);
+DSLASH_API int dslash_unpack_spinor(dslash_ctx *ctx, void *dst_canonical, const void *src_native, dslash_stream_t stream);
+DSLASH_API int dslash_pack_gauge(dslash_ctx *ctx, void *dst_native, const void *src_canonical, dslash_stream_t stream);
+
+/*
+ * Advisor-style variant selection (section 4.1.3; BASELINE.json configs[4]).
+ *   collapse_depth     DSLASH_VARIANT_TUNED (0): the tuned kernel; the other two arguments are ignored.
+ *                      1..4: the first `collapse_depth` of the loops (t, z, y, x) of Code 1
+ *                       are collapsed into one parallel iteration space; each parallel
+ *                      iteration runs the remaining inner loops serially in one thread.
+ *   threads_per_block  64, 128, 256, 512 or 1024.
+ *   sites_per_thread   1, 2 or 4 parallel iterations per thread, block-cyclic:
+ *                      iteration = (blockIdx*S + k)*threads_per_block + threadIdx, k = 0..S-1.
+ * The layout axis of the sweep is the ctx's own layout (create one ctx per layout).
+ * Errors: NULL, UNSUPPORTED.
+ */
+DSLASH_API int dslash_set_variant(dslash_ctx *ctx, int collapse_depth, int threads_per_block, int sites_per_thread);
+DSLASH_API int dslash_get_variant(const dslash_ctx *ctx, int *collapse_depth, int *threads_per_block, int *sites_per_thread);
+
+/* Enumeration of the sweep space of BASELINE.json configs[4]: 4 x 5 x 3 x 2 = 120 variants.
+ * dslash_variant_at(i, ...) writes variant i (0 <= i < dslash_variant_count()); layout is
+ * DSLASH_AOS or DSLASH_SOA.  Order: layout slowest, then collapse depth, threads/block, sites/thread.
+ * Errors: NULL, UNSUPPORTED (index out of range). */
+DSLASH_API int dslash_variant_count(void);
+DSLASH_API int dslash_variant_at(int index, int *collapse_depth, int *threads_per_block, int *sites_per_thread, int *layout);
+
+/*
+ * Tuning of the tuned kernel: the thread block covers a tile of tile[0] x tile[1] x tile[2] x tile[3]
+ * sites (x, y, z, t); each extent a power of two, product in {32, 64, ..., 1024}.  Lattice extents
+ * need not be multiples of the tile (edge threads idle).  Errors: NULL, UNSUPPORTED.
+ */
+DSLASH_API int dslash_set_tile(dslash_ctx *ctx, const int tile[4]);
+DSLASH_API int dslash_get_tile(const dslash_ctx *ctx, int tile[4]);
+
+/*
+ * End-to-end application from HOST buffers in the canonical layout at the ctx's precision
+ * (the path of PAPER.md:138-148: map to the device, run the kernel, map back):
+ *   H2D copy of gauge and in -> pack -> dslash_apply -> unpack -> D2H copy of out, then the stream is
+ *   synchronised.  With DSLASH_MAP_TOFROM all three fields travel both ways (what an offload without
+ *   data analysis does); with DSLASH_MAP_MINIMAL only gauge,in go to the device and only out comes back.
+ *   out_host, in_host, gauge_host   host pointers (pinned memory makes the copies asynchronous and
+ *   faster; pageable memory works).  DSLASH_MAP_TOFROM reads out_host and rewrites in_host/gauge_host
+ *   with the identical values.
+ * The ctx owns the device staging buffers (allocated on first use, freed by dslash_destroy).
+ * h2d_bytes / d2h_bytes (optional, may be NULL) receive the bytes copied in each direction.
+ * Errors: NULL, UNSUPPORTED (map_mode), NOMEM, CUDA.
+ */
+DSLASH_API int dslash_apply_host(dslash_ctx *ctx, void *out_host, const void *in_host, const void *gauge_host, int map_mode,
+                      dslash_stream_t stream, size_t *h2d_bytes, size_t *d2h_bytes);
+
+/* Number of kernels this ctx has launched since creation (bench.py's gpu_launches claim). */
+DSLASH_API long long dslash_launch_count(const dslash_ctx *ctx);
+
+/* The cudaError_t of the last failed CUDA call made through this ctx (0 = none). */
+DSLASH_API int dslash_last_cuda_error(const dslash_ctx *ctx);
+
+/* Static, NUL-terminated name of a status code ("DSLASH_OK", "DSLASH_ERR_ALIGN: ...", ...). */
+DSLASH_API const char *dslash_error_string(int status);
+
+/* Library version, "major.minor" as a static string. */
+DSLASH_API const char *dslash_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DSLASH_B200_H */

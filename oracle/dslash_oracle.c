@@ -38,7 +38,8 @@
  * NumPy straight from Eq. 1, P8 translation covariance, P9 even/odd parity, P10 norm bound and
  * linearity, P11 second moment.  Every exported function below is pinned by these.
  *
- * Build: gcc -O2 -std=c99 -fopenmp -fPIC -shared (see oracle/build.py).  OpenMP is used only to
+ * Build: gcc -O2 -std=c99 -fcx-limited-range -fopenmp -fPIC -shared (see oracle/build.py; the flag makes
+ * a complex product the four-multiply textbook formula instead of a call to __muldc3).  OpenMP is used only to
  * split the outermost (t) loop across cores when the oracle is timed as the CPU baseline.
  */
 #include <complex.h>

@@ -1,0 +1,196 @@
+"""Thin ctypes binding of libdslash_b200.so: the same names as include/dslash_b200.h, argument
+marshalling only.  Every step of the path runs in the library's CUDA kernels; there is no Python or
+CPU fallback.  Importing this module loads the library and raises ImportError if it is missing or
+does not export a declared symbol (build it with `python -m paper_2301_03636_b200.build`).
+
+Pointers are passed as plain integers (e.g. `tensor.data_ptr()`, `ndarray.ctypes.data`); streams as
+the integer value of a cudaStream_t (e.g. `torch.cuda.current_stream().cuda_stream`).  Functions
+that return a status in C raise DslashError on a non-zero status here and return their outputs.
+"""
+import ctypes
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libdslash_b200.so")
+
+DSLASH_FP64, DSLASH_FP32 = 0, 1
+DSLASH_AOS, DSLASH_SOA, DSLASH_RECON12 = 0, 1, 16
+DSLASH_OK = 0
+DSLASH_ERR_NULL, DSLASH_ERR_DIMS, DSLASH_ERR_PRECISION, DSLASH_ERR_LAYOUT = -1, -2, -3, -4
+DSLASH_ERR_ALIGN, DSLASH_ERR_ALIAS, DSLASH_ERR_UNSUPPORTED, DSLASH_ERR_CUDA, DSLASH_ERR_NOMEM = -5, -6, -7, -8, -9
+DSLASH_VARIANT_TUNED = 0
+DSLASH_MAP_MINIMAL, DSLASH_MAP_TOFROM = 0, 1
+
+_c_int_p = ctypes.POINTER(ctypes.c_int)
+_c_size_p = ctypes.POINTER(ctypes.c_size_t)
+_vp = ctypes.c_void_p
+
+# name -> (restype, argtypes); mirrors include/dslash_b200.h one to one
+SIGNATURES = {
+    "dslash_create": (ctypes.c_int, [ctypes.POINTER(_vp), _c_int_p, ctypes.c_int, ctypes.c_int]),
+    "dslash_destroy": (ctypes.c_int, [_vp]),
+    "dslash_apply": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp]),
+    "dslash_spinor_bytes": (ctypes.c_size_t, [_vp]),
+    "dslash_gauge_bytes": (ctypes.c_size_t, [_vp]),
+    "dslash_canonical_spinor_bytes": (ctypes.c_size_t, [_vp]),
+    "dslash_canonical_gauge_bytes": (ctypes.c_size_t, [_vp]),
+    "dslash_pack_spinor": (ctypes.c_int, [_vp, _vp, _vp, _vp]),
+    "dslash_unpack_spinor": (ctypes.c_int, [_vp, _vp, _vp, _vp]),
+    "dslash_pack_gauge": (ctypes.c_int, [_vp, _vp, _vp, _vp]),
+    "dslash_set_variant": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, ctypes.c_int]),
+    "dslash_get_variant": (ctypes.c_int, [_vp, _c_int_p, _c_int_p, _c_int_p]),
+    "dslash_variant_count": (ctypes.c_int, []),
+    "dslash_variant_at": (ctypes.c_int, [ctypes.c_int, _c_int_p, _c_int_p, _c_int_p, _c_int_p]),
+    "dslash_set_tile": (ctypes.c_int, [_vp, _c_int_p]),
+    "dslash_get_tile": (ctypes.c_int, [_vp, _c_int_p]),
+    "dslash_apply_host": (ctypes.c_int, [_vp, _vp, _vp, _vp, ctypes.c_int, _vp, _c_size_p, _c_size_p]),
+    "dslash_launch_count": (ctypes.c_longlong, [_vp]),
+    "dslash_last_cuda_error": (ctypes.c_int, [_vp]),
+    "dslash_error_string": (ctypes.c_char_p, [ctypes.c_int]),
+    "dslash_version": (ctypes.c_char_p, []),
+}
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            "libdslash_b200.so is missing (%s). Build it: python -m paper_2301_03636_b200.build. "
+            "There is no CPU fallback." % LIB_PATH)
+    try:
+        lib = ctypes.CDLL(LIB_PATH)
+    except OSError as e:  # pragma: no cover
+        raise ImportError("cannot load %s: %s" % (LIB_PATH, e))
+    for name, (res, args) in SIGNATURES.items():
+        try:
+            fn = getattr(lib, name)
+        except AttributeError:
+            raise ImportError("%s does not export %s" % (LIB_PATH, name))
+        fn.restype = res
+        fn.argtypes = args
+    return lib
+
+
+_lib = _load()
+
+
+class DslashError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = int(status)
+        super().__init__("%s: %s" % (where, dslash_error_string(status)))
+
+
+def _check(status, where):
+    if status != DSLASH_OK:
+        raise DslashError(status, where)
+
+
+def _ptr(p):
+    return _vp(int(p) if p else None)
+
+
+def dslash_error_string(status: int) -> str:
+    return _lib.dslash_error_string(int(status)).decode()
+
+
+def dslash_version() -> str:
+    return _lib.dslash_version().decode()
+
+
+def dslash_create(dims, precision: int, layout: int) -> int:
+    """Returns the ctx handle (an integer address). dims = (L_X, L_Y, L_Z, L_T)."""
+    ctx = _vp()
+    arr = (ctypes.c_int * 4)(*[int(d) for d in dims]) if dims is not None else None
+    _check(_lib.dslash_create(ctypes.byref(ctx), arr, int(precision), int(layout)), "dslash_create")
+    return ctx.value
+
+
+def dslash_destroy(ctx) -> None:
+    _check(_lib.dslash_destroy(_ptr(ctx)), "dslash_destroy")
+
+
+def dslash_apply(ctx, out, inp, gauge, stream=0) -> None:
+    _check(_lib.dslash_apply(_ptr(ctx), _ptr(out), _ptr(inp), _ptr(gauge), _ptr(stream)), "dslash_apply")
+
+
+def dslash_apply_status(ctx, out, inp, gauge, stream=0) -> int:
+    """dslash_apply returning the raw status instead of raising (error-path tests)."""
+    return int(_lib.dslash_apply(_ptr(ctx), _ptr(out), _ptr(inp), _ptr(gauge), _ptr(stream)))
+
+
+def dslash_spinor_bytes(ctx) -> int:
+    return int(_lib.dslash_spinor_bytes(_ptr(ctx)))
+
+
+def dslash_gauge_bytes(ctx) -> int:
+    return int(_lib.dslash_gauge_bytes(_ptr(ctx)))
+
+
+def dslash_canonical_spinor_bytes(ctx) -> int:
+    return int(_lib.dslash_canonical_spinor_bytes(_ptr(ctx)))
+
+
+def dslash_canonical_gauge_bytes(ctx) -> int:
+    return int(_lib.dslash_canonical_gauge_bytes(_ptr(ctx)))
+
+
+def dslash_pack_spinor(ctx, dst_native, src_canonical, stream=0) -> None:
+    _check(_lib.dslash_pack_spinor(_ptr(ctx), _ptr(dst_native), _ptr(src_canonical), _ptr(stream)), "dslash_pack_spinor")
+
+
+def dslash_unpack_spinor(ctx, dst_canonical, src_native, stream=0) -> None:
+    _check(_lib.dslash_unpack_spinor(_ptr(ctx), _ptr(dst_canonical), _ptr(src_native), _ptr(stream)),
+           "dslash_unpack_spinor")
+
+
+def dslash_pack_gauge(ctx, dst_native, src_canonical, stream=0) -> None:
+    _check(_lib.dslash_pack_gauge(_ptr(ctx), _ptr(dst_native), _ptr(src_canonical), _ptr(stream)), "dslash_pack_gauge")
+
+
+def dslash_set_variant(ctx, collapse_depth: int, threads_per_block: int = 0, sites_per_thread: int = 0) -> None:
+    _check(_lib.dslash_set_variant(_ptr(ctx), int(collapse_depth), int(threads_per_block), int(sites_per_thread)),
+           "dslash_set_variant")
+
+
+def dslash_get_variant(ctx):
+    d, b, s = ctypes.c_int(), ctypes.c_int(), ctypes.c_int()
+    _check(_lib.dslash_get_variant(_ptr(ctx), ctypes.byref(d), ctypes.byref(b), ctypes.byref(s)), "dslash_get_variant")
+    return d.value, b.value, s.value
+
+
+def dslash_variant_count() -> int:
+    return int(_lib.dslash_variant_count())
+
+
+def dslash_variant_at(index: int):
+    """(collapse_depth, threads_per_block, sites_per_thread, layout) of sweep variant `index`."""
+    d, b, s, l = ctypes.c_int(), ctypes.c_int(), ctypes.c_int(), ctypes.c_int()
+    _check(_lib.dslash_variant_at(int(index), ctypes.byref(d), ctypes.byref(b), ctypes.byref(s), ctypes.byref(l)),
+           "dslash_variant_at")
+    return d.value, b.value, s.value, l.value
+
+
+def dslash_set_tile(ctx, tile) -> None:
+    arr = (ctypes.c_int * 4)(*[int(t) for t in tile])
+    _check(_lib.dslash_set_tile(_ptr(ctx), arr), "dslash_set_tile")
+
+
+def dslash_get_tile(ctx):
+    arr = (ctypes.c_int * 4)()
+    _check(_lib.dslash_get_tile(_ptr(ctx), arr), "dslash_get_tile")
+    return tuple(arr)
+
+
+def dslash_apply_host(ctx, out_host, in_host, gauge_host, map_mode: int = DSLASH_MAP_MINIMAL, stream=0):
+    """Returns (h2d_bytes, d2h_bytes)."""
+    h2d, d2h = ctypes.c_size_t(), ctypes.c_size_t()
+    _check(_lib.dslash_apply_host(_ptr(ctx), _ptr(out_host), _ptr(in_host), _ptr(gauge_host), int(map_mode), _ptr(stream),
+                                  ctypes.byref(h2d), ctypes.byref(d2h)), "dslash_apply_host")
+    return h2d.value, d2h.value
+
+
+def dslash_launch_count(ctx) -> int:
+    return int(_lib.dslash_launch_count(_ptr(ctx)))
+
+
+def dslash_last_cuda_error(ctx) -> int:
+    return int(_lib.dslash_last_cuda_error(_ptr(ctx)))

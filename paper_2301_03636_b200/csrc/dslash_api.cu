@@ -1,0 +1,340 @@
+// dslash_api.cu -- the C ABI of libdslash_b200.so (see include/dslash_b200.h for the contract).
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <new>
+
+#include "../../include/dslash_b200.h"
+#include "dslash_kernels.cuh"
+
+using namespace dslash;
+
+struct dslash_ctx {
+    Geom geom;
+    int precision;
+    int layout_base;  // LAYOUT_AOS / LAYOUT_SOA
+    int recon;        // 18 or 12
+    int device;
+    int var_depth, var_tpb, var_spt;
+    int tile[4];
+    TileGeom tg;
+    long long launches;
+    int last_cuda;
+    // staging buffers of dslash_apply_host (device memory, owned)
+    void* d_can[3];  // canonical gauge, in, out
+    void* d_nat[3];  // native gauge, in, out (alias d_can when the native layout is the canonical one)
+};
+
+static int cuda_fail(dslash_ctx* c, cudaError_t e) {
+    if (c) c->last_cuda = (int)e;
+    return DSLASH_ERR_CUDA;
+}
+
+static size_t real_bytes(const dslash_ctx* c) { return c->precision == DSLASH_FP64 ? 8u : 4u; }
+
+static int ilog2_exact(int v) {
+    int l = 0;
+    while ((1 << l) < v) ++l;
+    return ((1 << l) == v) ? l : -1;
+}
+
+static void set_tile_geom(dslash_ctx* c, const int tile[4]) {
+    for (int d = 0; d < 4; ++d) {
+        c->tile[d] = tile[d];
+        c->tg.lb[d] = ilog2_exact(tile[d]);
+        c->tg.nt[d] = (c->geom.L[d] + tile[d] - 1) / tile[d];
+    }
+}
+
+// Default tile: grow towards 8 x 4 x 4 x 1 (128 threads), never beyond the next power of two of an extent;
+// leftover threads go to the other directions in the order t, z, y, x.
+static void default_tile(const dslash_ctx* c, int tile[4]) {
+    const int want[4] = {8, 4, 4, 1};
+    int cap[4];
+    for (int d = 0; d < 4; ++d) {
+        cap[d] = 1;
+        while (cap[d] < c->geom.L[d]) cap[d] <<= 1;
+        tile[d] = want[d] < cap[d] ? want[d] : cap[d];
+    }
+    const int order[4] = {3, 2, 1, 0};
+    bool grew = true;
+    while (tile[0] * tile[1] * tile[2] * tile[3] < 128 && grew) {
+        grew = false;
+        for (int k = 0; k < 4 && tile[0] * tile[1] * tile[2] * tile[3] < 128; ++k) {
+            const int d = order[k];
+            if (tile[d] < cap[d]) {
+                tile[d] <<= 1;
+                grew = true;
+            }
+        }
+    }
+}
+
+extern "C" {
+
+int dslash_create(dslash_ctx** ctx, const int dims[4], int precision, int layout) {
+    if (!ctx || !dims) return DSLASH_ERR_NULL;
+    *ctx = nullptr;
+    unsigned long long V = 1;
+    for (int d = 0; d < 4; ++d) {
+        if (dims[d] < 1) return DSLASH_ERR_DIMS;
+        V *= (unsigned long long)dims[d];
+        if (V * 36ull >= (1ull << 31)) return DSLASH_ERR_DIMS;
+    }
+    if (precision != DSLASH_FP64 && precision != DSLASH_FP32) return DSLASH_ERR_PRECISION;
+    const int base = layout & ~DSLASH_RECON12;
+    if (base != DSLASH_AOS && base != DSLASH_SOA) return DSLASH_ERR_LAYOUT;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) {
+        (void)cudaGetLastError();
+        return DSLASH_ERR_CUDA;
+    }
+    dslash_ctx* c = new (std::nothrow) dslash_ctx();
+    if (!c) return DSLASH_ERR_NOMEM;
+    for (int d = 0; d < 4; ++d) c->geom.L[d] = dims[d];
+    c->geom.V = (unsigned)V;
+    c->precision = precision;
+    c->layout_base = base == DSLASH_SOA ? LAYOUT_SOA : LAYOUT_AOS;
+    c->recon = (layout & DSLASH_RECON12) ? 12 : 18;
+    c->device = dev;
+    c->var_depth = DSLASH_VARIANT_TUNED;
+    c->var_tpb = 0;
+    c->var_spt = 0;
+    int tile[4];
+    default_tile(c, tile);
+    set_tile_geom(c, tile);
+    c->launches = 0;
+    c->last_cuda = 0;
+    for (int i = 0; i < 3; ++i) c->d_can[i] = c->d_nat[i] = nullptr;
+    *ctx = c;
+    return DSLASH_OK;
+}
+
+int dslash_destroy(dslash_ctx* c) {
+    if (!c) return DSLASH_OK;
+    int rc = DSLASH_OK;
+    bool any = false;
+    for (int i = 0; i < 3; ++i) any = any || c->d_can[i] || c->d_nat[i];
+    if (any) {
+        if (cudaDeviceSynchronize() != cudaSuccess) rc = DSLASH_ERR_CUDA;
+        for (int i = 0; i < 3; ++i) {
+            if (c->d_nat[i] && c->d_nat[i] != c->d_can[i]) cudaFree(c->d_nat[i]);
+            if (c->d_can[i]) cudaFree(c->d_can[i]);
+        }
+    }
+    delete c;
+    return rc;
+}
+
+size_t dslash_spinor_bytes(const dslash_ctx* c) { return c ? (size_t)c->geom.V * 24u * real_bytes(c) : 0; }
+size_t dslash_gauge_bytes(const dslash_ctx* c) {
+    return c ? (size_t)c->geom.V * 4u * (c->recon == 12 ? 12u : 18u) * real_bytes(c) : 0;
+}
+size_t dslash_canonical_spinor_bytes(const dslash_ctx* c) { return c ? (size_t)c->geom.V * 24u * real_bytes(c) : 0; }
+size_t dslash_canonical_gauge_bytes(const dslash_ctx* c) { return c ? (size_t)c->geom.V * 72u * real_bytes(c) : 0; }
+
+static bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+static bool overlap(const void* a, size_t na, const void* b, size_t nb) {
+    const uintptr_t A = reinterpret_cast<uintptr_t>(a), B = reinterpret_cast<uintptr_t>(b);
+    return A < B + nb && B < A + na;
+}
+
+int dslash_apply(dslash_ctx* c, void* out, const void* in, const void* gauge, dslash_stream_t stream) {
+    if (!c || !out || !in || !gauge) return DSLASH_ERR_NULL;
+    if (misaligned(out) || misaligned(in) || misaligned(gauge)) return DSLASH_ERR_ALIGN;
+    const size_t sb = dslash_spinor_bytes(c);
+    if (overlap(out, sb, in, sb)) return DSLASH_ERR_ALIAS;
+    LaunchArgs a{out, in, gauge, c->geom, static_cast<cudaStream_t>(stream)};
+    cudaError_t e;
+    if (c->var_depth == DSLASH_VARIANT_TUNED)
+        e = launch_tuned(c->precision, c->layout_base, c->recon, a, c->tg);
+    else
+        e = launch_variant(c->precision, c->layout_base, c->recon, a, c->var_depth, c->var_tpb, c->var_spt);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    c->launches += 1;
+    return DSLASH_OK;
+}
+
+int dslash_pack_spinor(dslash_ctx* c, void* dst, const void* src, dslash_stream_t stream) {
+    if (!c || !dst || !src) return DSLASH_ERR_NULL;
+    if (misaligned(dst) || misaligned(src)) return DSLASH_ERR_ALIGN;
+    cudaError_t e = launch_convert_spinor(c->precision, c->layout_base, dst, src, c->geom.V, 0, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    if (c->layout_base == LAYOUT_SOA) c->launches += 1;
+    return DSLASH_OK;
+}
+
+int dslash_unpack_spinor(dslash_ctx* c, void* dst, const void* src, dslash_stream_t stream) {
+    if (!c || !dst || !src) return DSLASH_ERR_NULL;
+    if (misaligned(dst) || misaligned(src)) return DSLASH_ERR_ALIGN;
+    cudaError_t e = launch_convert_spinor(c->precision, c->layout_base, dst, src, c->geom.V, 1, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    if (c->layout_base == LAYOUT_SOA) c->launches += 1;
+    return DSLASH_OK;
+}
+
+int dslash_pack_gauge(dslash_ctx* c, void* dst, const void* src, dslash_stream_t stream) {
+    if (!c || !dst || !src) return DSLASH_ERR_NULL;
+    if (misaligned(dst) || misaligned(src)) return DSLASH_ERR_ALIGN;
+    cudaError_t e = launch_pack_gauge(c->precision, c->layout_base, c->recon, dst, src, c->geom.V, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    if (!(c->layout_base == LAYOUT_AOS && c->recon == 18)) c->launches += 1;
+    return DSLASH_OK;
+}
+
+static const int kTpb[5] = {64, 128, 256, 512, 1024};
+static const int kSpt[3] = {1, 2, 4};
+
+int dslash_set_variant(dslash_ctx* c, int depth, int tpb, int spt) {
+    if (!c) return DSLASH_ERR_NULL;
+    if (depth == DSLASH_VARIANT_TUNED) {
+        c->var_depth = DSLASH_VARIANT_TUNED;
+        c->var_tpb = c->var_spt = 0;
+        return DSLASH_OK;
+    }
+    if (depth < 1 || depth > 4) return DSLASH_ERR_UNSUPPORTED;
+    bool ok = false;
+    for (int i = 0; i < 5; ++i) ok = ok || tpb == kTpb[i];
+    if (!ok) return DSLASH_ERR_UNSUPPORTED;
+    ok = false;
+    for (int i = 0; i < 3; ++i) ok = ok || spt == kSpt[i];
+    if (!ok) return DSLASH_ERR_UNSUPPORTED;
+    c->var_depth = depth;
+    c->var_tpb = tpb;
+    c->var_spt = spt;
+    return DSLASH_OK;
+}
+
+int dslash_get_variant(const dslash_ctx* c, int* depth, int* tpb, int* spt) {
+    if (!c || !depth || !tpb || !spt) return DSLASH_ERR_NULL;
+    *depth = c->var_depth;
+    *tpb = c->var_tpb;
+    *spt = c->var_spt;
+    return DSLASH_OK;
+}
+
+int dslash_variant_count(void) { return 2 * 4 * 5 * 3; }
+
+int dslash_variant_at(int index, int* depth, int* tpb, int* spt, int* layout) {
+    if (!depth || !tpb || !spt || !layout) return DSLASH_ERR_NULL;
+    if (index < 0 || index >= dslash_variant_count()) return DSLASH_ERR_UNSUPPORTED;
+    *spt = kSpt[index % 3];
+    index /= 3;
+    *tpb = kTpb[index % 5];
+    index /= 5;
+    *depth = 1 + index % 4;
+    index /= 4;
+    *layout = index == 0 ? DSLASH_AOS : DSLASH_SOA;
+    return DSLASH_OK;
+}
+
+int dslash_set_tile(dslash_ctx* c, const int tile[4]) {
+    if (!c || !tile) return DSLASH_ERR_NULL;
+    long long prod = 1;
+    for (int d = 0; d < 4; ++d) {
+        if (tile[d] < 1 || tile[d] > 1024 || ilog2_exact(tile[d]) < 0) return DSLASH_ERR_UNSUPPORTED;
+        prod *= tile[d];
+    }
+    if (prod < 32 || prod > 1024) return DSLASH_ERR_UNSUPPORTED;
+    set_tile_geom(c, tile);
+    return DSLASH_OK;
+}
+
+int dslash_get_tile(const dslash_ctx* c, int tile[4]) {
+    if (!c || !tile) return DSLASH_ERR_NULL;
+    for (int d = 0; d < 4; ++d) tile[d] = c->tile[d];
+    return DSLASH_OK;
+}
+
+int dslash_apply_host(dslash_ctx* c, void* out_host, const void* in_host, const void* gauge_host, int map_mode,
+                      dslash_stream_t stream_, size_t* h2d_bytes, size_t* d2h_bytes) {
+    if (!c || !out_host || !in_host || !gauge_host) return DSLASH_ERR_NULL;
+    if (map_mode != DSLASH_MAP_MINIMAL && map_mode != DSLASH_MAP_TOFROM) return DSLASH_ERR_UNSUPPORTED;
+    cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+    const size_t can_bytes[3] = {dslash_canonical_gauge_bytes(c), dslash_canonical_spinor_bytes(c),
+                                 dslash_canonical_spinor_bytes(c)};
+    const size_t nat_bytes[3] = {dslash_gauge_bytes(c), dslash_spinor_bytes(c), dslash_spinor_bytes(c)};
+    const bool native_is_canonical[3] = {c->layout_base == LAYOUT_AOS && c->recon == 18, c->layout_base == LAYOUT_AOS,
+                                         c->layout_base == LAYOUT_AOS};
+    for (int i = 0; i < 3; ++i) {
+        if (!c->d_can[i]) {
+            cudaError_t e = cudaMalloc(&c->d_can[i], can_bytes[i]);
+            if (e != cudaSuccess) {
+                c->d_can[i] = nullptr;
+                c->last_cuda = (int)e;
+                (void)cudaGetLastError();
+                return DSLASH_ERR_NOMEM;
+            }
+        }
+        if (!c->d_nat[i]) {
+            if (native_is_canonical[i]) {
+                c->d_nat[i] = c->d_can[i];
+            } else {
+                cudaError_t e = cudaMalloc(&c->d_nat[i], nat_bytes[i]);
+                if (e != cudaSuccess) {
+                    c->d_nat[i] = nullptr;
+                    c->last_cuda = (int)e;
+                    (void)cudaGetLastError();
+                    return DSLASH_ERR_NOMEM;
+                }
+            }
+        }
+    }
+    size_t h2d = 0, d2h = 0;
+    cudaError_t e;
+    // map(to: gauge, in) [+ map(tofrom: out) copies out in as well]
+    e = cudaMemcpyAsync(c->d_can[0], gauge_host, can_bytes[0], cudaMemcpyHostToDevice, stream);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    e = cudaMemcpyAsync(c->d_can[1], in_host, can_bytes[1], cudaMemcpyHostToDevice, stream);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    h2d += can_bytes[0] + can_bytes[1];
+    if (map_mode == DSLASH_MAP_TOFROM) {
+        e = cudaMemcpyAsync(c->d_can[2], out_host, can_bytes[2], cudaMemcpyHostToDevice, stream);
+        if (e != cudaSuccess) return cuda_fail(c, e);
+        h2d += can_bytes[2];
+    }
+    int rc;
+    if (!native_is_canonical[0] && (rc = dslash_pack_gauge(c, c->d_nat[0], c->d_can[0], stream)) != DSLASH_OK) return rc;
+    if (!native_is_canonical[1] && (rc = dslash_pack_spinor(c, c->d_nat[1], c->d_can[1], stream)) != DSLASH_OK) return rc;
+    if ((rc = dslash_apply(c, c->d_nat[2], c->d_nat[1], c->d_nat[0], stream)) != DSLASH_OK) return rc;
+    if (!native_is_canonical[2] && (rc = dslash_unpack_spinor(c, c->d_can[2], c->d_nat[2], stream)) != DSLASH_OK) return rc;
+    e = cudaMemcpyAsync(out_host, c->d_can[2], can_bytes[2], cudaMemcpyDeviceToHost, stream);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    d2h += can_bytes[2];
+    if (map_mode == DSLASH_MAP_TOFROM) {
+        e = cudaMemcpyAsync(const_cast<void*>(gauge_host), c->d_can[0], can_bytes[0], cudaMemcpyDeviceToHost, stream);
+        if (e != cudaSuccess) return cuda_fail(c, e);
+        e = cudaMemcpyAsync(const_cast<void*>(in_host), c->d_can[1], can_bytes[1], cudaMemcpyDeviceToHost, stream);
+        if (e != cudaSuccess) return cuda_fail(c, e);
+        d2h += can_bytes[0] + can_bytes[1];
+    }
+    e = cudaStreamSynchronize(stream);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    if (h2d_bytes) *h2d_bytes = h2d;
+    if (d2h_bytes) *d2h_bytes = d2h;
+    return DSLASH_OK;
+}
+
+long long dslash_launch_count(const dslash_ctx* c) { return c ? c->launches : 0; }
+int dslash_last_cuda_error(const dslash_ctx* c) { return c ? c->last_cuda : 0; }
+
+const char* dslash_error_string(int status) {
+    switch (status) {
+        case DSLASH_OK: return "DSLASH_OK";
+        case DSLASH_ERR_NULL: return "DSLASH_ERR_NULL: a required pointer argument is NULL";
+        case DSLASH_ERR_DIMS: return "DSLASH_ERR_DIMS: lattice extent < 1 or lattice too large for 32-bit indexing";
+        case DSLASH_ERR_PRECISION: return "DSLASH_ERR_PRECISION: precision must be DSLASH_FP64 or DSLASH_FP32";
+        case DSLASH_ERR_LAYOUT: return "DSLASH_ERR_LAYOUT: layout must be DSLASH_AOS or DSLASH_SOA, optionally | DSLASH_RECON12";
+        case DSLASH_ERR_ALIGN: return "DSLASH_ERR_ALIGN: field pointers must be 16-byte aligned";
+        case DSLASH_ERR_ALIAS: return "DSLASH_ERR_ALIAS: out must not overlap in";
+        case DSLASH_ERR_UNSUPPORTED: return "DSLASH_ERR_UNSUPPORTED: parameter outside the supported set";
+        case DSLASH_ERR_CUDA: return "DSLASH_ERR_CUDA: a CUDA runtime call failed (see dslash_last_cuda_error)";
+        case DSLASH_ERR_NOMEM: return "DSLASH_ERR_NOMEM: allocation failed";
+        default: return "DSLASH_ERR_?: unknown status code";
+    }
+}
+
+const char* dslash_version(void) { return "0.1"; }
+
+}  // extern "C"

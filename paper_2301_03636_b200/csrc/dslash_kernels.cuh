@@ -1,0 +1,37 @@
+// dslash_kernels.cuh -- kernel declarations shared by the translation units of libdslash_b200.so.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "dslash_site.cuh"
+
+namespace dslash {
+
+// Tile decomposition of the tuned kernel: a thread block covers 2^lb[0] x 2^lb[1] x 2^lb[2] x 2^lb[3]
+// sites; nt[d] = ceil(L[d] / 2^lb[d]) tiles along d; tiles are numbered x fastest.
+struct TileGeom {
+    int lb[4];
+    int nt[4];
+};
+
+struct LaunchArgs {
+    void* out;
+    const void* in;
+    const void* gauge;
+    Geom geom;
+    cudaStream_t stream;
+};
+
+// Advisor-style variant (SURVEY.md section 8(d) "Sweep variant semantics"): collapse the first `depth`
+// loops of (t,z,y,x); every parallel iteration runs the remaining loops serially.
+cudaError_t launch_variant(int precision, int layout_base, int recon, const LaunchArgs& a, int depth, int tpb, int spt);
+
+// Tuned kernel.
+cudaError_t launch_tuned(int precision, int layout_base, int recon, const LaunchArgs& a, const TileGeom& tg);
+
+// Layout module.  dir 0: canonical -> native (pack), 1: native -> canonical (unpack).
+cudaError_t launch_convert_spinor(int precision, int layout_base, void* dst, const void* src, unsigned V, int dir,
+                                  cudaStream_t stream);
+cudaError_t launch_pack_gauge(int precision, int layout_base, int recon, void* dst, const void* src, unsigned V,
+                              cudaStream_t stream);
+
+}  // namespace dslash

@@ -1,0 +1,105 @@
+"""Device-side plumbing around the C ABI: torch owns device memory and streams, nothing else.
+
+`Lattice` wraps one dslash_ctx plus the handful of copies a caller needs to get canonical NumPy
+fields to the device in the ctx's native layout and back.  All arithmetic and all layout
+conversion happen in libdslash_b200.so (dslash_pack_* / dslash_apply / dslash_unpack_spinor).
+"""
+import numpy as np
+import torch
+
+from . import binding as B
+
+PRECISIONS = {"f64": B.DSLASH_FP64, "f32": B.DSLASH_FP32}
+LAYOUTS = {"aos": B.DSLASH_AOS, "soa": B.DSLASH_SOA}
+
+
+class Lattice:
+    def __init__(self, dims, precision="f64", layout="soa", recon12=False, device="cuda:0"):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2301_03636_b200 needs a CUDA device; there is no CPU fallback")
+        self.dims = tuple(int(d) for d in dims)
+        self.volume = int(np.prod(self.dims))
+        self.precision, self.layout, self.recon12 = precision, layout, bool(recon12)
+        self.np_dtype = np.float64 if precision == "f64" else np.float32
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.ctx = B.dslash_create(self.dims, PRECISIONS[precision], LAYOUTS[layout] | (B.DSLASH_RECON12 if recon12 else 0))
+
+    # -- lifetime
+    def close(self):
+        if getattr(self, "ctx", None):
+            B.dslash_destroy(self.ctx)
+            self.ctx = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):  # pragma: no cover
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- memory
+    @staticmethod
+    def stream():
+        return torch.cuda.current_stream().cuda_stream
+
+    def _bytes(self, n):
+        return torch.empty(int(n), dtype=torch.uint8, device=self.device)
+
+    def new_spinor(self):
+        return self._bytes(B.dslash_spinor_bytes(self.ctx))
+
+    def new_gauge(self):
+        return self._bytes(B.dslash_gauge_bytes(self.ctx))
+
+    def _to_device(self, a):
+        a = np.ascontiguousarray(a, dtype=self.np_dtype)
+        return torch.from_numpy(a.reshape(-1).view(np.uint8)).to(self.device)
+
+    def upload_spinor(self, canonical):
+        """canonical NumPy spinor [T,Z,Y,X,4,3,2] -> native device buffer."""
+        assert canonical.size == self.volume * 24
+        src = self._to_device(canonical)
+        dst = self.new_spinor()
+        B.dslash_pack_spinor(self.ctx, dst.data_ptr(), src.data_ptr(), self.stream())
+        torch.cuda.current_stream().synchronize()
+        return dst
+
+    def upload_gauge(self, canonical):
+        """canonical NumPy gauge [T,Z,Y,X,4,3,3,2] (18 reals per link) -> native device buffer."""
+        assert canonical.size == self.volume * 72
+        src = self._to_device(canonical)
+        dst = self.new_gauge()
+        B.dslash_pack_gauge(self.ctx, dst.data_ptr(), src.data_ptr(), self.stream())
+        torch.cuda.current_stream().synchronize()
+        return dst
+
+    def download_spinor(self, native):
+        """native device spinor -> canonical NumPy [T,Z,Y,X,4,3,2] at the ctx's precision."""
+        dst = self._bytes(B.dslash_canonical_spinor_bytes(self.ctx))
+        B.dslash_unpack_spinor(self.ctx, dst.data_ptr(), native.data_ptr(), self.stream())
+        lx, ly, lz, lt = self.dims
+        return dst.cpu().numpy().view(self.np_dtype).reshape(lt, lz, ly, lx, 4, 3, 2)
+
+    # -- the operator
+    def apply(self, out, inp, gauge):
+        B.dslash_apply(self.ctx, out.data_ptr(), inp.data_ptr(), gauge.data_ptr(), self.stream())
+
+    def set_variant(self, depth, tpb=0, spt=0):
+        B.dslash_set_variant(self.ctx, depth, tpb, spt)
+
+    def set_tile(self, tile):
+        B.dslash_set_tile(self.ctx, tile)
+
+    def dslash(self, gauge_canonical, spinor_canonical):
+        """Convenience: canonical NumPy in -> canonical NumPy out (one application on the device)."""
+        g = self.upload_gauge(gauge_canonical)
+        p = self.upload_spinor(spinor_canonical)
+        o = self.new_spinor()
+        self.apply(o, p, g)
+        return self.download_spinor(o)

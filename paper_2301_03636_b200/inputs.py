@@ -22,6 +22,9 @@ Canonical layout: dims = (L_X, L_Y, L_Z, L_T), x 
 """
 from __future__ import annotations
 
+import concurrent.futures
+import os
+
 import numpy as np
 
 BASE_SEED = 230103636  # arXiv id of the paper; config k uses BASE_SEED + k
@@ -71,12 +74,26 @@ def check_su3(u: np.ndarray, tol: float = 5e-15) -> None:
         raise AssertionError("SU(3) generator post-condition failed: |UU^+-1|=%g |det-1|=%g" % (err_u, err_d))
 
 
+def _map_chunks(fn, nchunks: int) -> None:
+    """Run fn(c) for every chunk; chunks are independent (own RNG stream, own output slice), so a
+    thread pool changes nothing but the wall time (NumPy releases the GIL in its kernels)."""
+    workers = min(nchunks, len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1))
+    if workers <= 1:
+        for c in range(nchunks):
+            fn(c)
+        return
+    with concurrent.futures.ThreadPoolExecutor(max_workers=workers) as ex:
+        list(ex.map(fn, range(nchunks)))
+
+
 def gauge_field(dims, seed: int, check: bool = True) -> np.ndarray:
     """Haar-random SU(3) links, float64 [L_T, L_Z, L_Y, L_X, 4, 3, 3, 2]."""
     lx, ly, lz, lt = (int(d) for d in dims)
     v = volume(dims)
     out = np.empty((v, 4, 3, 3, 2), dtype=np.float64)
-    for c, s0 in enumerate(range(0, v, CHUNK_SITES)):
+
+    def one(c):
+        s0 = c * CHUNK_SITES
         n = min(CHUNK_SITES, v - s0)
         u = haar_su3(n * 4, _rng(seed, _STREAM_GAUGE, c))
         if check:
@@ -84,6 +101,8 @@ def gauge_field(dims, seed: int, check: bool = True) -> np.ndarray:
         blk = out[s0:s0 + n].reshape(n * 4, 3, 3, 2)
         blk[..., 0] = u.real
         blk[..., 1] = u.imag
+
+    _map_chunks(one, (v + CHUNK_SITES - 1) // CHUNK_SITES)
     return out.reshape(lt, lz, ly, lx, 4, 3, 3, 2)
 
 
@@ -92,9 +111,13 @@ def spinor_field(dims, seed: int) -> np.ndarray:
     lx, ly, lz, lt = (int(d) for d in dims)
     v = volume(dims)
     out = np.empty((v, 4, 3, 2), dtype=np.float64)
-    for c, s0 in enumerate(range(0, v, CHUNK_SITES)):
+
+    def one(c):
+        s0 = c * CHUNK_SITES
         n = min(CHUNK_SITES, v - s0)
         out[s0:s0 + n] = _rng(seed, _STREAM_SPINOR, c).standard_normal((n, 4, 3, 2))
+
+    _map_chunks(one, (v + CHUNK_SITES - 1) // CHUNK_SITES)
     return out.reshape(lt, lz, ly, lx, 4, 3, 2)
 
 

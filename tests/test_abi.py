@@ -1,0 +1,113 @@
+"""CPU-only checks of the C ABI: the library builds, loads, exports every symbol that
+include/dslash_b200.h declares, and validates arguments before touching CUDA.  No compute calls."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "dslash_b200.h")
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2301_03636_b200 import build
+    build.build()  # no-op when the in-tree .so is newer than its sources
+    from paper_2301_03636_b200 import binding
+    return binding
+
+
+def declared_symbols():
+    text = open(HEADER).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(dslash_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_header_declares_the_north_star_calls():
+    names = declared_symbols()
+    for must in ("dslash_create", "dslash_apply", "dslash_destroy", "dslash_pack_spinor", "dslash_unpack_spinor",
+                 "dslash_pack_gauge", "dslash_set_variant", "dslash_apply_host"):
+        assert must in names
+
+
+def test_library_exports_every_declared_symbol(B):
+    lib = ctypes.CDLL(B.LIB_PATH)
+    for name in declared_symbols():
+        assert hasattr(lib, name), name
+    # and the binding mirrors the header one to one
+    assert sorted(B.SIGNATURES) == declared_symbols()
+    for name in declared_symbols():
+        assert hasattr(B, name), "binding lacks %s" % name
+
+
+def test_error_strings(B):
+    assert B.dslash_error_string(0) == "DSLASH_OK"
+    for code in range(-9, 0):
+        s = B.dslash_error_string(code)
+        assert s.startswith("DSLASH_ERR_") and "?" not in s
+    assert "?" in B.dslash_error_string(-99)
+    assert B.dslash_version() == "0.1"
+
+
+def test_argument_validation_precedes_cuda(B):
+    with pytest.raises(B.DslashError) as e:
+        B.dslash_create(None, B.DSLASH_FP64, B.DSLASH_SOA)
+    assert e.value.status == B.DSLASH_ERR_NULL
+    for dims, prec, lay, want in [
+        ((4, 4, 0, 4), B.DSLASH_FP64, B.DSLASH_SOA, B.DSLASH_ERR_DIMS),
+        ((4, 4, -1, 4), B.DSLASH_FP64, B.DSLASH_SOA, B.DSLASH_ERR_DIMS),
+        ((128, 128, 128, 64), B.DSLASH_FP64, B.DSLASH_SOA, B.DSLASH_ERR_DIMS),  # 36 V >= 2^31
+        ((4, 4, 4, 4), 2, B.DSLASH_SOA, B.DSLASH_ERR_PRECISION),
+        ((4, 4, 4, 4), B.DSLASH_FP64, 2, B.DSLASH_ERR_LAYOUT),
+        ((4, 4, 4, 4), B.DSLASH_FP64, 32, B.DSLASH_ERR_LAYOUT),
+    ]:
+        with pytest.raises(B.DslashError) as e:
+            B.dslash_create(dims, prec, lay)
+        assert e.value.status == want, (dims, prec, lay)
+    # NULL ctx paths
+    assert B.dslash_spinor_bytes(None) == 0 and B.dslash_gauge_bytes(None) == 0
+    assert B.dslash_launch_count(None) == 0
+    B.dslash_destroy(None)  # no-op
+    assert B.dslash_apply_status(None, 16, 32, 48) == B.DSLASH_ERR_NULL
+    with pytest.raises(B.DslashError) as e:
+        B.dslash_set_variant(None, 1, 64, 1)
+    assert e.value.status == B.DSLASH_ERR_NULL
+
+
+def test_variant_enumeration_is_the_120_of_config_5(B):
+    n = B.dslash_variant_count()
+    assert n == 120
+    seen = {B.dslash_variant_at(i) for i in range(n)}
+    assert len(seen) == 120
+    assert {v[0] for v in seen} == {1, 2, 3, 4}
+    assert {v[1] for v in seen} == {64, 128, 256, 512, 1024}
+    assert {v[2] for v in seen} == {1, 2, 4}
+    assert {v[3] for v in seen} == {B.DSLASH_AOS, B.DSLASH_SOA}
+    for bad in (-1, 120):
+        with pytest.raises(B.DslashError) as e:
+            B.dslash_variant_at(bad)
+        assert e.value.status == B.DSLASH_ERR_UNSUPPORTED
+
+
+def test_no_cuda_device_is_an_error_not_a_fallback(B):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    with pytest.raises(B.DslashError) as e:
+        B.dslash_create((4, 4, 4, 4), B.DSLASH_FP64, B.DSLASH_SOA)
+    assert e.value.status == B.DSLASH_ERR_CUDA
+
+
+def test_product_does_not_import_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2301_03636_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", text, flags=re.M), f
+                assert "dslash_oracle" not in text, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c", ".h")):
+            text = open(os.path.join(ROOT, "oracle", f)).read()
+            assert not re.search(r"^\s*(import|from)\s+paper_2301_03636_b200\b", text, flags=re.M), f

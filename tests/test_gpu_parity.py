@@ -1,0 +1,271 @@
+"""GPU parity: the CUDA library (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star; metric = checks.parity_error, DESIGN.md Reading R10):
+    FP64 (18- and 12-real links)  e <= 1e-12
+    FP32                          e <= 1e-5   (oracle fed the fp32-rounded inputs promoted to fp64)
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f64": 1e-12, "f32": 1e-5}
+SEED = 230103636
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    import oracle
+    from paper_2301_03636_b200 import binding, checks, device, inputs
+    assert torch.cuda.is_available()
+
+    class E:
+        pass
+    e = E()
+    e.torch, e.oracle, e.B, e.checks, e.device, e.inputs = torch, oracle, binding, checks, device, inputs
+    return e
+
+
+_FIELD_CACHE = {}
+
+
+def fields_and_ref(env, dims, seed, precision, full=True, nsample=4096):
+    key = (tuple(dims), seed, precision, full)
+    if key not in _FIELD_CACHE:
+        _FIELD_CACHE.clear()  # keep one lattice at a time in host memory
+        g, p = env.inputs.fields(dims, seed, precision)
+        g64, p64 = env.inputs.promote(g), env.inputs.promote(p)
+        if full:
+            sites = None
+            ref = env.oracle.dslash(p64, g64, dims)
+        else:
+            sites = env.inputs.sample_sites(dims, nsample, seed)
+            ref = env.oracle.dslash_sites(p64, g64, dims, sites)
+        _FIELD_CACHE[key] = (g, p, ref, sites)
+    return _FIELD_CACHE[key]
+
+
+def gpu_vs_ref(env, lat, g, p, ref, sites=None):
+    out = lat.dslash(g, p)
+    if sites is not None:
+        out = out.reshape(-1, 4, 3, 2)[sites]
+    return env.checks.parity_error(out, ref)
+
+
+ALL_MODES = [(lay, r12) for lay in ("aos", "soa") for r12 in (False, True)]
+
+
+# ---------------------------------------------------------------- config 1: 4^4 FP64 (+ FP32), every layout
+@pytest.mark.parametrize("precision", ["f64", "f32"])
+@pytest.mark.parametrize("layout,recon12", ALL_MODES)
+def test_config1_4x4x4x4(env, precision, layout, recon12):
+    dims = (4, 4, 4, 4)
+    g, p, ref, _ = fields_and_ref(env, dims, SEED + 1, precision)
+    with env.device.Lattice(dims, precision, layout, recon12) as lat:
+        assert gpu_vs_ref(env, lat, g, p, ref) <= TOL[precision]
+        n0 = env.B.dslash_launch_count(lat.ctx)
+        o, pi, gi = lat.new_spinor(), lat.upload_spinor(p), lat.upload_gauge(g)
+        n1 = env.B.dslash_launch_count(lat.ctx)
+        lat.apply(o, pi, gi)
+        assert env.B.dslash_launch_count(lat.ctx) == n1 + 1  # exactly one kernel per apply
+        assert n1 >= n0
+
+
+# ---------------------------------------------------------------- ragged / degenerate lattices
+@pytest.mark.parametrize("dims", [(4, 6, 8, 10), (3, 5, 7, 2), (2, 2, 2, 2), (1, 1, 1, 1), (1, 2, 3, 4), (33, 3, 2, 5),
+                                  (10, 4, 6, 2)])
+@pytest.mark.parametrize("precision", ["f64", "f32"])
+def test_ragged_and_degenerate_extents(env, dims, precision):
+    g, p, ref, _ = fields_and_ref(env, dims, SEED + 11, precision)
+    for layout, recon12 in ALL_MODES:
+        with env.device.Lattice(dims, precision, layout, recon12) as lat:
+            assert gpu_vs_ref(env, lat, g, p, ref) <= TOL[precision], (layout, recon12, "tuned")
+            for depth, tpb, spt in [(4, 64, 1), (3, 128, 2), (2, 256, 4), (1, 512, 1), (4, 1024, 4)]:
+                lat.set_variant(depth, tpb, spt)
+                assert gpu_vs_ref(env, lat, g, p, ref) <= TOL[precision], (layout, recon12, depth, tpb, spt)
+
+
+@pytest.mark.parametrize("tile", [(32, 1, 1, 1), (8, 4, 4, 1), (4, 4, 4, 4), (2, 2, 2, 4), (16, 2, 2, 2), (8, 8, 8, 2),
+                                  (1, 1, 1, 32), (16, 4, 4, 4)])
+def test_tuned_kernel_every_tile_shape(env, tile):
+    dims = (12, 6, 10, 5)
+    g, p, ref, _ = fields_and_ref(env, dims, SEED + 12, "f64")
+    with env.device.Lattice(dims, "f64", "soa", False) as lat:
+        lat.set_tile(tile)
+        assert env.B.dslash_get_tile(lat.ctx) == tuple(tile)
+        assert gpu_vs_ref(env, lat, g, p, ref) <= TOL["f64"]
+
+
+# ---------------------------------------------------------------- config 2: 16^4 FP64
+@pytest.mark.parametrize("layout,recon12", ALL_MODES)
+def test_config2_16x16x16x16(env, layout, recon12):
+    dims = (16, 16, 16, 16)
+    g, p, ref, _ = fields_and_ref(env, dims, SEED + 2, "f64")
+    with env.device.Lattice(dims, "f64", layout, recon12) as lat:
+        assert gpu_vs_ref(env, lat, g, p, ref) <= TOL["f64"]
+
+
+# ---------------------------------------------------------------- config 5: all 120 sweep variants on 24^4 FP64
+def test_config5_all_120_variants_24x24x24x24(env):
+    dims = (24, 24, 24, 24)
+    g, p, ref, _ = fields_and_ref(env, dims, SEED + 5, "f64")
+    torch = env.torch
+    ref_t = torch.from_numpy(np.ascontiguousarray(ref)).cuda()
+    ref_c = torch.view_as_complex(ref_t)
+    rms = torch.sqrt(torch.mean(ref_c.abs() ** 2))
+    den = torch.maximum(ref_c.abs(), rms)
+    lats = {}
+    worst = 0.0
+    try:
+        for lay in ("aos", "soa"):
+            lat = env.device.Lattice(dims, "f64", lay, False)
+            lats[lay] = (lat, lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor(),
+                         lat._bytes(env.B.dslash_canonical_spinor_bytes(lat.ctx)))
+        for i in range(env.B.dslash_variant_count()):
+            depth, tpb, spt, layout = env.B.dslash_variant_at(i)
+            lat, gi, pi, o, can = lats["aos" if layout == env.B.DSLASH_AOS else "soa"]
+            o.zero_()
+            lat.set_variant(depth, tpb, spt)
+            lat.apply(o, pi, gi)
+            env.B.dslash_unpack_spinor(lat.ctx, can.data_ptr(), o.data_ptr(), lat.stream())
+            got_c = torch.view_as_complex(can.view(torch.float64).view(ref_t.shape))
+            e = float(((got_c - ref_c).abs() / den).max())  # same metric as checks.parity_error
+            assert e <= TOL["f64"], (depth, tpb, spt, layout, e)
+            worst = max(worst, e)
+        # and one variant through the NumPy metric, so the torch restatement above is itself checked
+        lat, gi, pi, o, can = lats["soa"]
+        lat.set_variant(4, 128, 1)
+        lat.apply(o, pi, gi)
+        e_np = env.checks.parity_error(lat.download_spinor(o), ref)
+        assert e_np <= TOL["f64"] and e_np > 0.0
+    finally:
+        for lat, *_ in lats.values():
+            lat.close()
+
+
+# ---------------------------------------------------------------- config 3: 32^3 x 64 FP64, 18- and 12-real links
+@pytest.mark.parametrize("recon12", [False, True])
+def test_config3_32x32x32x64_fp64(env, recon12):
+    dims = (32, 32, 32, 64)
+    g, p, ref, sites = fields_and_ref(env, dims, SEED + 3, "f64", full=False, nsample=8192)
+    with env.device.Lattice(dims, "f64", "soa", recon12) as lat:
+        assert gpu_vs_ref(env, lat, g, p, ref, sites) <= TOL["f64"]
+
+
+def test_config3_full_size_properties(env):
+    """Properties that hold at any size, on the bench configuration: unit gauge + constant spinor
+    gives 8 psi everywhere; translation of all fields by one site translates the result."""
+    dims = (32, 32, 32, 64)
+    lx, ly, lz, lt = dims
+    chi = np.random.default_rng(3).standard_normal((4, 3, 2))
+    psi = np.broadcast_to(chi, (lt, lz, ly, lx, 4, 3, 2))
+    u = np.zeros((lt, lz, ly, lx, 4, 3, 3, 2))
+    u[..., range(3), range(3), 0] = 1.0
+    with env.device.Lattice(dims, "f64", "soa", False) as lat:
+        out = lat.dslash(u, psi)
+        assert np.abs(out - 8.0 * psi).max() <= 1e-13
+
+
+# ---------------------------------------------------------------- config 4: 48^3 x 96 FP32 vs the FP64 oracle
+def test_config4_48x48x48x96_fp32(env):
+    dims = (48, 48, 48, 96)
+    g, p, ref, sites = fields_and_ref(env, dims, SEED + 4, "f32", full=False, nsample=8192)
+    with env.device.Lattice(dims, "f32", "soa", False) as lat:
+        assert gpu_vs_ref(env, lat, g, p, ref, sites) <= TOL["f32"]
+    _FIELD_CACHE.clear()
+
+
+# ---------------------------------------------------------------- invariants evaluated on the GPU itself
+def test_gpu_gauge_covariance_and_translation(env):
+    dims = (6, 4, 8, 10)
+    v = int(np.prod(dims))
+    g, p = env.inputs.fields(dims, SEED + 21)
+    gc = g[..., 0] + 1j * g[..., 1]
+    pc = p[..., 0] + 1j * p[..., 1]
+    G = env.inputs.haar_su3(v, np.random.default_rng(5)).reshape(dims[3], dims[2], dims[1], dims[0], 3, 3)
+    ug = np.empty_like(gc)
+    for mu in range(4):
+        ug[..., mu, :, :] = G @ gc[..., mu, :, :] @ np.conj(np.swapaxes(np.roll(G, -1, axis=3 - mu), -1, -2))
+    pg = np.einsum("tzyxij,tzyxaj->tzyxai", G, pc)
+    c2r = lambda a: np.ascontiguousarray(np.stack([a.real, a.imag], axis=-1))
+    with env.device.Lattice(dims, "f64", "soa", False) as lat:
+        lhs = lat.dslash(c2r(ug), c2r(pg))
+        rhs = lat.dslash(g, p)
+        rhs_c = np.einsum("tzyxij,tzyxaj->tzyxai", G, rhs[..., 0] + 1j * rhs[..., 1])
+        assert env.checks.parity_error(lhs, c2r(rhs_c)) <= 1e-12
+        for mu in range(4):
+            ax = 3 - mu
+            rolled = lat.dslash(np.roll(g, 1, axis=ax), np.roll(p, 1, axis=ax))
+            assert np.array_equal(rolled, np.roll(rhs, 1, axis=ax))  # same arithmetic, bit for bit
+
+
+# ---------------------------------------------------------------- layout module round trip
+@pytest.mark.parametrize("precision", ["f64", "f32"])
+@pytest.mark.parametrize("layout", ["aos", "soa"])
+def test_pack_unpack_round_trip_is_bit_exact(env, precision, layout):
+    dims = (5, 4, 3, 6)
+    g, p = env.inputs.fields(dims, SEED + 31, precision)
+    with env.device.Lattice(dims, precision, layout, False) as lat:
+        back = lat.download_spinor(lat.upload_spinor(p))
+        assert np.array_equal(back, p)
+        nat = lat.upload_gauge(g).cpu().numpy().view(lat.np_dtype)
+        v = lat.volume
+        if layout == "soa":
+            want = np.ascontiguousarray(np.moveaxis(g.reshape(v, 4, 9, 2), 0, 2)).reshape(-1)  # [mu][e][s][ri]
+        else:
+            want = g.reshape(-1)
+        assert np.array_equal(nat, want)
+    with env.device.Lattice(dims, precision, layout, True) as lat:
+        nat = lat.upload_gauge(g).cpu().numpy().view(lat.np_dtype)
+        g12 = g.reshape(v, 4, 3, 3, 2)[:, :, :2].reshape(v, 4, 6, 2)
+        want = np.ascontiguousarray(np.moveaxis(g12, 0, 2)).reshape(-1) if layout == "soa" else g12.reshape(-1)
+        assert np.array_equal(nat, want)
+        if layout == "soa" and precision == "f64":
+            ps = lat.upload_spinor(p).cpu().numpy().view(np.float64)
+            assert np.array_equal(ps, np.ascontiguousarray(np.moveaxis(p.reshape(v, 12, 2), 0, 1)).reshape(-1))
+
+
+# ---------------------------------------------------------------- error behaviour on a live context
+def test_error_paths_on_device(env):
+    B = env.B
+    with env.device.Lattice((4, 4, 4, 4), "f64", "soa", False) as lat:
+        o, p, g = lat.new_spinor(), lat.new_spinor(), lat.new_gauge()
+        assert B.dslash_apply_status(lat.ctx, o.data_ptr() + 8, p.data_ptr(), g.data_ptr()) == B.DSLASH_ERR_ALIGN
+        assert B.dslash_apply_status(lat.ctx, p.data_ptr(), p.data_ptr(), g.data_ptr()) == B.DSLASH_ERR_ALIAS
+        assert B.dslash_apply_status(lat.ctx, p.data_ptr() + 16, p.data_ptr(), g.data_ptr()) == B.DSLASH_ERR_ALIAS
+        assert B.dslash_apply_status(lat.ctx, 0, p.data_ptr(), g.data_ptr()) == B.DSLASH_ERR_NULL
+        for bad in [(5, 64, 1), (4, 96, 1), (4, 64, 3), (-1, 64, 1)]:
+            with pytest.raises(B.DslashError) as e:
+                lat.set_variant(*bad)
+            assert e.value.status == B.DSLASH_ERR_UNSUPPORTED
+        for bad in [(3, 4, 4, 4), (64, 32, 1, 1), (1, 1, 1, 1), (0, 4, 4, 4)]:
+            with pytest.raises(B.DslashError) as e:
+                lat.set_tile(bad)
+            assert e.value.status == B.DSLASH_ERR_UNSUPPORTED
+        lat.set_variant(3, 256, 2)
+        assert B.dslash_get_variant(lat.ctx) == (3, 256, 2)
+        lat.set_variant(B.DSLASH_VARIANT_TUNED)
+        assert B.dslash_get_variant(lat.ctx)[0] == B.DSLASH_VARIANT_TUNED
+        assert B.dslash_last_cuda_error(lat.ctx) == 0
+
+
+# ---------------------------------------------------------------- host entry point (e2e path) and its byte accounting
+@pytest.mark.parametrize("layout,recon12", [("soa", False), ("soa", True), ("aos", False)])
+def test_apply_host_matches_oracle_and_counts_bytes(env, layout, recon12):
+    dims = (8, 6, 4, 10)
+    g, p, ref, _ = fields_and_ref(env, dims, SEED + 41, "f64")
+    torch, B = env.torch, env.B
+    gh = torch.from_numpy(g.copy()).pin_memory()
+    ph = torch.from_numpy(p.copy()).pin_memory()
+    oh = torch.zeros(p.shape, dtype=torch.float64).pin_memory()
+    with env.device.Lattice(dims, "f64", layout, recon12) as lat:
+        h2d, d2h = B.dslash_apply_host(lat.ctx, oh.data_ptr(), ph.data_ptr(), gh.data_ptr(), B.DSLASH_MAP_MINIMAL, lat.stream())
+        assert env.checks.parity_error(oh.numpy(), ref) <= TOL["f64"]
+        assert (h2d, d2h) == (g.nbytes + p.nbytes, p.nbytes)
+        oh.zero_()
+        h2d2, d2h2 = B.dslash_apply_host(lat.ctx, oh.data_ptr(), ph.data_ptr(), gh.data_ptr(), B.DSLASH_MAP_TOFROM, lat.stream())
+        assert env.checks.parity_error(oh.numpy(), ref) <= TOL["f64"]
+        # PAPER.md:265 (Fig. 4): 1.5 GB without data analysis -> 0.75 GB with it, exactly 2:1
+        assert h2d2 + d2h2 == 2 * (h2d + d2h)
+        assert np.array_equal(gh.numpy(), g) and np.array_equal(ph.numpy(), p)
