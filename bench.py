@@ -162,12 +162,11 @@ def run_reference(args, cfg):
 
 
 # ------------------------------------------------------------------ the CUDA arm
-def time_applies(torch, lat, out, inp, gauge, steps, warmup, dist, sampler_index):
+def time_applies(torch, lat, out, inp, gauge, steps, warmup, group, sampler_index):
     for _ in range(warmup):
         lat.apply(out, inp, gauge)
     torch.cuda.synchronize()
-    if dist is not None:
-        dist.barrier()
+    group.barrier()
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with ClockSampler(sampler_index) as cs:
@@ -176,32 +175,21 @@ def time_applies(torch, lat, out, inp, gauge, steps, warmup, dist, sampler_index
             lat.apply(out, inp, gauge)
         e1.record()
         torch.cuda.synchronize()
-    if dist is not None:
-        dist.barrier()
-    ms = e0.elapsed_time(e1)
-    if dist is not None:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    group.barrier()
+    ms = group.max_over_ranks(e0.elapsed_time(e1))
     return ms, cs.summary()
 
 
 def run_cuda(args, cfg):
     import torch
     from paper_2301_03636_b200 import binding as B
-    from paper_2301_03636_b200 import device, inputs
+    from paper_2301_03636_b200 import device, inputs, replicas
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, world, local = replicas.env_ranks()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the CUDA library has no CPU fallback (use --impl reference for the oracle)")
     torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist_
-        dist_.init_process_group("nccl", device_id=torch.device("cuda", local))
-        dist = dist_
+    group = replicas.Group("nccl", torch.device("cuda", local))
     dims, prec = cfg["dims"], cfg["precision"]
     v = inputs.volume(dims)
     g, p = inputs.fields(dims, SEED + 3 + 1000 * rank, prec, check=False)  # every rank its own replica
@@ -217,10 +205,11 @@ def run_cuda(args, cfg):
                 lat.set_tile(args.tile)
             gd, pd, od = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
             n0 = B.dslash_launch_count(lat.ctx)
-            ms, ck = time_applies(torch, lat, od, pd, gd, args.steps, args.warmup, dist, local)
+            ms, ck = time_applies(torch, lat, od, pd, gd, args.steps, args.warmup, group, local)
             n1 = B.dslash_launch_count(lat.ctx)
             bps = bytes_per_site(prec, recon12)
-            results[tag] = dict(ms=ms, ms_per_step=ms / args.steps, gflops=FLOP_PER_SITE * v * world / (ms / args.steps) / 1e6,
+            results[tag] = dict(ms=ms, ms_per_step=ms / args.steps,
+                                gflops=replicas.whole_job_rate(FLOP_PER_SITE * v, world, ms / args.steps) / 1e9,
                                 gbs=bps * v / (ms / args.steps) / 1e6, bps=bps, recon12=recon12,
                                 tile=list(B.dslash_get_tile(lat.ctx)))
             if tag == "main":
@@ -247,20 +236,16 @@ def run_cuda(args, cfg):
             for _ in range(2):
                 h2d, d2h = B.dslash_apply_host(lat.ctx, oh.data_ptr(), ph.data_ptr(), gh.data_ptr(), B.DSLASH_MAP_MINIMAL, stream)
             torch.cuda.synchronize()
-            if dist is not None:
-                dist.barrier()
+            group.barrier()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record()
             for _ in range(n_e2e):
                 B.dslash_apply_host(lat.ctx, oh.data_ptr(), ph.data_ptr(), gh.data_ptr(), B.DSLASH_MAP_MINIMAL, stream)
             e1.record()
             torch.cuda.synchronize()
-            ms_e = e0.elapsed_time(e1)
-            if dist is not None:
-                t = torch.tensor([ms_e], dtype=torch.float64, device="cuda")
-                dist.all_reduce(t, op=dist.ReduceOp.MAX)
-                ms_e = float(t.item())
-            e2e = {"value": FLOP_PER_SITE * v * world / (ms_e / n_e2e) / 1e6, "unit": "GFLOP/s", "h2d_bytes_per_step": int(h2d),
+            group.barrier()
+            ms_e = group.max_over_ranks(e0.elapsed_time(e1))
+            e2e = {"value": replicas.whole_job_rate(FLOP_PER_SITE * v, world, ms_e / n_e2e) / 1e9, "unit": "GFLOP/s", "h2d_bytes_per_step": int(h2d),
                    "d2h_bytes_per_step": int(d2h), "ms_per_step": ms_e / n_e2e, "steps": n_e2e,
                    "path": "dslash_apply_host(DSLASH_MAP_MINIMAL), pinned host buffers, canonical layout"}
             del gh, ph, oh
@@ -289,8 +274,7 @@ def run_cuda(args, cfg):
             line["also"] = {"recon": 12 if o["recon12"] else 18, "value": o["gflops"], "ms_per_step": o["ms_per_step"],
                             "hbm_gbs": o["gbs"], "roofline_frac": o["gbs"] / peak}
         print(json.dumps(line))
-    if dist is not None:
-        dist.destroy_process_group()
+    group.close()
     return 0
 
 

@@ -34,11 +34,15 @@
  *   DSLASH_AOS                  the canonical layout itself (18 reals per link).
  *   DSLASH_AOS|DSLASH_RECON12   spinor canonical; gauge keeps rows 0,1 only:
  *                                 real[ (((s*4 + mu)*2 + row)*3 + col)*2 + ri ]
- *   DSLASH_SOA  ("structure of arrays", one 16-byte vector per site and component, unit stride in s)
- *       FP64 spinor  double2[ k*V + s ]           k = spin*3 + colour = 0..11      (re, im)
- *       FP32 spinor  float4 [ q*V + s ]           q = 0..5: components k = 2q, 2q+1 (re,im,re,im)
- *       FP64 gauge   double2[ (mu*R + e)*V + s ]  e = row*3 + col; R = 9, or 6 with DSLASH_RECON12
- *       FP32 gauge   float2 [ (mu*R + e)*V + s ]
+ *   DSLASH_SOA  (blocked "structure of arrays": sites are grouped in vectors of 32 consecutive site indices,
+ *                v = s / 32, l = s % 32; inside a vector every component is a contiguous run of 32 elements.
+ *                V is padded up to a multiple of 32 -- use dslash_*_bytes(); the padding is never read)
+ *       FP64 spinor  double2[ (v*12 + k)*32 + l ]          k = spin*3 + colour = 0..11      (re, im)
+ *       FP32 spinor  float4 [ (v*6  + q)*32 + l ]          q = 0..5: components k = 2q, 2q+1 (re,im,re,im)
+ *       FP64 gauge   double2[ ((v*4 + mu)*R + e)*32 + l ]  e = row*3 + col; R = 9, or 6 with DSLASH_RECON12
+ *       FP32 gauge   float2 [ ((v*4 + mu)*R + e)*32 + l ]
+ *     A warp that handles 32 consecutive sites reads one contiguous 512-byte run per component, and all
+ *     components of a site share one base address (the component stride is a compile-time constant).
  *   With DSLASH_RECON12 row 2 of every link is rebuilt in registers as conj(row0 x row1), which is
  *   exact for SU(3) input (DESIGN.md Reading R14).
  */
@@ -82,6 +86,16 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
 
 /* variant selection: collapse_depth DSLASH_VARIANT_TUNED selects the library's tuned kernel */
 #define DSLASH_VARIANT_TUNED 0
+
+/* kernel selection of the tuned path, dslash_set_kernel() */
+#define DSLASH_KERNEL_AUTO 0   /* the library picks (TMA-staged when the layout/lattice/tile allow it, else direct) */
+#define DSLASH_KERNEL_DIRECT 1 /* one thread per site, all neighbours gathered from global memory through L1/L2 */
+#define DSLASH_KERNEL_TMA 2    /* tile's own spinors and links staged in shared memory by TMA bulk tensor copies */
+
+/* options of the tuned kernels, dslash_set_option() */
+#define DSLASH_OPT_OCCUPANCY 2        /* 0: default register budget; 1: 128-register variant (more resident warps) */
+#define DSLASH_OPT_L2_POLICY 3        /* bit mask of L2 eviction hints: 1 spinor loads evict_last, 2 U_t loads evict_last,
+                                         4 U_x/U_y/U_z loads evict_first, 8 stores of `out` evict_first (0: none) */
 
 /* host<->device mapping modes of dslash_apply_host() (section 4.1.2) */
 #define DSLASH_MAP_MINIMAL 0 /* to: gauge, in;  from: out            (after the Advisor's data analysis) */
@@ -160,6 +174,25 @@ DSLASH_API int dslash_variant_at(int index, int *collapse_depth, int *threads_pe
  */
 DSLASH_API int dslash_set_tile(dslash_ctx *ctx, const int tile[4]);
 DSLASH_API int dslash_get_tile(const dslash_ctx *ctx, int tile[4]);
+
+/*
+ * Choose the implementation behind DSLASH_VARIANT_TUNED: DSLASH_KERNEL_AUTO (default), _DIRECT or _TMA.
+ * _TMA needs a DSLASH_SOA ctx, a tile whose x-extent is a multiple of 32 and divides L_X, the other tile
+ * extents <= the lattice extents, and 32..128 sites per tile;
+ * if it is selected explicitly and the current tile/lattice do not allow it, dslash_apply returns
+ * DSLASH_ERR_UNSUPPORTED (AUTO falls back to _DIRECT silently -- both are CUDA kernels of this library).
+ * dslash_get_kernel reports the kernel the next dslash_apply would launch (_DIRECT or _TMA).
+ * Errors: NULL, UNSUPPORTED (unknown value).
+ */
+DSLASH_API int dslash_set_kernel(dslash_ctx *ctx, int kernel);
+DSLASH_API int dslash_get_kernel(const dslash_ctx *ctx, int *kernel);
+
+/*
+ * Performance options of the tuned kernels (DSLASH_OPT_*); they never change results beyond rounding order.
+ * Errors: NULL, UNSUPPORTED (unknown option or value out of range).
+ */
+DSLASH_API int dslash_set_option(dslash_ctx *ctx, int option, int value);
+DSLASH_API int dslash_get_option(const dslash_ctx *ctx, int option, int *value);
 
 /*
  * End-to-end application from HOST buffers in the canonical layout at the ctx's precision

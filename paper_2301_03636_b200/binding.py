@@ -20,6 +20,8 @@ DSLASH_ERR_NULL, DSLASH_ERR_DIMS, DSLASH_ERR_PRECISION, DSLASH_ERR_LAYOUT = -1, 
 DSLASH_ERR_ALIGN, DSLASH_ERR_ALIAS, DSLASH_ERR_UNSUPPORTED, DSLASH_ERR_CUDA, DSLASH_ERR_NOMEM = -5, -6, -7, -8, -9
 DSLASH_VARIANT_TUNED = 0
 DSLASH_MAP_MINIMAL, DSLASH_MAP_TOFROM = 0, 1
+DSLASH_KERNEL_AUTO, DSLASH_KERNEL_DIRECT, DSLASH_KERNEL_TMA = 0, 1, 2
+DSLASH_OPT_OCCUPANCY, DSLASH_OPT_L2_POLICY = 2, 3
 
 _c_int_p = ctypes.POINTER(ctypes.c_int)
 _c_size_p = ctypes.POINTER(ctypes.c_size_t)
@@ -43,6 +45,10 @@ SIGNATURES = {
     "dslash_variant_at": (ctypes.c_int, [ctypes.c_int, _c_int_p, _c_int_p, _c_int_p, _c_int_p]),
     "dslash_set_tile": (ctypes.c_int, [_vp, _c_int_p]),
     "dslash_get_tile": (ctypes.c_int, [_vp, _c_int_p]),
+    "dslash_set_kernel": (ctypes.c_int, [_vp, ctypes.c_int]),
+    "dslash_get_kernel": (ctypes.c_int, [_vp, _c_int_p]),
+    "dslash_set_option": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int]),
+    "dslash_get_option": (ctypes.c_int, [_vp, ctypes.c_int, _c_int_p]),
     "dslash_apply_host": (ctypes.c_int, [_vp, _vp, _vp, _vp, ctypes.c_int, _vp, _c_size_p, _c_size_p]),
     "dslash_launch_count": (ctypes.c_longlong, [_vp]),
     "dslash_last_cuda_error": (ctypes.c_int, [_vp]),
@@ -178,6 +184,26 @@ def dslash_get_tile(ctx):
     arr = (ctypes.c_int * 4)()
     _check(_lib.dslash_get_tile(_ptr(ctx), arr), "dslash_get_tile")
     return tuple(arr)
+
+
+def dslash_set_kernel(ctx, kernel: int) -> None:
+    _check(_lib.dslash_set_kernel(_ptr(ctx), int(kernel)), "dslash_set_kernel")
+
+
+def dslash_get_kernel(ctx) -> int:
+    k = ctypes.c_int()
+    _check(_lib.dslash_get_kernel(_ptr(ctx), ctypes.byref(k)), "dslash_get_kernel")
+    return k.value
+
+
+def dslash_set_option(ctx, option: int, value: int) -> None:
+    _check(_lib.dslash_set_option(_ptr(ctx), int(option), int(value)), "dslash_set_option")
+
+
+def dslash_get_option(ctx, option: int) -> int:
+    v = ctypes.c_int()
+    _check(_lib.dslash_get_option(_ptr(ctx), int(option), ctypes.byref(v)), "dslash_get_option")
+    return v.value
 
 
 def dslash_apply_host(ctx, out_host, in_host, gauge_host, map_mode: int = DSLASH_MAP_MINIMAL, stream=0):

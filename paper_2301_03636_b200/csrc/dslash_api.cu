@@ -18,6 +18,8 @@ struct dslash_ctx {
     int var_depth, var_tpb, var_spt;
     int tile[4];
     TileGeom tg;
+    int kernel;  // DSLASH_KERNEL_*
+    TunedConfig cfg;
     long long launches;
     int last_cuda;
     // staging buffers of dslash_apply_host (device memory, owned)
@@ -104,6 +106,9 @@ int dslash_create(dslash_ctx** ctx, const int dims[4], int precision, int layout
     int tile[4];
     default_tile(c, tile);
     set_tile_geom(c, tile);
+    c->kernel = DSLASH_KERNEL_AUTO;
+    c->cfg.occupancy = 0;
+    c->cfg.l2_policy = 0;
     c->launches = 0;
     c->last_cuda = 0;
     for (int i = 0; i < 3; ++i) c->d_can[i] = c->d_nat[i] = nullptr;
@@ -127,12 +132,25 @@ int dslash_destroy(dslash_ctx* c) {
     return rc;
 }
 
-size_t dslash_spinor_bytes(const dslash_ctx* c) { return c ? (size_t)c->geom.V * 24u * real_bytes(c) : 0; }
+// sites a native field is allocated for: the SoA layout pads V up to a whole number of 32-site vectors
+static size_t native_sites(const dslash_ctx* c) {
+    return c->layout_base == LAYOUT_SOA ? (size_t)((c->geom.V + VL - 1u) / VL) * VL : (size_t)c->geom.V;
+}
+size_t dslash_spinor_bytes(const dslash_ctx* c) { return c ? native_sites(c) * 24u * real_bytes(c) : 0; }
 size_t dslash_gauge_bytes(const dslash_ctx* c) {
-    return c ? (size_t)c->geom.V * 4u * (c->recon == 12 ? 12u : 18u) * real_bytes(c) : 0;
+    return c ? native_sites(c) * 4u * (c->recon == 12 ? 12u : 18u) * real_bytes(c) : 0;
 }
 size_t dslash_canonical_spinor_bytes(const dslash_ctx* c) { return c ? (size_t)c->geom.V * 24u * real_bytes(c) : 0; }
 size_t dslash_canonical_gauge_bytes(const dslash_ctx* c) { return c ? (size_t)c->geom.V * 72u * real_bytes(c) : 0; }
+
+// The kernel dslash_apply will launch for the tuned path: DSLASH_KERNEL_DIRECT / _TMA, or -1 if _TMA was
+// requested explicitly but cannot run this configuration.
+static int resolve_kernel(const dslash_ctx* c) {
+    const bool can_tma = c->layout_base == LAYOUT_SOA && tma_eligible(c->precision, c->recon, c->geom, c->tg);
+    if (c->kernel == DSLASH_KERNEL_DIRECT) return DSLASH_KERNEL_DIRECT;
+    if (c->kernel == DSLASH_KERNEL_TMA) return can_tma ? DSLASH_KERNEL_TMA : -1;
+    return DSLASH_KERNEL_DIRECT;  // AUTO
+}
 
 static bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
 static bool overlap(const void* a, size_t na, const void* b, size_t nb) {
@@ -147,9 +165,12 @@ int dslash_apply(dslash_ctx* c, void* out, const void* in, const void* gauge, ds
     if (overlap(out, sb, in, sb)) return DSLASH_ERR_ALIAS;
     LaunchArgs a{out, in, gauge, c->geom, static_cast<cudaStream_t>(stream)};
     cudaError_t e;
-    if (c->var_depth == DSLASH_VARIANT_TUNED)
-        e = launch_tuned(c->precision, c->layout_base, c->recon, a, c->tg);
-    else
+    if (c->var_depth == DSLASH_VARIANT_TUNED) {
+        const int k = resolve_kernel(c);
+        if (k < 0) return DSLASH_ERR_UNSUPPORTED;
+        e = (k == DSLASH_KERNEL_TMA) ? launch_tma(c->precision, c->recon, a, c->tg)
+                                     : launch_tuned(c->precision, c->layout_base, c->recon, a, c->tg, c->cfg);
+    } else
         e = launch_variant(c->precision, c->layout_base, c->recon, a, c->var_depth, c->var_tpb, c->var_spt);
     if (e != cudaSuccess) return cuda_fail(c, e);
     c->launches += 1;
@@ -244,6 +265,46 @@ int dslash_set_tile(dslash_ctx* c, const int tile[4]) {
 int dslash_get_tile(const dslash_ctx* c, int tile[4]) {
     if (!c || !tile) return DSLASH_ERR_NULL;
     for (int d = 0; d < 4; ++d) tile[d] = c->tile[d];
+    return DSLASH_OK;
+}
+
+int dslash_set_option(dslash_ctx* c, int option, int value) {
+    if (!c) return DSLASH_ERR_NULL;
+    switch (option) {
+        case DSLASH_OPT_OCCUPANCY:
+            if (value < 0 || value > 1) return DSLASH_ERR_UNSUPPORTED;
+            c->cfg.occupancy = value;
+            return DSLASH_OK;
+        case DSLASH_OPT_L2_POLICY:
+            if (value < 0 || value > 15) return DSLASH_ERR_UNSUPPORTED;
+            c->cfg.l2_policy = value;
+            return DSLASH_OK;
+        default:
+            return DSLASH_ERR_UNSUPPORTED;
+    }
+}
+
+int dslash_get_option(const dslash_ctx* c, int option, int* value) {
+    if (!c || !value) return DSLASH_ERR_NULL;
+    switch (option) {
+        case DSLASH_OPT_OCCUPANCY: *value = c->cfg.occupancy; return DSLASH_OK;
+        case DSLASH_OPT_L2_POLICY: *value = c->cfg.l2_policy; return DSLASH_OK;
+        default: return DSLASH_ERR_UNSUPPORTED;
+    }
+}
+
+int dslash_set_kernel(dslash_ctx* c, int kernel) {
+    if (!c) return DSLASH_ERR_NULL;
+    if (kernel != DSLASH_KERNEL_AUTO && kernel != DSLASH_KERNEL_DIRECT && kernel != DSLASH_KERNEL_TMA)
+        return DSLASH_ERR_UNSUPPORTED;
+    c->kernel = kernel;
+    return DSLASH_OK;
+}
+
+int dslash_get_kernel(const dslash_ctx* c, int* kernel) {
+    if (!c || !kernel) return DSLASH_ERR_NULL;
+    const int k = resolve_kernel(c);
+    *kernel = k < 0 ? DSLASH_KERNEL_DIRECT : k;
     return DSLASH_OK;
 }
 

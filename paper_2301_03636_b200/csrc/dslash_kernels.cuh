@@ -25,8 +25,19 @@ struct LaunchArgs {
 // loops of (t,z,y,x); every parallel iteration runs the remaining loops serially.
 cudaError_t launch_variant(int precision, int layout_base, int recon, const LaunchArgs& a, int depth, int tpb, int spt);
 
-// Tuned kernel.
-cudaError_t launch_tuned(int precision, int layout_base, int recon, const LaunchArgs& a, const TileGeom& tg);
+// Options of the tuned kernels (dslash_set_option).
+struct TunedConfig {
+    int occupancy;         // 0: default register budget, 1: 128-register variant
+    int l2_policy;         // DSLASH_OPT_L2_POLICY bits (0: no cache hints)
+};
+
+// Tuned kernel (direct, register-staged).
+cudaError_t launch_tuned(int precision, int layout_base, int recon, const LaunchArgs& a, const TileGeom& tg,
+                         const TunedConfig& cfg);
+
+// TMA-staged kernel (SoA only): tile's own spinors + links by cp.async.bulk.tensor into shared memory.
+bool tma_eligible(int precision, int recon, const Geom& g, const TileGeom& tg);
+cudaError_t launch_tma(int precision, int recon, const LaunchArgs& a, const TileGeom& tg);
 
 // Layout module.  dir 0: canonical -> native (pack), 1: native -> canonical (unpack).
 cudaError_t launch_convert_spinor(int precision, int layout_base, void* dst, const void* src, unsigned V, int dir,

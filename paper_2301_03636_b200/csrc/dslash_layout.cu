@@ -1,21 +1,25 @@
 // dslash_layout.cu -- layout module: canonical AoS <-> native (north_star subsystem (1)).
 //
 // The paper only says the fields are flat one-dimensional arrays; the canonical layout
-// is that array with the loop order of PAPER.md:54.  The native SoA layout puts one 16-byte vector
-// per (component, site) with unit stride in the site index, so a warp's load of one component of 32
-// consecutive sites is one contiguous 512-byte run.  Pure data movement; bit-exact.
+// is that array with the loop order of PAPER.md:54.  The native SoA layout (dslash_site.cuh) groups sites
+// in vectors of 32 consecutive site indices and stores every component of a vector as one contiguous run,
+// so a warp's load of one component of 32 consecutive sites is one contiguous 512-byte run and all
+// components of a site share one base address.  Pure data movement; bit-exact.
 #include "dslash_kernels.cuh"
 
 namespace dslash {
 
-// dst[u*V + s] = src[s*NU + u] (dir 0)   or   dst[s*NU + u] = src[u*V + s] (dir 1); one thread per SoA element.
+// dir 0: dst[soa(s,u)] = src[s*NU + u]   dir 1: dst[s*NU + u] = src[soa(s,u)]; one thread per (vector, u, lane).
 template <typename U>
 __global__ void __launch_bounds__(256) transpose_units_kernel(U* __restrict__ dst, const U* __restrict__ src, unsigned V,
-                                                              int NU, int dir) {
-    const size_t n = (size_t)V * (size_t)NU;
+                                                              unsigned NU, int dir) {
+    const size_t n = (size_t)((V + VL - 1u) / VL) * NU * VL;  // padded SoA size
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-        const unsigned u = (unsigned)(i / V);
-        const unsigned s = (unsigned)(i - (size_t)u * V);
+        const unsigned lane = (unsigned)(i & (VL - 1u));
+        const size_t vu = i >> VL_LOG2;
+        const unsigned u = (unsigned)(vu % NU);
+        const unsigned s = (unsigned)(vu / NU) * VL + lane;
+        if (s >= V) continue;  // padding of the last vector
         const size_t aos = (size_t)s * NU + u;
         if (dir == 0)
             dst[i] = src[aos];
@@ -24,20 +28,28 @@ __global__ void __launch_bounds__(256) transpose_units_kernel(U* __restrict__ ds
     }
 }
 
-// Gauge pack.  Canonical: src[(s*4 + mu)*9 + e].  SoA: dst[(mu*R + e)*V + s];  AoS: dst[(s*4 + mu)*R + e];  e < R.
+// Gauge pack.  Canonical: src[(s*4 + mu)*9 + e].  SoA: dst[soa(s, mu*R + e) with 4R components];
+// AoS (12-real): dst[(s*4 + mu)*R + e];  e < R.
 template <typename U>
-__global__ void __launch_bounds__(256) pack_gauge_kernel(U* __restrict__ dst, const U* __restrict__ src, unsigned V, int R,
+__global__ void __launch_bounds__(256) pack_gauge_kernel(U* __restrict__ dst, const U* __restrict__ src, unsigned V, unsigned R,
                                                          int soa) {
-    const size_t n = (size_t)V * 4u * (size_t)R;
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-        if (soa) {
-            const unsigned me = (unsigned)(i / V);  // mu*R + e
-            const unsigned s = (unsigned)(i - (size_t)me * V);
-            const unsigned mu = me / (unsigned)R, e = me - mu * (unsigned)R;
+    if (soa) {
+        const unsigned NU = 4u * R;
+        const size_t n = (size_t)((V + VL - 1u) / VL) * NU * VL;
+        for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+            const unsigned lane = (unsigned)(i & (VL - 1u));
+            const size_t vu = i >> VL_LOG2;
+            const unsigned me = (unsigned)(vu % NU);  // mu*R + e
+            const unsigned s = (unsigned)(vu / NU) * VL + lane;
+            if (s >= V) continue;
+            const unsigned mu = me / R, e = me - mu * R;
             dst[i] = src[((size_t)s * 4u + mu) * 9u + e];
-        } else {
-            const size_t sm = i / (unsigned)R;  // s*4 + mu
-            const unsigned e = (unsigned)(i - sm * (unsigned)R);
+        }
+    } else {
+        const size_t n = (size_t)V * 4u * R;
+        for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+            const size_t sm = i / R;  // s*4 + mu
+            const unsigned e = (unsigned)(i - sm * R);
             dst[i] = src[sm * 9u + e];
         }
     }
@@ -53,7 +65,7 @@ cudaError_t launch_convert_spinor(int precision, int layout_base, void* dst, con
                                   cudaStream_t stream) {
     const size_t bytes = (size_t)V * 24u * (precision == 0 ? 8u : 4u);
     if (layout_base == LAYOUT_AOS) return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, stream);
-    const int NU = precision == 0 ? 12 : 6;  // 16-byte units per site
+    const unsigned NU = precision == 0 ? 12u : 6u;  // 16-byte units per site
     transpose_units_kernel<uint4><<<grid_for((size_t)V * NU), 256, 0, stream>>>(reinterpret_cast<uint4*>(dst),
                                                                                  reinterpret_cast<const uint4*>(src), V, NU, dir);
     return cudaGetLastError();
@@ -61,7 +73,7 @@ cudaError_t launch_convert_spinor(int precision, int layout_base, void* dst, con
 
 cudaError_t launch_pack_gauge(int precision, int layout_base, int recon, void* dst, const void* src, unsigned V,
                               cudaStream_t stream) {
-    const int R = recon == 12 ? 6 : 9;
+    const unsigned R = recon == 12 ? 6u : 9u;
     if (layout_base == LAYOUT_AOS && R == 9)
         return cudaMemcpyAsync(dst, src, (size_t)V * 72u * (precision == 0 ? 8u : 4u), cudaMemcpyDeviceToDevice, stream);
     const size_t n = (size_t)V * 4u * (size_t)R;

@@ -18,6 +18,18 @@ namespace dslash {
 
 enum : int { LAYOUT_AOS = 0, LAYOUT_SOA = 1 };
 
+// The SoA layout is blocked ("array of structures of arrays"): sites are grouped in vectors of VL = 32
+// consecutive site indices; within a vector every component is a contiguous run of 32 elements.
+//   spinor  unit16[ (s / 32) * (NU * 32) + k * 32 + (s % 32) ]          NU = 12 (fp64, double2) or 6 (fp32, float4)
+//   gauge   vec2  [ ((s / 32) * 4 + mu) * (R * 32) + e * 32 + (s % 32) ]  R = 9 or 6
+// A warp that handles 32 consecutive sites still reads one contiguous 512-byte (fp32 links: 256-byte) run
+// per component, but the component stride is the compile-time constant 32 elements, so the 12 (9) loads of
+// a spinor (link) share ONE 64-bit base address and differ only in the instruction's immediate offset
+// (SASS: LDG.E.128 [R.64 + imm]) -- the planar [k][V] form spent ~4.5 integer instructions per load on
+// addresses.  V is padded up to a multiple of 32; the padding is never read by the operator.
+constexpr unsigned VL = 32u;
+constexpr unsigned VL_LOG2 = 5u;
+
 struct Geom {
     int L[4];    // L_X, L_Y, L_Z, L_T
     unsigned V;  // number of sites
@@ -42,6 +54,66 @@ __device__ __forceinline__ cplx<Real> c_sub_i(cplx<Real> a, cplx<Real> b) { retu
 
 __device__ __forceinline__ double fma_(double a, double b, double c) { return fma(a, b, c); }
 __device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a, b, c); }
+
+// ------------------------------------------------------------------ global loads/stores with an optional L2 eviction policy
+// HINT = false: plain read-only loads (__ldg) and plain stores.  HINT = true: the same accesses carry a 64-bit L2
+// cache policy made by `createpolicy` (evict_last for data that is re-read one or two time-slices later,
+// evict_first for data that is dead after this access) -- SASS LDG/STG with a desc[UR] operand.
+struct Policies {
+    uint64_t psi, u_t, u_s, out;  // spinor loads, U_t loads, U_x/U_y/U_z loads, stores of `out`
+};
+enum : int { POLICY_NORMAL = 0, POLICY_EVICT_LAST = 1, POLICY_EVICT_FIRST = 2 };
+__device__ __forceinline__ uint64_t make_policy(int kind) {
+    uint64_t p;
+    if (kind == POLICY_EVICT_LAST)
+        asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    else if (kind == POLICY_EVICT_FIRST)
+        asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    else
+        asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+template <bool HINT>
+__device__ __forceinline__ double2 ld_ro(const double2* p, uint64_t pol) {
+    if (!HINT) return __ldg(p);
+    double2 v;
+    asm volatile("ld.global.nc.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol));
+    return v;
+}
+template <bool HINT>
+__device__ __forceinline__ float4 ld_ro(const float4* p, uint64_t pol) {
+    if (!HINT) return __ldg(p);
+    float4 v;
+    asm volatile("ld.global.nc.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;"
+                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+                 : "l"(p), "l"(pol));
+    return v;
+}
+template <bool HINT>
+__device__ __forceinline__ float2 ld_ro(const float2* p, uint64_t pol) {
+    if (!HINT) return __ldg(p);
+    float2 v;
+    asm volatile("ld.global.nc.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;" : "=f"(v.x), "=f"(v.y) : "l"(p), "l"(pol));
+    return v;
+}
+template <bool HINT>
+__device__ __forceinline__ void st_g(double2* p, double2 v, uint64_t pol) {
+    if (!HINT) {
+        *p = v;
+        return;
+    }
+    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1,%2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+}
+template <bool HINT>
+__device__ __forceinline__ void st_g(float4* p, float4 v, uint64_t pol) {
+    if (!HINT) {
+        *p = v;
+        return;
+    }
+    asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1,%2,%3,%4}, %5;" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w),
+                 "l"(pol)
+                 : "memory");
+}
 
 // acc += a * b
 template <typename Real>
@@ -85,71 +157,48 @@ __device__ __forceinline__ cplx<Real> c_mul_conj(cplx<Real> a, cplx<Real> b) {
 template <typename Real, int LAYOUT>
 struct SpinorIO;
 
-template <>
-struct SpinorIO<double, LAYOUT_AOS> {
-    __device__ __forceinline__ static void load(cplx<double> (&psi)[12], const void* base, unsigned V, unsigned s) {
-        const double2* p = reinterpret_cast<const double2*>(base) + (size_t)s * 12;
+template <int LAYOUT>
+struct SpinorIO<double, LAYOUT> {
+    __device__ __forceinline__ static size_t idx(unsigned V, unsigned s, int k) {
+        return LAYOUT == LAYOUT_AOS ? (size_t)s * 12 + k : (size_t)(s >> VL_LOG2) * (12u * VL) + (s & (VL - 1u)) + (unsigned)k * VL;
+    }
+    template <bool HINT = false>
+    __device__ __forceinline__ static void load(cplx<double> (&psi)[12], const void* base, unsigned V, unsigned s, uint64_t pol = 0) {
+        const double2* p = reinterpret_cast<const double2*>(base);
 #pragma unroll
         for (int k = 0; k < 12; ++k) {
-            double2 v = __ldg(p + k);
+            double2 v = ld_ro<HINT>(p + idx(V, s, k), pol);
             psi[k] = {v.x, v.y};
         }
     }
-    __device__ __forceinline__ static void store(void* base, unsigned V, unsigned s, const cplx<double> (&psi)[12]) {
-        double2* p = reinterpret_cast<double2*>(base) + (size_t)s * 12;
+    template <bool HINT = false>
+    __device__ __forceinline__ static void store(void* base, unsigned V, unsigned s, const cplx<double> (&psi)[12], uint64_t pol = 0) {
+        double2* p = reinterpret_cast<double2*>(base);
 #pragma unroll
-        for (int k = 0; k < 12; ++k) p[k] = make_double2(psi[k].re, psi[k].im);
+        for (int k = 0; k < 12; ++k) st_g<HINT>(p + idx(V, s, k), make_double2(psi[k].re, psi[k].im), pol);
     }
 };
-template <>
-struct SpinorIO<double, LAYOUT_SOA> {
-    __device__ __forceinline__ static void load(cplx<double> (&psi)[12], const void* base, unsigned V, unsigned s) {
-        const double2* p = reinterpret_cast<const double2*>(base) + s;
-#pragma unroll
-        for (int k = 0; k < 12; ++k) {
-            double2 v = __ldg(p + (size_t)k * V);
-            psi[k] = {v.x, v.y};
-        }
+template <int LAYOUT>
+struct SpinorIO<float, LAYOUT> {
+    __device__ __forceinline__ static size_t idx(unsigned V, unsigned s, int q) {
+        return LAYOUT == LAYOUT_AOS ? (size_t)s * 6 + q : (size_t)(s >> VL_LOG2) * (6u * VL) + (s & (VL - 1u)) + (unsigned)q * VL;
     }
-    __device__ __forceinline__ static void store(void* base, unsigned V, unsigned s, const cplx<double> (&psi)[12]) {
-        double2* p = reinterpret_cast<double2*>(base) + s;
-#pragma unroll
-        for (int k = 0; k < 12; ++k) p[(size_t)k * V] = make_double2(psi[k].re, psi[k].im);
-    }
-};
-template <>
-struct SpinorIO<float, LAYOUT_AOS> {
-    __device__ __forceinline__ static void load(cplx<float> (&psi)[12], const void* base, unsigned V, unsigned s) {
-        const float4* p = reinterpret_cast<const float4*>(base) + (size_t)s * 6;
+    template <bool HINT = false>
+    __device__ __forceinline__ static void load(cplx<float> (&psi)[12], const void* base, unsigned V, unsigned s, uint64_t pol = 0) {
+        const float4* p = reinterpret_cast<const float4*>(base);
 #pragma unroll
         for (int q = 0; q < 6; ++q) {
-            float4 v = __ldg(p + q);
+            float4 v = ld_ro<HINT>(p + idx(V, s, q), pol);
             psi[2 * q] = {v.x, v.y};
             psi[2 * q + 1] = {v.z, v.w};
         }
     }
-    __device__ __forceinline__ static void store(void* base, unsigned V, unsigned s, const cplx<float> (&psi)[12]) {
-        float4* p = reinterpret_cast<float4*>(base) + (size_t)s * 6;
-#pragma unroll
-        for (int q = 0; q < 6; ++q) p[q] = make_float4(psi[2 * q].re, psi[2 * q].im, psi[2 * q + 1].re, psi[2 * q + 1].im);
-    }
-};
-template <>
-struct SpinorIO<float, LAYOUT_SOA> {
-    __device__ __forceinline__ static void load(cplx<float> (&psi)[12], const void* base, unsigned V, unsigned s) {
-        const float4* p = reinterpret_cast<const float4*>(base) + s;
-#pragma unroll
-        for (int q = 0; q < 6; ++q) {
-            float4 v = __ldg(p + (size_t)q * V);
-            psi[2 * q] = {v.x, v.y};
-            psi[2 * q + 1] = {v.z, v.w};
-        }
-    }
-    __device__ __forceinline__ static void store(void* base, unsigned V, unsigned s, const cplx<float> (&psi)[12]) {
-        float4* p = reinterpret_cast<float4*>(base) + s;
+    template <bool HINT = false>
+    __device__ __forceinline__ static void store(void* base, unsigned V, unsigned s, const cplx<float> (&psi)[12], uint64_t pol = 0) {
+        float4* p = reinterpret_cast<float4*>(base);
 #pragma unroll
         for (int q = 0; q < 6; ++q)
-            p[(size_t)q * V] = make_float4(psi[2 * q].re, psi[2 * q].im, psi[2 * q + 1].re, psi[2 * q + 1].im);
+            st_g<HINT>(p + idx(V, s, q), make_float4(psi[2 * q].re, psi[2 * q].im, psi[2 * q + 1].re, psi[2 * q + 1].im), pol);
     }
 };
 
@@ -166,8 +215,8 @@ struct vec2<float> {
 
 // Link U_mu(s): 9 complex entries u[row*3+col]; with RECON == 12 only rows 0,1 are stored and row 2
 // is rebuilt as conj(row0 x row1) (exact for SU(3), DESIGN.md Reading R14).
-template <typename Real, int LAYOUT, int RECON>
-__device__ __forceinline__ void load_link(cplx<Real> (&u)[9], const void* base, unsigned V, unsigned s, int mu) {
+template <typename Real, int LAYOUT, int RECON, bool HINT = false>
+__device__ __forceinline__ void load_link(cplx<Real> (&u)[9], const void* base, unsigned V, unsigned s, int mu, uint64_t pol = 0) {
     using V2 = typename vec2<Real>::type;
     constexpr int R = (RECON == 12) ? 6 : 9;
     const V2* p = reinterpret_cast<const V2*>(base);
@@ -175,14 +224,14 @@ __device__ __forceinline__ void load_link(cplx<Real> (&u)[9], const void* base, 
         p += (size_t)(s * 4u + (unsigned)mu) * R;
 #pragma unroll
         for (int e = 0; e < R; ++e) {
-            V2 v = __ldg(p + e);
+            V2 v = ld_ro<HINT>(p + e, pol);
             u[e] = {v.x, v.y};
         }
     } else {
-        p += (size_t)(mu * R) * V + s;
+        p += (size_t)((s >> VL_LOG2) * 4u + (unsigned)mu) * (R * VL) + (s & (VL - 1u));
 #pragma unroll
         for (int e = 0; e < R; ++e) {
-            V2 v = __ldg(p + (size_t)e * V);
+            V2 v = ld_ro<HINT>(p + e * VL, pol);
             u[e] = {v.x, v.y};
         }
     }
@@ -230,34 +279,37 @@ __device__ __forceinline__ void project(cplx<Real> (&h)[6], const cplx<Real> (&p
 //   MU 2: r2 = +-i h0, r3 = -+i h1    MU 3: r2 = -+ h0, r3 = -+ h1       (upper sign: SIGN = -1)
 template <int MU, int SIGN, bool FIRST, typename Real>
 __device__ __forceinline__ void reconstruct_accumulate(cplx<Real> (&acc)[12], const cplx<Real> (&h)[6]) {
+    constexpr bool M = SIGN < 0;  // the (1 - gamma) projector
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         const cplx<Real> h0 = h[c], h1 = h[3 + c];
-        cplx<Real> r2, r3;
-        const cplx<Real> zero = {Real(0), Real(0)};
-        if (MU == 0) {
-            r2 = (SIGN < 0) ? c_add_i(zero, h1) : c_sub_i(zero, h1);
-            r3 = (SIGN < 0) ? c_add_i(zero, h0) : c_sub_i(zero, h0);
-        } else if (MU == 1) {
-            r2 = (SIGN < 0) ? c_sub(zero, h1) : h1;
-            r3 = (SIGN < 0) ? h0 : c_sub(zero, h0);
-        } else if (MU == 2) {
-            r2 = (SIGN < 0) ? c_add_i(zero, h0) : c_sub_i(zero, h0);
-            r3 = (SIGN < 0) ? c_sub_i(zero, h1) : c_add_i(zero, h1);
-        } else {
-            r2 = (SIGN < 0) ? c_sub(zero, h0) : h0;
-            r3 = (SIGN < 0) ? c_sub(zero, h1) : h1;
+        // rows 2,3 are updated in place (acc +- h, acc +- i h) so that no separate negation is executed
+        cplx<Real> a2 = acc[6 + c], a3 = acc[9 + c];
+        if (FIRST) {
+            a2 = {Real(0), Real(0)};
+            a3 = {Real(0), Real(0)};
         }
+        if (MU == 0) {          // r2 = +-i h1, r3 = +-i h0
+            a2 = M ? c_add_i(a2, h1) : c_sub_i(a2, h1);
+            a3 = M ? c_add_i(a3, h0) : c_sub_i(a3, h0);
+        } else if (MU == 1) {   // r2 = -+ h1, r3 = +- h0
+            a2 = M ? c_sub(a2, h1) : c_add(a2, h1);
+            a3 = M ? c_add(a3, h0) : c_sub(a3, h0);
+        } else if (MU == 2) {   // r2 = +-i h0, r3 = -+i h1
+            a2 = M ? c_add_i(a2, h0) : c_sub_i(a2, h0);
+            a3 = M ? c_sub_i(a3, h1) : c_add_i(a3, h1);
+        } else {                // r2 = -+ h0, r3 = -+ h1
+            a2 = M ? c_sub(a2, h0) : c_add(a2, h0);
+            a3 = M ? c_sub(a3, h1) : c_add(a3, h1);
+        }
+        acc[6 + c] = a2;
+        acc[9 + c] = a3;
         if (FIRST) {
             acc[c] = h0;
             acc[3 + c] = h1;
-            acc[6 + c] = r2;
-            acc[9 + c] = r3;
         } else {
             acc[c] = c_add(acc[c], h0);
             acc[3 + c] = c_add(acc[3 + c], h1);
-            acc[6 + c] = c_add(acc[6 + c], r2);
-            acc[9 + c] = c_add(acc[9 + c], r3);
         }
     }
 }
@@ -284,12 +336,12 @@ __device__ __forceinline__ void su3_mul(cplx<Real> (&hp)[6], const cplx<Real> (&
 }
 
 // One hop: acc (+)= R_{MU,SIGN}( U^(dagger) P_{MU,SIGN} psi(sn) ), link taken at site sl.
-template <int MU, int SIGN, bool FIRST, typename Real, int LAYOUT, int RECON>
+template <int MU, int SIGN, bool FIRST, typename Real, int LAYOUT, int RECON, bool HINT = false>
 __device__ __forceinline__ void hop(cplx<Real> (&acc)[12], const void* in, const void* gauge, unsigned V, unsigned sn,
-                                    unsigned sl) {
+                                    unsigned sl, uint64_t pol_psi = 0, uint64_t pol_u = 0) {
     cplx<Real> psi[12], h[6], hp[6], u[9];
-    SpinorIO<Real, LAYOUT>::load(psi, in, V, sn);
-    load_link<Real, LAYOUT, RECON>(u, gauge, V, sl, MU);
+    SpinorIO<Real, LAYOUT>::template load<HINT>(psi, in, V, sn, pol_psi);
+    load_link<Real, LAYOUT, RECON, HINT>(u, gauge, V, sl, MU, pol_u);
     project<MU, SIGN>(h, psi);
     su3_mul<(SIGN > 0)>(hp, u, h);
     reconstruct_accumulate<MU, SIGN, FIRST>(acc, hp);
@@ -297,9 +349,9 @@ __device__ __forceinline__ void hop(cplx<Real> (&acc)[12], const void* in, const
 
 // out(s) for the site with coordinates (x, y, z, t), s = x + L_X*(y + L_Y*(z + L_Z*t)).
 // Neighbour coordinates wrap modulo L_mu (the Kronecker deltas of Eq. 1 on a periodic lattice).
-template <typename Real, int LAYOUT, int RECON>
+template <typename Real, int LAYOUT, int RECON, bool HINT = false>
 __device__ __forceinline__ void dslash_site(void* out, const void* in, const void* gauge, const Geom& g, int x, int y,
-                                            int z, int t, unsigned s) {
+                                            int z, int t, unsigned s, const Policies& pol = Policies{0, 0, 0, 0}) {
     const unsigned V = g.V;
     const unsigned sx = 1u, sy = (unsigned)g.L[0], sz = sy * (unsigned)g.L[1], st = sz * (unsigned)g.L[2];
     const unsigned xf = (x + 1 == g.L[0]) ? s - (unsigned)(g.L[0] - 1) * sx : s + sx;
@@ -312,15 +364,15 @@ __device__ __forceinline__ void dslash_site(void* out, const void* in, const voi
     const unsigned tb = (t == 0) ? s + (unsigned)(g.L[3] - 1) * st : s - st;
 
     cplx<Real> acc[12];
-    hop<0, -1, true, Real, LAYOUT, RECON>(acc, in, gauge, V, xf, s);
-    hop<0, +1, false, Real, LAYOUT, RECON>(acc, in, gauge, V, xb, xb);
-    hop<1, -1, false, Real, LAYOUT, RECON>(acc, in, gauge, V, yf, s);
-    hop<1, +1, false, Real, LAYOUT, RECON>(acc, in, gauge, V, yb, yb);
-    hop<2, -1, false, Real, LAYOUT, RECON>(acc, in, gauge, V, zf, s);
-    hop<2, +1, false, Real, LAYOUT, RECON>(acc, in, gauge, V, zb, zb);
-    hop<3, -1, false, Real, LAYOUT, RECON>(acc, in, gauge, V, tf, s);
-    hop<3, +1, false, Real, LAYOUT, RECON>(acc, in, gauge, V, tb, tb);
-    SpinorIO<Real, LAYOUT>::store(out, V, s, acc);
+    hop<0, -1, true, Real, LAYOUT, RECON, HINT>(acc, in, gauge, V, xf, s, pol.psi, pol.u_s);
+    hop<0, +1, false, Real, LAYOUT, RECON, HINT>(acc, in, gauge, V, xb, xb, pol.psi, pol.u_s);
+    hop<1, -1, false, Real, LAYOUT, RECON, HINT>(acc, in, gauge, V, yf, s, pol.psi, pol.u_s);
+    hop<1, +1, false, Real, LAYOUT, RECON, HINT>(acc, in, gauge, V, yb, yb, pol.psi, pol.u_s);
+    hop<2, -1, false, Real, LAYOUT, RECON, HINT>(acc, in, gauge, V, zf, s, pol.psi, pol.u_s);
+    hop<2, +1, false, Real, LAYOUT, RECON, HINT>(acc, in, gauge, V, zb, zb, pol.psi, pol.u_s);
+    hop<3, -1, false, Real, LAYOUT, RECON, HINT>(acc, in, gauge, V, tf, s, pol.psi, pol.u_t);
+    hop<3, +1, false, Real, LAYOUT, RECON, HINT>(acc, in, gauge, V, tb, tb, pol.psi, pol.u_t);
+    SpinorIO<Real, LAYOUT>::template store<HINT>(out, V, s, acc, pol.out);
 }
 
 }  // namespace dslash

@@ -1,18 +1,29 @@
-// dslash_tuned.cu -- the tuned Dslash kernel for sm_100a.
+// dslash_tuned.cu -- the direct (register-staged) tuned Dslash kernel for sm_100a.
 //
-// One thread per site; the thread block covers a 4-D tile of sites (x fastest inside the tile) so that
-// the +-mu neighbours of most sites of a block belong to the same block and their spinors / backward
-// links are served from the SM's L1 instead of L2 (hard part 1).  Tiles are numbered
-// x fastest, so blocks that run at the same time touch adjacent memory and the halos they share stay
-// in the 126 MB L2; HBM sees each field once per application.  See DESIGN.md "Kernels".
+// One thread per site; the thread block covers a 4-D tile of sites (x fastest inside the tile).  Tiles are
+// numbered x fastest, so blocks that run at the same time touch adjacent memory and the halos they share
+// stay in the 126 MB L2; HBM sees each field about once per application (profiles/: 1.11x).
+// With the blocked SoA layout the 12 (9) loads of a spinor (link) share one base address, which took the
+// kernel from ~2100 to ~1500 SASS instructions per site -- that matters because under sustained load the
+// B200 runs this kernel against its 1 kW power cap (SM clock ~1.4 GHz), not against a fixed clock.
+//
+// Options (dslash_set_option; both measured as no gain on 32^3x64 and left off by default):
+//   OCCUPANCY 1       compile-time variant limited to 128 registers (16 instead of 12 warps per SM).
+//   L2_POLICY bits    per-access L2 eviction policies (createpolicy + ld/st .L2::cache_hint): 1 spinor loads evict_last,
+//                     2 U_t loads evict_last, 4 U_x/U_y/U_z loads evict_first, 8 stores of `out` evict_first.
+// See DESIGN.md section 6.
 #include "dslash_kernels.cuh"
 
 namespace dslash {
 
-template <typename Real, int LAYOUT, int RECON, int MAXTPB, int MINBLK>
+struct TunedOpts {
+    int l2_policy;  // DSLASH_OPT_L2_POLICY bits
+};
+
+template <typename Real, int LAYOUT, int RECON, int MAXTPB, int MINBLK, bool HINT>
 __global__ void __launch_bounds__(MAXTPB, MINBLK)
     dslash_tuned_kernel(void* __restrict__ out, const void* __restrict__ in, const void* __restrict__ gauge, Geom g,
-                        TileGeom tg) {
+                        TileGeom tg, TunedOpts opt) {
     // tile coordinates of this block
     unsigned b = blockIdx.x;
     const unsigned bx = b % (unsigned)tg.nt[0];
@@ -32,33 +43,55 @@ __global__ void __launch_bounds__(MAXTPB, MINBLK)
     const int t = (int)((bt << tg.lb[3]) + r);
     if (x >= g.L[0] || y >= g.L[1] || z >= g.L[2] || t >= g.L[3]) return;
     const unsigned s = (unsigned)x + (unsigned)g.L[0] * ((unsigned)y + (unsigned)g.L[1] * ((unsigned)z + (unsigned)g.L[2] * (unsigned)t));
-    dslash_site<Real, LAYOUT, RECON>(out, in, gauge, g, x, y, z, t, s);
+    Policies pol{0, 0, 0, 0};
+    if (HINT) {
+        pol.psi = make_policy((opt.l2_policy & 1) ? POLICY_EVICT_LAST : POLICY_NORMAL);
+        pol.u_t = make_policy((opt.l2_policy & 2) ? POLICY_EVICT_LAST : POLICY_NORMAL);
+        pol.u_s = make_policy((opt.l2_policy & 4) ? POLICY_EVICT_FIRST : POLICY_NORMAL);
+        pol.out = make_policy((opt.l2_policy & 8) ? POLICY_EVICT_FIRST : POLICY_NORMAL);
+    }
+    dslash_site<Real, LAYOUT, RECON, HINT>(out, in, gauge, g, x, y, z, t, s, pol);
 }
 
-template <typename Real, int LAYOUT, int RECON>
-static cudaError_t launch_tuned_t(const LaunchArgs& a, const TileGeom& tg) {
+template <typename Real, int LAYOUT, int RECON, bool HINT>
+static cudaError_t launch_tuned_s(const LaunchArgs& a, const TileGeom& tg, const TunedConfig& cfg) {
     const int tpb = 1 << (tg.lb[0] + tg.lb[1] + tg.lb[2] + tg.lb[3]);
     const unsigned grid = (unsigned)tg.nt[0] * (unsigned)tg.nt[1] * (unsigned)tg.nt[2] * (unsigned)tg.nt[3];
-    if (tpb <= 128)
-        dslash_tuned_kernel<Real, LAYOUT, RECON, 128, 3><<<grid, tpb, 0, a.stream>>>(a.out, a.in, a.gauge, a.geom, tg);
-    else if (tpb <= 256)
-        dslash_tuned_kernel<Real, LAYOUT, RECON, 256, 1><<<grid, tpb, 0, a.stream>>>(a.out, a.in, a.gauge, a.geom, tg);
+    TunedOpts o{cfg.l2_policy};
+#define DSLASH_LAUNCH(MAXTPB, MINBLK) \
+    dslash_tuned_kernel<Real, LAYOUT, RECON, MAXTPB, MINBLK, HINT><<<grid, tpb, 0, a.stream>>>(a.out, a.in, a.gauge, a.geom, tg, o)
+    if (tpb <= 128) {
+        if (cfg.occupancy >= 1)
+            DSLASH_LAUNCH(128, 4);
+        else
+            DSLASH_LAUNCH(128, 3);
+    } else if (tpb <= 256)
+        DSLASH_LAUNCH(256, 1);
     else if (tpb <= 512)
-        dslash_tuned_kernel<Real, LAYOUT, RECON, 512, 1><<<grid, tpb, 0, a.stream>>>(a.out, a.in, a.gauge, a.geom, tg);
+        DSLASH_LAUNCH(512, 1);
     else
-        dslash_tuned_kernel<Real, LAYOUT, RECON, 1024, 1><<<grid, tpb, 0, a.stream>>>(a.out, a.in, a.gauge, a.geom, tg);
+        DSLASH_LAUNCH(1024, 1);
+#undef DSLASH_LAUNCH
     return cudaGetLastError();
 }
 
-template <typename Real>
-static cudaError_t launch_tuned_p(int layout_base, int recon, const LaunchArgs& a, const TileGeom& tg) {
-    if (layout_base == LAYOUT_AOS)
-        return recon == 12 ? launch_tuned_t<Real, LAYOUT_AOS, 12>(a, tg) : launch_tuned_t<Real, LAYOUT_AOS, 18>(a, tg);
-    return recon == 12 ? launch_tuned_t<Real, LAYOUT_SOA, 12>(a, tg) : launch_tuned_t<Real, LAYOUT_SOA, 18>(a, tg);
+template <typename Real, int LAYOUT, int RECON>
+static cudaError_t launch_tuned_t(const LaunchArgs& a, const TileGeom& tg, const TunedConfig& cfg) {
+    return cfg.l2_policy ? launch_tuned_s<Real, LAYOUT, RECON, true>(a, tg, cfg)
+                                : launch_tuned_s<Real, LAYOUT, RECON, false>(a, tg, cfg);
 }
 
-cudaError_t launch_tuned(int precision, int layout_base, int recon, const LaunchArgs& a, const TileGeom& tg) {
-    return precision == 0 ? launch_tuned_p<double>(layout_base, recon, a, tg) : launch_tuned_p<float>(layout_base, recon, a, tg);
+template <typename Real>
+static cudaError_t launch_tuned_p(int layout_base, int recon, const LaunchArgs& a, const TileGeom& tg, const TunedConfig& cfg) {
+    if (layout_base == LAYOUT_AOS)
+        return recon == 12 ? launch_tuned_t<Real, LAYOUT_AOS, 12>(a, tg, cfg) : launch_tuned_t<Real, LAYOUT_AOS, 18>(a, tg, cfg);
+    return recon == 12 ? launch_tuned_t<Real, LAYOUT_SOA, 12>(a, tg, cfg) : launch_tuned_t<Real, LAYOUT_SOA, 18>(a, tg, cfg);
+}
+
+cudaError_t launch_tuned(int precision, int layout_base, int recon, const LaunchArgs& a, const TileGeom& tg,
+                         const TunedConfig& cfg) {
+    return precision == 0 ? launch_tuned_p<double>(layout_base, recon, a, tg, cfg)
+                          : launch_tuned_p<float>(layout_base, recon, a, tg, cfg);
 }
 
 }  // namespace dslash

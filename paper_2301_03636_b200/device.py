@@ -96,6 +96,10 @@ class Lattice:
     def set_tile(self, tile):
         B.dslash_set_tile(self.ctx, tile)
 
+    def set_kernel(self, kernel):
+        B.dslash_set_kernel(self.ctx, {"auto": B.DSLASH_KERNEL_AUTO, "direct": B.DSLASH_KERNEL_DIRECT,
+                                       "tma": B.DSLASH_KERNEL_TMA}.get(kernel, kernel))
+
     def dslash(self, gauge_canonical, spinor_canonical):
         """Convenience: canonical NumPy in -> canonical NumPy out (one application on the device)."""
         g = self.upload_gauge(gauge_canonical)

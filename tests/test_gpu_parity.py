@@ -97,6 +97,41 @@ def test_tuned_kernel_every_tile_shape(env, tile):
         assert gpu_vs_ref(env, lat, g, p, ref) <= TOL["f64"]
 
 
+# ---------------------------------------------------------------- the TMA-staged kernel (SoA), selected explicitly
+@pytest.mark.parametrize("dims,tile", [
+    ((32, 4, 4, 4), (32, 2, 2, 1)), ((32, 4, 4, 4), (32, 1, 2, 2)), ((32, 4, 4, 4), (32, 4, 1, 1)), ((32, 4, 4, 4), (32, 1, 1, 1)),
+    ((32, 2, 2, 1), (32, 2, 2, 1)),          # a single tile: every neighbour wraps
+    ((32, 6, 5, 3), (32, 4, 1, 1)),          # ragged: partial tiles (inactive warps) in y
+    ((32, 3, 5, 7), (32, 2, 2, 1)), ((64, 4, 2, 6), (32, 2, 1, 2)), ((64, 2, 3, 2), (64, 2, 1, 1)),
+])
+@pytest.mark.parametrize("precision", ["f64", "f32"])
+@pytest.mark.parametrize("recon12", [False, True])
+def test_tma_kernel_parity(env, dims, tile, precision, recon12):
+    g, p, ref, _ = fields_and_ref(env, dims, SEED + 13, precision)
+    with env.device.Lattice(dims, precision, "soa", recon12) as lat:
+        lat.set_tile(tile)
+        lat.set_kernel("tma")
+        assert env.B.dslash_get_kernel(lat.ctx) == env.B.DSLASH_KERNEL_TMA
+        assert gpu_vs_ref(env, lat, g, p, ref) <= TOL[precision]
+
+
+def test_tma_kernel_refuses_what_it_cannot_run(env):
+    B = env.B
+    with env.device.Lattice((4, 4, 4, 4), "f64", "aos", False) as lat:  # AoS: no TMA path
+        lat.set_kernel("tma")
+        o, p, g = lat.new_spinor(), lat.new_spinor(), lat.new_gauge()
+        assert B.dslash_apply_status(lat.ctx, o.data_ptr(), p.data_ptr(), g.data_ptr()) == B.DSLASH_ERR_UNSUPPORTED
+        lat.set_kernel("auto")
+        assert B.dslash_apply_status(lat.ctx, o.data_ptr(), p.data_ptr(), g.data_ptr()) == B.DSLASH_OK
+    with env.device.Lattice((16, 4, 4, 4), "f64", "soa", False) as lat:
+        lat.set_tile((16, 4, 2, 1))  # tile rows are not whole 32-site vectors
+        lat.set_kernel("tma")
+        o, p, g = lat.new_spinor(), lat.new_spinor(), lat.new_gauge()
+        assert B.dslash_apply_status(lat.ctx, o.data_ptr(), p.data_ptr(), g.data_ptr()) == B.DSLASH_ERR_UNSUPPORTED
+        with pytest.raises(B.DslashError):
+            B.dslash_set_kernel(lat.ctx, 7)
+
+
 # ---------------------------------------------------------------- config 2: 16^4 FP64
 @pytest.mark.parametrize("layout,recon12", ALL_MODES)
 def test_config2_16x16x16x16(env, layout, recon12):
@@ -203,27 +238,45 @@ def test_gpu_gauge_covariance_and_translation(env):
 # ---------------------------------------------------------------- layout module round trip
 @pytest.mark.parametrize("precision", ["f64", "f32"])
 @pytest.mark.parametrize("layout", ["aos", "soa"])
-def test_pack_unpack_round_trip_is_bit_exact(env, precision, layout):
-    dims = (5, 4, 3, 6)
+@pytest.mark.parametrize("dims", [(8, 4, 3, 4), (5, 4, 3, 6)])  # V a multiple of 32 / a ragged last vector
+def test_pack_unpack_round_trip_is_bit_exact(env, precision, layout, dims):
     g, p = env.inputs.fields(dims, SEED + 31, precision)
     with env.device.Lattice(dims, precision, layout, False) as lat:
         back = lat.download_spinor(lat.upload_spinor(p))
         assert np.array_equal(back, p)
         nat = lat.upload_gauge(g).cpu().numpy().view(lat.np_dtype)
         v = lat.volume
-        if layout == "soa":
-            want = np.ascontiguousarray(np.moveaxis(g.reshape(v, 4, 9, 2), 0, 2)).reshape(-1)  # [mu][e][s][ri]
-        else:
-            want = g.reshape(-1)
-        assert np.array_equal(nat, want)
+        assert np.array_equal(nat[:soa_ref(g.reshape(v, 36, 2), layout).size], soa_ref(g.reshape(v, 36, 2), layout))
     with env.device.Lattice(dims, precision, layout, True) as lat:
         nat = lat.upload_gauge(g).cpu().numpy().view(lat.np_dtype)
-        g12 = g.reshape(v, 4, 3, 3, 2)[:, :, :2].reshape(v, 4, 6, 2)
-        want = np.ascontiguousarray(np.moveaxis(g12, 0, 2)).reshape(-1) if layout == "soa" else g12.reshape(-1)
-        assert np.array_equal(nat, want)
-        if layout == "soa" and precision == "f64":
-            ps = lat.upload_spinor(p).cpu().numpy().view(np.float64)
-            assert np.array_equal(ps, np.ascontiguousarray(np.moveaxis(p.reshape(v, 12, 2), 0, 1)).reshape(-1))
+        g12 = np.ascontiguousarray(g.reshape(v, 4, 3, 3, 2)[:, :, :2]).reshape(v, 24, 2)
+        assert np.array_equal(nat[:soa_ref(g12, layout).size], soa_ref(g12, layout))
+        ps = lat.upload_spinor(p).cpu().numpy().view(lat.np_dtype)
+        pref = soa_ref(p.reshape(v, 12, 2), layout)
+        assert np.array_equal(ps[:pref.size], pref)
+
+
+def soa_ref(a, layout):
+    """Reference native image of a canonical [V, ncomp, 2] field (NumPy, layout arithmetic only).
+    soa: blocked SoA of include/dslash_b200.h -- [ceil(V/32)][ncomp][32][2] for 16-byte (fp64) or 8-byte (fp32
+    link) elements; fp32 spinors pair components (2q, 2q+1) into float4 units: [v][6][32][4].  The last
+    vector is compared only up to the last real site."""
+    v, nc, _ = a.shape
+    if layout == "aos":
+        return a.reshape(-1)
+    nv = (v + 31) // 32
+    pad = np.zeros((nv * 32, nc, 2), dtype=a.dtype)
+    pad[:v] = a
+    if a.dtype == np.float32 and nc == 12:  # fp32 spinor: float4 units
+        out = pad.reshape(nv, 32, 6, 4).transpose(0, 2, 1, 3)
+    else:
+        out = pad.reshape(nv, 32, nc, 2).transpose(0, 2, 1, 3)
+    flat = np.ascontiguousarray(out).reshape(-1)
+    # drop the (unspecified) padding tail: keep whole vectors only if V is a multiple of 32
+    if v % 32:
+        full = (v // 32) * 32 * nc * 2
+        return flat[:full]
+    return flat
 
 
 # ---------------------------------------------------------------- error behaviour on a live context
