@@ -43,7 +43,10 @@ CONFIGS = {
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture (profiles/); None until captured for that workload.
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {
+    # profiles/r01_ncu_tuned_kernel.txt, capture r01b: 1.6467 GB read + 0.3914 GB written (mean of 2 launches)
+    "32x32x32x64_f64_soa_r18": 2037656000,
+}
 
 
 def bytes_per_site(precision, recon12):
@@ -67,7 +70,7 @@ class ClockSampler:
                0x80: "hw_power_brake_slowdown"}
 
     def __init__(self, index):
-        self.samples, self.reasons, self.max_mhz, self.ok = [], set(), None, False
+        self.samples, self.power, self.reasons, self.max_mhz, self.ok = [], [], set(), None, False
         self._stop = threading.Event()
         try:
             import pynvml
@@ -84,6 +87,7 @@ class ClockSampler:
         while not self._stop.is_set():
             try:
                 self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
                 try:
                     r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
                 except Exception:
@@ -109,8 +113,9 @@ class ClockSampler:
     def summary(self):
         if not self.ok or not self.samples:
             return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": 0}
-        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
-                "samples": len(self.samples)}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_min_mhz": int(min(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples),
+                "power_w": float(np.median(self.power)) if self.power else None}
 
 
 # ------------------------------------------------------------------ CPU oracle legs
@@ -203,6 +208,10 @@ def run_cuda(args, cfg):
         with device.Lattice(dims, prec, args.layout, recon12, device="cuda:%d" % local) as lat:
             if args.tile:
                 lat.set_tile(args.tile)
+            if args.occupancy is not None:
+                B.dslash_set_option(lat.ctx, B.DSLASH_OPT_OCCUPANCY, args.occupancy)
+            if args.kernel:
+                lat.set_kernel(args.kernel)
             gd, pd, od = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
             n0 = B.dslash_launch_count(lat.ctx)
             ms, ck = time_applies(torch, lat, od, pd, gd, args.steps, args.warmup, group, local)
@@ -211,9 +220,17 @@ def run_cuda(args, cfg):
             results[tag] = dict(ms=ms, ms_per_step=ms / args.steps,
                                 gflops=replicas.whole_job_rate(FLOP_PER_SITE * v, world, ms / args.steps) / 1e9,
                                 gbs=bps * v / (ms / args.steps) / 1e6, bps=bps, recon12=recon12,
-                                tile=list(B.dslash_get_tile(lat.ctx)))
+                                tile=list(B.dslash_get_tile(lat.ctx)),
+                                kernel={B.DSLASH_KERNEL_DIRECT: "direct", B.DSLASH_KERNEL_TMA: "tma"}[B.dslash_get_kernel(lat.ctx)],
+                                occupancy=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_OCCUPANCY))
             if tag == "main":
                 clocks, launches = ck, n1 - n0 - args.warmup
+                if args.sustained_steps > 0:
+                    # the same kernel after ~0.6 s of continuous load, when the board runs against its power cap
+                    ms_s, ck_s = time_applies(torch, lat, od, pd, gd, args.sustained_steps, args.heat_steps, group, local)
+                    results["sustained"] = dict(ms_per_step=ms_s / args.sustained_steps, clocks=ck_s,
+                                                gbs=bps * v / (ms_s / args.sustained_steps) / 1e6,
+                                                gflops=replicas.whole_job_rate(FLOP_PER_SITE * v, world, ms_s / args.sustained_steps) / 1e9)
             del gd, pd, od
 
     main = results["main"]
@@ -253,9 +270,10 @@ def run_cuda(args, cfg):
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         g64, p64 = inputs.promote(g), inputs.promote(p)
-        gf, dt, cores, n = oracle_timing(dims, g64, p64, min(v, args.cpu_sites), 1, 0)
-        cpu_baseline = {"value": gf, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "seconds": dt,
-                        "sample": "1 application to %d of %d sites (%s)" % (n, v, "whole lattice" if n == v else "seeded sample")}
+        gf, dt, cores, n = oracle_timing(dims, g64, p64, min(v, args.cpu_sites), 3, 1)
+        cpu_baseline = {"value": gf, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "seconds_per_application": dt,
+                        "sample": "mean of 3 applications (after 1 warm-up) to %d of %d sites (%s)"
+                                  % (n, v, "whole lattice" if n == v else "seeded sample")}
 
     if rank == 0:
         line = {
@@ -263,12 +281,18 @@ def run_cuda(args, cfg):
             "warmup": args.warmup, "ms_per_step": main["ms_per_step"], "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": prec, "data": "synthetic",
             "config": {"workload": cfg["name"], "dims": list(dims), "layout": args.layout, "recon": 12 if main["recon12"] else 18,
-                       "tile": main["tile"], "sites": v, "parallelism": "replicas x%d" % world,
+                       "tile": main["tile"], "kernel": main["kernel"], "occupancy_option": main["occupancy"], "sites": v, "parallelism": "replicas x%d" % world,
                        "l2": "inputs larger than L2: %.2f GB working set per apply vs 126 MB L2, no flush needed"
                              % (main["bps"] * v / 1e9)},
             "hbm_gbs": main["gbs"], "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "clocks": clocks,
             "gpu_launches": int(launches),
         }
+        if "sustained" in results:
+            su = results["sustained"]
+            line["sustained"] = {"value": su["gflops"], "ms_per_step": su["ms_per_step"], "hbm_gbs": su["gbs"],
+                                 "roofline_frac": su["gbs"] / peak, "steps": args.sustained_steps, "heat_steps": args.heat_steps,
+                                 "clocks": su["clocks"],
+                                 "note": "same launches after heat_steps back-to-back applies: SM clock under the 1 kW power cap"}
         if "other_recon" in results:
             o = results["other_recon"]
             line["also"] = {"recon": 12 if o["recon12"] else 18, "value": o["gflops"], "ms_per_step": o["ms_per_step"],
@@ -365,12 +389,16 @@ def run_sweep(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=500)
-    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=100)  # 10 warm-up + 100 applies
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--sustained-steps", type=int, default=300, help="0: skip the power-capped (sustained) measurement")
+    ap.add_argument("--heat-steps", type=int, default=1500)
     ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
     ap.add_argument("--config", choices=sorted(CONFIGS), default="3")
     ap.add_argument("--layout", choices=["soa", "aos"], default="soa")
     ap.add_argument("--tile", type=int, nargs=4, default=None, help="tile of the tuned kernel (x y z t)")
+    ap.add_argument("--occupancy", type=int, default=None, help="DSLASH_OPT_OCCUPANCY override")
+    ap.add_argument("--kernel", choices=["auto", "direct", "tma"], default=None)
     ap.add_argument("--both-recon", action="store_true", default=True, help="also time the other link compression")
     ap.add_argument("--one-recon", dest="both_recon", action="store_false")
     ap.add_argument("--no-e2e", action="store_true")

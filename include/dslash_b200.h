@@ -93,7 +93,8 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
 #define DSLASH_KERNEL_TMA 2    /* tile's own spinors and links staged in shared memory by TMA bulk tensor copies */
 
 /* options of the tuned kernels, dslash_set_option() */
-#define DSLASH_OPT_OCCUPANCY 2        /* 0: default register budget; 1: 128-register variant (more resident warps) */
+#define DSLASH_OPT_OCCUPANCY 2        /* blocks of <= 128 threads: 0 = 168 registers/thread (12 warps/SM), 1 = 128 (16 warps),
+                                         2 = 255 (8 warps, deeper load hoisting) */
 #define DSLASH_OPT_L2_POLICY 3        /* bit mask of L2 eviction hints: 1 spinor loads evict_last, 2 U_t loads evict_last,
                                          4 U_x/U_y/U_z loads evict_first, 8 stores of `out` evict_first (0: none) */
 

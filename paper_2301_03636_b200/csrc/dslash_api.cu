@@ -48,21 +48,28 @@ static void set_tile_geom(dslash_ctx* c, const int tile[4]) {
     }
 }
 
-// Default tile: grow towards 8 x 4 x 4 x 1 (128 threads), never beyond the next power of two of an extent;
-// leftover threads go to the other directions in the order t, z, y, x.
+// Default tile of the tuned kernel (measured on B200, profiles/): x-extent = the largest power of two <= 32 that
+// divides L_X (a warp then reads whole 32-site vectors or aligned halves of them), 2-4 rows in y, 2 planes in z,
+// about 128 sites per block for wide rows and 64 for narrow ones; never beyond the next power of two of an extent.
 static void default_tile(const dslash_ctx* c, int tile[4]) {
-    const int want[4] = {8, 4, 4, 1};
     int cap[4];
     for (int d = 0; d < 4; ++d) {
         cap[d] = 1;
         while (cap[d] < c->geom.L[d]) cap[d] <<= 1;
-        tile[d] = want[d] < cap[d] ? want[d] : cap[d];
     }
+    int bx = 32;
+    while (bx > 1 && (c->geom.L[0] % bx)) bx >>= 1;
+    if (bx < 4) bx = cap[0] < 8 ? cap[0] : 8;  // odd or tiny L_X: edge threads idle instead
+    int by = 64 / bx;
+    if (by < 1) by = 1;
+    if (by > 4) by = 4;
+    const int want[4] = {bx, by, 2, 1};
+    for (int d = 0; d < 4; ++d) tile[d] = want[d] < cap[d] ? want[d] : cap[d];
     const int order[4] = {3, 2, 1, 0};
     bool grew = true;
-    while (tile[0] * tile[1] * tile[2] * tile[3] < 128 && grew) {
+    while (tile[0] * tile[1] * tile[2] * tile[3] < 64 && grew) {
         grew = false;
-        for (int k = 0; k < 4 && tile[0] * tile[1] * tile[2] * tile[3] < 128; ++k) {
+        for (int k = 0; k < 4 && tile[0] * tile[1] * tile[2] * tile[3] < 64; ++k) {
             const int d = order[k];
             if (tile[d] < cap[d]) {
                 tile[d] <<= 1;
@@ -107,7 +114,7 @@ int dslash_create(dslash_ctx** ctx, const int dims[4], int precision, int layout
     default_tile(c, tile);
     set_tile_geom(c, tile);
     c->kernel = DSLASH_KERNEL_AUTO;
-    c->cfg.occupancy = 0;
+    c->cfg.occupancy = precision == DSLASH_FP64 ? 2 : 1;  // measured: fp64 wants registers (ILP), fp32 wants warps
     c->cfg.l2_policy = 0;
     c->launches = 0;
     c->last_cuda = 0;
@@ -272,7 +279,7 @@ int dslash_set_option(dslash_ctx* c, int option, int value) {
     if (!c) return DSLASH_ERR_NULL;
     switch (option) {
         case DSLASH_OPT_OCCUPANCY:
-            if (value < 0 || value > 1) return DSLASH_ERR_UNSUPPORTED;
+            if (value < 0 || value > 2) return DSLASH_ERR_UNSUPPORTED;
             c->cfg.occupancy = value;
             return DSLASH_OK;
         case DSLASH_OPT_L2_POLICY:

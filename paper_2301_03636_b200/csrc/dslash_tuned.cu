@@ -8,7 +8,8 @@
 // B200 runs this kernel against its 1 kW power cap (SM clock ~1.4 GHz), not against a fixed clock.
 //
 // Options (dslash_set_option; both measured as no gain on 32^3x64 and left off by default):
-//   OCCUPANCY 1       compile-time variant limited to 128 registers (16 instead of 12 warps per SM).
+//   OCCUPANCY 1 / 2   compile-time variants for blocks of <= 128 threads: 1 = 128 registers (16 warps per SM),
+//                     2 = 255 registers (8 warps per SM, deeper load hoisting); 0 = 168 registers (12 warps).
 //   L2_POLICY bits    per-access L2 eviction policies (createpolicy + ld/st .L2::cache_hint): 1 spinor loads evict_last,
 //                     2 U_t loads evict_last, 4 U_x/U_y/U_z loads evict_first, 8 stores of `out` evict_first.
 // See DESIGN.md section 6.
@@ -61,8 +62,10 @@ static cudaError_t launch_tuned_s(const LaunchArgs& a, const TileGeom& tg, const
 #define DSLASH_LAUNCH(MAXTPB, MINBLK) \
     dslash_tuned_kernel<Real, LAYOUT, RECON, MAXTPB, MINBLK, HINT><<<grid, tpb, 0, a.stream>>>(a.out, a.in, a.gauge, a.geom, tg, o)
     if (tpb <= 128) {
-        if (cfg.occupancy >= 1)
+        if (cfg.occupancy == 1)
             DSLASH_LAUNCH(128, 4);
+        else if (cfg.occupancy == 2)
+            DSLASH_LAUNCH(128, 2);
         else
             DSLASH_LAUNCH(128, 3);
     } else if (tpb <= 256)
