@@ -90,7 +90,8 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
 /* kernel selection of the tuned path, dslash_set_kernel() */
 #define DSLASH_KERNEL_AUTO 0   /* the library picks (TMA-staged when the layout/lattice/tile allow it, else direct) */
 #define DSLASH_KERNEL_DIRECT 1 /* one thread per site, all neighbours gathered from global memory through L1/L2 */
-#define DSLASH_KERNEL_TMA 2    /* tile's own spinors and links staged in shared memory by TMA bulk tensor copies */
+#define DSLASH_KERNEL_TMA 2    /* tile's own spinors and links staged in shared memory by TMA bulk copies */
+#define DSLASH_KERNEL_TMA_LINKS 3 /* only the tile's own links staged by TMA bulk copies; spinors gathered directly */
 
 /* options of the tuned kernels, dslash_set_option() */
 #define DSLASH_OPT_OCCUPANCY 2        /* blocks of <= 128 threads: 0 = 168 registers/thread (12 warps/SM), 1 = 128 (16 warps),
@@ -177,12 +178,12 @@ DSLASH_API int dslash_set_tile(dslash_ctx *ctx, const int tile[4]);
 DSLASH_API int dslash_get_tile(const dslash_ctx *ctx, int tile[4]);
 
 /*
- * Choose the implementation behind DSLASH_VARIANT_TUNED: DSLASH_KERNEL_AUTO (default), _DIRECT or _TMA.
- * _TMA needs a DSLASH_SOA ctx, a tile whose x-extent is a multiple of 32 and divides L_X, the other tile
+ * Choose the implementation behind DSLASH_VARIANT_TUNED: DSLASH_KERNEL_AUTO (default), _DIRECT, _TMA or _TMA_LINKS.
+ * _TMA and _TMA_LINKS need a DSLASH_SOA ctx, a tile whose x-extent is a multiple of 32 and divides L_X, the other tile
  * extents <= the lattice extents, and 32..128 sites per tile;
  * if it is selected explicitly and the current tile/lattice do not allow it, dslash_apply returns
  * DSLASH_ERR_UNSUPPORTED (AUTO falls back to _DIRECT silently -- both are CUDA kernels of this library).
- * dslash_get_kernel reports the kernel the next dslash_apply would launch (_DIRECT or _TMA).
+ * dslash_get_kernel reports the kernel the next dslash_apply would launch (_DIRECT, _TMA or _TMA_LINKS).
  * Errors: NULL, UNSUPPORTED (unknown value).
  */
 DSLASH_API int dslash_set_kernel(dslash_ctx *ctx, int kernel);

@@ -20,7 +20,7 @@ DSLASH_ERR_NULL, DSLASH_ERR_DIMS, DSLASH_ERR_PRECISION, DSLASH_ERR_LAYOUT = -1, 
 DSLASH_ERR_ALIGN, DSLASH_ERR_ALIAS, DSLASH_ERR_UNSUPPORTED, DSLASH_ERR_CUDA, DSLASH_ERR_NOMEM = -5, -6, -7, -8, -9
 DSLASH_VARIANT_TUNED = 0
 DSLASH_MAP_MINIMAL, DSLASH_MAP_TOFROM = 0, 1
-DSLASH_KERNEL_AUTO, DSLASH_KERNEL_DIRECT, DSLASH_KERNEL_TMA = 0, 1, 2
+DSLASH_KERNEL_AUTO, DSLASH_KERNEL_DIRECT, DSLASH_KERNEL_TMA, DSLASH_KERNEL_TMA_LINKS = 0, 1, 2, 3
 DSLASH_OPT_OCCUPANCY, DSLASH_OPT_L2_POLICY = 2, 3
 
 _c_int_p = ctypes.POINTER(ctypes.c_int)

@@ -155,7 +155,7 @@ size_t dslash_canonical_gauge_bytes(const dslash_ctx* c) { return c ? (size_t)c-
 static int resolve_kernel(const dslash_ctx* c) {
     const bool can_tma = c->layout_base == LAYOUT_SOA && tma_eligible(c->precision, c->recon, c->geom, c->tg);
     if (c->kernel == DSLASH_KERNEL_DIRECT) return DSLASH_KERNEL_DIRECT;
-    if (c->kernel == DSLASH_KERNEL_TMA) return can_tma ? DSLASH_KERNEL_TMA : -1;
+    if (c->kernel == DSLASH_KERNEL_TMA || c->kernel == DSLASH_KERNEL_TMA_LINKS) return can_tma ? c->kernel : -1;
     return DSLASH_KERNEL_DIRECT;  // AUTO
 }
 
@@ -175,8 +175,8 @@ int dslash_apply(dslash_ctx* c, void* out, const void* in, const void* gauge, ds
     if (c->var_depth == DSLASH_VARIANT_TUNED) {
         const int k = resolve_kernel(c);
         if (k < 0) return DSLASH_ERR_UNSUPPORTED;
-        e = (k == DSLASH_KERNEL_TMA) ? launch_tma(c->precision, c->recon, a, c->tg)
-                                     : launch_tuned(c->precision, c->layout_base, c->recon, a, c->tg, c->cfg);
+        e = (k == DSLASH_KERNEL_DIRECT) ? launch_tuned(c->precision, c->layout_base, c->recon, a, c->tg, c->cfg)
+                                        : launch_tma(c->precision, c->recon, a, c->tg, k == DSLASH_KERNEL_TMA_LINKS);
     } else
         e = launch_variant(c->precision, c->layout_base, c->recon, a, c->var_depth, c->var_tpb, c->var_spt);
     if (e != cudaSuccess) return cuda_fail(c, e);
@@ -302,7 +302,8 @@ int dslash_get_option(const dslash_ctx* c, int option, int* value) {
 
 int dslash_set_kernel(dslash_ctx* c, int kernel) {
     if (!c) return DSLASH_ERR_NULL;
-    if (kernel != DSLASH_KERNEL_AUTO && kernel != DSLASH_KERNEL_DIRECT && kernel != DSLASH_KERNEL_TMA)
+    if (kernel != DSLASH_KERNEL_AUTO && kernel != DSLASH_KERNEL_DIRECT && kernel != DSLASH_KERNEL_TMA &&
+        kernel != DSLASH_KERNEL_TMA_LINKS)
         return DSLASH_ERR_UNSUPPORTED;
     c->kernel = kernel;
     return DSLASH_OK;

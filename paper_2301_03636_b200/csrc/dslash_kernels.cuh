@@ -37,7 +37,7 @@ cudaError_t launch_tuned(int precision, int layout_base, int recon, const Launch
 
 // TMA-staged kernel (SoA only): tile's own spinors + links by cp.async.bulk.tensor into shared memory.
 bool tma_eligible(int precision, int recon, const Geom& g, const TileGeom& tg);
-cudaError_t launch_tma(int precision, int recon, const LaunchArgs& a, const TileGeom& tg);
+cudaError_t launch_tma(int precision, int recon, const LaunchArgs& a, const TileGeom& tg, bool links_only);
 
 // Layout module.  dir 0: canonical -> native (pack), 1: native -> canonical (unpack).
 cudaError_t launch_convert_spinor(int precision, int layout_base, void* dst, const void* src, unsigned V, int dir,

@@ -228,6 +228,98 @@ __global__ void __launch_bounds__(128, 2)
     }
 }
 
+// ------------------------------------------------------------------ links-only staging ("TMA-lite")
+// Only the tile's own links U_mu(x) (60 % of the compulsory bytes, used by the four forward hops) are bulk-copied to
+// shared memory.  All spinors and the backward links are gathered from global memory in straight-line code exactly as in
+// the direct kernel (so the compiler keeps overlapping the loads of the next hop with the arithmetic of the current one),
+// but the four backward hops run first and the four forward hops -- which need no register-staged link loads any more --
+// run after the mbarrier wait.  36 of the 168 register-staged 16-byte loads per site disappear and their DRAM latency is
+// taken by the TMA unit instead of by a warp.
+template <int MU, typename Real, int RECON>
+__device__ __forceinline__ void hop_fwd_smemlink(cplx<Real> (&acc)[12], const void* in, const void* u_s, unsigned V, unsigned sn,
+                                                 unsigned ltid) {
+    cplx<Real> psi[12], h[6], hp[6], u[9];
+    SpinorIO<Real, LAYOUT_SOA>::load(psi, in, V, sn);
+    load_link_smem<Real, RECON>(u, u_s, ltid, MU);
+    project<MU, -1>(h, psi);
+    su3_mul<false>(hp, u, h);
+    reconstruct_accumulate<MU, -1, false>(acc, hp);
+}
+
+template <typename Real, int RECON>
+__global__ void __launch_bounds__(128, 2)
+    dslash_tma_links_kernel(void* __restrict__ out, const void* __restrict__ in, const void* __restrict__ gauge, const Geom g,
+                            const TileGeom tg) {
+    constexpr unsigned U_VEC_BYTES = 4u * (RECON == 12 ? 12u : 18u) * VL * sizeof(Real);
+    extern __shared__ __align__(128) unsigned char smem[];
+    const unsigned T = blockDim.x;
+    const unsigned nvec = T >> VL_LOG2;
+    unsigned char* u_s = smem;
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem + nvec * U_VEC_BYTES);
+
+    unsigned b = blockIdx.x;
+    const unsigned tbx = b % (unsigned)tg.nt[0];
+    b /= (unsigned)tg.nt[0];
+    const unsigned tby = b % (unsigned)tg.nt[1];
+    b /= (unsigned)tg.nt[1];
+    const unsigned tbz = b % (unsigned)tg.nt[2];
+    const unsigned tbt = b / (unsigned)tg.nt[2];
+    const int x0 = (int)(tbx << tg.lb[0]), y0 = (int)(tby << tg.lb[1]), z0 = (int)(tbz << tg.lb[2]), t0 = (int)(tbt << tg.lb[3]);
+    const unsigned tid = threadIdx.x;
+    unsigned r = tid;
+    const int x = x0 + (int)(r & ((1u << tg.lb[0]) - 1u));
+    r >>= tg.lb[0];
+    const int y = y0 + (int)(r & ((1u << tg.lb[1]) - 1u));
+    r >>= tg.lb[1];
+    const int z = z0 + (int)(r & ((1u << tg.lb[2]) - 1u));
+    r >>= tg.lb[2];
+    const int t = t0 + (int)r;
+    const bool active = (y < g.L[1]) && (z < g.L[2]) && (t < g.L[3]);
+    const unsigned V = g.V;
+    const unsigned sy = (unsigned)g.L[0], sz = sy * (unsigned)g.L[1], st = sz * (unsigned)g.L[2];
+    const unsigned s = (unsigned)x + sy * (unsigned)y + sz * (unsigned)z + st * (unsigned)t;
+
+    const unsigned rows_y = min((unsigned)(g.L[1] - y0), 1u << tg.lb[1]);
+    const unsigned rows_z = min((unsigned)(g.L[2] - z0), 1u << tg.lb[2]);
+    const unsigned rows_t = min((unsigned)(g.L[3] - t0), 1u << tg.lb[3]);
+    const unsigned nactive_vec = (rows_y * rows_z * rows_t) << (tg.lb[0] - (int)VL_LOG2);
+
+    if (tid == 0) {
+        mbar_init(bar, 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (tid == 0) mbar_arrive_expect_tx(bar, nactive_vec * U_VEC_BYTES);
+    __syncthreads();
+    if (active && (tid & (VL - 1u)) == 0)
+        bulk_g2s(u_s + (tid >> VL_LOG2) * U_VEC_BYTES,
+                 reinterpret_cast<const unsigned char*>(gauge) + (size_t)(s >> VL_LOG2) * U_VEC_BYTES, U_VEC_BYTES, bar);
+
+    cplx<Real> acc[12];
+    if (active) {
+        const unsigned xf = (x + 1 == g.L[0]) ? s - (unsigned)(g.L[0] - 1) : s + 1u;
+        const unsigned xb = (x == 0) ? s + (unsigned)(g.L[0] - 1) : s - 1u;
+        const unsigned yf = (y + 1 == g.L[1]) ? s - (unsigned)(g.L[1] - 1) * sy : s + sy;
+        const unsigned yb = (y == 0) ? s + (unsigned)(g.L[1] - 1) * sy : s - sy;
+        const unsigned zf = (z + 1 == g.L[2]) ? s - (unsigned)(g.L[2] - 1) * sz : s + sz;
+        const unsigned zb = (z == 0) ? s + (unsigned)(g.L[2] - 1) * sz : s - sz;
+        const unsigned tf = (t + 1 == g.L[3]) ? s - (unsigned)(g.L[3] - 1) * st : s + st;
+        const unsigned tb = (t == 0) ? s + (unsigned)(g.L[3] - 1) * st : s - st;
+        // backward hops: everything from global memory
+        hop<3, +1, true, Real, LAYOUT_SOA, RECON>(acc, in, gauge, V, tb, tb);
+        hop<2, +1, false, Real, LAYOUT_SOA, RECON>(acc, in, gauge, V, zb, zb);
+        hop<1, +1, false, Real, LAYOUT_SOA, RECON>(acc, in, gauge, V, yb, yb);
+        hop<0, +1, false, Real, LAYOUT_SOA, RECON>(acc, in, gauge, V, xb, xb);
+        mbar_wait(bar, 0);
+        // forward hops: spinor from global memory, own link from shared memory
+        hop_fwd_smemlink<0, Real, RECON>(acc, in, u_s, V, xf, tid);
+        hop_fwd_smemlink<1, Real, RECON>(acc, in, u_s, V, yf, tid);
+        hop_fwd_smemlink<2, Real, RECON>(acc, in, u_s, V, zf, tid);
+        hop_fwd_smemlink<3, Real, RECON>(acc, in, u_s, V, tf, tid);
+        SpinorIO<Real, LAYOUT_SOA>::store(out, V, s, acc);
+    }
+}
+
 // ------------------------------------------------------------------ host side
 static size_t tma_smem_bytes(int precision, int recon, int T) {
     const size_t rb = precision == 0 ? 8u : 4u;
@@ -247,26 +339,32 @@ bool tma_eligible(int precision, int recon, const Geom& g, const TileGeom& tg) {
     return tma_smem_bytes(precision, recon, T) <= 113u * 1024u;
 }
 
-template <typename Real, int RECON>
+template <typename Real, int RECON, bool LINKS_ONLY>
 static cudaError_t launch_tma_t(const LaunchArgs& a, const TileGeom& tg) {
     const int T = 1 << (tg.lb[0] + tg.lb[1] + tg.lb[2] + tg.lb[3]);
-    const size_t smem = tma_smem_bytes(sizeof(Real) == 8 ? 0 : 1, RECON, T);
+    const int prec = sizeof(Real) == 8 ? 0 : 1;
+    const size_t smem = LINKS_ONLY ? tma_smem_bytes(prec, RECON, T) - (size_t)T * 24u * sizeof(Real) : tma_smem_bytes(prec, RECON, T);
+    auto kernel = LINKS_ONLY ? dslash_tma_links_kernel<Real, RECON> : dslash_tma_kernel<Real, RECON>;
     static bool attr_set = false;  // per template instantiation
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(dslash_tma_kernel<Real, RECON>, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024);
         if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(dslash_tma_kernel<Real, RECON>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+        e = cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, LINKS_ONLY ? 75 : 100);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
     const unsigned grid = (unsigned)tg.nt[0] * (unsigned)tg.nt[1] * (unsigned)tg.nt[2] * (unsigned)tg.nt[3];
-    dslash_tma_kernel<Real, RECON><<<grid, T, smem, a.stream>>>(a.out, a.in, a.gauge, a.geom, tg);
+    kernel<<<grid, T, smem, a.stream>>>(a.out, a.in, a.gauge, a.geom, tg);
     return cudaGetLastError();
 }
 
-cudaError_t launch_tma(int precision, int recon, const LaunchArgs& a, const TileGeom& tg) {
-    if (precision == 0) return recon == 12 ? launch_tma_t<double, 12>(a, tg) : launch_tma_t<double, 18>(a, tg);
-    return recon == 12 ? launch_tma_t<float, 12>(a, tg) : launch_tma_t<float, 18>(a, tg);
+cudaError_t launch_tma(int precision, int recon, const LaunchArgs& a, const TileGeom& tg, bool links_only) {
+    if (links_only) {
+        if (precision == 0) return recon == 12 ? launch_tma_t<double, 12, true>(a, tg) : launch_tma_t<double, 18, true>(a, tg);
+        return recon == 12 ? launch_tma_t<float, 12, true>(a, tg) : launch_tma_t<float, 18, true>(a, tg);
+    }
+    if (precision == 0) return recon == 12 ? launch_tma_t<double, 12, false>(a, tg) : launch_tma_t<double, 18, false>(a, tg);
+    return recon == 12 ? launch_tma_t<float, 12, false>(a, tg) : launch_tma_t<float, 18, false>(a, tg);
 }
 
 }  // namespace dslash

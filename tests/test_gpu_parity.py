@@ -106,12 +106,14 @@ def test_tuned_kernel_every_tile_shape(env, tile):
 ])
 @pytest.mark.parametrize("precision", ["f64", "f32"])
 @pytest.mark.parametrize("recon12", [False, True])
-def test_tma_kernel_parity(env, dims, tile, precision, recon12):
+@pytest.mark.parametrize("kernel", ["tma", "tma_links"])
+def test_tma_kernel_parity(env, dims, tile, precision, recon12, kernel):
     g, p, ref, _ = fields_and_ref(env, dims, SEED + 13, precision)
     with env.device.Lattice(dims, precision, "soa", recon12) as lat:
         lat.set_tile(tile)
-        lat.set_kernel("tma")
-        assert env.B.dslash_get_kernel(lat.ctx) == env.B.DSLASH_KERNEL_TMA
+        lat.set_kernel(kernel)
+        want = env.B.DSLASH_KERNEL_TMA if kernel == "tma" else env.B.DSLASH_KERNEL_TMA_LINKS
+        assert env.B.dslash_get_kernel(lat.ctx) == want
         assert gpu_vs_ref(env, lat, g, p, ref) <= TOL[precision]
 
 
