@@ -87,6 +87,11 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
 /* variant selection: collapse_depth DSLASH_VARIANT_TUNED selects the library's tuned kernel */
 #define DSLASH_VARIANT_TUNED 0
 
+/* schedules of the paper's offload variants, dslash_set_omp_variant() */
+#define DSLASH_SCHED_STATIC 0
+#define DSLASH_SCHED_DYNAMIC 1
+#define DSLASH_SCHED_GUIDED 2
+
 /* kernel selection of the tuned path, dslash_set_kernel() */
 #define DSLASH_KERNEL_AUTO 0   /* the library picks (TMA-staged when the layout/lattice/tile allow it, else direct) */
 #define DSLASH_KERNEL_DIRECT 1 /* one thread per site, all neighbours gathered from global memory through L1/L2 */
@@ -168,6 +173,25 @@ DSLASH_API int dslash_get_variant(const dslash_ctx *ctx, int *collapse_depth, in
  * Errors: NULL, UNSUPPORTED (index out of range). */
 DSLASH_API int dslash_variant_count(void);
 DSLASH_API int dslash_variant_at(int index, int *collapse_depth, int *threads_per_block, int *sites_per_thread, int *layout);
+
+/*
+ * The paper's own variant space (section 4.1.3, Table 1).  For num_loops nested loops (1..4) a
+ * variant is (parallel_position x, distribute_collapse a, parallel_collapse b, schedule, map_mode):
+ *   x in 0..num_loops-1;  a = 0 if x == 0 (combined `teams distribute parallel for`), else 1 <= a <= x;
+ *   1 <= b <= num_loops - x;  schedule in DSLASH_SCHED_*;  map_mode in DSLASH_MAP_* (the two host<->device
+ *   data-transfer modes; it only matters to dslash_apply_host).
+ * dslash_omp_variant_count(num_loops) = 6, 18, 42, 84 for 1..4 loops (Table 1; 0 for any other num_loops);
+ * dslash_omp_variant_at enumerates them (order: x, then a, then b, then schedule, then map_mode fastest).
+ * dslash_set_omp_variant selects the CUDA analogue of one loop structure for dslash_apply on the four Dslash loops
+ * (t,z,y,x): a team is a thread block of team_size threads (32..256, multiple of 32), the league has num_teams blocks
+ * (clamped to the distribute space; 0 = 4 per SM).  dslash_set_variant(ctx, DSLASH_VARIANT_TUNED, 0, 0) leaves it.
+ * Errors: NULL, UNSUPPORTED (outside the space above).
+ */
+DSLASH_API int dslash_omp_variant_count(int num_loops);
+DSLASH_API int dslash_omp_variant_at(int num_loops, int index, int *parallel_position, int *distribute_collapse,
+                                     int *parallel_collapse, int *schedule, int *map_mode);
+DSLASH_API int dslash_set_omp_variant(dslash_ctx *ctx, int parallel_position, int distribute_collapse, int parallel_collapse,
+                                      int schedule, int num_teams, int team_size);
 
 /*
  * Tuning of the tuned kernel: the thread block covers a tile of tile[0] x tile[1] x tile[2] x tile[3]

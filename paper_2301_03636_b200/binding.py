@@ -22,6 +22,7 @@ DSLASH_VARIANT_TUNED = 0
 DSLASH_MAP_MINIMAL, DSLASH_MAP_TOFROM = 0, 1
 DSLASH_KERNEL_AUTO, DSLASH_KERNEL_DIRECT, DSLASH_KERNEL_TMA, DSLASH_KERNEL_TMA_LINKS = 0, 1, 2, 3
 DSLASH_OPT_OCCUPANCY, DSLASH_OPT_L2_POLICY = 2, 3
+DSLASH_SCHED_STATIC, DSLASH_SCHED_DYNAMIC, DSLASH_SCHED_GUIDED = 0, 1, 2
 
 _c_int_p = ctypes.POINTER(ctypes.c_int)
 _c_size_p = ctypes.POINTER(ctypes.c_size_t)
@@ -43,6 +44,10 @@ SIGNATURES = {
     "dslash_get_variant": (ctypes.c_int, [_vp, _c_int_p, _c_int_p, _c_int_p]),
     "dslash_variant_count": (ctypes.c_int, []),
     "dslash_variant_at": (ctypes.c_int, [ctypes.c_int, _c_int_p, _c_int_p, _c_int_p, _c_int_p]),
+    "dslash_omp_variant_count": (ctypes.c_int, [ctypes.c_int]),
+    "dslash_omp_variant_at": (ctypes.c_int, [ctypes.c_int, ctypes.c_int, _c_int_p, _c_int_p, _c_int_p, _c_int_p, _c_int_p]),
+    "dslash_set_omp_variant": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                               ctypes.c_int]),
     "dslash_set_tile": (ctypes.c_int, [_vp, _c_int_p]),
     "dslash_get_tile": (ctypes.c_int, [_vp, _c_int_p]),
     "dslash_set_kernel": (ctypes.c_int, [_vp, ctypes.c_int]),
@@ -173,6 +178,23 @@ def dslash_variant_at(index: int):
     _check(_lib.dslash_variant_at(int(index), ctypes.byref(d), ctypes.byref(b), ctypes.byref(s), ctypes.byref(l)),
            "dslash_variant_at")
     return d.value, b.value, s.value, l.value
+
+
+def dslash_omp_variant_count(num_loops: int) -> int:
+    return int(_lib.dslash_omp_variant_count(int(num_loops)))
+
+
+def dslash_omp_variant_at(num_loops: int, index: int):
+    """(parallel_position, distribute_collapse, parallel_collapse, schedule, map_mode) of the paper's variant `index`."""
+    v = [ctypes.c_int() for _ in range(5)]
+    _check(_lib.dslash_omp_variant_at(int(num_loops), int(index), *[ctypes.byref(i) for i in v]), "dslash_omp_variant_at")
+    return tuple(i.value for i in v)
+
+
+def dslash_set_omp_variant(ctx, parallel_position: int, distribute_collapse: int, parallel_collapse: int, schedule: int,
+                           num_teams: int = 0, team_size: int = 128) -> None:
+    _check(_lib.dslash_set_omp_variant(_ptr(ctx), int(parallel_position), int(distribute_collapse), int(parallel_collapse),
+                                       int(schedule), int(num_teams), int(team_size)), "dslash_set_omp_variant")
 
 
 def dslash_set_tile(ctx, tile) -> None:

@@ -15,7 +15,8 @@ struct dslash_ctx {
     int layout_base;  // LAYOUT_AOS / LAYOUT_SOA
     int recon;        // 18 or 12
     int device;
-    int var_depth, var_tpb, var_spt;
+    int var_depth, var_tpb, var_spt;  // var_depth: 0 tuned, 1..4 collapse-depth sweep variant, -1 OpenMP-style variant
+    int omp_x, omp_a, omp_b, omp_sched, omp_teams, omp_team_size;
     int tile[4];
     TileGeom tg;
     int kernel;  // DSLASH_KERNEL_*
@@ -177,6 +178,9 @@ int dslash_apply(dslash_ctx* c, void* out, const void* in, const void* gauge, ds
         if (k < 0) return DSLASH_ERR_UNSUPPORTED;
         e = (k == DSLASH_KERNEL_DIRECT) ? launch_tuned(c->precision, c->layout_base, c->recon, a, c->tg, c->cfg)
                                         : launch_tma(c->precision, c->recon, a, c->tg, k == DSLASH_KERNEL_TMA_LINKS);
+    } else if (c->var_depth < 0) {
+        e = launch_omp_variant(c->precision, c->layout_base, c->recon, a, c->omp_a, c->omp_x, c->omp_b, c->omp_sched, c->omp_teams,
+                               c->omp_team_size);
     } else
         e = launch_variant(c->precision, c->layout_base, c->recon, a, c->var_depth, c->var_tpb, c->var_spt);
     if (e != cudaSuccess) return cuda_fail(c, e);
@@ -254,6 +258,62 @@ int dslash_variant_at(int index, int* depth, int* tpb, int* spt, int* layout) {
     *depth = 1 + index % 4;
     index /= 4;
     *layout = index == 0 ? DSLASH_AOS : DSLASH_SOA;
+    return DSLASH_OK;
+}
+
+// loop structures for num_loops loops: x = 0: b = 1..N;  x >= 1: a = 1..x, b = 1..N-x
+static bool omp_structure_valid(int N, int x, int a, int b) {
+    if (N < 1 || N > 4 || x < 0 || x >= N || b < 1 || b > N - x) return false;
+    return x == 0 ? a == 0 : (a >= 1 && a <= x);
+}
+
+int dslash_omp_variant_count(int num_loops) {
+    if (num_loops < 1 || num_loops > 4) return 0;
+    int structures = 0;
+    for (int x = 0; x < num_loops; ++x) structures += (x == 0) ? num_loops : x * (num_loops - x);
+    return structures * 3 * 2;  // x schedules x data-transfer modes
+}
+
+int dslash_omp_variant_at(int num_loops, int index, int* px, int* pa, int* pb, int* psched, int* pmap) {
+    if (!px || !pa || !pb || !psched || !pmap) return DSLASH_ERR_NULL;
+    if (index < 0 || index >= dslash_omp_variant_count(num_loops)) return DSLASH_ERR_UNSUPPORTED;
+    const int map_mode = index % 2, sched = (index / 2) % 3;
+    int st = index / 6;
+    for (int x = 0; x < num_loops; ++x) {
+        const int a_lo = x == 0 ? 0 : 1, a_hi = x == 0 ? 0 : x;
+        for (int a = a_lo; a <= a_hi; ++a)
+            for (int b = 1; b <= num_loops - x; ++b) {
+                if (st == 0) {
+                    *px = x;
+                    *pa = a;
+                    *pb = b;
+                    *psched = sched;
+                    *pmap = map_mode == 0 ? DSLASH_MAP_TOFROM : DSLASH_MAP_MINIMAL;
+                    return DSLASH_OK;
+                }
+                --st;
+            }
+    }
+    return DSLASH_ERR_UNSUPPORTED;
+}
+
+int dslash_set_omp_variant(dslash_ctx* c, int x, int a, int b, int sched, int num_teams, int team_size) {
+    if (!c) return DSLASH_ERR_NULL;
+    if (!omp_structure_valid(4, x, a, b)) return DSLASH_ERR_UNSUPPORTED;
+    if (sched != DSLASH_SCHED_STATIC && sched != DSLASH_SCHED_DYNAMIC && sched != DSLASH_SCHED_GUIDED) return DSLASH_ERR_UNSUPPORTED;
+    if (team_size < 32 || team_size > 256 || team_size % 32 || num_teams < 0) return DSLASH_ERR_UNSUPPORTED;
+    if (num_teams == 0) {
+        int sms = 148;
+        if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess) (void)cudaGetLastError();
+        num_teams = 4 * sms;
+    }
+    c->var_depth = -1;
+    c->omp_x = x;
+    c->omp_a = a;
+    c->omp_b = b;
+    c->omp_sched = sched;
+    c->omp_teams = num_teams;
+    c->omp_team_size = team_size;
     return DSLASH_OK;
 }
 

@@ -25,6 +25,11 @@ struct LaunchArgs {
 // loops of (t,z,y,x); every parallel iteration runs the remaining loops serially.
 cudaError_t launch_variant(int precision, int layout_base, int recon, const LaunchArgs& a, int depth, int tpb, int spt);
 
+// The paper's exact variant space: distribute collapse da (0 if x == 0), parallel-for position x,
+// parallel-for collapse b, schedule 0/1/2 = static/dynamic/guided, league and team size.
+cudaError_t launch_omp_variant(int precision, int layout_base, int recon, const LaunchArgs& a, int da, int x, int b, int sched,
+                               int teams, int team_size);
+
 // Options of the tuned kernels (dslash_set_option).
 struct TunedConfig {
     int occupancy;         // 0: default register budget, 1: 128-register variant

@@ -90,6 +90,33 @@ def test_variant_enumeration_is_the_120_of_config_5(B):
         assert e.value.status == B.DSLASH_ERR_UNSUPPORTED
 
 
+def test_omp_variant_space_reproduces_table_1(B):
+    """PAPER.md:166-173 (Table 1): 6, 18, 42, 84 variants for 1..4 nested loops (tests/golden/table1_variant_counts.txt)."""
+    golden = {}
+    for line in open(os.path.join(ROOT, "tests", "golden", "table1_variant_counts.txt")):
+        if line.strip() and not line.startswith("#"):
+            n, v = line.split()
+            golden[int(n)] = int(v)
+    assert golden == {1: 6, 2: 18, 3: 42, 4: 84}
+    for n, want in golden.items():
+        assert B.dslash_omp_variant_count(n) == want
+        seen = set()
+        for i in range(want):
+            x, a, b, sched, mode = B.dslash_omp_variant_at(n, i)
+            assert 0 <= x < n and 1 <= b <= n - x  # PAPER.md:162: max collapse of parallel for is NUM - x
+            assert (a == 0) if x == 0 else (1 <= a <= x)  # PAPER.md:162: max collapse of teams distribute is x
+            assert sched in (B.DSLASH_SCHED_STATIC, B.DSLASH_SCHED_DYNAMIC, B.DSLASH_SCHED_GUIDED)
+            assert mode in (B.DSLASH_MAP_MINIMAL, B.DSLASH_MAP_TOFROM)
+            seen.add((x, a, b, sched, mode))
+        assert len(seen) == want
+        for bad in (-1, want):
+            with pytest.raises(B.DslashError):
+                B.dslash_omp_variant_at(n, bad)
+    assert B.dslash_omp_variant_count(0) == 0 and B.dslash_omp_variant_count(5) == 0
+    # loop structures alone: 1, 3, 7, 14
+    assert [B.dslash_omp_variant_count(n) // 6 for n in (1, 2, 3, 4)] == [1, 3, 7, 14]
+
+
 def test_no_cuda_device_is_an_error_not_a_fallback(B):
     import torch
     if torch.cuda.is_available():

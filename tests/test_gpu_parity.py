@@ -181,6 +181,35 @@ def test_config5_all_120_variants_24x24x24x24(env):
             lat.close()
 
 
+# ---------------------------------------------------------------- the paper's own 84-variant space (42 kernels x 2 map modes)
+@pytest.mark.parametrize("dims", [(4, 6, 8, 10), (3, 5, 2, 7)])
+def test_all_omp_style_variants_match_the_oracle(env, dims):
+    B = env.B
+    g, p, ref, _ = fields_and_ref(env, dims, SEED + 15, "f64")
+    structures = set()
+    for i in range(B.dslash_omp_variant_count(4)):
+        x, a, b, sched, _mode = B.dslash_omp_variant_at(4, i)
+        structures.add((x, a, b, sched))
+    assert len(structures) == 42
+    for layout in ("soa", "aos"):
+        with env.device.Lattice(dims, "f64", layout, False) as lat:
+            gi, pi, o = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
+            for (x, a, b, sched) in sorted(structures):
+                for teams, team_size in ((0, 128), (3, 32), (7, 256)):
+                    B.dslash_set_omp_variant(lat.ctx, x, a, b, sched, teams, team_size)
+                    o.zero_()
+                    lat.apply(o, pi, gi)
+                    e = env.checks.parity_error(lat.download_spinor(o), ref)
+                    assert e <= TOL["f64"], (layout, x, a, b, sched, teams, team_size, e)
+            for bad in [(0, 1, 1, 0), (1, 0, 1, 0), (1, 2, 1, 0), (2, 1, 3, 0), (4, 1, 1, 0), (0, 0, 5, 0), (0, 0, 1, 3)]:
+                with pytest.raises(B.DslashError):
+                    B.dslash_set_omp_variant(lat.ctx, *bad)
+            with pytest.raises(B.DslashError):
+                B.dslash_set_omp_variant(lat.ctx, 0, 0, 4, 0, 0, 48)
+            lat.set_variant(B.DSLASH_VARIANT_TUNED)
+            assert env.checks.parity_error(lat.dslash(g, p), ref) <= TOL["f64"]
+
+
 # ---------------------------------------------------------------- config 3: 32^3 x 64 FP64, 18- and 12-real links
 @pytest.mark.parametrize("recon12", [False, True])
 def test_config3_32x32x32x64_fp64(env, recon12):
