@@ -87,6 +87,12 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
 /* variant selection: collapse_depth DSLASH_VARIANT_TUNED selects the library's tuned kernel */
 #define DSLASH_VARIANT_TUNED 0
 
+/* operators of dslash_apply_op() */
+#define DSLASH_OP_D 0        /* Eq. 1 */
+#define DSLASH_OP_D_DAGGER 1 /* its adjoint: Eq. 1 with gamma_mu -> -gamma_mu (= gamma_5 D gamma_5) */
+#define DSLASH_OP_M 2        /* Wilson matrix M = (4 + mass) - D/2 */
+#define DSLASH_OP_M_DAGGER 3 /* M^dagger = (4 + mass) - D^dagger/2 */
+
 /* schedules of the paper's offload variants, dslash_set_omp_variant() */
 #define DSLASH_SCHED_STATIC 0
 #define DSLASH_SCHED_DYNAMIC 1
@@ -212,6 +218,25 @@ DSLASH_API int dslash_get_tile(const dslash_ctx *ctx, int tile[4]);
  */
 DSLASH_API int dslash_set_kernel(dslash_ctx *ctx, int kernel);
 DSLASH_API int dslash_get_kernel(const dslash_ctx *ctx, int *kernel);
+
+/*
+ * The operators a caller of Dslash needs next (the paper: D is the "unpreconditioned Dirac operator", and
+ * "is called several times throughout the LQCD application").
+ * dslash_apply_op: out = OP in with OP one of DSLASH_OP_* (mass is used by _M and _M_DAGGER only); same buffers, layouts,
+ *   alignment and aliasing rules as dslash_apply; one kernel launch on `stream`; uses the ctx's tile (<= 128 sites; a
+ *   larger tile returns DSLASH_ERR_UNSUPPORTED), ignores the variant/kernel selection.
+ * dslash_cg_solve: conjugate gradient on the normal equations M^dagger M x = b, started from x = 0, stopped when
+ *   |r| / |b| <= tol or after max_iter iterations.  x, b: device spinors in the native layout (x is overwritten, b is
+ *   not modified); the ctx owns four work spinors (allocated on first use).  Reductions are two-pass fp64 sums
+ *   (deterministic).  The call synchronises `stream` (it reads the residual every iteration).  iterations / rel_residual
+ *   (optional, may be NULL) receive the iteration count and the final |r|/|b| of the recurrence.
+ *   Returns DSLASH_OK also when max_iter was reached without convergence (check rel_residual).
+ * Errors: NULL, ALIGN, ALIAS, UNSUPPORTED (op, tile, tol <= 0, max_iter < 1), NOMEM, CUDA.
+ */
+DSLASH_API int dslash_apply_op(dslash_ctx *ctx, int op, double mass, void *out, const void *in, const void *gauge,
+                               dslash_stream_t stream);
+DSLASH_API int dslash_cg_solve(dslash_ctx *ctx, void *x, const void *b, const void *gauge, double mass, double tol, int max_iter,
+                               int *iterations, double *rel_residual, dslash_stream_t stream);
 
 /*
  * Performance options of the tuned kernels (DSLASH_OPT_*); they never change results beyond rounding order.

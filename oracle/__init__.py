@@ -31,6 +31,8 @@ def _lib():
         lib.oracle_gamma.restype = None
         lib.oracle_dslash.argtypes = [dbl_p, dbl_p, dbl_p, int_p, ctypes.c_int]
         lib.oracle_dslash.restype = ctypes.c_int
+        lib.oracle_dslash_dagger.argtypes = [dbl_p, dbl_p, dbl_p, int_p, ctypes.c_int]
+        lib.oracle_dslash_dagger.restype = ctypes.c_int
         lib.oracle_dslash_sites.argtypes = [dbl_p, dbl_p, dbl_p, int_p, ctypes.POINTER(ctypes.c_int64),
                                             ctypes.c_int64, ctypes.c_int]
         lib.oracle_dslash_sites.restype = ctypes.c_int
@@ -72,6 +74,22 @@ def dslash(psi: np.ndarray, gauge: np.ndarray, dims, nthreads: int = 0) -> np.nd
     if rc != 0:
         raise RuntimeError("oracle_dslash failed: %d" % rc)
     return out
+
+
+def dslash_dagger(psi: np.ndarray, gauge: np.ndarray, dims, nthreads: int = 0) -> np.ndarray:
+    """out = D^dagger[gauge] psi: Eq. 1 with gamma_mu -> -gamma_mu (DESIGN.md Reading R19)."""
+    psi, gauge, cdims, (lx, ly, lz, lt), _ = _check(psi, gauge, dims)
+    out = np.empty((lt, lz, ly, lx, 4, 3, 2), dtype=np.float64)
+    rc = _lib().oracle_dslash_dagger(_dp(out), _dp(psi), _dp(gauge), cdims, int(nthreads))
+    if rc != 0:
+        raise RuntimeError("oracle_dslash_dagger failed: %d" % rc)
+    return out
+
+
+def wilson(psi: np.ndarray, gauge: np.ndarray, dims, mass: float, dagger: bool = False, nthreads: int = 0) -> np.ndarray:
+    """M psi = (4 + mass) psi - D psi / 2 (dagger: with D^dagger): the Wilson matrix whose hopping term is Eq. 1."""
+    d = (dslash_dagger if dagger else dslash)(psi, gauge, dims, nthreads)
+    return (4.0 + float(mass)) * np.ascontiguousarray(psi, dtype=np.float64).reshape(d.shape) - 0.5 * d
 
 
 def dslash_sites(psi: np.ndarray, gauge: np.ndarray, dims, sites, nthreads: int = 0) -> np.ndarray:

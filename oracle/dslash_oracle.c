@@ -115,9 +115,13 @@ static cplx link_at(const double *gauge, size_t s, int mu, int i, int j) {
     return p[0] + p[1] * I;
 }
 
-/* out24 <- (D psi)(x) for the one site with coordinates coord = {x,y,z,t}.  Eq. 1 term by term. */
+/* out24 <- (D psi)(x) (sigma = +1) or (D^dagger psi)(x) (sigma = -1) for the one site with coordinates
+ * coord = {x,y,z,t}.  Eq. 1 term by term.  The adjoint of Eq. 1 follows from gamma_mu^dagger = gamma_mu and
+ * (U_mu(x) delta_{x+mu,y})^dagger = U_mu(x)^dagger delta_{x,y+mu}: relabelling, D^dagger is Eq. 1 with
+ * gamma_mu -> -gamma_mu, i.e. the projectors (1 - sigma*gamma_mu) forward and (1 + sigma*gamma_mu) backward
+ * (DESIGN.md Reading R19; pinned by <phi, D psi> = <D^dagger phi, psi> and by gamma_5 D gamma_5 = D^dagger). */
 static void dslash_one_site(double *out24, const double *psi, const double *gauge, const int dims[4],
-                            const int coord[4]) {
+                            const int coord[4], double sigma) {
     cplx acc[NS][NC];
     for (int a = 0; a < NS; ++a)
         for (int i = 0; i < NC; ++i) acc[a][i] = 0.0;
@@ -132,19 +136,19 @@ static void dslash_one_site(double *out24, const double *psi, const double *gaug
         const size_t sf = site_index(dims, fwd);
         const size_t sb = site_index(dims, bwd);
 
-        /* forward:  (1 - gamma_mu)[a][b] U_mu(x)[i][j] psi(x+mu^)[b][j] */
+        /* forward:  (1 - sigma*gamma_mu)[a][b] U_mu(x)[i][j] psi(x+mu^)[b][j] */
         for (int a = 0; a < NS; ++a)
             for (int i = 0; i < NC; ++i)
                 for (int b = 0; b < NS; ++b) {
-                    const cplx pm = (a == b ? 1.0 : 0.0) - gamma_entry(mu, a, b);
+                    const cplx pm = (a == b ? 1.0 : 0.0) - sigma * gamma_entry(mu, a, b);
                     for (int j = 0; j < NC; ++j) acc[a][i] += pm * link_at(gauge, s, mu, i, j) * spinor_at(psi, sf, b, j);
                 }
 
-        /* backward: (1 + gamma_mu)[a][b] conj(U_mu(x-mu^)[j][i]) psi(x-mu^)[b][j] */
+        /* backward: (1 + sigma*gamma_mu)[a][b] conj(U_mu(x-mu^)[j][i]) psi(x-mu^)[b][j] */
         for (int a = 0; a < NS; ++a)
             for (int i = 0; i < NC; ++i)
                 for (int b = 0; b < NS; ++b) {
-                    const cplx pp = (a == b ? 1.0 : 0.0) + gamma_entry(mu, a, b);
+                    const cplx pp = (a == b ? 1.0 : 0.0) + sigma * gamma_entry(mu, a, b);
                     for (int j = 0; j < NC; ++j)
                         acc[a][i] += pp * conj(link_at(gauge, sb, mu, j, i)) * spinor_at(psi, sb, b, j);
                 }
@@ -159,7 +163,7 @@ static void dslash_one_site(double *out24, const double *psi, const double *gaug
 
 /* out <- D[gauge] psi on the whole lattice.  dims = {L_X, L_Y, L_Z, L_T}, each >= 1.
  * Four explicit loops t,z,y,x as in Code 1.  nthreads <= 0: all cores. */
-int oracle_dslash(double *out, const double *psi, const double *gauge, const int dims[4], int nthreads) {
+static int dslash_all(double *out, const double *psi, const double *gauge, const int dims[4], int nthreads, double sigma) {
     if (!out || !psi || !gauge || !dims) return -1;
     for (int d = 0; d < 4; ++d)
         if (dims[d] < 1) return -2;
@@ -176,9 +180,18 @@ int oracle_dslash(double *out, const double *psi, const double *gauge, const int
                 for (int x = 0; x < dims[0]; ++x) {
                     const int coord[4] = {x, y, z, t};
                     const size_t s = site_index(dims, coord);
-                    dslash_one_site(out + s * (NS * NC * 2), psi, gauge, dims, coord);
+                    dslash_one_site(out + s * (NS * NC * 2), psi, gauge, dims, coord, sigma);
                 }
     return 0;
+}
+
+int oracle_dslash(double *out, const double *psi, const double *gauge, const int dims[4], int nthreads) {
+    return dslash_all(out, psi, gauge, dims, nthreads, 1.0);
+}
+
+/* out <- D^dagger[gauge] psi on the whole lattice (see dslash_one_site). */
+int oracle_dslash_dagger(double *out, const double *psi, const double *gauge, const int dims[4], int nthreads) {
+    return dslash_all(out, psi, gauge, dims, nthreads, -1.0);
 }
 
 /* out[n][24] <- (D psi)(sites[k]) for a list of linear site indices: the "one by one" form used
@@ -205,7 +218,7 @@ int oracle_dslash_sites(double *out, const double *psi, const double *gauge, con
         coord[1] = (int)(r % dims[1]); r /= dims[1];
         coord[2] = (int)(r % dims[2]); r /= dims[2];
         coord[3] = (int)r;
-        dslash_one_site(out + k * (NS * NC * 2), psi, gauge, dims, coord);
+        dslash_one_site(out + k * (NS * NC * 2), psi, gauge, dims, coord, 1.0);
     }
     return 0;
 }

@@ -23,6 +23,7 @@ DSLASH_MAP_MINIMAL, DSLASH_MAP_TOFROM = 0, 1
 DSLASH_KERNEL_AUTO, DSLASH_KERNEL_DIRECT, DSLASH_KERNEL_TMA, DSLASH_KERNEL_TMA_LINKS = 0, 1, 2, 3
 DSLASH_OPT_OCCUPANCY, DSLASH_OPT_L2_POLICY = 2, 3
 DSLASH_SCHED_STATIC, DSLASH_SCHED_DYNAMIC, DSLASH_SCHED_GUIDED = 0, 1, 2
+DSLASH_OP_D, DSLASH_OP_D_DAGGER, DSLASH_OP_M, DSLASH_OP_M_DAGGER = 0, 1, 2, 3
 
 _c_int_p = ctypes.POINTER(ctypes.c_int)
 _c_size_p = ctypes.POINTER(ctypes.c_size_t)
@@ -33,6 +34,9 @@ SIGNATURES = {
     "dslash_create": (ctypes.c_int, [ctypes.POINTER(_vp), _c_int_p, ctypes.c_int, ctypes.c_int]),
     "dslash_destroy": (ctypes.c_int, [_vp]),
     "dslash_apply": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp]),
+    "dslash_apply_op": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_double, _vp, _vp, _vp, _vp]),
+    "dslash_cg_solve": (ctypes.c_int, [_vp, _vp, _vp, _vp, ctypes.c_double, ctypes.c_double, ctypes.c_int, _c_int_p,
+                                        ctypes.POINTER(ctypes.c_double), _vp]),
     "dslash_spinor_bytes": (ctypes.c_size_t, [_vp]),
     "dslash_gauge_bytes": (ctypes.c_size_t, [_vp]),
     "dslash_canonical_spinor_bytes": (ctypes.c_size_t, [_vp]),
@@ -126,6 +130,19 @@ def dslash_apply(ctx, out, inp, gauge, stream=0) -> None:
 def dslash_apply_status(ctx, out, inp, gauge, stream=0) -> int:
     """dslash_apply returning the raw status instead of raising (error-path tests)."""
     return int(_lib.dslash_apply(_ptr(ctx), _ptr(out), _ptr(inp), _ptr(gauge), _ptr(stream)))
+
+
+def dslash_apply_op(ctx, op: int, mass: float, out, inp, gauge, stream=0) -> None:
+    _check(_lib.dslash_apply_op(_ptr(ctx), int(op), float(mass), _ptr(out), _ptr(inp), _ptr(gauge), _ptr(stream)),
+           "dslash_apply_op")
+
+
+def dslash_cg_solve(ctx, x, b, gauge, mass: float, tol: float, max_iter: int, stream=0):
+    """Returns (iterations, rel_residual)."""
+    it, rel = ctypes.c_int(), ctypes.c_double()
+    _check(_lib.dslash_cg_solve(_ptr(ctx), _ptr(x), _ptr(b), _ptr(gauge), float(mass), float(tol), int(max_iter),
+                                ctypes.byref(it), ctypes.byref(rel), _ptr(stream)), "dslash_cg_solve")
+    return it.value, rel.value
 
 
 def dslash_spinor_bytes(ctx) -> int:

@@ -1,5 +1,6 @@
 // dslash_api.cu -- the C ABI of libdslash_b200.so (see include/dslash_b200.h for the contract).
 #include <cuda_runtime.h>
+#include <math.h>
 #include <stdint.h>
 
 #include <new>
@@ -26,6 +27,9 @@ struct dslash_ctx {
     // staging buffers of dslash_apply_host (device memory, owned)
     void* d_can[3];  // canonical gauge, in, out
     void* d_nat[3];  // native gauge, in, out (alias d_can when the native layout is the canonical one)
+    // workspace of dslash_cg_solve (device memory, owned): r, p, t, q spinors; reduction scratch; one result
+    void* cg_vec[4];
+    double* cg_scratch;
 };
 
 static int cuda_fail(dslash_ctx* c, cudaError_t e) {
@@ -120,6 +124,8 @@ int dslash_create(dslash_ctx** ctx, const int dims[4], int precision, int layout
     c->launches = 0;
     c->last_cuda = 0;
     for (int i = 0; i < 3; ++i) c->d_can[i] = c->d_nat[i] = nullptr;
+    for (int i = 0; i < 4; ++i) c->cg_vec[i] = nullptr;
+    c->cg_scratch = nullptr;
     *ctx = c;
     return DSLASH_OK;
 }
@@ -127,10 +133,14 @@ int dslash_create(dslash_ctx** ctx, const int dims[4], int precision, int layout
 int dslash_destroy(dslash_ctx* c) {
     if (!c) return DSLASH_OK;
     int rc = DSLASH_OK;
-    bool any = false;
+    bool any = c->cg_scratch != nullptr;
     for (int i = 0; i < 3; ++i) any = any || c->d_can[i] || c->d_nat[i];
+    for (int i = 0; i < 4; ++i) any = any || c->cg_vec[i];
     if (any) {
         if (cudaDeviceSynchronize() != cudaSuccess) rc = DSLASH_ERR_CUDA;
+        for (int i = 0; i < 4; ++i)
+            if (c->cg_vec[i]) cudaFree(c->cg_vec[i]);
+        if (c->cg_scratch) cudaFree(c->cg_scratch);
         for (int i = 0; i < 3; ++i) {
             if (c->d_nat[i] && c->d_nat[i] != c->d_can[i]) cudaFree(c->d_nat[i]);
             if (c->d_can[i]) cudaFree(c->d_can[i]);
@@ -185,6 +195,106 @@ int dslash_apply(dslash_ctx* c, void* out, const void* in, const void* gauge, ds
         e = launch_variant(c->precision, c->layout_base, c->recon, a, c->var_depth, c->var_tpb, c->var_spt);
     if (e != cudaSuccess) return cuda_fail(c, e);
     c->launches += 1;
+    return DSLASH_OK;
+}
+
+int dslash_apply_op(dslash_ctx* c, int op, double mass, void* out, const void* in, const void* gauge, dslash_stream_t stream) {
+    if (!c || !out || !in || !gauge) return DSLASH_ERR_NULL;
+    if (op < DSLASH_OP_D || op > DSLASH_OP_M_DAGGER) return DSLASH_ERR_UNSUPPORTED;
+    if (misaligned(out) || misaligned(in) || misaligned(gauge)) return DSLASH_ERR_ALIGN;
+    const size_t sb = dslash_spinor_bytes(c);
+    if (overlap(out, sb, in, sb)) return DSLASH_ERR_ALIAS;
+    if (c->tile[0] * c->tile[1] * c->tile[2] * c->tile[3] > 128) return DSLASH_ERR_UNSUPPORTED;
+    LaunchArgs a{out, in, gauge, c->geom, static_cast<cudaStream_t>(stream)};
+    cudaError_t e = launch_op(c->precision, c->layout_base, c->recon, a, c->tg, op, mass);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    c->launches += 1;
+    return DSLASH_OK;
+}
+
+int dslash_cg_solve(dslash_ctx* c, void* x, const void* b, const void* gauge, double mass, double tol, int max_iter, int* iterations,
+                    double* rel_residual, dslash_stream_t stream_) {
+    if (!c || !x || !b || !gauge) return DSLASH_ERR_NULL;
+    if (!(tol > 0.0) || max_iter < 1) return DSLASH_ERR_UNSUPPORTED;
+    if (misaligned(x) || misaligned(b) || misaligned(gauge)) return DSLASH_ERR_ALIGN;
+    const size_t sb = dslash_spinor_bytes(c);
+    if (overlap(x, sb, b, sb)) return DSLASH_ERR_ALIAS;
+    if (c->tile[0] * c->tile[1] * c->tile[2] * c->tile[3] > 128) return DSLASH_ERR_UNSUPPORTED;
+    cudaStream_t st = static_cast<cudaStream_t>(stream_);
+    cudaError_t e;
+    for (int i = 0; i < 4; ++i)
+        if (!c->cg_vec[i]) {
+            e = cudaMalloc(&c->cg_vec[i], sb);
+            if (e != cudaSuccess) {
+                c->cg_vec[i] = nullptr;
+                c->last_cuda = (int)e;
+                (void)cudaGetLastError();
+                return DSLASH_ERR_NOMEM;
+            }
+            if ((e = cudaMemsetAsync(c->cg_vec[i], 0, sb, st)) != cudaSuccess) return cuda_fail(c, e);
+        }
+    if (!c->cg_scratch) {
+        e = cudaMalloc(reinterpret_cast<void**>(&c->cg_scratch), sizeof(double) * (size_t)(reduction_scratch_doubles() + 1));
+        if (e != cudaSuccess) {
+            c->cg_scratch = nullptr;
+            c->last_cuda = (int)e;
+            (void)cudaGetLastError();
+            return DSLASH_ERR_NOMEM;
+        }
+    }
+    void *r = c->cg_vec[0], *p = c->cg_vec[1], *t = c->cg_vec[2], *q = c->cg_vec[3];
+    double* d_res = c->cg_scratch + reduction_scratch_doubles();
+    const int prec = c->precision, lay = c->layout_base;
+    const unsigned V = c->geom.V;
+    // <u, v> on the device, value read back (synchronises the stream)
+    auto dot = [&](const void* u, const void* v, double* host) -> cudaError_t {
+        cudaError_t er = launch_dot(prec, lay, V, d_res, c->cg_scratch, u, v, st);
+        if (er != cudaSuccess) return er;
+        c->launches += 2;
+        er = cudaMemcpyAsync(host, d_res, sizeof(double), cudaMemcpyDeviceToHost, st);
+        if (er != cudaSuccess) return er;
+        return cudaStreamSynchronize(st);
+    };
+    auto op = [&](int which, void* o, const void* i) -> cudaError_t {
+        LaunchArgs a{o, i, gauge, c->geom, st};
+        c->launches += 1;
+        return launch_op(prec, lay, c->recon, a, c->tg, which, mass);
+    };
+    auto axpby = [&](void* y, const void* xx, double aa, double bb) -> cudaError_t {
+        c->launches += 1;
+        return launch_axpby(prec, lay, V, y, xx, aa, bb, st);
+    };
+#define CG_TRY(call)                                  \
+    do {                                              \
+        if ((e = (call)) != cudaSuccess) return cuda_fail(c, e); \
+    } while (0)
+    CG_TRY(cudaMemsetAsync(x, 0, sb, st));
+    CG_TRY(cudaMemcpyAsync(r, b, sb, cudaMemcpyDeviceToDevice, st));
+    CG_TRY(cudaMemcpyAsync(p, b, sb, cudaMemcpyDeviceToDevice, st));
+    double rr = 0.0, bb = 0.0, pAp = 0.0, rr_new = 0.0;
+    CG_TRY(dot(r, r, &rr));
+    bb = rr;
+    int it = 0;
+    double rel = bb > 0.0 ? 1.0 : 0.0;
+    if (bb > 0.0) {
+        for (it = 1; it <= max_iter; ++it) {
+            CG_TRY(op(DSLASH_OP_M, t, p));
+            CG_TRY(dot(t, t, &pAp));
+            CG_TRY(op(DSLASH_OP_M_DAGGER, q, t));
+            const double alpha = rr / pAp;
+            CG_TRY(axpby(x, p, alpha, 1.0));
+            CG_TRY(axpby(r, q, -alpha, 1.0));
+            CG_TRY(dot(r, r, &rr_new));
+            rel = sqrt(rr_new / bb);
+            if (rel <= tol) break;
+            CG_TRY(axpby(p, r, 1.0, rr_new / rr));
+            rr = rr_new;
+        }
+        if (it > max_iter) it = max_iter;
+    }
+#undef CG_TRY
+    if (iterations) *iterations = it;
+    if (rel_residual) *rel_residual = rel;
     return DSLASH_OK;
 }
 

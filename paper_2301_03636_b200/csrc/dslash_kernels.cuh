@@ -44,6 +44,13 @@ cudaError_t launch_tuned(int precision, int layout_base, int recon, const Launch
 bool tma_eligible(int precision, int recon, const Geom& g, const TileGeom& tg);
 cudaError_t launch_tma(int precision, int recon, const LaunchArgs& a, const TileGeom& tg, bool links_only);
 
+// Operators around Dslash (dslash_ops.cu): op 0 D, 1 D^dagger, 2 M = (4+m) - D/2, 3 M^dagger; solver vector kernels.
+cudaError_t launch_op(int precision, int layout_base, int recon, const LaunchArgs& a, const TileGeom& tg, int op, double mass);
+cudaError_t launch_axpby(int precision, int layout_base, unsigned V, void* y, const void* x, double a, double b, cudaStream_t st);
+cudaError_t launch_dot(int precision, int layout_base, unsigned V, double* result, double* scratch, const void* x, const void* y,
+                       cudaStream_t st);
+int reduction_scratch_doubles();
+
 // Layout module.  dir 0: canonical -> native (pack), 1: native -> canonical (unpack).
 cudaError_t launch_convert_spinor(int precision, int layout_base, void* dst, const void* src, unsigned V, int dir,
                                   cudaStream_t stream);

@@ -1,0 +1,253 @@
+// dslash_ops.cu -- the operators around Dslash that its callers use:
+//   D^dagger, the Wilson matrix M = (4 + m) - D/2 and M^dagger, and a conjugate-gradient solve of M^dagger M x = b.
+//
+// PAPER.md:52 calls Eq. 1 the "unpreconditioned Dirac operator" and PAPER.md:54 notes that it "is called several times
+// throughout the LQCD application": the caller is a Krylov solver for the Wilson matrix, which is what is provided
+// here.  D^dagger follows from Eq. 1 by taking the adjoint: gamma_mu is hermitian, so
+//   (D^dagger psi)(x) = sum_mu [ (1 + gamma_mu) U_mu(x) psi(x+mu^) + (1 - gamma_mu) U_mu(x-mu^)^dagger psi(x-mu^) ],
+// i.e. Eq. 1 with gamma_mu -> -gamma_mu (also = gamma_5 D gamma_5, oracle pin P5).
+//
+// One kernel serves all four operators: the projector sign is a run-time +-1 that enters the projection and the
+// reconstruction as the multiplier of an FMA (a + s*b costs the same as a + b and is bit-identical for s = +-1), and
+// the epilogue out = a*in(x) + b*acc is a uniform branch.
+#include "dslash_kernels.cuh"
+
+namespace dslash {
+
+// h = P psi for the projector (1 + s*gamma_MU), s = +-1
+template <int MU, typename Real>
+__device__ __forceinline__ void project_rt(cplx<Real> (&h)[6], const cplx<Real> (&psi)[12], Real s) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const cplx<Real> p0 = psi[c], p1 = psi[3 + c], p2 = psi[6 + c], p3 = psi[9 + c];
+        if (MU == 0) {          // h0 = p0 + s i p3, h1 = p1 + s i p2
+            h[c] = {fma_(-s, p3.im, p0.re), fma_(s, p3.re, p0.im)};
+            h[3 + c] = {fma_(-s, p2.im, p1.re), fma_(s, p2.re, p1.im)};
+        } else if (MU == 1) {   // h0 = p0 - s p3, h1 = p1 + s p2
+            h[c] = {fma_(-s, p3.re, p0.re), fma_(-s, p3.im, p0.im)};
+            h[3 + c] = {fma_(s, p2.re, p1.re), fma_(s, p2.im, p1.im)};
+        } else if (MU == 2) {   // h0 = p0 + s i p2, h1 = p1 - s i p3
+            h[c] = {fma_(-s, p2.im, p0.re), fma_(s, p2.re, p0.im)};
+            h[3 + c] = {fma_(s, p3.im, p1.re), fma_(-s, p3.re, p1.im)};
+        } else {                // h0 = p0 + s p2, h1 = p1 + s p3
+            h[c] = {fma_(s, p2.re, p0.re), fma_(s, p2.im, p0.im)};
+            h[3 + c] = {fma_(s, p3.re, p1.re), fma_(s, p3.im, p1.im)};
+        }
+    }
+}
+
+// acc += R(h): rows 0,1 += h0,h1; rows 2,3 from the projector (1 + s*gamma_MU):
+//   MU 0: r2 = -s i h1, r3 = -s i h0    MU 1: r2 = s h1, r3 = -s h0    MU 2: r2 = -s i h0, r3 = s i h1    MU 3: r2 = s h0, r3 = s h1
+template <int MU, typename Real>
+__device__ __forceinline__ void reconstruct_accumulate_rt(cplx<Real> (&acc)[12], const cplx<Real> (&h)[6], Real s) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const cplx<Real> h0 = h[c], h1 = h[3 + c];
+        cplx<Real> a2 = acc[6 + c], a3 = acc[9 + c];
+        if (MU == 0) {
+            a2 = {fma_(s, h1.im, a2.re), fma_(-s, h1.re, a2.im)};
+            a3 = {fma_(s, h0.im, a3.re), fma_(-s, h0.re, a3.im)};
+        } else if (MU == 1) {
+            a2 = {fma_(s, h1.re, a2.re), fma_(s, h1.im, a2.im)};
+            a3 = {fma_(-s, h0.re, a3.re), fma_(-s, h0.im, a3.im)};
+        } else if (MU == 2) {
+            a2 = {fma_(s, h0.im, a2.re), fma_(-s, h0.re, a2.im)};
+            a3 = {fma_(-s, h1.im, a3.re), fma_(s, h1.re, a3.im)};
+        } else {
+            a2 = {fma_(s, h0.re, a2.re), fma_(s, h0.im, a2.im)};
+            a3 = {fma_(s, h1.re, a3.re), fma_(s, h1.im, a3.im)};
+        }
+        acc[6 + c] = a2;
+        acc[9 + c] = a3;
+        acc[c] = c_add(acc[c], h0);
+        acc[3 + c] = c_add(acc[3 + c], h1);
+    }
+}
+
+template <int MU, bool UDAG, typename Real, int LAYOUT, int RECON>
+__device__ __forceinline__ void hop_rt(cplx<Real> (&acc)[12], const void* in, const void* gauge, unsigned V, unsigned sn, unsigned sl,
+                                       Real s) {
+    cplx<Real> psi[12], h[6], hp[6], u[9];
+    SpinorIO<Real, LAYOUT>::load(psi, in, V, sn);
+    load_link<Real, LAYOUT, RECON>(u, gauge, V, sl, MU);
+    project_rt<MU>(h, psi, s);
+    su3_mul<UDAG>(hp, u, h);
+    reconstruct_accumulate_rt<MU>(acc, hp, s);
+}
+
+struct OpParams {
+    double sigma;  // +1: D (forward projector 1 - gamma), -1: D^dagger (forward projector 1 + gamma)
+    double a, b;   // out = a * in(x) + b * (D or D^dagger in)(x)
+    int xpay;      // 0: out = b * acc only when b != 1 is not needed either (plain D / D^dagger)
+};
+
+template <typename Real, int LAYOUT, int RECON, int MINBLK>
+__global__ void __launch_bounds__(128, MINBLK)
+    dslash_op_kernel(void* __restrict__ out, const void* __restrict__ in, const void* __restrict__ gauge, Geom g, TileGeom tg,
+                     OpParams op) {
+    unsigned b = blockIdx.x;
+    const unsigned bx = b % (unsigned)tg.nt[0];
+    b /= (unsigned)tg.nt[0];
+    const unsigned by = b % (unsigned)tg.nt[1];
+    b /= (unsigned)tg.nt[1];
+    const unsigned bz = b % (unsigned)tg.nt[2];
+    const unsigned bt = b / (unsigned)tg.nt[2];
+    unsigned r = threadIdx.x;
+    const int x = (int)((bx << tg.lb[0]) + (r & ((1u << tg.lb[0]) - 1u)));
+    r >>= tg.lb[0];
+    const int y = (int)((by << tg.lb[1]) + (r & ((1u << tg.lb[1]) - 1u)));
+    r >>= tg.lb[1];
+    const int z = (int)((bz << tg.lb[2]) + (r & ((1u << tg.lb[2]) - 1u)));
+    r >>= tg.lb[2];
+    const int t = (int)((bt << tg.lb[3]) + r);
+    if (x >= g.L[0] || y >= g.L[1] || z >= g.L[2] || t >= g.L[3]) return;
+    const unsigned V = g.V;
+    const unsigned sy = (unsigned)g.L[0], sz = sy * (unsigned)g.L[1], st = sz * (unsigned)g.L[2];
+    const unsigned s = (unsigned)x + sy * (unsigned)y + sz * (unsigned)z + st * (unsigned)t;
+    const unsigned xf = (x + 1 == g.L[0]) ? s - (unsigned)(g.L[0] - 1) : s + 1u;
+    const unsigned xb = (x == 0) ? s + (unsigned)(g.L[0] - 1) : s - 1u;
+    const unsigned yf = (y + 1 == g.L[1]) ? s - (unsigned)(g.L[1] - 1) * sy : s + sy;
+    const unsigned yb = (y == 0) ? s + (unsigned)(g.L[1] - 1) * sy : s - sy;
+    const unsigned zf = (z + 1 == g.L[2]) ? s - (unsigned)(g.L[2] - 1) * sz : s + sz;
+    const unsigned zb = (z == 0) ? s + (unsigned)(g.L[2] - 1) * sz : s - sz;
+    const unsigned tf = (t + 1 == g.L[3]) ? s - (unsigned)(g.L[3] - 1) * st : s + st;
+    const unsigned tb = (t == 0) ? s + (unsigned)(g.L[3] - 1) * st : s - st;
+
+    const Real sf = (Real)(-op.sigma), sb = (Real)op.sigma;  // forward projector 1 - sigma*gamma, backward 1 + sigma*gamma
+    cplx<Real> acc[12];
+#pragma unroll
+    for (int k = 0; k < 12; ++k) acc[k] = {Real(0), Real(0)};
+    hop_rt<0, false, Real, LAYOUT, RECON>(acc, in, gauge, V, xf, s, sf);
+    hop_rt<0, true, Real, LAYOUT, RECON>(acc, in, gauge, V, xb, xb, sb);
+    hop_rt<1, false, Real, LAYOUT, RECON>(acc, in, gauge, V, yf, s, sf);
+    hop_rt<1, true, Real, LAYOUT, RECON>(acc, in, gauge, V, yb, yb, sb);
+    hop_rt<2, false, Real, LAYOUT, RECON>(acc, in, gauge, V, zf, s, sf);
+    hop_rt<2, true, Real, LAYOUT, RECON>(acc, in, gauge, V, zb, zb, sb);
+    hop_rt<3, false, Real, LAYOUT, RECON>(acc, in, gauge, V, tf, s, sf);
+    hop_rt<3, true, Real, LAYOUT, RECON>(acc, in, gauge, V, tb, tb, sb);
+    if (op.xpay) {
+        cplx<Real> c[12];
+        SpinorIO<Real, LAYOUT>::load(c, in, V, s);
+        const Real a = (Real)op.a, bb = (Real)op.b;
+#pragma unroll
+        for (int k = 0; k < 12; ++k) acc[k] = {fma_(bb, acc[k].re, a * c[k].re), fma_(bb, acc[k].im, a * c[k].im)};
+    }
+    SpinorIO<Real, LAYOUT>::store(out, V, s, acc);
+}
+
+template <typename Real, int LAYOUT, int RECON>
+static cudaError_t launch_op_t(const LaunchArgs& a, const TileGeom& tg, const OpParams& op) {
+    const int tpb = 1 << (tg.lb[0] + tg.lb[1] + tg.lb[2] + tg.lb[3]);
+    if (tpb > 128) return cudaErrorInvalidConfiguration;
+    const unsigned grid = (unsigned)tg.nt[0] * (unsigned)tg.nt[1] * (unsigned)tg.nt[2] * (unsigned)tg.nt[3];
+    constexpr int MINBLK = sizeof(Real) == 8 ? 2 : 4;  // same register budgets as the tuned Dslash kernel
+    dslash_op_kernel<Real, LAYOUT, RECON, MINBLK><<<grid, tpb, 0, a.stream>>>(a.out, a.in, a.gauge, a.geom, tg, op);
+    return cudaGetLastError();
+}
+
+// op: 0 D, 1 D^dagger, 2 M = (4+m) - D/2, 3 M^dagger
+cudaError_t launch_op(int precision, int layout_base, int recon, const LaunchArgs& a, const TileGeom& tg, int op, double mass) {
+    OpParams p;
+    p.sigma = (op == 1 || op == 3) ? -1.0 : 1.0;
+    p.xpay = (op >= 2);
+    p.a = 4.0 + mass;
+    p.b = -0.5;
+#define DSLASH_OP(REAL)                                                                                   \
+    (layout_base == LAYOUT_AOS ? (recon == 12 ? launch_op_t<REAL, LAYOUT_AOS, 12>(a, tg, p)              \
+                                              : launch_op_t<REAL, LAYOUT_AOS, 18>(a, tg, p))             \
+                               : (recon == 12 ? launch_op_t<REAL, LAYOUT_SOA, 12>(a, tg, p)              \
+                                              : launch_op_t<REAL, LAYOUT_SOA, 18>(a, tg, p)))
+    return precision == 0 ? DSLASH_OP(double) : DSLASH_OP(float);
+#undef DSLASH_OP
+}
+
+// ------------------------------------------------------------------ vector kernels for the solver
+// Fields are treated as arrays of reals in the native layout.  With the blocked SoA layout the last vector may contain
+// padding sites; `valid(i)` masks them out of the reductions and the updates leave them untouched.
+struct FieldShape {
+    size_t n;       // reals in the buffer (including padding)
+    unsigned V;     // real sites
+    int soa;        // blocked SoA?
+    unsigned rpv;   // reals per vector = 24 * 32
+    unsigned rpu;   // reals per 16-byte unit row: fp64 2, fp32 4  (lane index = (i / rpu) % 32)
+};
+__device__ __forceinline__ bool valid(const FieldShape& f, size_t i) {
+    if (!f.soa) return true;
+    const unsigned v = (unsigned)(i / f.rpv);
+    const unsigned lane = (unsigned)((i / f.rpu) & (VL - 1u));
+    return v * VL + lane < f.V;
+}
+
+// y = a*x + b*y   (a, b real)
+template <typename Real>
+__global__ void __launch_bounds__(256) axpby_kernel(Real* __restrict__ y, const Real* __restrict__ x, double a, double b, FieldShape f) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < f.n; i += (size_t)gridDim.x * blockDim.x)
+        if (valid(f, i)) y[i] = (Real)(a * (double)x[i] + b * (double)y[i]);
+}
+
+// partial[block] = sum_i x[i]*y[i] over the block's grid-stride range, accumulated in fp64 (deterministic two-pass sum)
+template <typename Real>
+__global__ void __launch_bounds__(256) dot_partial_kernel(double* __restrict__ partial, const Real* __restrict__ x,
+                                                          const Real* __restrict__ y, FieldShape f) {
+    double s = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < f.n; i += (size_t)gridDim.x * blockDim.x)
+        if (valid(f, i)) s += (double)x[i] * (double)y[i];
+    __shared__ double sh[256];
+    sh[threadIdx.x] = s;
+    __syncthreads();
+    for (int w = 128; w > 0; w >>= 1) {
+        if ((int)threadIdx.x < w) sh[threadIdx.x] += sh[threadIdx.x + w];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partial[blockIdx.x] = sh[0];
+}
+__global__ void __launch_bounds__(256) dot_final_kernel(double* __restrict__ result, const double* __restrict__ partial, int n) {
+    __shared__ double sh[256];
+    double s = 0.0;
+    for (int i = threadIdx.x; i < n; i += 256) s += partial[i];
+    sh[threadIdx.x] = s;
+    __syncthreads();
+    for (int w = 128; w > 0; w >>= 1) {
+        if ((int)threadIdx.x < w) sh[threadIdx.x] += sh[threadIdx.x + w];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *result = sh[0];
+}
+
+static FieldShape shape_of(int precision, int layout_base, unsigned V) {
+    FieldShape f;
+    f.V = V;
+    f.soa = layout_base == LAYOUT_SOA;
+    const size_t sites = f.soa ? (size_t)((V + VL - 1u) / VL) * VL : (size_t)V;
+    f.n = sites * 24u;
+    f.rpv = 24u * VL;
+    f.rpu = precision == 0 ? 2u : 4u;
+    return f;
+}
+
+static const int kRedBlocks = 592;
+
+cudaError_t launch_axpby(int precision, int layout_base, unsigned V, void* y, const void* x, double a, double b, cudaStream_t st) {
+    const FieldShape f = shape_of(precision, layout_base, V);
+    if (precision == 0)
+        axpby_kernel<double><<<kRedBlocks, 256, 0, st>>>(static_cast<double*>(y), static_cast<const double*>(x), a, b, f);
+    else
+        axpby_kernel<float><<<kRedBlocks, 256, 0, st>>>(static_cast<float*>(y), static_cast<const float*>(x), a, b, f);
+    return cudaGetLastError();
+}
+
+// result (device double) = <x, y> real inner product; scratch holds kRedBlocks doubles
+cudaError_t launch_dot(int precision, int layout_base, unsigned V, double* result, double* scratch, const void* x, const void* y,
+                       cudaStream_t st) {
+    const FieldShape f = shape_of(precision, layout_base, V);
+    if (precision == 0)
+        dot_partial_kernel<double><<<kRedBlocks, 256, 0, st>>>(scratch, static_cast<const double*>(x), static_cast<const double*>(y), f);
+    else
+        dot_partial_kernel<float><<<kRedBlocks, 256, 0, st>>>(scratch, static_cast<const float*>(x), static_cast<const float*>(y), f);
+    dot_final_kernel<<<1, 256, 0, st>>>(result, scratch, kRedBlocks);
+    return cudaGetLastError();
+}
+
+int reduction_scratch_doubles() { return kRedBlocks; }
+
+}  // namespace dslash

@@ -90,6 +90,13 @@ class Lattice:
     def apply(self, out, inp, gauge):
         B.dslash_apply(self.ctx, out.data_ptr(), inp.data_ptr(), gauge.data_ptr(), self.stream())
 
+    def apply_op(self, op, mass, out, inp, gauge):
+        B.dslash_apply_op(self.ctx, op, mass, out.data_ptr(), inp.data_ptr(), gauge.data_ptr(), self.stream())
+
+    def cg_solve(self, x, b, gauge, mass, tol, max_iter):
+        """x <- solution of M^dagger M x = b (native device buffers); returns (iterations, rel_residual)."""
+        return B.dslash_cg_solve(self.ctx, x.data_ptr(), b.data_ptr(), gauge.data_ptr(), mass, tol, max_iter, self.stream())
+
     def set_variant(self, depth, tpb=0, spt=0):
         B.dslash_set_variant(self.ctx, depth, tpb, spt)
 

@@ -210,6 +210,65 @@ def test_all_omp_style_variants_match_the_oracle(env, dims):
             assert env.checks.parity_error(lat.dslash(g, p), ref) <= TOL["f64"]
 
 
+# ---------------------------------------------------------------- operators around Dslash: D^dagger, M, M^dagger, CG
+@pytest.mark.parametrize("dims", [(4, 6, 8, 10), (3, 5, 2, 7), (32, 4, 2, 4)])
+@pytest.mark.parametrize("precision", ["f64", "f32"])
+@pytest.mark.parametrize("layout,recon12", ALL_MODES)
+def test_apply_op_matches_the_oracle(env, dims, precision, layout, recon12):
+    B = env.B
+    g, p = env.inputs.fields(dims, SEED + 16, precision)
+    g64, p64 = env.inputs.promote(g), env.inputs.promote(p)
+    mass = -0.3
+    refs = {B.DSLASH_OP_D: env.oracle.dslash(p64, g64, dims), B.DSLASH_OP_D_DAGGER: env.oracle.dslash_dagger(p64, g64, dims),
+            B.DSLASH_OP_M: env.oracle.wilson(p64, g64, dims, mass), B.DSLASH_OP_M_DAGGER: env.oracle.wilson(p64, g64, dims, mass, dagger=True)}
+    with env.device.Lattice(dims, precision, layout, recon12) as lat:
+        gi, pi, o = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
+        for op, ref in refs.items():
+            o.zero_()
+            lat.apply_op(op, mass, o, pi, gi)
+            assert env.checks.parity_error(lat.download_spinor(o), ref) <= TOL[precision], op
+        assert B.dslash_apply_status(lat.ctx, o.data_ptr(), pi.data_ptr(), gi.data_ptr()) == B.DSLASH_OK
+        with pytest.raises(B.DslashError) as e:
+            B.dslash_apply_op(lat.ctx, 4, 0.0, o.data_ptr(), pi.data_ptr(), gi.data_ptr())
+        assert e.value.status == B.DSLASH_ERR_UNSUPPORTED
+        with pytest.raises(B.DslashError) as e:
+            B.dslash_apply_op(lat.ctx, 0, 0.0, pi.data_ptr(), pi.data_ptr(), gi.data_ptr())
+        assert e.value.status == B.DSLASH_ERR_ALIAS
+
+
+@pytest.mark.parametrize("dims,precision,layout,tol", [((8, 8, 8, 8), "f64", "soa", 1e-10), ((6, 4, 10, 5), "f64", "aos", 1e-10),
+                                                       ((8, 8, 8, 8), "f32", "soa", 1e-5)])
+def test_cg_solves_the_normal_equations(env, dims, precision, layout, tol):
+    """x = CG(M^dagger M, b): the residual |M^dagger M x - b| / |b| is evaluated independently with the fp64 oracle."""
+    B = env.B
+    g, b = env.inputs.fields(dims, SEED + 17, precision)
+    g64, b64 = env.inputs.promote(g), env.inputs.promote(b)
+    mass = 0.2
+    with env.device.Lattice(dims, precision, layout, False) as lat:
+        gi, bi, x = lat.upload_gauge(g), lat.upload_spinor(b), lat.new_spinor()
+        n0 = B.dslash_launch_count(lat.ctx)
+        iters, rel = lat.cg_solve(x, bi, gi, mass, tol, 500)
+        assert 1 <= iters < 500 and rel <= tol
+        assert B.dslash_launch_count(lat.ctx) >= n0 + 9 * (iters - 1)
+        xs = env.inputs.promote(lat.download_spinor(x))
+        mx = env.oracle.wilson(xs, g64, dims, mass)
+        mdmx = env.oracle.wilson(mx, g64, dims, mass, dagger=True)
+        res = np.linalg.norm(mdmx - b64.reshape(mdmx.shape)) / np.linalg.norm(b64)
+        assert res <= (5 * tol if precision == "f64" else 5e-5), res
+        # b is not modified, a second solve reproduces the first bit for bit (deterministic reductions)
+        assert np.array_equal(lat.download_spinor(bi), b)
+        x2 = lat.new_spinor()
+        iters2, rel2 = lat.cg_solve(x2, bi, gi, mass, tol, 500)
+        assert (iters2, rel2) == (iters, rel) and np.array_equal(lat.download_spinor(x2), lat.download_spinor(x))
+        # max_iter reached is reported, not an error
+        it3, rel3 = lat.cg_solve(x2, bi, gi, mass, 1e-30, 3)
+        assert it3 == 3 and rel3 > 1e-30
+        for bad in [dict(tol=0.0, max_iter=10), dict(tol=1e-8, max_iter=0)]:
+            with pytest.raises(B.DslashError) as e:
+                lat.cg_solve(x2, bi, gi, mass, bad["tol"], bad["max_iter"])
+            assert e.value.status == B.DSLASH_ERR_UNSUPPORTED
+
+
 # ---------------------------------------------------------------- config 3: 32^3 x 64 FP64, 18- and 12-real links
 @pytest.mark.parametrize("recon12", [False, True])
 def test_config3_32x32x32x64_fp64(env, recon12):

@@ -234,6 +234,51 @@ def test_p5_gamma5_hermiticity_dense_2x2x2x2():
     assert np.abs(d.conj().T - dense_from_eq1(u, dims, gam=-G)).max() < 1e-14
 
 
+def test_dagger_is_the_adjoint_and_gamma5_conjugate():
+    """oracle_dslash_dagger (Reading R19): <phi, D psi> = <D^dagger phi, psi>; D^dagger = gamma5 D gamma5; and on the
+    dense 2^4 matrix D^dagger is the conjugate transpose."""
+    dims = DISTINCT
+    u = random_gauge(dims, 33)
+    psi, phi = random_spinor(dims, 34), random_spinor(dims, 35)
+    d_psi = apply(u, psi, dims)
+    dd_phi = r2c(oracle.dslash_dagger(c2r(phi), c2r(u), dims))
+    lhs = np.vdot(phi, d_psi)
+    rhs = np.vdot(dd_phi, psi)
+    assert abs(lhs - rhs) <= 1e-12 * abs(lhs)
+    g5 = np.array([1.0, 1.0, -1.0, -1.0])[:, None]
+    assert np.abs(dd_phi - g5 * apply(u, g5 * phi, dims)).max() < 2e-13
+    small = (2, 2, 2, 2)
+    us = random_gauge(small, 36)
+    n = 16 * 12
+    cols = np.zeros((n, n), dtype=np.complex128)
+    for k in range(n):
+        e = np.zeros(n, dtype=np.complex128)
+        e[k] = 1.0
+        cols[:, k] = r2c(oracle.dslash_dagger(c2r(e.reshape(shape4(small) + (4, 3))), c2r(us), small)).reshape(n)
+    assert np.abs(cols - dense_from_eq1(us, small).conj().T).max() < 1e-14
+
+
+def test_wilson_matrix_definition_and_normal_operator_is_positive():
+    dims = (4, 2, 6, 4)
+    u = random_gauge(dims, 37)
+    psi = random_spinor(dims, 38)
+    m = 0.1
+    mp = r2c(oracle.wilson(c2r(psi), c2r(u), dims, m))
+    assert np.abs(mp - ((4.0 + m) * psi - 0.5 * apply(u, psi, dims))).max() < 1e-14
+    # free field: M e^{ipx} chi = [(4 + m) - sum cos p + i sum gamma sin p] e^{ipx} chi
+    n = (1, 0, 2, 3)
+    p = [2.0 * np.pi * n[k] / dims[k] for k in range(4)]
+    x, y, z, t = coords(dims)
+    phase = np.exp(1j * (p[0] * x + p[1] * y + p[2] * z + p[3] * t))
+    chi = np.random.default_rng(3).standard_normal((4, 3)) + 0j
+    got = r2c(oracle.wilson(c2r(phase[..., None, None] * chi), c2r(unit_gauge(dims)), dims, m))
+    mm = (4.0 + m) * ID4 - 0.5 * free_matrix(p)
+    assert np.abs(got - phase[..., None, None] * (mm @ chi)).max() < 2e-13
+    # <psi, M^dagger M psi> = |M psi|^2 > 0
+    mdm = r2c(oracle.wilson(c2r(mp), c2r(u), dims, m, dagger=True))
+    assert abs(np.vdot(psi, mdm) - np.vdot(mp, mp)) <= 1e-12 * abs(np.vdot(mp, mp))
+
+
 # ------------------------------------------------------------------ P6
 def _gauge_transform(u, psi, g, dims):
     ug = np.empty_like(u)
