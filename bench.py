@@ -481,6 +481,43 @@ def run_advisor(args):
     return 0
 
 
+# ------------------------------------------------------------------ the solver around Dslash
+def run_cg(args):
+    """CG on M^dagger M (dslash_cg_solve) on a BASELINE lattice: what "called several times throughout the LQCD
+    application" (PAPER.md:54) looks like.  Reports iterations, time per iteration and the operator throughput."""
+    import torch
+    from paper_2301_03636_b200 import binding as B
+    from paper_2301_03636_b200 import device, inputs
+    cfg = CONFIGS[args.config]
+    dims, prec = cfg["dims"], cfg["precision"]
+    v = inputs.volume(dims)
+    g, b = inputs.fields(dims, SEED + 7, prec, check=False)
+    with device.Lattice(dims, prec, args.layout, cfg["recon12"]) as lat:
+        gd, bd, xd = lat.upload_gauge(g), lat.upload_spinor(b), lat.new_spinor()
+        lat.cg_solve(xd, bd, gd, args.cg_mass, 1e-2, 5)  # warm-up (allocates the work spinors)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n0 = B.dslash_launch_count(lat.ctx)
+        e0.record()
+        iters, rel = lat.cg_solve(xd, bd, gd, args.cg_mass, args.cg_tol, args.cg_max_iter)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        launches = B.dslash_launch_count(lat.ctx) - n0
+        # per iteration: M and M^dagger (1320 + 72 flop/site each: the epilogue a*psi + b*acc is 24 mul + 24 fma), |t|^2 (48),
+        # the fused update x += alpha p, r -= alpha q, |r|^2 (4*24 + 48), p = r + beta p (48)
+        flop_it = v * (2 * (1320 + 72) + 48 + 144 + 48)
+        rb = 8 if prec == "f64" else 4
+        # bytes: two operator applies (+ centre spinor), |t|^2 reads t, the fused update reads 4 and writes 2, p-update reads 2 writes 1
+        bytes_it = v * (2 * (bytes_per_site(prec, cfg["recon12"]) + 24 * rb) + (1 + 6 + 3) * 24 * rb)
+        line = {"cg": "dslash_cg_solve, M^dagger M x = b", "workload": cfg["name"], "dims": list(dims), "mass": args.cg_mass,
+                "tol": args.cg_tol, "iterations": iters, "rel_residual": rel, "ms_total": ms, "ms_per_iteration": ms / max(iters, 1),
+                "gflops": flop_it * iters / ms / 1e6, "algorithmic_gbs": bytes_it * iters / ms / 1e6, "gpu_launches": int(launches),
+                "dtype": prec, "data": "synthetic"}
+        print(json.dumps(line))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -507,6 +544,10 @@ def main():
     ap.add_argument("--advisor-dims", type=int, nargs=4, default=[32, 32, 32, 16])
     ap.add_argument("--advisor-csv", default=os.path.join(ROOT, "gpurun_out", "advisor_variants.csv"))
     ap.add_argument("--team-size", type=int, default=128)
+    ap.add_argument("--cg", action="store_true", help="time dslash_cg_solve on the --config lattice")
+    ap.add_argument("--cg-mass", type=float, default=0.2)
+    ap.add_argument("--cg-tol", type=float, default=1e-8)
+    ap.add_argument("--cg-max-iter", type=int, default=2000)
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "cuda" and not args.sweep:
         args.warmup = 3  # timing rule: at least 3 warm-up steps
@@ -514,6 +555,8 @@ def main():
         return run_sweep(args)
     if args.advisor:
         return run_advisor(args)
+    if args.cg:
+        return run_cg(args)
     cfg = CONFIGS[args.config]
     if args.impl == "reference":
         return run_reference(args, cfg)

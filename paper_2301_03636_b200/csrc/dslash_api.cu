@@ -282,9 +282,11 @@ int dslash_cg_solve(dslash_ctx* c, void* x, const void* b, const void* gauge, do
             CG_TRY(dot(t, t, &pAp));
             CG_TRY(op(DSLASH_OP_M_DAGGER, q, t));
             const double alpha = rr / pAp;
-            CG_TRY(axpby(x, p, alpha, 1.0));
-            CG_TRY(axpby(r, q, -alpha, 1.0));
-            CG_TRY(dot(r, r, &rr_new));
+            // x += alpha p, r -= alpha q, rr_new = |r|^2 in one pass over the four fields
+            CG_TRY(launch_cg_update(prec, lay, V, x, r, p, q, alpha, d_res, c->cg_scratch, st));
+            c->launches += 2;
+            CG_TRY(cudaMemcpyAsync(&rr_new, d_res, sizeof(double), cudaMemcpyDeviceToHost, st));
+            CG_TRY(cudaStreamSynchronize(st));
             rel = sqrt(rr_new / bb);
             if (rel <= tol) break;
             CG_TRY(axpby(p, r, 1.0, rr_new / rr));

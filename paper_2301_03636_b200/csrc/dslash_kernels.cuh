@@ -49,6 +49,8 @@ cudaError_t launch_op(int precision, int layout_base, int recon, const LaunchArg
 cudaError_t launch_axpby(int precision, int layout_base, unsigned V, void* y, const void* x, double a, double b, cudaStream_t st);
 cudaError_t launch_dot(int precision, int layout_base, unsigned V, double* result, double* scratch, const void* x, const void* y,
                        cudaStream_t st);
+cudaError_t launch_cg_update(int precision, int layout_base, unsigned V, void* x, void* r, const void* p, const void* q, double alpha,
+                             double* result, double* scratch, cudaStream_t st);
 int reduction_scratch_doubles();
 
 // Layout module.  dir 0: canonical -> native (pack), 1: native -> canonical (unpack).

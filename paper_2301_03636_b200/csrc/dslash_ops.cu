@@ -162,36 +162,54 @@ cudaError_t launch_op(int precision, int layout_base, int recon, const LaunchArg
 }
 
 // ------------------------------------------------------------------ vector kernels for the solver
-// Fields are treated as arrays of reals in the native layout.  With the blocked SoA layout the last vector may contain
-// padding sites; `valid(i)` masks them out of the reductions and the updates leave them untouched.
+// Fields are treated as arrays of 16-byte units in the native layout (fp64: one complex number, fp32: two).  With the
+// blocked SoA layout the last vector may contain padding sites; `valid(u)` masks them out of the reductions and the
+// updates leave them untouched (they are zero in the solver's own work spinors).
 struct FieldShape {
-    size_t n;       // reals in the buffer (including padding)
+    size_t nunits;  // 16-byte units in the buffer (including padding)
     unsigned V;     // real sites
     int soa;        // blocked SoA?
-    unsigned rpv;   // reals per vector = 24 * 32
-    unsigned rpu;   // reals per 16-byte unit row: fp64 2, fp32 4  (lane index = (i / rpu) % 32)
+    unsigned upv;   // units per vector: 12 * 32 (fp64) or 6 * 32 (fp32)
 };
-__device__ __forceinline__ bool valid(const FieldShape& f, size_t i) {
+__device__ __forceinline__ bool valid(const FieldShape& f, size_t u) {
     if (!f.soa) return true;
-    const unsigned v = (unsigned)(i / f.rpv);
-    const unsigned lane = (unsigned)((i / f.rpu) & (VL - 1u));
-    return v * VL + lane < f.V;
+    const unsigned v = (unsigned)(u / f.upv);
+    return v * VL + (unsigned)(u & (VL - 1u)) < f.V;
 }
 
-// y = a*x + b*y   (a, b real)
 template <typename Real>
-__global__ void __launch_bounds__(256) axpby_kernel(Real* __restrict__ y, const Real* __restrict__ x, double a, double b, FieldShape f) {
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < f.n; i += (size_t)gridDim.x * blockDim.x)
-        if (valid(f, i)) y[i] = (Real)(a * (double)x[i] + b * (double)y[i]);
+struct U16;
+template <>
+struct U16<double> {
+    using type = double2;
+    static constexpr int N = 2;
+};
+template <>
+struct U16<float> {
+    using type = float4;
+    static constexpr int N = 4;
+};
+template <typename Real>
+__device__ __forceinline__ void unpack(const typename U16<Real>::type& v, double (&a)[4]);
+template <>
+__device__ __forceinline__ void unpack<double>(const double2& v, double (&a)[4]) {
+    a[0] = v.x;
+    a[1] = v.y;
+}
+template <>
+__device__ __forceinline__ void unpack<float>(const float4& v, double (&a)[4]) {
+    a[0] = v.x;
+    a[1] = v.y;
+    a[2] = v.z;
+    a[3] = v.w;
+}
+__device__ __forceinline__ void pack(double2& v, const double (&a)[4]) { v = make_double2(a[0], a[1]); }
+__device__ __forceinline__ void pack(float4& v, const double (&a)[4]) {
+    v = make_float4((float)a[0], (float)a[1], (float)a[2], (float)a[3]);
 }
 
-// partial[block] = sum_i x[i]*y[i] over the block's grid-stride range, accumulated in fp64 (deterministic two-pass sum)
-template <typename Real>
-__global__ void __launch_bounds__(256) dot_partial_kernel(double* __restrict__ partial, const Real* __restrict__ x,
-                                                          const Real* __restrict__ y, FieldShape f) {
-    double s = 0.0;
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < f.n; i += (size_t)gridDim.x * blockDim.x)
-        if (valid(f, i)) s += (double)x[i] * (double)y[i];
+// block-level fp64 sum -> partial[blockIdx.x]
+__device__ __forceinline__ void block_sum_to(double* partial, double s) {
     __shared__ double sh[256];
     sh[threadIdx.x] = s;
     __syncthreads();
@@ -200,6 +218,80 @@ __global__ void __launch_bounds__(256) dot_partial_kernel(double* __restrict__ p
         __syncthreads();
     }
     if (threadIdx.x == 0) partial[blockIdx.x] = sh[0];
+}
+
+// y = a*x + b*y   (a, b real)
+template <typename Real>
+__global__ void __launch_bounds__(256) axpby_kernel(void* __restrict__ y_, const void* __restrict__ x_, double a, double b,
+                                                    FieldShape f) {
+    using U = typename U16<Real>::type;
+    U* y = static_cast<U*>(y_);
+    const U* x = static_cast<const U*>(x_);
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < f.nunits; i += (size_t)gridDim.x * blockDim.x) {
+        if (!valid(f, i)) continue;
+        double xv[4], yv[4];
+        unpack<Real>(x[i], xv);
+        unpack<Real>(y[i], yv);
+#pragma unroll
+        for (int k = 0; k < U16<Real>::N; ++k) yv[k] = a * xv[k] + b * yv[k];
+        U o;
+        pack(o, yv);
+        y[i] = o;
+    }
+}
+
+// the fused CG update: x += alpha*p;  r -= alpha*q;  partial[block] = sum |r|^2  (fp64 accumulation)
+template <typename Real>
+__global__ void __launch_bounds__(256) cg_update_kernel(void* __restrict__ x_, void* __restrict__ r_, const void* __restrict__ p_,
+                                                        const void* __restrict__ q_, double alpha, double* __restrict__ partial,
+                                                        FieldShape f) {
+    using U = typename U16<Real>::type;
+    U* x = static_cast<U*>(x_);
+    U* r = static_cast<U*>(r_);
+    const U* p = static_cast<const U*>(p_);
+    const U* q = static_cast<const U*>(q_);
+    double s = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < f.nunits; i += (size_t)gridDim.x * blockDim.x) {
+        if (!valid(f, i)) continue;
+        double xv[4], rv[4], pv[4], qv[4];
+        unpack<Real>(x[i], xv);
+        unpack<Real>(r[i], rv);
+        unpack<Real>(p[i], pv);
+        unpack<Real>(q[i], qv);
+        U xo, ro;
+#pragma unroll
+        for (int k = 0; k < U16<Real>::N; ++k) {
+            xv[k] += alpha * pv[k];
+            rv[k] -= alpha * qv[k];
+        }
+        pack(xo, xv);
+        pack(ro, rv);
+        unpack<Real>(ro, rv);  // the norm is taken of r as it is stored (fp32 contexts round here)
+#pragma unroll
+        for (int k = 0; k < U16<Real>::N; ++k) s += rv[k] * rv[k];
+        x[i] = xo;
+        r[i] = ro;
+    }
+    block_sum_to(partial, s);
+}
+
+// partial[block] = sum_i x[i]*y[i] over the block's grid-stride range, accumulated in fp64 (deterministic two-pass sum)
+template <typename Real>
+__global__ void __launch_bounds__(256) dot_partial_kernel(double* __restrict__ partial, const void* __restrict__ x_,
+                                                          const void* __restrict__ y_, FieldShape f) {
+    using U = typename U16<Real>::type;
+    const U* x = static_cast<const U*>(x_);
+    const U* y = static_cast<const U*>(y_);
+    double s = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < f.nunits; i += (size_t)gridDim.x * blockDim.x) {
+        if (!valid(f, i)) continue;
+        double xv[4], yv[4];
+        unpack<Real>(x[i], xv);
+        unpack<Real>(y[i], yv);
+#pragma unroll
+        for (int k = 0; k < U16<Real>::N; ++k) s += xv[k] * yv[k];
+    }
+    block_sum_to(partial, s);
 }
 __global__ void __launch_bounds__(256) dot_final_kernel(double* __restrict__ result, const double* __restrict__ partial, int n) {
     __shared__ double sh[256];
@@ -219,20 +311,20 @@ static FieldShape shape_of(int precision, int layout_base, unsigned V) {
     f.V = V;
     f.soa = layout_base == LAYOUT_SOA;
     const size_t sites = f.soa ? (size_t)((V + VL - 1u) / VL) * VL : (size_t)V;
-    f.n = sites * 24u;
-    f.rpv = 24u * VL;
-    f.rpu = precision == 0 ? 2u : 4u;
+    const unsigned ups = precision == 0 ? 12u : 6u;  // 16-byte units per site
+    f.nunits = sites * ups;
+    f.upv = ups * VL;
     return f;
 }
 
-static const int kRedBlocks = 592;
+static const int kRedBlocks = 1184;  // 8 blocks of 256 threads per SM
 
 cudaError_t launch_axpby(int precision, int layout_base, unsigned V, void* y, const void* x, double a, double b, cudaStream_t st) {
     const FieldShape f = shape_of(precision, layout_base, V);
     if (precision == 0)
-        axpby_kernel<double><<<kRedBlocks, 256, 0, st>>>(static_cast<double*>(y), static_cast<const double*>(x), a, b, f);
+        axpby_kernel<double><<<kRedBlocks, 256, 0, st>>>(y, x, a, b, f);
     else
-        axpby_kernel<float><<<kRedBlocks, 256, 0, st>>>(static_cast<float*>(y), static_cast<const float*>(x), a, b, f);
+        axpby_kernel<float><<<kRedBlocks, 256, 0, st>>>(y, x, a, b, f);
     return cudaGetLastError();
 }
 
@@ -241,9 +333,21 @@ cudaError_t launch_dot(int precision, int layout_base, unsigned V, double* resul
                        cudaStream_t st) {
     const FieldShape f = shape_of(precision, layout_base, V);
     if (precision == 0)
-        dot_partial_kernel<double><<<kRedBlocks, 256, 0, st>>>(scratch, static_cast<const double*>(x), static_cast<const double*>(y), f);
+        dot_partial_kernel<double><<<kRedBlocks, 256, 0, st>>>(scratch, x, y, f);
     else
-        dot_partial_kernel<float><<<kRedBlocks, 256, 0, st>>>(scratch, static_cast<const float*>(x), static_cast<const float*>(y), f);
+        dot_partial_kernel<float><<<kRedBlocks, 256, 0, st>>>(scratch, x, y, f);
+    dot_final_kernel<<<1, 256, 0, st>>>(result, scratch, kRedBlocks);
+    return cudaGetLastError();
+}
+
+// x += alpha p, r -= alpha q, result = |r|^2
+cudaError_t launch_cg_update(int precision, int layout_base, unsigned V, void* x, void* r, const void* p, const void* q, double alpha,
+                             double* result, double* scratch, cudaStream_t st) {
+    const FieldShape f = shape_of(precision, layout_base, V);
+    if (precision == 0)
+        cg_update_kernel<double><<<kRedBlocks, 256, 0, st>>>(x, r, p, q, alpha, scratch, f);
+    else
+        cg_update_kernel<float><<<kRedBlocks, 256, 0, st>>>(x, r, p, q, alpha, scratch, f);
     dot_final_kernel<<<1, 256, 0, st>>>(result, scratch, kRedBlocks);
     return cudaGetLastError();
 }

@@ -249,7 +249,7 @@ def test_cg_solves_the_normal_equations(env, dims, precision, layout, tol):
         n0 = B.dslash_launch_count(lat.ctx)
         iters, rel = lat.cg_solve(x, bi, gi, mass, tol, 500)
         assert 1 <= iters < 500 and rel <= tol
-        assert B.dslash_launch_count(lat.ctx) >= n0 + 9 * (iters - 1)
+        assert B.dslash_launch_count(lat.ctx) >= n0 + 7 * (iters - 1)
         xs = env.inputs.promote(lat.download_spinor(x))
         mx = env.oracle.wilson(xs, g64, dims, mass)
         mdmx = env.oracle.wilson(mx, g64, dims, mass, dagger=True)
