@@ -208,6 +208,18 @@ DSLASH_API int dslash_set_tile(dslash_ctx *ctx, const int tile[4]);
 DSLASH_API int dslash_get_tile(const dslash_ctx *ctx, int tile[4]);
 
 /*
+ * Restrict dslash_apply / dslash_apply_op to the time slices t_begin <= t < t_end (default: the whole lattice); sites
+ * outside the range are neither computed nor written.  This is the hook of the multi-GPU slab decomposition
+ * (paper_2301_03636_b200/slab.py): a rank's local lattice carries one ghost slice at each end in t, only the interior
+ * slices are computed, and the interior can be launched while the ghost slices are still being exchanged.
+ * With a partial range the tuned path always uses the direct kernel; the sweep variants and dslash_cg_solve need the
+ * full range (DSLASH_ERR_UNSUPPORTED otherwise).
+ * Errors: NULL, UNSUPPORTED (not 0 <= t_begin < t_end <= L_T).
+ */
+DSLASH_API int dslash_set_time_range(dslash_ctx *ctx, int t_begin, int t_end);
+DSLASH_API int dslash_get_time_range(const dslash_ctx *ctx, int *t_begin, int *t_end);
+
+/*
  * Choose the implementation behind DSLASH_VARIANT_TUNED: DSLASH_KERNEL_AUTO (default), _DIRECT, _TMA or _TMA_LINKS.
  * _TMA and _TMA_LINKS need a DSLASH_SOA ctx, a tile whose x-extent is a multiple of 32 and divides L_X, the other tile
  * extents <= the lattice extents, and 32..128 sites per tile;

@@ -54,6 +54,8 @@ SIGNATURES = {
                                                ctypes.c_int]),
     "dslash_set_tile": (ctypes.c_int, [_vp, _c_int_p]),
     "dslash_get_tile": (ctypes.c_int, [_vp, _c_int_p]),
+    "dslash_set_time_range": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int]),
+    "dslash_get_time_range": (ctypes.c_int, [_vp, _c_int_p, _c_int_p]),
     "dslash_set_kernel": (ctypes.c_int, [_vp, ctypes.c_int]),
     "dslash_get_kernel": (ctypes.c_int, [_vp, _c_int_p]),
     "dslash_set_option": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int]),
@@ -223,6 +225,16 @@ def dslash_get_tile(ctx):
     arr = (ctypes.c_int * 4)()
     _check(_lib.dslash_get_tile(_ptr(ctx), arr), "dslash_get_tile")
     return tuple(arr)
+
+
+def dslash_set_time_range(ctx, t_begin: int, t_end: int) -> None:
+    _check(_lib.dslash_set_time_range(_ptr(ctx), int(t_begin), int(t_end)), "dslash_set_time_range")
+
+
+def dslash_get_time_range(ctx):
+    a, b = ctypes.c_int(), ctypes.c_int()
+    _check(_lib.dslash_get_time_range(_ptr(ctx), ctypes.byref(a), ctypes.byref(b)), "dslash_get_time_range")
+    return a.value, b.value
 
 
 def dslash_set_kernel(ctx, kernel: int) -> None:

@@ -51,7 +51,9 @@ static void set_tile_geom(dslash_ctx* c, const int tile[4]) {
         c->tg.lb[d] = ilog2_exact(tile[d]);
         c->tg.nt[d] = (c->geom.L[d] + tile[d] - 1) / tile[d];
     }
+    c->tg.nt[3] = (c->tg.t_end - c->tg.t_begin + tile[3] - 1) / tile[3];  // tiles in t cover the active range only
 }
+static bool full_time_range(const dslash_ctx* c) { return c->tg.t_begin == 0 && c->tg.t_end == c->geom.L[3]; }
 
 // Default tile of the tuned kernel (measured on B200, profiles/): x-extent = the largest power of two <= 32 that
 // divides L_X (a warp then reads whole 32-site vectors or aligned halves of them), 2-4 rows in y, 2 planes in z,
@@ -115,6 +117,8 @@ int dslash_create(dslash_ctx** ctx, const int dims[4], int precision, int layout
     c->var_depth = DSLASH_VARIANT_TUNED;
     c->var_tpb = 0;
     c->var_spt = 0;
+    c->tg.t_begin = 0;
+    c->tg.t_end = dims[3];
     int tile[4];
     default_tile(c, tile);
     set_tile_geom(c, tile);
@@ -164,7 +168,7 @@ size_t dslash_canonical_gauge_bytes(const dslash_ctx* c) { return c ? (size_t)c-
 // The kernel dslash_apply will launch for the tuned path: DSLASH_KERNEL_DIRECT / _TMA, or -1 if _TMA was
 // requested explicitly but cannot run this configuration.
 static int resolve_kernel(const dslash_ctx* c) {
-    const bool can_tma = c->layout_base == LAYOUT_SOA && tma_eligible(c->precision, c->recon, c->geom, c->tg);
+    const bool can_tma = c->layout_base == LAYOUT_SOA && full_time_range(c) && tma_eligible(c->precision, c->recon, c->geom, c->tg);
     if (c->kernel == DSLASH_KERNEL_DIRECT) return DSLASH_KERNEL_DIRECT;
     if (c->kernel == DSLASH_KERNEL_TMA || c->kernel == DSLASH_KERNEL_TMA_LINKS) return can_tma ? c->kernel : -1;
     return DSLASH_KERNEL_DIRECT;  // AUTO
@@ -188,6 +192,8 @@ int dslash_apply(dslash_ctx* c, void* out, const void* in, const void* gauge, ds
         if (k < 0) return DSLASH_ERR_UNSUPPORTED;
         e = (k == DSLASH_KERNEL_DIRECT) ? launch_tuned(c->precision, c->layout_base, c->recon, a, c->tg, c->cfg)
                                         : launch_tma(c->precision, c->recon, a, c->tg, k == DSLASH_KERNEL_TMA_LINKS);
+    } else if (!full_time_range(c)) {
+        return DSLASH_ERR_UNSUPPORTED;  // the variant kernels always sweep the whole lattice
     } else if (c->var_depth < 0) {
         e = launch_omp_variant(c->precision, c->layout_base, c->recon, a, c->omp_a, c->omp_x, c->omp_b, c->omp_sched, c->omp_teams,
                                c->omp_team_size);
@@ -215,7 +221,7 @@ int dslash_apply_op(dslash_ctx* c, int op, double mass, void* out, const void* i
 int dslash_cg_solve(dslash_ctx* c, void* x, const void* b, const void* gauge, double mass, double tol, int max_iter, int* iterations,
                     double* rel_residual, dslash_stream_t stream_) {
     if (!c || !x || !b || !gauge) return DSLASH_ERR_NULL;
-    if (!(tol > 0.0) || max_iter < 1) return DSLASH_ERR_UNSUPPORTED;
+    if (!(tol > 0.0) || max_iter < 1 || !full_time_range(c)) return DSLASH_ERR_UNSUPPORTED;
     if (misaligned(x) || misaligned(b) || misaligned(gauge)) return DSLASH_ERR_ALIGN;
     const size_t sb = dslash_spinor_bytes(c);
     if (overlap(x, sb, b, sb)) return DSLASH_ERR_ALIAS;
@@ -438,6 +444,22 @@ int dslash_set_tile(dslash_ctx* c, const int tile[4]) {
     }
     if (prod < 32 || prod > 1024) return DSLASH_ERR_UNSUPPORTED;
     set_tile_geom(c, tile);
+    return DSLASH_OK;
+}
+
+int dslash_set_time_range(dslash_ctx* c, int t_begin, int t_end) {
+    if (!c) return DSLASH_ERR_NULL;
+    if (t_begin < 0 || t_end > c->geom.L[3] || t_begin >= t_end) return DSLASH_ERR_UNSUPPORTED;
+    c->tg.t_begin = t_begin;
+    c->tg.t_end = t_end;
+    set_tile_geom(c, c->tile);
+    return DSLASH_OK;
+}
+
+int dslash_get_time_range(const dslash_ctx* c, int* t_begin, int* t_end) {
+    if (!c || !t_begin || !t_end) return DSLASH_ERR_NULL;
+    *t_begin = c->tg.t_begin;
+    *t_end = c->tg.t_end;
     return DSLASH_OK;
 }
 

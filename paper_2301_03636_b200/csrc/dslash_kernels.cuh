@@ -11,6 +11,7 @@ namespace dslash {
 struct TileGeom {
     int lb[4];
     int nt[4];
+    int t_begin, t_end;  // time slices [t_begin, t_end) are computed (dslash_set_time_range); nt[3] tiles cover that range
 };
 
 struct LaunchArgs {

@@ -99,8 +99,8 @@ __global__ void __launch_bounds__(128, MINBLK)
     r >>= tg.lb[1];
     const int z = (int)((bz << tg.lb[2]) + (r & ((1u << tg.lb[2]) - 1u)));
     r >>= tg.lb[2];
-    const int t = (int)((bt << tg.lb[3]) + r);
-    if (x >= g.L[0] || y >= g.L[1] || z >= g.L[2] || t >= g.L[3]) return;
+    const int t = tg.t_begin + (int)((bt << tg.lb[3]) + r);
+    if (x >= g.L[0] || y >= g.L[1] || z >= g.L[2] || t >= tg.t_end) return;
     const unsigned V = g.V;
     const unsigned sy = (unsigned)g.L[0], sz = sy * (unsigned)g.L[1], st = sz * (unsigned)g.L[2];
     const unsigned s = (unsigned)x + sy * (unsigned)y + sz * (unsigned)z + st * (unsigned)t;

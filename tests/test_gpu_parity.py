@@ -269,6 +269,69 @@ def test_cg_solves_the_normal_equations(env, dims, precision, layout, tol):
             assert e.value.status == B.DSLASH_ERR_UNSUPPORTED
 
 
+# ---------------------------------------------------------------- multi-GPU slab decomposition, ranks emulated in one process
+@pytest.mark.parametrize("world", [1, 2, 3, 4])
+@pytest.mark.parametrize("precision,layout,recon12", [("f64", "soa", False), ("f64", "aos", True), ("f32", "soa", True)])
+def test_slab_decomposition_reproduces_the_single_lattice_result(env, world, precision, layout, recon12):
+    """T-slabs with ghost slices + halo exchange + dslash_set_time_range (interior first, then the two boundary
+    slices) must give the oracle's result for the GLOBAL lattice.  One GPU is available, so the `world` ranks are
+    emulated in one process and the exchange is a device copy between their buffers (slab.exchange_halos_in_process);
+    the torch.distributed path is covered on CPU by tests/test_multirank_gloo.py."""
+    from paper_2301_03636_b200 import slab
+    dims = (8, 4, 4, 12)
+    g, p, ref, _ = fields_and_ref(env, dims, SEED + 18, precision)
+    ranks = [slab.SlabDslash(dims, precision, layout, recon12, rank=r, world=world) for r in range(world)]
+    try:
+        gauges = [rk.upload_gauge(g) for rk in ranks]
+        ins = [rk.upload_spinor(p) for rk in ranks]
+        outs = [rk.lat.new_spinor() for rk in ranks]
+        geoms = [rk.geom for rk in ranks]
+        done = []
+
+        def exchange_all(_buf, nbytes):  # the first rank that asks triggers the exchange for everybody
+            if not done:
+                slab.exchange_halos_in_process(ins, geoms, nbytes)
+                done.append(True)
+            return []
+        for rk in ranks:
+            rk._exchange = exchange_all
+        for rk, o, i, gg in zip(ranks, outs, ins, gauges):
+            o.zero_()
+            rk.apply(o, i, gg)
+        env.torch.cuda.synchronize()
+        got = np.concatenate([rk.download_interior(o) for rk, o in zip(ranks, outs)], axis=0)
+        assert got.shape == ref.shape
+        assert env.checks.parity_error(got, ref) <= TOL[precision]
+        assert env.B.dslash_get_time_range(ranks[0].lat.ctx) == (0, ranks[0].geom.lt + 2)
+    finally:
+        for rk in ranks:
+            rk.close()
+
+
+def test_time_range_only_touches_its_slices(env):
+    B = env.B
+    dims = (8, 4, 4, 6)
+    g, p, ref, _ = fields_and_ref(env, dims, SEED + 19, "f64")
+    with env.device.Lattice(dims, "f64", "soa", False) as lat:
+        gi, pi, o = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
+        o.zero_()
+        B.dslash_set_time_range(lat.ctx, 2, 5)
+        lat.apply(o, pi, gi)
+        out = lat.download_spinor(o)
+        assert env.checks.parity_error(out[2:5], ref[2:5]) <= TOL["f64"]
+        assert np.all(out[:2] == 0) and np.all(out[5:] == 0)
+        lat.apply_op(B.DSLASH_OP_D_DAGGER, 0.0, o, pi, gi)
+        assert np.all(lat.download_spinor(o)[:2] == 0)
+        lat.set_variant(4, 128, 1)
+        assert B.dslash_apply_status(lat.ctx, o.data_ptr(), pi.data_ptr(), gi.data_ptr()) == B.DSLASH_ERR_UNSUPPORTED
+        lat.set_variant(B.DSLASH_VARIANT_TUNED)
+        for bad in [(-1, 3), (3, 3), (2, 7)]:
+            with pytest.raises(B.DslashError):
+                B.dslash_set_time_range(lat.ctx, *bad)
+        B.dslash_set_time_range(lat.ctx, 0, 6)
+        assert env.checks.parity_error(lat.dslash(g, p), ref) <= TOL["f64"]
+
+
 # ---------------------------------------------------------------- config 3: 32^3 x 64 FP64, 18- and 12-real links
 @pytest.mark.parametrize("recon12", [False, True])
 def test_config3_32x32x32x64_fp64(env, recon12):
