@@ -108,7 +108,9 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
 #define DSLASH_OPT_OCCUPANCY 2        /* blocks of <= 128 threads: 0 = 168 registers/thread (12 warps/SM), 1 = 128 (16 warps),
                                          2 = 255 (8 warps, deeper load hoisting) */
 #define DSLASH_OPT_L2_POLICY 3        /* bit mask of L2 eviction hints: 1 spinor loads evict_last, 2 U_t loads evict_last,
-                                         4 U_x/U_y/U_z loads evict_first, 8 stores of `out` evict_first (0: none) */
+                                         4 U_x/U_y/U_z loads evict_first, 8 stores of `out` evict_first,
+                                         16 t-direction loads bypass L1 allocation (0: none) */
+#define DSLASH_OPT_L1_CARVEOUT 4      /* direct kernel: preferred shared-memory carve-out in percent, -1 = driver default */
 
 /* host<->device mapping modes of dslash_apply_host() (section 4.1.2) */
 #define DSLASH_MAP_MINIMAL 0 /* to: gauge, in;  from: out            (after the Advisor's data analysis) */

@@ -125,6 +125,7 @@ int dslash_create(dslash_ctx** ctx, const int dims[4], int precision, int layout
     c->kernel = DSLASH_KERNEL_AUTO;
     c->cfg.occupancy = precision == DSLASH_FP64 ? 2 : 1;  // measured: fp64 wants registers (ILP), fp32 wants warps
     c->cfg.l2_policy = 0;
+    c->cfg.l1_carveout = -1;
     c->launches = 0;
     c->last_cuda = 0;
     for (int i = 0; i < 3; ++i) c->d_can[i] = c->d_nat[i] = nullptr;
@@ -477,8 +478,12 @@ int dslash_set_option(dslash_ctx* c, int option, int value) {
             c->cfg.occupancy = value;
             return DSLASH_OK;
         case DSLASH_OPT_L2_POLICY:
-            if (value < 0 || value > 15) return DSLASH_ERR_UNSUPPORTED;
+            if (value < 0 || value > 31) return DSLASH_ERR_UNSUPPORTED;
             c->cfg.l2_policy = value;
+            return DSLASH_OK;
+        case DSLASH_OPT_L1_CARVEOUT:
+            if (value < -1 || value > 100) return DSLASH_ERR_UNSUPPORTED;
+            c->cfg.l1_carveout = value;
             return DSLASH_OK;
         default:
             return DSLASH_ERR_UNSUPPORTED;
@@ -490,6 +495,7 @@ int dslash_get_option(const dslash_ctx* c, int option, int* value) {
     switch (option) {
         case DSLASH_OPT_OCCUPANCY: *value = c->cfg.occupancy; return DSLASH_OK;
         case DSLASH_OPT_L2_POLICY: *value = c->cfg.l2_policy; return DSLASH_OK;
+        case DSLASH_OPT_L1_CARVEOUT: *value = c->cfg.l1_carveout; return DSLASH_OK;
         default: return DSLASH_ERR_UNSUPPORTED;
     }
 }

@@ -35,6 +35,7 @@ cudaError_t launch_omp_variant(int precision, int layout_base, int recon, const 
 struct TunedConfig {
     int occupancy;         // 0: default register budget, 1: 128-register variant
     int l2_policy;         // DSLASH_OPT_L2_POLICY bits (0: no cache hints)
+    int l1_carveout;       // preferred shared-memory carve-out of the direct kernel in percent (-1: driver default)
 };
 
 // Tuned kernel (direct, register-staged).

@@ -73,30 +73,42 @@ __device__ __forceinline__ uint64_t make_policy(int kind) {
         asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
     return p;
 }
-template <bool HINT>
+// HINT: 0 plain __ldg, 1 with the L2 policy, 2 with the L2 policy and L1::no_allocate (data with no reuse inside the block)
+template <int HINT>
 __device__ __forceinline__ double2 ld_ro(const double2* p, uint64_t pol) {
-    if (!HINT) return __ldg(p);
+    if (HINT == 0) return __ldg(p);
     double2 v;
-    asm volatile("ld.global.nc.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol));
+    if (HINT == 2)
+        asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol));
+    else
+        asm volatile("ld.global.nc.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol));
     return v;
 }
-template <bool HINT>
+template <int HINT>
 __device__ __forceinline__ float4 ld_ro(const float4* p, uint64_t pol) {
-    if (!HINT) return __ldg(p);
+    if (HINT == 0) return __ldg(p);
     float4 v;
-    asm volatile("ld.global.nc.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;"
-                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
-                 : "l"(p), "l"(pol));
+    if (HINT == 2)
+        asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;"
+                     : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+                     : "l"(p), "l"(pol));
+    else
+        asm volatile("ld.global.nc.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;"
+                     : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+                     : "l"(p), "l"(pol));
     return v;
 }
-template <bool HINT>
+template <int HINT>
 __device__ __forceinline__ float2 ld_ro(const float2* p, uint64_t pol) {
-    if (!HINT) return __ldg(p);
+    if (HINT == 0) return __ldg(p);
     float2 v;
-    asm volatile("ld.global.nc.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;" : "=f"(v.x), "=f"(v.y) : "l"(p), "l"(pol));
+    if (HINT == 2)
+        asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;" : "=f"(v.x), "=f"(v.y) : "l"(p), "l"(pol));
+    else
+        asm volatile("ld.global.nc.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;" : "=f"(v.x), "=f"(v.y) : "l"(p), "l"(pol));
     return v;
 }
-template <bool HINT>
+template <int HINT>
 __device__ __forceinline__ void st_g(double2* p, double2 v, uint64_t pol) {
     if (!HINT) {
         *p = v;
@@ -104,7 +116,7 @@ __device__ __forceinline__ void st_g(double2* p, double2 v, uint64_t pol) {
     }
     asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1,%2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
 }
-template <bool HINT>
+template <int HINT>
 __device__ __forceinline__ void st_g(float4* p, float4 v, uint64_t pol) {
     if (!HINT) {
         *p = v;
@@ -162,7 +174,7 @@ struct SpinorIO<double, LAYOUT> {
     __device__ __forceinline__ static size_t idx(unsigned V, unsigned s, int k) {
         return LAYOUT == LAYOUT_AOS ? (size_t)s * 12 + k : (size_t)(s >> VL_LOG2) * (12u * VL) + (s & (VL - 1u)) + (unsigned)k * VL;
     }
-    template <bool HINT = false>
+    template <int HINT = 0>
     __device__ __forceinline__ static void load(cplx<double> (&psi)[12], const void* base, unsigned V, unsigned s, uint64_t pol = 0) {
         const double2* p = reinterpret_cast<const double2*>(base);
 #pragma unroll
@@ -171,7 +183,7 @@ struct SpinorIO<double, LAYOUT> {
             psi[k] = {v.x, v.y};
         }
     }
-    template <bool HINT = false>
+    template <int HINT = 0>
     __device__ __forceinline__ static void store(void* base, unsigned V, unsigned s, const cplx<double> (&psi)[12], uint64_t pol = 0) {
         double2* p = reinterpret_cast<double2*>(base);
 #pragma unroll
@@ -183,7 +195,7 @@ struct SpinorIO<float, LAYOUT> {
     __device__ __forceinline__ static size_t idx(unsigned V, unsigned s, int q) {
         return LAYOUT == LAYOUT_AOS ? (size_t)s * 6 + q : (size_t)(s >> VL_LOG2) * (6u * VL) + (s & (VL - 1u)) + (unsigned)q * VL;
     }
-    template <bool HINT = false>
+    template <int HINT = 0>
     __device__ __forceinline__ static void load(cplx<float> (&psi)[12], const void* base, unsigned V, unsigned s, uint64_t pol = 0) {
         const float4* p = reinterpret_cast<const float4*>(base);
 #pragma unroll
@@ -193,7 +205,7 @@ struct SpinorIO<float, LAYOUT> {
             psi[2 * q + 1] = {v.z, v.w};
         }
     }
-    template <bool HINT = false>
+    template <int HINT = 0>
     __device__ __forceinline__ static void store(void* base, unsigned V, unsigned s, const cplx<float> (&psi)[12], uint64_t pol = 0) {
         float4* p = reinterpret_cast<float4*>(base);
 #pragma unroll
@@ -215,7 +227,7 @@ struct vec2<float> {
 
 // Link U_mu(s): 9 complex entries u[row*3+col]; with RECON == 12 only rows 0,1 are stored and row 2
 // is rebuilt as conj(row0 x row1) (exact for SU(3), DESIGN.md Reading R14).
-template <typename Real, int LAYOUT, int RECON, bool HINT = false>
+template <typename Real, int LAYOUT, int RECON, int HINT = 0>
 __device__ __forceinline__ void load_link(cplx<Real> (&u)[9], const void* base, unsigned V, unsigned s, int mu, uint64_t pol = 0) {
     using V2 = typename vec2<Real>::type;
     constexpr int R = (RECON == 12) ? 6 : 9;
@@ -336,7 +348,7 @@ __device__ __forceinline__ void su3_mul(cplx<Real> (&hp)[6], const cplx<Real> (&
 }
 
 // One hop: acc (+)= R_{MU,SIGN}( U^(dagger) P_{MU,SIGN} psi(sn) ), link taken at site sl.
-template <int MU, int SIGN, bool FIRST, typename Real, int LAYOUT, int RECON, bool HINT = false>
+template <int MU, int SIGN, bool FIRST, typename Real, int LAYOUT, int RECON, int HINT = 0>
 __device__ __forceinline__ void hop(cplx<Real> (&acc)[12], const void* in, const void* gauge, unsigned V, unsigned sn,
                                     unsigned sl, uint64_t pol_psi = 0, uint64_t pol_u = 0) {
     cplx<Real> psi[12], h[6], hp[6], u[9];
@@ -349,7 +361,7 @@ __device__ __forceinline__ void hop(cplx<Real> (&acc)[12], const void* in, const
 
 // out(s) for the site with coordinates (x, y, z, t), s = x + L_X*(y + L_Y*(z + L_Z*t)).
 // Neighbour coordinates wrap modulo L_mu (the Kronecker deltas of Eq. 1 on a periodic lattice).
-template <typename Real, int LAYOUT, int RECON, bool HINT = false>
+template <typename Real, int LAYOUT, int RECON, int HINT = 0>
 __device__ __forceinline__ void dslash_site(void* out, const void* in, const void* gauge, const Geom& g, int x, int y,
                                             int z, int t, unsigned s, const Policies& pol = Policies{0, 0, 0, 0}) {
     const unsigned V = g.V;
@@ -364,15 +376,16 @@ __device__ __forceinline__ void dslash_site(void* out, const void* in, const voi
     const unsigned tb = (t == 0) ? s + (unsigned)(g.L[3] - 1) * st : s - st;
 
     cplx<Real> acc[12];
-    hop<0, -1, true, Real, LAYOUT, RECON, HINT>(acc, in, gauge, V, xf, s, pol.psi, pol.u_s);
-    hop<0, +1, false, Real, LAYOUT, RECON, HINT>(acc, in, gauge, V, xb, xb, pol.psi, pol.u_s);
-    hop<1, -1, false, Real, LAYOUT, RECON, HINT>(acc, in, gauge, V, yf, s, pol.psi, pol.u_s);
-    hop<1, +1, false, Real, LAYOUT, RECON, HINT>(acc, in, gauge, V, yb, yb, pol.psi, pol.u_s);
-    hop<2, -1, false, Real, LAYOUT, RECON, HINT>(acc, in, gauge, V, zf, s, pol.psi, pol.u_s);
-    hop<2, +1, false, Real, LAYOUT, RECON, HINT>(acc, in, gauge, V, zb, zb, pol.psi, pol.u_s);
+    hop<0, -1, true, Real, LAYOUT, RECON, (HINT ? 1 : 0)>(acc, in, gauge, V, xf, s, pol.psi, pol.u_s);
+    hop<0, +1, false, Real, LAYOUT, RECON, (HINT ? 1 : 0)>(acc, in, gauge, V, xb, xb, pol.psi, pol.u_s);
+    hop<1, -1, false, Real, LAYOUT, RECON, (HINT ? 1 : 0)>(acc, in, gauge, V, yf, s, pol.psi, pol.u_s);
+    hop<1, +1, false, Real, LAYOUT, RECON, (HINT ? 1 : 0)>(acc, in, gauge, V, yb, yb, pol.psi, pol.u_s);
+    hop<2, -1, false, Real, LAYOUT, RECON, (HINT ? 1 : 0)>(acc, in, gauge, V, zf, s, pol.psi, pol.u_s);
+    hop<2, +1, false, Real, LAYOUT, RECON, (HINT ? 1 : 0)>(acc, in, gauge, V, zb, zb, pol.psi, pol.u_s);
+    // HINT == 2: the t-direction loads bypass L1 allocation (a block's tile is one slice thick in t: no reuse inside the block)
     hop<3, -1, false, Real, LAYOUT, RECON, HINT>(acc, in, gauge, V, tf, s, pol.psi, pol.u_t);
     hop<3, +1, false, Real, LAYOUT, RECON, HINT>(acc, in, gauge, V, tb, tb, pol.psi, pol.u_t);
-    SpinorIO<Real, LAYOUT>::template store<HINT>(out, V, s, acc, pol.out);
+    SpinorIO<Real, LAYOUT>::template store<(HINT ? 1 : 0)>(out, V, s, acc, pol.out);
 }
 
 }  // namespace dslash

@@ -11,7 +11,9 @@
 //   OCCUPANCY 1 / 2   compile-time variants for blocks of <= 128 threads: 1 = 128 registers (16 warps per SM),
 //                     2 = 255 registers (8 warps per SM, deeper load hoisting); 0 = 168 registers (12 warps).
 //   L2_POLICY bits    per-access L2 eviction policies (createpolicy + ld/st .L2::cache_hint): 1 spinor loads evict_last,
-//                     2 U_t loads evict_last, 4 U_x/U_y/U_z loads evict_first, 8 stores of `out` evict_first.
+//                     2 U_t loads evict_last, 4 U_x/U_y/U_z loads evict_first, 8 stores of `out` evict_first,
+//                     16 t-direction loads with L1::no_allocate.
+//   L1_CARVEOUT       preferred shared-memory carve-out in percent (the kernel uses no shared memory: 0 = all L1).
 // See DESIGN.md section 6.
 #include "dslash_kernels.cuh"
 
@@ -21,7 +23,7 @@ struct TunedOpts {
     int l2_policy;  // DSLASH_OPT_L2_POLICY bits
 };
 
-template <typename Real, int LAYOUT, int RECON, int MAXTPB, int MINBLK, bool HINT>
+template <typename Real, int LAYOUT, int RECON, int MAXTPB, int MINBLK, int HINT>
 __global__ void __launch_bounds__(MAXTPB, MINBLK)
     dslash_tuned_kernel(void* __restrict__ out, const void* __restrict__ in, const void* __restrict__ gauge, Geom g,
                         TileGeom tg, TunedOpts opt) {
@@ -54,13 +56,22 @@ __global__ void __launch_bounds__(MAXTPB, MINBLK)
     dslash_site<Real, LAYOUT, RECON, HINT>(out, in, gauge, g, x, y, z, t, s, pol);
 }
 
-template <typename Real, int LAYOUT, int RECON, bool HINT>
+template <typename Real, int LAYOUT, int RECON, int HINT>
 static cudaError_t launch_tuned_s(const LaunchArgs& a, const TileGeom& tg, const TunedConfig& cfg) {
     const int tpb = 1 << (tg.lb[0] + tg.lb[1] + tg.lb[2] + tg.lb[3]);
     const unsigned grid = (unsigned)tg.nt[0] * (unsigned)tg.nt[1] * (unsigned)tg.nt[2] * (unsigned)tg.nt[3];
     TunedOpts o{cfg.l2_policy};
-#define DSLASH_LAUNCH(MAXTPB, MINBLK) \
-    dslash_tuned_kernel<Real, LAYOUT, RECON, MAXTPB, MINBLK, HINT><<<grid, tpb, 0, a.stream>>>(a.out, a.in, a.gauge, a.geom, tg, o)
+#define DSLASH_LAUNCH(MAXTPB, MINBLK)                                                                                        \
+    do {                                                                                                                     \
+        static int carve_set = -1;                                                                                           \
+        if (carve_set != cfg.l1_carveout) {                                                                                  \
+            cudaFuncSetAttribute(dslash_tuned_kernel<Real, LAYOUT, RECON, MAXTPB, MINBLK, HINT>,                             \
+                                 cudaFuncAttributePreferredSharedMemoryCarveout, cfg.l1_carveout);                          \
+            carve_set = cfg.l1_carveout;                                                                                     \
+        }                                                                                                                    \
+        dslash_tuned_kernel<Real, LAYOUT, RECON, MAXTPB, MINBLK, HINT><<<grid, tpb, 0, a.stream>>>(a.out, a.in, a.gauge,     \
+                                                                                                   a.geom, tg, o);         \
+    } while (0)
     if (tpb <= 128) {
         if (cfg.occupancy == 1)
             DSLASH_LAUNCH(128, 4);
@@ -80,8 +91,8 @@ static cudaError_t launch_tuned_s(const LaunchArgs& a, const TileGeom& tg, const
 
 template <typename Real, int LAYOUT, int RECON>
 static cudaError_t launch_tuned_t(const LaunchArgs& a, const TileGeom& tg, const TunedConfig& cfg) {
-    return cfg.l2_policy ? launch_tuned_s<Real, LAYOUT, RECON, true>(a, tg, cfg)
-                                : launch_tuned_s<Real, LAYOUT, RECON, false>(a, tg, cfg);
+    if (cfg.l2_policy & 16) return launch_tuned_s<Real, LAYOUT, RECON, 2>(a, tg, cfg);
+    return cfg.l2_policy ? launch_tuned_s<Real, LAYOUT, RECON, 1>(a, tg, cfg) : launch_tuned_s<Real, LAYOUT, RECON, 0>(a, tg, cfg);
 }
 
 template <typename Real>
