@@ -213,6 +213,8 @@ def run_cuda(args, cfg):
                 B.dslash_set_option(lat.ctx, B.DSLASH_OPT_OCCUPANCY, args.occupancy)
             if args.kernel:
                 lat.set_kernel(args.kernel)
+            if args.x_shuffle is not None:
+                B.dslash_set_option(lat.ctx, B.DSLASH_OPT_X_SHUFFLE, args.x_shuffle)
             gd, pd, od = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
             n0 = B.dslash_launch_count(lat.ctx)
             ms, ck = time_applies(torch, lat, od, pd, gd, args.steps, args.warmup, group, local)
@@ -223,7 +225,8 @@ def run_cuda(args, cfg):
                                 gbs=bps * v / (ms / args.steps) / 1e6, bps=bps, recon12=recon12,
                                 tile=list(B.dslash_get_tile(lat.ctx)),
                                 kernel={B.DSLASH_KERNEL_DIRECT: "direct", B.DSLASH_KERNEL_TMA: "tma"}[B.dslash_get_kernel(lat.ctx)],
-                                occupancy=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_OCCUPANCY))
+                                occupancy=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_OCCUPANCY),
+                                x_shuffle=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_X_SHUFFLE))
             if tag == "main":
                 clocks, launches = ck, n1 - n0 - args.warmup
                 if args.sustained_steps > 0:
@@ -282,7 +285,8 @@ def run_cuda(args, cfg):
             "warmup": args.warmup, "ms_per_step": main["ms_per_step"], "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": prec, "data": "synthetic",
             "config": {"workload": cfg["name"], "dims": list(dims), "layout": args.layout, "recon": 12 if main["recon12"] else 18,
-                       "tile": main["tile"], "kernel": main["kernel"], "occupancy_option": main["occupancy"], "sites": v, "parallelism": "replicas x%d" % world,
+                       "tile": main["tile"], "kernel": main["kernel"], "occupancy_option": main["occupancy"],
+                       "x_shuffle_option": main["x_shuffle"], "sites": v, "parallelism": "replicas x%d" % world,
                        "l2": "inputs larger than L2: %.2f GB working set per apply vs 126 MB L2, no flush needed"
                              % (main["bps"] * v / 1e9)},
             "hbm_gbs": main["gbs"], "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "clocks": clocks,
@@ -587,6 +591,7 @@ def main():
     ap.add_argument("--tile", type=int, nargs=4, default=None, help="tile of the tuned kernel (x y z t)")
     ap.add_argument("--occupancy", type=int, default=None, help="DSLASH_OPT_OCCUPANCY override")
     ap.add_argument("--kernel", choices=["auto", "direct", "tma"], default=None)
+    ap.add_argument("--x-shuffle", type=int, choices=[0, 1], default=None, help="DSLASH_OPT_X_SHUFFLE override")
     ap.add_argument("--both-recon", action="store_true", default=True, help="also time the other link compression")
     ap.add_argument("--one-recon", dest="both_recon", action="store_false")
     ap.add_argument("--no-e2e", action="store_true")

@@ -111,6 +111,10 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
                                          4 U_x/U_y/U_z loads evict_first, 8 stores of `out` evict_first,
                                          16 t-direction loads bypass L1 allocation (0: none) */
 #define DSLASH_OPT_L1_CARVEOUT 4      /* direct kernel: preferred shared-memory carve-out in percent, -1 = driver default */
+#define DSLASH_OPT_X_SHUFFLE 5        /* direct kernel: 1 (default for FP64; FP32 defaults to 0) = when a whole x row sits inside one warp
+                                         (tile x-extent == L_X, a power of two <= 32) the two x hops are exchanged between
+                                         lanes by warp shuffles instead of loaded; 0 = always load them.  Same result, bit
+                                         for bit */
 
 /* host<->device mapping modes of dslash_apply_host() (section 4.1.2) */
 #define DSLASH_MAP_MINIMAL 0 /* to: gauge, in;  from: out            (after the Advisor's data analysis) */

@@ -36,7 +36,9 @@ struct TunedConfig {
     int occupancy;         // 0: default register budget, 1: 128-register variant
     int l2_policy;         // DSLASH_OPT_L2_POLICY bits (0: no cache hints)
     int l1_carveout;       // preferred shared-memory carve-out of the direct kernel in percent (-1: driver default)
+    int x_shuffle;         // 1: exchange the x hops inside the warp when the tile allows it (fp64 default), 0: always load them
 };
+bool x_shuffle_eligible(const Geom& g, const TileGeom& tg);
 
 // Tuned kernel (direct, register-staged).
 cudaError_t launch_tuned(int precision, int layout_base, int recon, const LaunchArgs& a, const TileGeom& tg,

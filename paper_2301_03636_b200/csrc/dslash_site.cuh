@@ -359,11 +359,54 @@ __device__ __forceinline__ void hop(cplx<Real> (&acc)[12], const void* in, const
     reconstruct_accumulate<MU, SIGN, FIRST>(acc, hp);
 }
 
+// ------------------------------------------------------------------ x hops exchanged inside the warp
+// When a whole x row lives in one warp (tile x-extent == L_X, a power of two <= 32, so lane bits [0, log2 L_X) are the
+// x coordinate and x+-1 wraps inside the row), the two x hops need no neighbour loads at all.  Each thread loads its OWN
+// psi(s) and U_x(s) once (aligned, 21 loads instead of 42 shifted ones) and computes the two half-spinors its neighbours
+// want from it:   hm = P^-_x psi(s)                (the site at x-1 multiplies it by its own U_x: forward hop there)
+//                 w  = U_x(s)^dagger P^+_x psi(s)  (the complete backward-hop contribution of the site at x+1)
+// and the warp rotates them by one lane with shuffles.  The arithmetic per site is the same as two hop<> calls (two
+// projections, two SU(3) products), and so is the result, bit for bit; with RECON == 12 row 2 of U_x(s) is rebuilt once
+// instead of twice.  Measured on 32^3x64 fp64: 0.351 -> 0.331 ms (profiles/).
+__device__ __forceinline__ double shfl_(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
+__device__ __forceinline__ float shfl_(float v, int src) { return __shfl_sync(0xffffffffu, v, src); }
+
+// lanes holding the x+1 / x-1 neighbours of this thread's site (wrap inside the row segment of the warp)
+__device__ __forceinline__ void x_shuffle_lanes(int LX, int& lane_fwd, int& lane_bwd) {
+    const int lane = (int)(threadIdx.x & 31u), m = LX - 1;
+    lane_fwd = (lane & ~m) | ((lane + 1) & m);
+    lane_bwd = (lane & ~m) | ((lane - 1) & m);
+}
+
+template <typename Real, int LAYOUT, int RECON, int HINT = 0>
+__device__ __forceinline__ void x_hops_shuffle(cplx<Real> (&acc)[12], const void* in, const void* gauge, unsigned V, unsigned s,
+                                               int lane_fwd, int lane_bwd, uint64_t pol_psi = 0, uint64_t pol_u = 0) {
+    cplx<Real> psi[12], u[9], hm[6], hq[6], w[6], hp[6];
+    SpinorIO<Real, LAYOUT>::template load<HINT>(psi, in, V, s, pol_psi);
+    load_link<Real, LAYOUT, RECON, HINT>(u, gauge, V, s, 0, pol_u);
+    project<0, -1>(hm, psi);
+    project<0, +1>(hq, psi);
+    su3_mul<true>(w, u, hq);
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        hm[k].re = shfl_(hm[k].re, lane_fwd);
+        hm[k].im = shfl_(hm[k].im, lane_fwd);
+        w[k].re = shfl_(w[k].re, lane_bwd);
+        w[k].im = shfl_(w[k].im, lane_bwd);
+    }
+    su3_mul<false>(hp, u, hm);
+    reconstruct_accumulate<0, -1, true>(acc, hp);
+    reconstruct_accumulate<0, +1, false>(acc, w);
+}
+
 // out(s) for the site with coordinates (x, y, z, t), s = x + L_X*(y + L_Y*(z + L_Z*t)).
 // Neighbour coordinates wrap modulo L_mu (the Kronecker deltas of Eq. 1 on a periodic lattice).
-template <typename Real, int LAYOUT, int RECON, int HINT = 0>
+// XSHFL: the x hops come from x_hops_shuffle (every lane of the warp must make the call; `active` = false lanes
+// compute on a clamped site and skip the store).
+template <typename Real, int LAYOUT, int RECON, int HINT = 0, bool XSHFL = false>
 __device__ __forceinline__ void dslash_site(void* out, const void* in, const void* gauge, const Geom& g, int x, int y,
-                                            int z, int t, unsigned s, const Policies& pol = Policies{0, 0, 0, 0}) {
+                                            int z, int t, unsigned s, const Policies& pol = Policies{0, 0, 0, 0},
+                                            bool active = true) {
     const unsigned V = g.V;
     const unsigned sx = 1u, sy = (unsigned)g.L[0], sz = sy * (unsigned)g.L[1], st = sz * (unsigned)g.L[2];
     const unsigned xf = (x + 1 == g.L[0]) ? s - (unsigned)(g.L[0] - 1) * sx : s + sx;
@@ -376,8 +419,14 @@ __device__ __forceinline__ void dslash_site(void* out, const void* in, const voi
     const unsigned tb = (t == 0) ? s + (unsigned)(g.L[3] - 1) * st : s - st;
 
     cplx<Real> acc[12];
-    hop<0, -1, true, Real, LAYOUT, RECON, (HINT ? 1 : 0)>(acc, in, gauge, V, xf, s, pol.psi, pol.u_s);
-    hop<0, +1, false, Real, LAYOUT, RECON, (HINT ? 1 : 0)>(acc, in, gauge, V, xb, xb, pol.psi, pol.u_s);
+    if (XSHFL) {
+        int lane_fwd, lane_bwd;
+        x_shuffle_lanes(g.L[0], lane_fwd, lane_bwd);
+        x_hops_shuffle<Real, LAYOUT, RECON, (HINT ? 1 : 0)>(acc, in, gauge, V, s, lane_fwd, lane_bwd, pol.psi, pol.u_s);
+    } else {
+        hop<0, -1, true, Real, LAYOUT, RECON, (HINT ? 1 : 0)>(acc, in, gauge, V, xf, s, pol.psi, pol.u_s);
+        hop<0, +1, false, Real, LAYOUT, RECON, (HINT ? 1 : 0)>(acc, in, gauge, V, xb, xb, pol.psi, pol.u_s);
+    }
     hop<1, -1, false, Real, LAYOUT, RECON, (HINT ? 1 : 0)>(acc, in, gauge, V, yf, s, pol.psi, pol.u_s);
     hop<1, +1, false, Real, LAYOUT, RECON, (HINT ? 1 : 0)>(acc, in, gauge, V, yb, yb, pol.psi, pol.u_s);
     hop<2, -1, false, Real, LAYOUT, RECON, (HINT ? 1 : 0)>(acc, in, gauge, V, zf, s, pol.psi, pol.u_s);
@@ -385,7 +434,7 @@ __device__ __forceinline__ void dslash_site(void* out, const void* in, const voi
     // HINT == 2: the t-direction loads bypass L1 allocation (a block's tile is one slice thick in t: no reuse inside the block)
     hop<3, -1, false, Real, LAYOUT, RECON, HINT>(acc, in, gauge, V, tf, s, pol.psi, pol.u_t);
     hop<3, +1, false, Real, LAYOUT, RECON, HINT>(acc, in, gauge, V, tb, tb, pol.psi, pol.u_t);
-    SpinorIO<Real, LAYOUT>::template store<(HINT ? 1 : 0)>(out, V, s, acc, pol.out);
+    if (active) SpinorIO<Real, LAYOUT>::template store<(HINT ? 1 : 0)>(out, V, s, acc, pol.out);
 }
 
 }  // namespace dslash

@@ -23,7 +23,15 @@ struct TunedOpts {
     int l2_policy;  // DSLASH_OPT_L2_POLICY bits
 };
 
-template <typename Real, int LAYOUT, int RECON, int MAXTPB, int MINBLK, int HINT>
+// A whole x row inside one warp: tile x-extent == L_X, L_X a power of two <= 32 (the tile has >= 32 threads and
+// x is its fastest thread index, so lane bits [0, log2 L_X) are the x coordinate).
+bool x_shuffle_eligible(const Geom& g, const TileGeom& tg) {
+    const int lx = g.L[0];
+    return lx <= 32 && (lx & (lx - 1)) == 0 && (1 << tg.lb[0]) == lx &&
+           (tg.lb[0] + tg.lb[1] + tg.lb[2] + tg.lb[3]) >= 5;
+}
+
+template <typename Real, int LAYOUT, int RECON, int MAXTPB, int MINBLK, int HINT, bool XSHFL>
 __global__ void __launch_bounds__(MAXTPB, MINBLK)
     dslash_tuned_kernel(void* __restrict__ out, const void* __restrict__ in, const void* __restrict__ gauge, Geom g,
                         TileGeom tg, TunedOpts opt) {
@@ -39,12 +47,22 @@ __global__ void __launch_bounds__(MAXTPB, MINBLK)
     unsigned r = threadIdx.x;
     const int x = (int)((bx << tg.lb[0]) + (r & ((1u << tg.lb[0]) - 1u)));
     r >>= tg.lb[0];
-    const int y = (int)((by << tg.lb[1]) + (r & ((1u << tg.lb[1]) - 1u)));
+    int y = (int)((by << tg.lb[1]) + (r & ((1u << tg.lb[1]) - 1u)));
     r >>= tg.lb[1];
-    const int z = (int)((bz << tg.lb[2]) + (r & ((1u << tg.lb[2]) - 1u)));
+    int z = (int)((bz << tg.lb[2]) + (r & ((1u << tg.lb[2]) - 1u)));
     r >>= tg.lb[2];
-    const int t = tg.t_begin + (int)((bt << tg.lb[3]) + r);
-    if (x >= g.L[0] || y >= g.L[1] || z >= g.L[2] || t >= tg.t_end) return;
+    int t = tg.t_begin + (int)((bt << tg.lb[3]) + r);
+    const bool active = !(x >= g.L[0] || y >= g.L[1] || z >= g.L[2] || t >= tg.t_end);
+    if (!XSHFL) {
+        if (!active) return;
+    } else {
+        // the warp shuffles of the x hops need every lane: rows beyond a ragged tile edge compute a clamped site and do
+        // not store (x is always in range: the tile's x-extent is L_X)
+        if (__all_sync(0xffffffffu, !active)) return;
+        y = min(y, g.L[1] - 1);
+        z = min(z, g.L[2] - 1);
+        t = min(t, tg.t_end - 1);
+    }
     const unsigned s = (unsigned)x + (unsigned)g.L[0] * ((unsigned)y + (unsigned)g.L[1] * ((unsigned)z + (unsigned)g.L[2] * (unsigned)t));
     Policies pol{0, 0, 0, 0};
     if (HINT) {
@@ -53,10 +71,10 @@ __global__ void __launch_bounds__(MAXTPB, MINBLK)
         pol.u_s = make_policy((opt.l2_policy & 4) ? POLICY_EVICT_FIRST : POLICY_NORMAL);
         pol.out = make_policy((opt.l2_policy & 8) ? POLICY_EVICT_FIRST : POLICY_NORMAL);
     }
-    dslash_site<Real, LAYOUT, RECON, HINT>(out, in, gauge, g, x, y, z, t, s, pol);
+    dslash_site<Real, LAYOUT, RECON, HINT, XSHFL>(out, in, gauge, g, x, y, z, t, s, pol, active);
 }
 
-template <typename Real, int LAYOUT, int RECON, int HINT>
+template <typename Real, int LAYOUT, int RECON, int HINT, bool XSHFL>
 static cudaError_t launch_tuned_s(const LaunchArgs& a, const TileGeom& tg, const TunedConfig& cfg) {
     const int tpb = 1 << (tg.lb[0] + tg.lb[1] + tg.lb[2] + tg.lb[3]);
     const unsigned grid = (unsigned)tg.nt[0] * (unsigned)tg.nt[1] * (unsigned)tg.nt[2] * (unsigned)tg.nt[3];
@@ -65,12 +83,13 @@ static cudaError_t launch_tuned_s(const LaunchArgs& a, const TileGeom& tg, const
     do {                                                                                                                     \
         static int carve_set = -1;                                                                                           \
         if (carve_set != cfg.l1_carveout) {                                                                                  \
-            cudaFuncSetAttribute(dslash_tuned_kernel<Real, LAYOUT, RECON, MAXTPB, MINBLK, HINT>,                             \
+            cudaFuncSetAttribute(dslash_tuned_kernel<Real, LAYOUT, RECON, MAXTPB, MINBLK, HINT, XSHFL>,                             \
                                  cudaFuncAttributePreferredSharedMemoryCarveout, cfg.l1_carveout);                          \
             carve_set = cfg.l1_carveout;                                                                                     \
         }                                                                                                                    \
-        dslash_tuned_kernel<Real, LAYOUT, RECON, MAXTPB, MINBLK, HINT><<<grid, tpb, 0, a.stream>>>(a.out, a.in, a.gauge,     \
-                                                                                                   a.geom, tg, o);         \
+        dslash_tuned_kernel<Real, LAYOUT, RECON, MAXTPB, MINBLK, HINT, XSHFL><<<grid, tpb, 0, a.stream>>>(a.out, a.in,        \
+                                                                                                          a.gauge, a.geom, \
+                                                                                                          tg, o);          \
     } while (0)
     if (tpb <= 128) {
         if (cfg.occupancy == 1)
@@ -91,8 +110,11 @@ static cudaError_t launch_tuned_s(const LaunchArgs& a, const TileGeom& tg, const
 
 template <typename Real, int LAYOUT, int RECON>
 static cudaError_t launch_tuned_t(const LaunchArgs& a, const TileGeom& tg, const TunedConfig& cfg) {
-    if (cfg.l2_policy & 16) return launch_tuned_s<Real, LAYOUT, RECON, 2>(a, tg, cfg);
-    return cfg.l2_policy ? launch_tuned_s<Real, LAYOUT, RECON, 1>(a, tg, cfg) : launch_tuned_s<Real, LAYOUT, RECON, 0>(a, tg, cfg);
+    if (cfg.l2_policy & 16) return launch_tuned_s<Real, LAYOUT, RECON, 2, false>(a, tg, cfg);
+    if (cfg.l2_policy) return launch_tuned_s<Real, LAYOUT, RECON, 1, false>(a, tg, cfg);
+    // x hops by warp shuffle when a whole x row sits inside one warp (see x_hops_shuffle in dslash_site.cuh)
+    if (cfg.x_shuffle && x_shuffle_eligible(a.geom, tg)) return launch_tuned_s<Real, LAYOUT, RECON, 0, true>(a, tg, cfg);
+    return launch_tuned_s<Real, LAYOUT, RECON, 0, false>(a, tg, cfg);
 }
 
 template <typename Real>

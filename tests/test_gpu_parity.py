@@ -97,6 +97,38 @@ def test_tuned_kernel_every_tile_shape(env, tile):
         assert gpu_vs_ref(env, lat, g, p, ref) <= TOL["f64"]
 
 
+# ---------------------------------------------------------------- x hops by warp shuffle (DSLASH_OPT_X_SHUFFLE)
+@pytest.mark.parametrize("dims,tile", [
+    ((32, 3, 5, 2), (32, 2, 2, 1)),   # one row per warp, ragged tiles in y and z (clamped rows that do not store)
+    ((32, 4, 2, 3), (32, 1, 1, 2)),   # ragged in t
+    ((16, 3, 3, 3), (16, 2, 2, 1)),   # two rows per warp, one of them beyond the edge in some warps
+    ((8, 5, 3, 2), (8, 4, 2, 1)),     # four rows per warp
+    ((4, 6, 2, 5), (4, 4, 2, 2)),
+    ((2, 3, 2, 5), (2, 4, 2, 4)),     # L_X = 2: x+1 and x-1 are the same lane
+    ((1, 2, 3, 4), (1, 2, 4, 4)),     # L_X = 1: the neighbour is the site itself
+    ((16, 4, 4, 4), (16, 4, 4, 4)),   # 1024-thread tile
+])
+@pytest.mark.parametrize("precision", ["f64", "f32"])
+def test_x_shuffle_kernel_matches_the_oracle_and_the_loading_kernel_bit_for_bit(env, dims, tile, precision):
+    g, p, ref, _ = fields_and_ref(env, dims, SEED + 14, precision)
+    for layout, recon12 in ALL_MODES:
+        with env.device.Lattice(dims, precision, layout, recon12) as lat:
+            lat.set_tile(tile)
+            assert env.B.dslash_get_option(lat.ctx, env.B.DSLASH_OPT_X_SHUFFLE) == (1 if precision == "f64" else 0)  # default
+            gi, pi = lat.upload_gauge(g), lat.upload_spinor(p)
+            outs = {}
+            for on in (1, 0):
+                env.B.dslash_set_option(lat.ctx, env.B.DSLASH_OPT_X_SHUFFLE, on)
+                o = lat.new_spinor()
+                o.fill_(0x7f)  # a site the kernel forgot to store would stay NaN-like garbage
+                lat.apply(o, pi, gi)
+                outs[on] = lat.download_spinor(o)
+                assert env.checks.parity_error(outs[on], ref) <= TOL[precision], (layout, recon12, on)
+            # same arithmetic in the same order; with 12-real links the shuffle path rebuilds row 2 of U_x(s) once for
+            # both hops, from the same two rows: still the same bits
+            assert np.array_equal(outs[1], outs[0]), (layout, recon12)
+
+
 # ---------------------------------------------------------------- the TMA-staged kernel (SoA), selected explicitly
 @pytest.mark.parametrize("dims,tile", [
     ((32, 4, 4, 4), (32, 2, 2, 1)), ((32, 4, 4, 4), (32, 1, 2, 2)), ((32, 4, 4, 4), (32, 4, 1, 1)), ((32, 4, 4, 4), (32, 1, 1, 1)),
