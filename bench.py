@@ -45,8 +45,8 @@ CONFIGS = {
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture (profiles/); None until captured for that workload.
 NCU_TRAFFIC_BYTES = {
-    # profiles/r01_ncu_tuned_kernel.txt, capture r01b: 1.6467 GB read + 0.3914 GB written (mean of 2 launches)
-    "32x32x32x64_f64_soa_r18": 2037656000,
+    # profiles/r01_ncu_tuned_kernel.txt, capture r01c: 1.6424 GB read + 0.3903 GB written (mean of 2 launches)
+    "32x32x32x64_f64_soa_r18": 2032698000,
 }
 
 

@@ -92,6 +92,40 @@ def wilson(psi: np.ndarray, gauge: np.ndarray, dims, mass: float, dagger: bool =
     return (4.0 + float(mass)) * np.ascontiguousarray(psi, dtype=np.float64).reshape(d.shape) - 0.5 * d
 
 
+def parity_mask(dims) -> np.ndarray:
+    """bool [T, Z, Y, X]: True on the odd sites, (x + y + z + t) mod 2 == 1."""
+    lx, ly, lz, lt = (int(d) for d in dims)
+    t, z, y, x = np.meshgrid(np.arange(lt), np.arange(lz), np.arange(ly), np.arange(lx), indexing="ij")
+    return ((x + y + z + t) & 1).astype(bool)
+
+
+def dslash_parity(psi: np.ndarray, gauge: np.ndarray, dims, out_parity: int, dagger: bool = False, nthreads: int = 0) -> np.ndarray:
+    """The checkerboarded hopping term by its definition: restrict Eq. 1 to input on the sites of parity 1 - out_parity and
+    output on the sites of parity out_parity (all extents even, so every neighbour of a site has the other parity):
+        D_{p,1-p} = P_p D P_{1-p},   P_p = projector on the sites with (x+y+z+t) mod 2 == p.
+    Takes and returns full-lattice arrays; entries outside the respective parity are ignored / returned as 0."""
+    if any(int(d) % 2 for d in dims):
+        raise ValueError("even-odd decomposition needs even extents")
+    odd = parity_mask(dims)
+    keep_in = odd if out_parity == 0 else ~odd
+    src = np.ascontiguousarray(psi, dtype=np.float64).reshape(odd.shape + (4, 3, 2)) * keep_in[..., None, None, None]
+    d = (dslash_dagger if dagger else dslash)(src, gauge, dims, nthreads)
+    return d * (~keep_in)[..., None, None, None]
+
+
+def schur_even(psi: np.ndarray, gauge: np.ndarray, dims, mass: float, dagger: bool = False, nthreads: int = 0) -> np.ndarray:
+    """The even-odd preconditioned Wilson matrix on the even sites: the Schur complement of M = (4+m) - D/2 with respect
+    to its odd-odd block (4+m)*1,
+        Mhat = (4+m) - D_eo D_oe / (4 (4+m))        (dagger: with D^dagger in both factors),
+    written as the two restricted applications it is.  Full-lattice arrays; odd-site entries of the result are 0."""
+    a = 4.0 + float(mass)
+    even = ~parity_mask(dims)
+    pe = np.ascontiguousarray(psi, dtype=np.float64).reshape(even.shape + (4, 3, 2)) * even[..., None, None, None]
+    t_o = dslash_parity(pe, gauge, dims, 1, dagger, nthreads)   # D_oe psi_e
+    t_e = dslash_parity(t_o, gauge, dims, 0, dagger, nthreads)  # D_eo D_oe psi_e
+    return a * pe - t_e / (4.0 * a)
+
+
 def dslash_sites(psi: np.ndarray, gauge: np.ndarray, dims, sites, nthreads: int = 0) -> np.ndarray:
     """(D psi)(s) for the linear site indices `sites`; returns float64 [n, 4, 3, 2]."""
     psi, gauge, cdims, _, _ = _check(psi, gauge, dims)
