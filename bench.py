@@ -578,6 +578,73 @@ def run_cg(args):
     return 0
 
 
+def run_eo(args):
+    """Even-odd (checkerboarded) form on a BASELINE lattice: time of one D_{eo} application and of the Schur complement Mhat,
+    then dslash_eo_solve (M x = b through Mhat) beside dslash_cg_solve on the same right-hand side."""
+    import torch
+    from paper_2301_03636_b200 import binding as B
+    from paper_2301_03636_b200 import device, inputs
+    cfg = CONFIGS[args.config]
+    dims, prec = cfg["dims"], cfg["precision"]
+    v = inputs.volume(dims)
+    rb = 8 if prec == "f64" else 4
+    g, b = inputs.fields(dims, SEED + 7, prec, check=False)
+    with device.Lattice(dims, prec, args.layout, cfg["recon12"]) as lat:
+        ge = lat.upload_eo_gauge(g)
+        be, bo = lat.upload_eo_spinor(b, 0), lat.upload_eo_spinor(b, 1)
+        xe, xo, tmp = lat.new_eo_spinor(), lat.new_eo_spinor(), lat.new_eo_spinor()
+
+        def timed(fn, steps, warmup):
+            for _ in range(warmup):
+                fn()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(steps):
+                fn()
+            e1.record()
+            torch.cuda.synchronize()
+            return e0.elapsed_time(e1) / steps
+
+        ms_d = timed(lambda: lat.eo_apply(0, 0, xe, bo, ge), args.steps, args.warmup)
+        ms_m = timed(lambda: lat.eo_apply_schur(0, args.cg_mass, xe, be, tmp, ge), args.steps, args.warmup)
+        # one D_{p,1-p}: V/2 output sites x 1320 flop; bytes: in half + all links (forward links of the output parity, backward
+        # links of the input parity) + out half
+        link_b = (12 if cfg["recon12"] else 18) * 4 * rb
+        bytes_d = v * (24 * rb // 2 + link_b + 24 * rb // 2)
+        lat.eo_solve(xe, xo, be, bo, ge, args.cg_mass, 1e-2, 5)  # warm-up (allocates the work fields)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n0 = B.dslash_launch_count(lat.ctx)
+        e0.record()
+        iters, rel = lat.eo_solve(xe, xo, be, bo, ge, args.cg_mass, args.cg_tol, args.cg_max_iter)
+        e1.record()
+        torch.cuda.synchronize()
+        ms_solve, launches = e0.elapsed_time(e1), B.dslash_launch_count(lat.ctx) - n0
+        del ge
+        gd, bd, xd = lat.upload_gauge(g), lat.upload_spinor(b), lat.new_spinor()
+        lat.cg_solve(xd, bd, gd, args.cg_mass, 1e-2, 5)
+        torch.cuda.synchronize()
+        e0.record()
+        iters_plain, rel_plain = lat.cg_solve(xd, bd, gd, args.cg_mass, args.cg_tol, args.cg_max_iter)
+        e1.record()
+        torch.cuda.synchronize()
+        ms_plain = e0.elapsed_time(e1)
+        line = {"eo": "checkerboarded Dslash, Schur complement, dslash_eo_solve", "workload": cfg["name"], "dims": list(dims),
+                "mass": args.cg_mass, "tol": args.cg_tol,
+                "d_eo": {"ms": ms_d, "gflops": 1320 * (v // 2) / ms_d / 1e6, "algorithmic_gbs": bytes_d / ms_d / 1e6,
+                         "algorithmic_bytes": bytes_d},
+                "mhat": {"ms": ms_m, "gflops": (2 * 1320 + 72) * (v // 2) / ms_m / 1e6,
+                         "algorithmic_gbs": (2 * bytes_d + v // 2 * 24 * rb) / ms_m / 1e6},
+                "eo_solve": {"iterations": iters, "rel_residual": rel, "ms_total": ms_solve, "ms_per_iteration": ms_solve / max(iters, 1),
+                             "gpu_launches": int(launches)},
+                "plain_cg": {"iterations": iters_plain, "rel_residual": rel_plain, "ms_total": ms_plain,
+                             "ms_per_iteration": ms_plain / max(iters_plain, 1)},
+                "speedup_vs_plain_cg": ms_plain / ms_solve, "dtype": prec, "data": "synthetic"}
+        print(json.dumps(line))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -608,6 +675,7 @@ def main():
     ap.add_argument("--advisor-csv", default=os.path.join(ROOT, "gpurun_out", "advisor_variants.csv"))
     ap.add_argument("--team-size", type=int, default=128)
     ap.add_argument("--cg", action="store_true", help="time dslash_cg_solve on the --config lattice")
+    ap.add_argument("--eo", action="store_true", help="time the even-odd operator, Mhat and dslash_eo_solve on the --config lattice")
     ap.add_argument("--cg-mass", type=float, default=0.2)
     ap.add_argument("--cg-tol", type=float, default=1e-8)
     ap.add_argument("--cg-max-iter", type=int, default=2000)
@@ -620,6 +688,8 @@ def main():
         return run_advisor(args)
     if args.cg:
         return run_cg(args)
+    if args.eo:
+        return run_eo(args)
     cfg = CONFIGS[args.config]
     if args.impl == "reference":
         return run_reference(args, cfg)

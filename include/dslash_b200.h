@@ -257,6 +257,53 @@ DSLASH_API int dslash_cg_solve(dslash_ctx *ctx, void *x, const void *b, const vo
                                int *iterations, double *rel_residual, dslash_stream_t stream);
 
 /*
+ * Even-odd (checkerboarded) form of Eq. 1 (PAPER.md:52 calls Eq. 1 the
+ * "unpreconditioned" operator -- this is the preconditioned one).  Requires every extent to be even: then Eq. 1 couples
+ * a site only to sites of the other parity, parity(x) = (x+y+z+t) mod 2, 0 = even, and
+ *     D_{p,1-p} = P_p D P_{1-p}                           (P_p = projector on the sites of parity p)
+ *     Mhat = (4+mass) - D_eo D_oe / (4 (4+mass))          (Schur complement of M = (4+mass) - D/2 on the even sites)
+ * Solving M x = b then reduces to  Mhat x_e = b_e + D_eo b_o / (2 (4+mass)),  x_o = (b_o + D_oe x_e / 2) / (4+mass).
+ *
+ * Checkerboard layout: the site s of parity p has the half-index h = s >> 1 (L_X is even), s = 2h + ((p+y+z+t) & 1).
+ *   half-lattice spinor   a native spinor field (the ctx's AoS or blocked-SoA formulas) over the V/2 "sites" h of one parity;
+ *                         dslash_eo_spinor_bytes() bytes.
+ *   checkerboarded gauge  two native gauge fields over h, the links U_mu(s) of the even sites first, then (at byte offset
+ *                         dslash_eo_gauge_bytes()/2) those of the odd sites; rows 0,1 only with DSLASH_RECON12.
+ * dslash_eo_pack_spinor / _unpack_spinor / _pack_gauge convert from / to the canonical full-lattice arrays (device
+ * pointers; unpack writes only the sites of `parity` and leaves the others untouched).
+ *
+ * dslash_eo_apply        out = D_{p,1-p} in (dagger = 1: D^dagger), p = out_parity; `in` lives on parity 1-p.
+ * dslash_eo_apply_xpay   out = a * c + b * D_{p,1-p} in;  c = half-lattice field of parity p, only read; it must not
+ *                        overlap out.
+ * dslash_eo_apply_schur  out_even = Mhat in_even (dagger = 1: Mhat^dagger); tmp_odd = caller's half-lattice scratch field.
+ *                        Two launches, the axpy fused into the second.
+ * dslash_eo_cg_solve     conjugate gradients on Mhat^dagger Mhat x_even = b_even (same conventions, determinism and error
+ *                        behaviour as dslash_cg_solve; the ctx owns five half-lattice work fields).
+ * dslash_eo_solve        solves the full Wilson system M x = b through the preconditioned one: forms the right-hand side
+ *                        above, runs dslash_eo_cg_solve on Mhat^dagger Mhat x_e = Mhat^dagger (.), reconstructs x_o.  x and b are
+ *                        given as their even and odd halves (four distinct half-lattice fields); rel_residual is that of the
+ *                        normal equations.  7 launches around the CG.
+ * All asynchronous on `stream` except dslash_eo_cg_solve / dslash_eo_solve, which synchronise it.
+ * Errors: NULL, DIMS (an extent is odd), UNSUPPORTED (parity/dagger not 0/1, 4+mass == 0, tol, max_iter), ALIGN,
+ * ALIAS (out overlaps in; x overlaps b), NOMEM, CUDA.  dslash_eo_*_bytes return 0 when an extent is odd.
+ */
+DSLASH_API size_t dslash_eo_spinor_bytes(const dslash_ctx *ctx);
+DSLASH_API size_t dslash_eo_gauge_bytes(const dslash_ctx *ctx);
+DSLASH_API int dslash_eo_pack_spinor(dslash_ctx *ctx, void *dst_half, const void *src_canonical, int parity, dslash_stream_t stream);
+DSLASH_API int dslash_eo_unpack_spinor(dslash_ctx *ctx, void *dst_canonical, const void *src_half, int parity, dslash_stream_t stream);
+DSLASH_API int dslash_eo_pack_gauge(dslash_ctx *ctx, void *dst_eo, const void *src_canonical, dslash_stream_t stream);
+DSLASH_API int dslash_eo_apply(dslash_ctx *ctx, int out_parity, int dagger, void *out, const void *in, const void *gauge_eo,
+                               dslash_stream_t stream);
+DSLASH_API int dslash_eo_apply_xpay(dslash_ctx *ctx, int out_parity, int dagger, void *out, const void *in, const void *gauge_eo,
+                                    const void *c, double a, double b, dslash_stream_t stream);
+DSLASH_API int dslash_eo_apply_schur(dslash_ctx *ctx, int dagger, double mass, void *out_even, const void *in_even, void *tmp_odd,
+                                     const void *gauge_eo, dslash_stream_t stream);
+DSLASH_API int dslash_eo_cg_solve(dslash_ctx *ctx, void *x_even, const void *b_even, const void *gauge_eo, double mass, double tol,
+                                  int max_iter, int *iterations, double *rel_residual, dslash_stream_t stream);
+DSLASH_API int dslash_eo_solve(dslash_ctx *ctx, void *x_even, void *x_odd, const void *b_even, const void *b_odd, const void *gauge_eo,
+                               double mass, double tol, int max_iter, int *iterations, double *rel_residual, dslash_stream_t stream);
+
+/*
  * Performance options of the tuned kernels (DSLASH_OPT_*); they never change results beyond rounding order.
  * Errors: NULL, UNSUPPORTED (unknown option or value out of range).
  */

@@ -37,6 +37,19 @@ SIGNATURES = {
     "dslash_apply_op": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_double, _vp, _vp, _vp, _vp]),
     "dslash_cg_solve": (ctypes.c_int, [_vp, _vp, _vp, _vp, ctypes.c_double, ctypes.c_double, ctypes.c_int, _c_int_p,
                                         ctypes.POINTER(ctypes.c_double), _vp]),
+    "dslash_eo_spinor_bytes": (ctypes.c_size_t, [_vp]),
+    "dslash_eo_gauge_bytes": (ctypes.c_size_t, [_vp]),
+    "dslash_eo_pack_spinor": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int, _vp]),
+    "dslash_eo_unpack_spinor": (ctypes.c_int, [_vp, _vp, _vp, ctypes.c_int, _vp]),
+    "dslash_eo_pack_gauge": (ctypes.c_int, [_vp, _vp, _vp, _vp]),
+    "dslash_eo_apply": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp, _vp]),
+    "dslash_eo_apply_xpay": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp, _vp, ctypes.c_double, ctypes.c_double,
+                                             _vp]),
+    "dslash_eo_apply_schur": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_double, _vp, _vp, _vp, _vp, _vp]),
+    "dslash_eo_cg_solve": (ctypes.c_int, [_vp, _vp, _vp, _vp, ctypes.c_double, ctypes.c_double, ctypes.c_int, _c_int_p,
+                                           ctypes.POINTER(ctypes.c_double), _vp]),
+    "dslash_eo_solve": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_double, ctypes.c_double, ctypes.c_int, _c_int_p,
+                                        ctypes.POINTER(ctypes.c_double), _vp]),
     "dslash_spinor_bytes": (ctypes.c_size_t, [_vp]),
     "dslash_gauge_bytes": (ctypes.c_size_t, [_vp]),
     "dslash_canonical_spinor_bytes": (ctypes.c_size_t, [_vp]),
@@ -144,6 +157,64 @@ def dslash_cg_solve(ctx, x, b, gauge, mass: float, tol: float, max_iter: int, st
     it, rel = ctypes.c_int(), ctypes.c_double()
     _check(_lib.dslash_cg_solve(_ptr(ctx), _ptr(x), _ptr(b), _ptr(gauge), float(mass), float(tol), int(max_iter),
                                 ctypes.byref(it), ctypes.byref(rel), _ptr(stream)), "dslash_cg_solve")
+    return it.value, rel.value
+
+
+def dslash_eo_spinor_bytes(ctx) -> int:
+    return int(_lib.dslash_eo_spinor_bytes(_ptr(ctx)))
+
+
+def dslash_eo_gauge_bytes(ctx) -> int:
+    return int(_lib.dslash_eo_gauge_bytes(_ptr(ctx)))
+
+
+def dslash_eo_pack_spinor(ctx, dst_half, src_canonical, parity: int, stream=0) -> None:
+    _check(_lib.dslash_eo_pack_spinor(_ptr(ctx), _ptr(dst_half), _ptr(src_canonical), int(parity), _ptr(stream)),
+           "dslash_eo_pack_spinor")
+
+
+def dslash_eo_unpack_spinor(ctx, dst_canonical, src_half, parity: int, stream=0) -> None:
+    _check(_lib.dslash_eo_unpack_spinor(_ptr(ctx), _ptr(dst_canonical), _ptr(src_half), int(parity), _ptr(stream)),
+           "dslash_eo_unpack_spinor")
+
+
+def dslash_eo_pack_gauge(ctx, dst_eo, src_canonical, stream=0) -> None:
+    _check(_lib.dslash_eo_pack_gauge(_ptr(ctx), _ptr(dst_eo), _ptr(src_canonical), _ptr(stream)), "dslash_eo_pack_gauge")
+
+
+def dslash_eo_apply(ctx, out_parity: int, dagger: int, out, inp, gauge_eo, stream=0) -> None:
+    _check(_lib.dslash_eo_apply(_ptr(ctx), int(out_parity), int(dagger), _ptr(out), _ptr(inp), _ptr(gauge_eo), _ptr(stream)),
+           "dslash_eo_apply")
+
+
+def dslash_eo_apply_status(ctx, out_parity: int, dagger: int, out, inp, gauge_eo, stream=0) -> int:
+    """dslash_eo_apply returning the raw status instead of raising (error-path tests)."""
+    return int(_lib.dslash_eo_apply(_ptr(ctx), int(out_parity), int(dagger), _ptr(out), _ptr(inp), _ptr(gauge_eo), _ptr(stream)))
+
+
+def dslash_eo_apply_xpay(ctx, out_parity: int, dagger: int, out, inp, gauge_eo, c, a: float, b: float, stream=0) -> None:
+    _check(_lib.dslash_eo_apply_xpay(_ptr(ctx), int(out_parity), int(dagger), _ptr(out), _ptr(inp), _ptr(gauge_eo), _ptr(c),
+                                     float(a), float(b), _ptr(stream)), "dslash_eo_apply_xpay")
+
+
+def dslash_eo_apply_schur(ctx, dagger: int, mass: float, out_even, in_even, tmp_odd, gauge_eo, stream=0) -> None:
+    _check(_lib.dslash_eo_apply_schur(_ptr(ctx), int(dagger), float(mass), _ptr(out_even), _ptr(in_even), _ptr(tmp_odd),
+                                      _ptr(gauge_eo), _ptr(stream)), "dslash_eo_apply_schur")
+
+
+def dslash_eo_cg_solve(ctx, x_even, b_even, gauge_eo, mass: float, tol: float, max_iter: int, stream=0):
+    """Returns (iterations, rel_residual)."""
+    it, rel = ctypes.c_int(), ctypes.c_double()
+    _check(_lib.dslash_eo_cg_solve(_ptr(ctx), _ptr(x_even), _ptr(b_even), _ptr(gauge_eo), float(mass), float(tol), int(max_iter),
+                                   ctypes.byref(it), ctypes.byref(rel), _ptr(stream)), "dslash_eo_cg_solve")
+    return it.value, rel.value
+
+
+def dslash_eo_solve(ctx, x_even, x_odd, b_even, b_odd, gauge_eo, mass: float, tol: float, max_iter: int, stream=0):
+    """Returns (iterations, rel_residual)."""
+    it, rel = ctypes.c_int(), ctypes.c_double()
+    _check(_lib.dslash_eo_solve(_ptr(ctx), _ptr(x_even), _ptr(x_odd), _ptr(b_even), _ptr(b_odd), _ptr(gauge_eo), float(mass),
+                                float(tol), int(max_iter), ctypes.byref(it), ctypes.byref(rel), _ptr(stream)), "dslash_eo_solve")
     return it.value, rel.value
 
 

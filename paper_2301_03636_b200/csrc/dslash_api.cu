@@ -30,6 +30,12 @@ struct dslash_ctx {
     // workspace of dslash_cg_solve (device memory, owned): r, p, t, q spinors; reduction scratch; one result
     void* cg_vec[4];
     double* cg_scratch;
+    // even-odd (checkerboard) form: half geometry {L_X/2, L_Y, L_Z, L_T}, its tile decomposition, solver workspace
+    // (r, p, t, q, the odd-parity temporary of Mhat, the right-hand side of dslash_eo_solve); eo_ok = all extents even
+    bool eo_ok;
+    Geom gh;
+    TileGeom tg_eo;
+    void* eo_vec[6];
 };
 
 static int cuda_fail(dslash_ctx* c, cudaError_t e) {
@@ -58,14 +64,14 @@ static bool full_time_range(const dslash_ctx* c) { return c->tg.t_begin == 0 && 
 // Default tile of the tuned kernel (measured on B200, profiles/): x-extent = the largest power of two <= 32 that
 // divides L_X (a warp then reads whole 32-site vectors or aligned halves of them), 2-4 rows in y, 2 planes in z,
 // about 128 sites per block for wide rows and 64 for narrow ones; never beyond the next power of two of an extent.
-static void default_tile(const dslash_ctx* c, int tile[4]) {
+static void default_tile(const Geom& geom, int tile[4]) {
     int cap[4];
     for (int d = 0; d < 4; ++d) {
         cap[d] = 1;
-        while (cap[d] < c->geom.L[d]) cap[d] <<= 1;
+        while (cap[d] < geom.L[d]) cap[d] <<= 1;
     }
     int bx = 32;
-    while (bx > 1 && (c->geom.L[0] % bx)) bx >>= 1;
+    while (bx > 1 && (geom.L[0] % bx)) bx >>= 1;
     if (bx < 4) bx = cap[0] < 8 ? cap[0] : 8;  // odd or tiny L_X: edge threads idle instead
     int by = 64 / bx;
     if (by < 1) by = 1;
@@ -84,6 +90,88 @@ static void default_tile(const dslash_ctx* c, int tile[4]) {
             }
         }
     }
+}
+
+// Conjugate gradients on the normal equations A^dagger A x = b for a field of V sites (sb bytes) in the ctx's native
+// layout.  applyA(t, p) / applyAdag(q, t) enqueue the operator on `st` and return the number of kernels they launched
+// (negative: a cudaError_t, negated).  vec = {r, p, t, q} work fields, zero-initialised when first allocated so that the
+// padding of a blocked-SoA field stays zero.  Deterministic: every reduction is a fixed-order two-pass fp64 sum.
+template <typename OpA, typename OpAdag>
+static int cg_normal_equations(dslash_ctx* c, unsigned V, size_t sb, void** vec, void* x, const void* b, double tol, int max_iter,
+                               int* iterations, double* rel_residual, cudaStream_t st, OpA applyA, OpAdag applyAdag) {
+    cudaError_t e;
+    for (int i = 0; i < 4; ++i)
+        if (!vec[i]) {
+            e = cudaMalloc(&vec[i], sb);
+            if (e != cudaSuccess) {
+                vec[i] = nullptr;
+                c->last_cuda = (int)e;
+                (void)cudaGetLastError();
+                return DSLASH_ERR_NOMEM;
+            }
+            if ((e = cudaMemsetAsync(vec[i], 0, sb, st)) != cudaSuccess) return cuda_fail(c, e);
+        }
+    if (!c->cg_scratch) {
+        e = cudaMalloc(reinterpret_cast<void**>(&c->cg_scratch), sizeof(double) * (size_t)(reduction_scratch_doubles() + 1));
+        if (e != cudaSuccess) {
+            c->cg_scratch = nullptr;
+            c->last_cuda = (int)e;
+            (void)cudaGetLastError();
+            return DSLASH_ERR_NOMEM;
+        }
+    }
+    void *r = vec[0], *p = vec[1], *t = vec[2], *q = vec[3];
+    double* d_res = c->cg_scratch + reduction_scratch_doubles();
+    const int prec = c->precision, lay = c->layout_base;
+    // <u, v> on the device, value read back (synchronises the stream)
+    auto dot = [&](const void* u, const void* v, double* host) -> cudaError_t {
+        cudaError_t er = launch_dot(prec, lay, V, d_res, c->cg_scratch, u, v, st);
+        if (er != cudaSuccess) return er;
+        c->launches += 2;
+        er = cudaMemcpyAsync(host, d_res, sizeof(double), cudaMemcpyDeviceToHost, st);
+        if (er != cudaSuccess) return er;
+        return cudaStreamSynchronize(st);
+    };
+    auto op = [&](int n) -> cudaError_t {
+        if (n < 0) return (cudaError_t)(-n);
+        c->launches += n;
+        return cudaSuccess;
+    };
+#define CG_TRY(call)                                  \
+    do {                                              \
+        if ((e = (call)) != cudaSuccess) return cuda_fail(c, e); \
+    } while (0)
+    CG_TRY(cudaMemsetAsync(x, 0, sb, st));
+    CG_TRY(cudaMemcpyAsync(r, b, sb, cudaMemcpyDeviceToDevice, st));
+    CG_TRY(cudaMemcpyAsync(p, b, sb, cudaMemcpyDeviceToDevice, st));
+    double rr = 0.0, bb = 0.0, pAp = 0.0, rr_new = 0.0;
+    CG_TRY(dot(r, r, &rr));
+    bb = rr;
+    int it = 0;
+    double rel = bb > 0.0 ? 1.0 : 0.0;
+    if (bb > 0.0) {
+        for (it = 1; it <= max_iter; ++it) {
+            CG_TRY(op(applyA(t, p)));
+            CG_TRY(dot(t, t, &pAp));
+            CG_TRY(op(applyAdag(q, t)));
+            const double alpha = rr / pAp;
+            // x += alpha p, r -= alpha q, rr_new = |r|^2 in one pass over the four fields
+            CG_TRY(launch_cg_update(prec, lay, V, x, r, p, q, alpha, d_res, c->cg_scratch, st));
+            c->launches += 2;
+            CG_TRY(cudaMemcpyAsync(&rr_new, d_res, sizeof(double), cudaMemcpyDeviceToHost, st));
+            CG_TRY(cudaStreamSynchronize(st));
+            rel = sqrt(rr_new / bb);
+            if (rel <= tol) break;
+            CG_TRY(launch_axpby(prec, lay, V, p, r, 1.0, rr_new / rr, st));
+            c->launches += 1;
+            rr = rr_new;
+        }
+        if (it > max_iter) it = max_iter;
+    }
+#undef CG_TRY
+    if (iterations) *iterations = it;
+    if (rel_residual) *rel_residual = rel;
+    return DSLASH_OK;
 }
 
 extern "C" {
@@ -120,8 +208,23 @@ int dslash_create(dslash_ctx** ctx, const int dims[4], int precision, int layout
     c->tg.t_begin = 0;
     c->tg.t_end = dims[3];
     int tile[4];
-    default_tile(c, tile);
+    default_tile(c->geom, tile);
     set_tile_geom(c, tile);
+    c->eo_ok = true;
+    for (int d = 0; d < 4; ++d) c->eo_ok = c->eo_ok && (dims[d] % 2 == 0);
+    if (c->eo_ok) {
+        c->gh = c->geom;
+        c->gh.L[0] = dims[0] / 2;
+        c->gh.V = c->geom.V / 2u;
+        default_tile(c->gh, tile);
+        for (int d = 0; d < 4; ++d) {
+            c->tg_eo.lb[d] = ilog2_exact(tile[d]);
+            c->tg_eo.nt[d] = (c->gh.L[d] + tile[d] - 1) / tile[d];
+        }
+        c->tg_eo.t_begin = 0;
+        c->tg_eo.t_end = dims[3];
+    }
+    for (int i = 0; i < 6; ++i) c->eo_vec[i] = nullptr;
     c->kernel = DSLASH_KERNEL_AUTO;
     c->cfg.occupancy = precision == DSLASH_FP64 ? 2 : 1;  // measured: fp64 wants registers (ILP), fp32 wants warps
     c->cfg.l2_policy = 0;
@@ -142,8 +245,11 @@ int dslash_destroy(dslash_ctx* c) {
     bool any = c->cg_scratch != nullptr;
     for (int i = 0; i < 3; ++i) any = any || c->d_can[i] || c->d_nat[i];
     for (int i = 0; i < 4; ++i) any = any || c->cg_vec[i];
+    for (int i = 0; i < 6; ++i) any = any || c->eo_vec[i];
     if (any) {
         if (cudaDeviceSynchronize() != cudaSuccess) rc = DSLASH_ERR_CUDA;
+        for (int i = 0; i < 6; ++i)
+            if (c->eo_vec[i]) cudaFree(c->eo_vec[i]);
         for (int i = 0; i < 4; ++i)
             if (c->cg_vec[i]) cudaFree(c->cg_vec[i]);
         if (c->cg_scratch) cudaFree(c->cg_scratch);
@@ -229,83 +335,160 @@ int dslash_cg_solve(dslash_ctx* c, void* x, const void* b, const void* gauge, do
     if (overlap(x, sb, b, sb)) return DSLASH_ERR_ALIAS;
     if (c->tile[0] * c->tile[1] * c->tile[2] * c->tile[3] > 128) return DSLASH_ERR_UNSUPPORTED;
     cudaStream_t st = static_cast<cudaStream_t>(stream_);
-    cudaError_t e;
-    for (int i = 0; i < 4; ++i)
-        if (!c->cg_vec[i]) {
-            e = cudaMalloc(&c->cg_vec[i], sb);
-            if (e != cudaSuccess) {
-                c->cg_vec[i] = nullptr;
-                c->last_cuda = (int)e;
-                (void)cudaGetLastError();
-                return DSLASH_ERR_NOMEM;
-            }
-            if ((e = cudaMemsetAsync(c->cg_vec[i], 0, sb, st)) != cudaSuccess) return cuda_fail(c, e);
-        }
-    if (!c->cg_scratch) {
-        e = cudaMalloc(reinterpret_cast<void**>(&c->cg_scratch), sizeof(double) * (size_t)(reduction_scratch_doubles() + 1));
-        if (e != cudaSuccess) {
-            c->cg_scratch = nullptr;
-            c->last_cuda = (int)e;
-            (void)cudaGetLastError();
-            return DSLASH_ERR_NOMEM;
-        }
-    }
-    void *r = c->cg_vec[0], *p = c->cg_vec[1], *t = c->cg_vec[2], *q = c->cg_vec[3];
-    double* d_res = c->cg_scratch + reduction_scratch_doubles();
-    const int prec = c->precision, lay = c->layout_base;
-    const unsigned V = c->geom.V;
-    // <u, v> on the device, value read back (synchronises the stream)
-    auto dot = [&](const void* u, const void* v, double* host) -> cudaError_t {
-        cudaError_t er = launch_dot(prec, lay, V, d_res, c->cg_scratch, u, v, st);
-        if (er != cudaSuccess) return er;
-        c->launches += 2;
-        er = cudaMemcpyAsync(host, d_res, sizeof(double), cudaMemcpyDeviceToHost, st);
-        if (er != cudaSuccess) return er;
-        return cudaStreamSynchronize(st);
-    };
-    auto op = [&](int which, void* o, const void* i) -> cudaError_t {
+    auto op = [&](int which, void* o, const void* i) -> int {
         LaunchArgs a{o, i, gauge, c->geom, st};
-        c->launches += 1;
-        return launch_op(prec, lay, c->recon, a, c->tg, which, mass);
+        const cudaError_t e = launch_op(c->precision, c->layout_base, c->recon, a, c->tg, which, mass);
+        return e == cudaSuccess ? 1 : -(int)e;
     };
-    auto axpby = [&](void* y, const void* xx, double aa, double bb) -> cudaError_t {
-        c->launches += 1;
-        return launch_axpby(prec, lay, V, y, xx, aa, bb, st);
-    };
-#define CG_TRY(call)                                  \
-    do {                                              \
-        if ((e = (call)) != cudaSuccess) return cuda_fail(c, e); \
-    } while (0)
-    CG_TRY(cudaMemsetAsync(x, 0, sb, st));
-    CG_TRY(cudaMemcpyAsync(r, b, sb, cudaMemcpyDeviceToDevice, st));
-    CG_TRY(cudaMemcpyAsync(p, b, sb, cudaMemcpyDeviceToDevice, st));
-    double rr = 0.0, bb = 0.0, pAp = 0.0, rr_new = 0.0;
-    CG_TRY(dot(r, r, &rr));
-    bb = rr;
-    int it = 0;
-    double rel = bb > 0.0 ? 1.0 : 0.0;
-    if (bb > 0.0) {
-        for (it = 1; it <= max_iter; ++it) {
-            CG_TRY(op(DSLASH_OP_M, t, p));
-            CG_TRY(dot(t, t, &pAp));
-            CG_TRY(op(DSLASH_OP_M_DAGGER, q, t));
-            const double alpha = rr / pAp;
-            // x += alpha p, r -= alpha q, rr_new = |r|^2 in one pass over the four fields
-            CG_TRY(launch_cg_update(prec, lay, V, x, r, p, q, alpha, d_res, c->cg_scratch, st));
-            c->launches += 2;
-            CG_TRY(cudaMemcpyAsync(&rr_new, d_res, sizeof(double), cudaMemcpyDeviceToHost, st));
-            CG_TRY(cudaStreamSynchronize(st));
-            rel = sqrt(rr_new / bb);
-            if (rel <= tol) break;
-            CG_TRY(axpby(p, r, 1.0, rr_new / rr));
-            rr = rr_new;
-        }
-        if (it > max_iter) it = max_iter;
-    }
-#undef CG_TRY
-    if (iterations) *iterations = it;
-    if (rel_residual) *rel_residual = rel;
+    return cg_normal_equations(
+        c, c->geom.V, sb, c->cg_vec, x, b, tol, max_iter, iterations, rel_residual, st,
+        [&](void* o, const void* i) { return op(DSLASH_OP_M, o, i); }, [&](void* o, const void* i) { return op(DSLASH_OP_M_DAGGER, o, i); });
+}
+
+/* ------------------------------------------------------------------ even-odd (checkerboarded) form */
+static size_t eo_native_sites(const dslash_ctx* c) {
+    return c->layout_base == LAYOUT_SOA ? (size_t)((c->gh.V + VL - 1u) / VL) * VL : (size_t)c->gh.V;
+}
+static size_t eo_gauge_half_bytes(const dslash_ctx* c) { return eo_native_sites(c) * 4u * (c->recon == 12 ? 12u : 18u) * real_bytes(c); }
+
+size_t dslash_eo_spinor_bytes(const dslash_ctx* c) { return (c && c->eo_ok) ? eo_native_sites(c) * 24u * real_bytes(c) : 0; }
+size_t dslash_eo_gauge_bytes(const dslash_ctx* c) { return (c && c->eo_ok) ? 2u * eo_gauge_half_bytes(c) : 0; }
+
+int dslash_eo_pack_spinor(dslash_ctx* c, void* dst_half, const void* src_canonical, int parity, dslash_stream_t stream) {
+    if (!c || !dst_half || !src_canonical) return DSLASH_ERR_NULL;
+    if (!c->eo_ok) return DSLASH_ERR_DIMS;
+    if (parity != 0 && parity != 1) return DSLASH_ERR_UNSUPPORTED;
+    if (misaligned(dst_half) || misaligned(src_canonical)) return DSLASH_ERR_ALIGN;
+    cudaError_t e = launch_eo_convert_spinor(c->precision, c->layout_base, dst_half, src_canonical, c->gh, parity, 0,
+                                             static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    c->launches += 1;
     return DSLASH_OK;
+}
+
+int dslash_eo_unpack_spinor(dslash_ctx* c, void* dst_canonical, const void* src_half, int parity, dslash_stream_t stream) {
+    if (!c || !dst_canonical || !src_half) return DSLASH_ERR_NULL;
+    if (!c->eo_ok) return DSLASH_ERR_DIMS;
+    if (parity != 0 && parity != 1) return DSLASH_ERR_UNSUPPORTED;
+    if (misaligned(dst_canonical) || misaligned(src_half)) return DSLASH_ERR_ALIGN;
+    cudaError_t e = launch_eo_convert_spinor(c->precision, c->layout_base, dst_canonical, src_half, c->gh, parity, 1,
+                                             static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    c->launches += 1;
+    return DSLASH_OK;
+}
+
+int dslash_eo_pack_gauge(dslash_ctx* c, void* dst_eo, const void* src_canonical, dslash_stream_t stream) {
+    if (!c || !dst_eo || !src_canonical) return DSLASH_ERR_NULL;
+    if (!c->eo_ok) return DSLASH_ERR_DIMS;
+    if (misaligned(dst_eo) || misaligned(src_canonical)) return DSLASH_ERR_ALIGN;
+    cudaError_t e = launch_eo_pack_gauge(c->precision, c->layout_base, c->recon, dst_eo, src_canonical, eo_gauge_half_bytes(c), c->gh,
+                                         static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    c->launches += 2;
+    return DSLASH_OK;
+}
+
+// half-lattice work field i of the ctx, allocated (and zeroed, so that blocked-SoA padding is zero) on first use
+static int eo_work_field(dslash_ctx* c, int i, cudaStream_t st) {
+    if (c->eo_vec[i]) return DSLASH_OK;
+    const size_t sb = dslash_eo_spinor_bytes(c);
+    cudaError_t e = cudaMalloc(&c->eo_vec[i], sb);
+    if (e != cudaSuccess) {
+        c->eo_vec[i] = nullptr;
+        c->last_cuda = (int)e;
+        (void)cudaGetLastError();
+        return DSLASH_ERR_NOMEM;
+    }
+    if ((e = cudaMemsetAsync(c->eo_vec[i], 0, sb, st)) != cudaSuccess) return cuda_fail(c, e);
+    return DSLASH_OK;
+}
+
+static int eo_apply_checked(dslash_ctx* c, int out_parity, int dagger, void* out, const void* in, const void* gauge_eo, int xpay,
+                            const void* cfield, double a, double b, dslash_stream_t stream) {
+    if (!c || !out || !in || !gauge_eo || (xpay && !cfield)) return DSLASH_ERR_NULL;
+    if (!c->eo_ok) return DSLASH_ERR_DIMS;
+    if ((out_parity != 0 && out_parity != 1) || (dagger != 0 && dagger != 1)) return DSLASH_ERR_UNSUPPORTED;
+    if (misaligned(out) || misaligned(in) || misaligned(gauge_eo) || (xpay && misaligned(cfield))) return DSLASH_ERR_ALIGN;
+    const size_t sb = dslash_eo_spinor_bytes(c);
+    if (overlap(out, sb, in, sb) || (xpay && overlap(out, sb, cfield, sb))) return DSLASH_ERR_ALIAS;
+    cudaError_t e = launch_eo(c->precision, c->layout_base, c->recon, out, in, gauge_eo, eo_gauge_half_bytes(c), c->gh, c->tg_eo,
+                              out_parity, dagger, xpay, a, b, cfield, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    c->launches += 1;
+    return DSLASH_OK;
+}
+
+int dslash_eo_apply(dslash_ctx* c, int out_parity, int dagger, void* out, const void* in, const void* gauge_eo, dslash_stream_t stream) {
+    return eo_apply_checked(c, out_parity, dagger, out, in, gauge_eo, 0, nullptr, 0.0, 1.0, stream);
+}
+
+int dslash_eo_apply_xpay(dslash_ctx* c, int out_parity, int dagger, void* out, const void* in, const void* gauge_eo, const void* cfield,
+                         double a, double b, dslash_stream_t stream) {
+    return eo_apply_checked(c, out_parity, dagger, out, in, gauge_eo, 1, cfield, a, b, stream);
+}
+
+int dslash_eo_apply_schur(dslash_ctx* c, int dagger, double mass, void* out_even, const void* in_even, void* tmp_odd, const void* gauge_eo,
+                          dslash_stream_t stream) {
+    if (!tmp_odd) return DSLASH_ERR_NULL;
+    const double a = 4.0 + mass;
+    if (!(a != 0.0)) return DSLASH_ERR_UNSUPPORTED;
+    int rc = eo_apply_checked(c, 1, dagger, tmp_odd, in_even, gauge_eo, 0, nullptr, 0.0, 1.0, stream);  // D_oe in
+    if (rc != DSLASH_OK) return rc;
+    return eo_apply_checked(c, 0, dagger, out_even, tmp_odd, gauge_eo, 1, in_even, a, -1.0 / (4.0 * a), stream);  // a in - D_eo(.)/(4a)
+}
+
+int dslash_eo_cg_solve(dslash_ctx* c, void* x_even, const void* b_even, const void* gauge_eo, double mass, double tol, int max_iter,
+                       int* iterations, double* rel_residual, dslash_stream_t stream_) {
+    if (!c || !x_even || !b_even || !gauge_eo) return DSLASH_ERR_NULL;
+    if (!c->eo_ok) return DSLASH_ERR_DIMS;
+    const double a = 4.0 + mass;
+    if (!(tol > 0.0) || max_iter < 1 || !(a != 0.0)) return DSLASH_ERR_UNSUPPORTED;
+    if (misaligned(x_even) || misaligned(b_even) || misaligned(gauge_eo)) return DSLASH_ERR_ALIGN;
+    const size_t sb = dslash_eo_spinor_bytes(c);
+    if (overlap(x_even, sb, b_even, sb)) return DSLASH_ERR_ALIAS;
+    cudaStream_t st = static_cast<cudaStream_t>(stream_);
+    const int rc_alloc = eo_work_field(c, 4, st);
+    if (rc_alloc != DSLASH_OK) return rc_alloc;
+    void* tmp = c->eo_vec[4];
+    const size_t ghb = eo_gauge_half_bytes(c);
+    auto schur = [&](int dagger, void* o, const void* i) -> int {
+        cudaError_t e = launch_eo(c->precision, c->layout_base, c->recon, tmp, i, gauge_eo, ghb, c->gh, c->tg_eo, 1, dagger, 0, 0.0, 1.0,
+                                  nullptr, st);
+        if (e != cudaSuccess) return -(int)e;
+        e = launch_eo(c->precision, c->layout_base, c->recon, o, tmp, gauge_eo, ghb, c->gh, c->tg_eo, 0, dagger, 1, a, -1.0 / (4.0 * a), i,
+                      st);
+        return e == cudaSuccess ? 2 : -(int)e;
+    };
+    return cg_normal_equations(
+        c, c->gh.V, sb, c->eo_vec, x_even, b_even, tol, max_iter, iterations, rel_residual, st,
+        [&](void* o, const void* i) { return schur(0, o, i); }, [&](void* o, const void* i) { return schur(1, o, i); });
+}
+
+int dslash_eo_solve(dslash_ctx* c, void* x_even, void* x_odd, const void* b_even, const void* b_odd, const void* gauge_eo, double mass,
+                    double tol, int max_iter, int* iterations, double* rel_residual, dslash_stream_t stream) {
+    if (!c || !x_even || !x_odd || !b_even || !b_odd || !gauge_eo) return DSLASH_ERR_NULL;
+    if (!c->eo_ok) return DSLASH_ERR_DIMS;
+    const double a = 4.0 + mass;
+    if (!(a != 0.0)) return DSLASH_ERR_UNSUPPORTED;
+    const size_t sb = dslash_eo_spinor_bytes(c);
+    const void* f[5] = {x_even, x_odd, b_even, b_odd, gauge_eo};
+    for (int i = 0; i < 5; ++i)
+        if (misaligned(f[i])) return DSLASH_ERR_ALIGN;
+    for (int i = 0; i < 4; ++i)
+        for (int j = i + 1; j < 4; ++j)
+            if (overlap(f[i], sb, f[j], sb)) return DSLASH_ERR_ALIAS;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    int rc;
+    if ((rc = eo_work_field(c, 4, st)) != DSLASH_OK || (rc = eo_work_field(c, 5, st)) != DSLASH_OK) return rc;
+    void *tmp = c->eo_vec[4], *rhs = c->eo_vec[5];
+    // bhat = b_e + D_eo b_o / (2a), held in x_odd until the end
+    if ((rc = dslash_eo_apply_xpay(c, 0, 0, x_odd, b_odd, gauge_eo, b_even, 1.0, 0.5 / a, stream)) != DSLASH_OK) return rc;
+    // normal equations: Mhat^dagger Mhat x_e = Mhat^dagger bhat
+    if ((rc = dslash_eo_apply_schur(c, 1, mass, rhs, x_odd, tmp, gauge_eo, stream)) != DSLASH_OK) return rc;
+    if ((rc = dslash_eo_cg_solve(c, x_even, rhs, gauge_eo, mass, tol, max_iter, iterations, rel_residual, stream)) != DSLASH_OK) return rc;
+    // x_o = (b_o + D_oe x_e / 2) / a
+    return dslash_eo_apply_xpay(c, 1, 0, x_odd, x_even, gauge_eo, b_odd, 1.0 / a, 0.5 / a, stream);
 }
 
 int dslash_pack_spinor(dslash_ctx* c, void* dst, const void* src, dslash_stream_t stream) {

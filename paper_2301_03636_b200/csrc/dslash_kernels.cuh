@@ -57,6 +57,15 @@ cudaError_t launch_cg_update(int precision, int layout_base, unsigned V, void* x
                              double* result, double* scratch, cudaStream_t st);
 int reduction_scratch_doubles();
 
+// Even-odd (checkerboarded) operator and its layout kernels (dslash_eo.cu).  gh = half geometry {L_X/2, L_Y, L_Z, L_T}, V/2.
+cudaError_t launch_eo(int precision, int layout_base, int recon, void* out, const void* in, const void* gauge_eo,
+                      size_t gauge_half_bytes, const Geom& gh, const TileGeom& tg, int parity, int dagger, int xpay, double a,
+                      double b, const void* c, cudaStream_t st);
+cudaError_t launch_eo_convert_spinor(int precision, int layout_base, void* dst, const void* src, const Geom& gh, int parity, int dir,
+                                     cudaStream_t st);
+cudaError_t launch_eo_pack_gauge(int precision, int layout_base, int recon, void* dst_eo, const void* src, size_t gauge_half_bytes,
+                                 const Geom& gh, cudaStream_t st);
+
 // Layout module.  dir 0: canonical -> native (pack), 1: native -> canonical (unpack).
 cudaError_t launch_convert_spinor(int precision, int layout_base, void* dst, const void* src, unsigned V, int dir,
                                   cudaStream_t stream);

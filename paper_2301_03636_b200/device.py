@@ -97,6 +97,52 @@ class Lattice:
         """x <- solution of M^dagger M x = b (native device buffers); returns (iterations, rel_residual)."""
         return B.dslash_cg_solve(self.ctx, x.data_ptr(), b.data_ptr(), gauge.data_ptr(), mass, tol, max_iter, self.stream())
 
+    # -- even-odd (checkerboarded) form; all extents even
+    def new_eo_spinor(self):
+        return self._bytes(B.dslash_eo_spinor_bytes(self.ctx)).zero_()
+
+    def upload_eo_spinor(self, canonical, parity):
+        """canonical full-lattice NumPy spinor -> native half-lattice device buffer holding its sites of `parity`."""
+        assert canonical.size == self.volume * 24
+        src = self._to_device(canonical)
+        dst = self.new_eo_spinor()
+        B.dslash_eo_pack_spinor(self.ctx, dst.data_ptr(), src.data_ptr(), parity, self.stream())
+        torch.cuda.current_stream().synchronize()
+        return dst
+
+    def upload_eo_gauge(self, canonical):
+        assert canonical.size == self.volume * 72
+        src = self._to_device(canonical)
+        dst = self._bytes(B.dslash_eo_gauge_bytes(self.ctx))
+        B.dslash_eo_pack_gauge(self.ctx, dst.data_ptr(), src.data_ptr(), self.stream())
+        torch.cuda.current_stream().synchronize()
+        return dst
+
+    def download_eo_spinor(self, halves):
+        """{parity: native half-lattice buffer} -> canonical full-lattice NumPy spinor (absent parities are zero)."""
+        dst = self._bytes(B.dslash_canonical_spinor_bytes(self.ctx)).zero_()
+        for parity, buf in halves.items():
+            B.dslash_eo_unpack_spinor(self.ctx, dst.data_ptr(), buf.data_ptr(), parity, self.stream())
+        lx, ly, lz, lt = self.dims
+        return dst.cpu().numpy().view(self.np_dtype).reshape(lt, lz, ly, lx, 4, 3, 2)
+
+    def eo_apply(self, out_parity, dagger, out, inp, gauge_eo):
+        B.dslash_eo_apply(self.ctx, out_parity, dagger, out.data_ptr(), inp.data_ptr(), gauge_eo.data_ptr(), self.stream())
+
+    def eo_apply_schur(self, dagger, mass, out_even, in_even, tmp_odd, gauge_eo):
+        B.dslash_eo_apply_schur(self.ctx, dagger, mass, out_even.data_ptr(), in_even.data_ptr(), tmp_odd.data_ptr(),
+                                gauge_eo.data_ptr(), self.stream())
+
+    def eo_cg_solve(self, x_even, b_even, gauge_eo, mass, tol, max_iter):
+        """x_even <- solution of Mhat^dagger Mhat x = b_even; returns (iterations, rel_residual)."""
+        return B.dslash_eo_cg_solve(self.ctx, x_even.data_ptr(), b_even.data_ptr(), gauge_eo.data_ptr(), mass, tol, max_iter,
+                                    self.stream())
+
+    def eo_solve(self, x_even, x_odd, b_even, b_odd, gauge_eo, mass, tol, max_iter):
+        """(x_even, x_odd) <- solution of M x = b through the even-odd preconditioned system."""
+        return B.dslash_eo_solve(self.ctx, x_even.data_ptr(), x_odd.data_ptr(), b_even.data_ptr(), b_odd.data_ptr(),
+                                 gauge_eo.data_ptr(), mass, tol, max_iter, self.stream())
+
     def set_variant(self, depth, tpb=0, spt=0):
         B.dslash_set_variant(self.ctx, depth, tpb, spt)
 
