@@ -215,6 +215,8 @@ def run_cuda(args, cfg):
                 lat.set_kernel(args.kernel)
             if args.x_shuffle is not None:
                 B.dslash_set_option(lat.ctx, B.DSLASH_OPT_X_SHUFFLE, args.x_shuffle)
+            if args.t_chunk is not None:
+                B.dslash_set_option(lat.ctx, B.DSLASH_OPT_T_CHUNK, args.t_chunk)
             gd, pd, od = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
             n0 = B.dslash_launch_count(lat.ctx)
             ms, ck = time_applies(torch, lat, od, pd, gd, args.steps, args.warmup, group, local)
@@ -224,7 +226,9 @@ def run_cuda(args, cfg):
                                 gflops=replicas.whole_job_rate(FLOP_PER_SITE * v, world, ms / args.steps) / 1e9,
                                 gbs=bps * v / (ms / args.steps) / 1e6, bps=bps, recon12=recon12,
                                 tile=list(B.dslash_get_tile(lat.ctx)),
-                                kernel={B.DSLASH_KERNEL_DIRECT: "direct", B.DSLASH_KERNEL_TMA: "tma"}[B.dslash_get_kernel(lat.ctx)],
+                                kernel={B.DSLASH_KERNEL_DIRECT: "direct", B.DSLASH_KERNEL_TMA: "tma", B.DSLASH_KERNEL_TMA_LINKS: "tma_links",
+                                        B.DSLASH_KERNEL_RING: "ring"}[B.dslash_get_kernel(lat.ctx)],
+                                t_chunk=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_T_CHUNK),
                                 occupancy=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_OCCUPANCY),
                                 x_shuffle=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_X_SHUFFLE))
             if tag == "main":
@@ -286,7 +290,7 @@ def run_cuda(args, cfg):
             "vs_baseline": None, "dtype": prec, "data": "synthetic",
             "config": {"workload": cfg["name"], "dims": list(dims), "layout": args.layout, "recon": 12 if main["recon12"] else 18,
                        "tile": main["tile"], "kernel": main["kernel"], "occupancy_option": main["occupancy"],
-                       "x_shuffle_option": main["x_shuffle"], "sites": v, "parallelism": "replicas x%d" % world,
+                       "x_shuffle_option": main["x_shuffle"], "t_chunk_option": main["t_chunk"], "sites": v, "parallelism": "replicas x%d" % world,
                        "l2": "inputs larger than L2: %.2f GB working set per apply vs 126 MB L2, no flush needed"
                              % (main["bps"] * v / 1e9)},
             "hbm_gbs": main["gbs"], "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "clocks": clocks,
@@ -657,7 +661,8 @@ def main():
     ap.add_argument("--layout", choices=["soa", "aos"], default="soa")
     ap.add_argument("--tile", type=int, nargs=4, default=None, help="tile of the tuned kernel (x y z t)")
     ap.add_argument("--occupancy", type=int, default=None, help="DSLASH_OPT_OCCUPANCY override")
-    ap.add_argument("--kernel", choices=["auto", "direct", "tma"], default=None)
+    ap.add_argument("--kernel", choices=["auto", "direct", "tma", "tma_links", "ring"], default=None)
+    ap.add_argument("--t-chunk", type=int, default=None, help="DSLASH_OPT_T_CHUNK override (ring kernel)")
     ap.add_argument("--x-shuffle", type=int, choices=[0, 1], default=None, help="DSLASH_OPT_X_SHUFFLE override")
     ap.add_argument("--both-recon", action="store_true", default=True, help="also time the other link compression")
     ap.add_argument("--one-recon", dest="both_recon", action="store_false")

@@ -103,6 +103,9 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
 #define DSLASH_KERNEL_DIRECT 1 /* one thread per site, all neighbours gathered from global memory through L1/L2 */
 #define DSLASH_KERNEL_TMA 2    /* tile's own spinors and links staged in shared memory by TMA bulk copies */
 #define DSLASH_KERNEL_TMA_LINKS 3 /* only the tile's own links staged by TMA bulk copies; spinors gathered directly */
+#define DSLASH_KERNEL_RING 4   /* t-marching with the tile's spinor rows of t, t+1, t+2 in a shared-memory ring filled by bulk
+                                  async copies one step ahead (blocked SoA, tile 32 x by x bz x 1 that tiles the lattice exactly,
+                                  L_X a multiple of 32); bit-identical to DSLASH_KERNEL_DIRECT */
 
 /* options of the tuned kernels, dslash_set_option() */
 #define DSLASH_OPT_OCCUPANCY 2        /* blocks of <= 128 threads: 0 = 168 registers/thread (12 warps/SM), 1 = 128 (16 warps),
@@ -115,6 +118,8 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
                                          (tile x-extent == L_X, a power of two <= 32) the two x hops are exchanged between
                                          lanes by warp shuffles instead of loaded; 0 = always load them.  Same result, bit
                                          for bit */
+
+#define DSLASH_OPT_T_CHUNK 6          /* ring kernel: time slices a block marches through, 1..L_T (0 = library default 8) */
 
 /* host<->device mapping modes of dslash_apply_host() (section 4.1.2) */
 #define DSLASH_MAP_MINIMAL 0 /* to: gauge, in;  from: out            (after the Advisor's data analysis) */

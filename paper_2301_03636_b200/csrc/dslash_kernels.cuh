@@ -36,6 +36,7 @@ struct TunedConfig {
     int occupancy;         // 0: default register budget, 1: 128-register variant
     int l2_policy;         // DSLASH_OPT_L2_POLICY bits (0: no cache hints)
     int l1_carveout;       // preferred shared-memory carve-out of the direct kernel in percent (-1: driver default)
+    int t_chunk;           // time slices a block of the ring kernel marches through (0: default)
     int x_shuffle;         // 1: exchange the x hops inside the warp when the tile allows it (fp64 default), 0: always load them
 };
 bool x_shuffle_eligible(const Geom& g, const TileGeom& tg);
@@ -43,6 +44,10 @@ bool x_shuffle_eligible(const Geom& g, const TileGeom& tg);
 // Tuned kernel (direct, register-staged).
 cudaError_t launch_tuned(int precision, int layout_base, int recon, const LaunchArgs& a, const TileGeom& tg,
                          const TunedConfig& cfg);
+
+// t-marching kernel with a shared-memory ring of spinor time slices fed by bulk async copies (dslash_ring.cu).
+bool ring_eligible(int layout_base, const Geom& g, const TileGeom& tg);
+cudaError_t launch_ring(int precision, int layout_base, int recon, const LaunchArgs& a, const TileGeom& tg, const TunedConfig& cfg);
 
 // TMA-staged kernel (SoA only): tile's own spinors + links by cp.async.bulk.tensor into shared memory.
 bool tma_eligible(int precision, int recon, const Geom& g, const TileGeom& tg);

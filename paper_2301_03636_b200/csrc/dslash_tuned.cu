@@ -83,7 +83,7 @@ static cudaError_t launch_tuned_s(const LaunchArgs& a, const TileGeom& tg, const
     do {                                                                                                                     \
         static int carve_set = -1;                                                                                           \
         if (carve_set != cfg.l1_carveout) {                                                                                  \
-            cudaFuncSetAttribute(dslash_tuned_kernel<Real, LAYOUT, RECON, MAXTPB, MINBLK, HINT, XSHFL>,                             \
+            cudaFuncSetAttribute(dslash_tuned_kernel<Real, LAYOUT, RECON, MAXTPB, MINBLK, HINT, XSHFL>,                           \
                                  cudaFuncAttributePreferredSharedMemoryCarveout, cfg.l1_carveout);                          \
             carve_set = cfg.l1_carveout;                                                                                     \
         }                                                                                                                    \

@@ -166,6 +166,60 @@ def test_tma_kernel_refuses_what_it_cannot_run(env):
             B.dslash_set_kernel(lat.ctx, 7)
 
 
+# ---------------------------------------------------------------- the t-marching ring kernel (SoA), selected explicitly
+@pytest.mark.parametrize("dims,tile,chunk", [
+    ((32, 4, 4, 8), (32, 2, 2, 1), 0),        # default chunk (8): one chunk
+    ((32, 4, 4, 8), (32, 2, 2, 1), 3),        # chunks of 3, 3, 2 steps: ring wrap-around, parity flips, short last chunk
+    ((32, 4, 4, 7), (32, 4, 1, 1), 1),        # one step per block: prologue + a single step
+    ((32, 4, 4, 7), (32, 1, 4, 1), 7),        # the whole time extent in one block: forward hop of the last step wraps to t = 0
+    ((32, 2, 2, 5), (32, 2, 2, 1), 2),        # a single spatial tile: every y/z neighbour is in the tile or wraps through global
+    ((32, 8, 4, 4), (32, 4, 2, 1), 4),        # 8 warps per block
+    ((32, 6, 4, 4), (32, 2, 1, 1), 2),        # L_Y = 6 tiled by 2
+    ((64, 4, 2, 6), (32, 2, 1, 1), 4),        # L_X = 64: x hops loaded (no whole row in a warp), two x tiles
+    ((32, 2, 6, 3), (32, 1, 1, 1), 2),        # one warp per block, no in-tile neighbours
+])
+@pytest.mark.parametrize("precision", ["f64", "f32"])
+@pytest.mark.parametrize("recon12", [False, True])
+def test_ring_kernel_matches_the_oracle_and_the_direct_kernel_bit_for_bit(env, dims, tile, chunk, precision, recon12):
+    B = env.B
+    g, p, ref, _ = fields_and_ref(env, dims, SEED + 19, precision)
+    with env.device.Lattice(dims, precision, "soa", recon12) as lat:
+        gi, pi, o = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
+        lat.set_tile(tile)
+        lat.apply(o, pi, gi)
+        direct = lat.download_spinor(o)
+        lat.set_kernel("ring")
+        B.dslash_set_option(lat.ctx, B.DSLASH_OPT_T_CHUNK, chunk)
+        assert B.dslash_get_kernel(lat.ctx) == B.DSLASH_KERNEL_RING and B.dslash_get_option(lat.ctx, B.DSLASH_OPT_T_CHUNK) == chunk
+        o.zero_()
+        lat.apply(o, pi, gi)
+        got = lat.download_spinor(o)
+        assert env.checks.parity_error(got, ref) <= TOL[precision]
+        assert np.array_equal(got, direct)  # same arithmetic in the same order
+        # a time range (multi-GPU slab interior) with the ring kernel: only its slices are written
+        if dims[3] >= 4:
+            B.dslash_set_time_range(lat.ctx, 1, dims[3] - 1)
+            o.zero_()
+            lat.apply(o, pi, gi)
+            part = lat.download_spinor(o)
+            assert np.array_equal(part[1:-1], direct[1:-1]) and not part[0].any() and not part[-1].any()
+
+
+def test_ring_kernel_refuses_what_it_cannot_run(env):
+    B = env.B
+    for dims, layout, tile in [((32, 4, 4, 4), "aos", (32, 2, 2, 1)),   # AoS rows are not contiguous vectors
+                               ((16, 4, 4, 4), "soa", (16, 4, 2, 1)),   # rows shorter than a 32-site vector
+                               ((32, 6, 4, 4), "soa", (32, 4, 1, 1)),   # tile does not divide L_Y
+                               ((32, 4, 4, 4), "soa", (32, 2, 1, 2))]:  # tile with a t extent
+        with env.device.Lattice(dims, "f64", layout, False) as lat:
+            lat.set_tile(tile)
+            lat.set_kernel("ring")
+            o, p, g = lat.new_spinor(), lat.new_spinor(), lat.new_gauge()
+            assert B.dslash_apply_status(lat.ctx, o.data_ptr(), p.data_ptr(), g.data_ptr()) == B.DSLASH_ERR_UNSUPPORTED, (dims, tile)
+            with pytest.raises(B.DslashError):
+                B.dslash_set_option(lat.ctx, B.DSLASH_OPT_T_CHUNK, dims[3] + 1)
+
+
 # ---------------------------------------------------------------- config 2: 16^4 FP64
 @pytest.mark.parametrize("layout,recon12", ALL_MODES)
 def test_config2_16x16x16x16(env, layout, recon12):
