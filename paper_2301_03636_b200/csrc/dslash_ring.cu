@@ -1,17 +1,19 @@
 // dslash_ring.cu -- t-marching Dslash kernel with a shared-memory ring of spinor time slices (DSLASH_KERNEL_RING), sm_100a.
 //
 // Same operator, same per-hop arithmetic and the same hop order as dslash_tuned.cu (Eq. 1; results
-// bit-identical).  What changes is where the spinors come from.  Measured (profiles/): the direct kernel moves 1.95 KB per
-// site from L2 into the SMs for 0.96 KB of compulsory HBM traffic and sits on the L2->SM throughput limit (~12 TB/s
-// chip-wide), not on HBM.  Here a block owns a SPATIAL tile of 32 x by x bz sites (one warp per x row = one 32-site vector of
-// the blocked SoA layout) and marches over a chunk of time slices.  The spinors of the tile's rows at t, t+1 (and t+2 in
-// flight) live in a ring of three shared-memory slots, each row brought in ONCE by one cp.async.bulk (TMA unit, SASS UBLKCP;
-// a row is 6 KB contiguous in fp64) a full step before it is needed, completion counted on one mbarrier per slot.  A step
-// reads from shared memory: the site's own spinor (x hops by warp shuffle), the in-tile y and z neighbours, psi(x,t+1); the
-// backward-t contribution w = U_t(x,t-1)^dagger P^+ psi(x,t-1) is carried in registers from the previous step, when both
-// operands were at hand.  Only the y/z halo spinors and the links still come through L1/L2.  Per site the SM now pulls
-//     psi: 1 (new slice) + 2/by (y halo) + 2/bz (z halo) vectors instead of 5;  links: U_t(x,t-1) no longer loaded
-// i.e. ~1.3 KB (32x2x2) instead of 1.95 KB.
+// bit-identical).  What changes is where the spinors come from.  The direct kernel moves 1.95 KB per site from L2 into the
+// SMs for 0.96 KB of compulsory HBM traffic.  Here a block owns a SPATIAL tile of 32 x by x bz sites (one warp per x row =
+// one 32-site vector of the blocked SoA layout) and marches over a chunk of time slices.  The spinors of the tile's rows at
+// t, t+1 (and t+2 in flight) live in a ring of three shared-memory slots, each row brought in ONCE by one cp.async.bulk (TMA
+// unit, SASS UBLKCP; a row is 6 KB contiguous in fp64) a full step before it is needed, completion counted on one mbarrier
+// per slot.  A step reads from shared memory: the site's own spinor (x hops by warp shuffle), the in-tile y and z
+// neighbours, psi(x,t+1); the backward-t contribution w = U_t(x,t-1)^dagger P^+ psi(x,t-1) is carried in registers from the
+// previous step, when both operands were at hand.  Only the y/z halo spinors and the links still come through L1/L2.
+//
+// MEASURED (profiles/r01d_ncu_direct_ring_eo.txt, 32^3x64 fp64): L2->SM traffic 4.07 -> 2.97 GB per launch and 45 % fewer
+// LSU load sectors, as designed -- but 0.40 ms against 0.34 ms for the direct kernel: inside the marching loop the eight
+// link-load wait points of a step are serialised and the kernel is bound by latency, not by L2->SM throughput.  It is
+// therefore opt-in (dslash_set_kernel), kept because it is the correct pipeline skeleton for staging the LINKS the same way.
 //
 // Synchronisation per step: one __syncthreads() (all warps are done with the slot that is refilled next), lane 0 of every
 // warp issues the bulk copy of its row for t+2 and arrives on that slot's mbarrier with the byte count, every thread waits

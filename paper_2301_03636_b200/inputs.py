@@ -156,3 +156,15 @@ def sample_sites(dims, n: int, seed: int) -> np.ndarray:
     rng = np.random.default_rng([int(seed), 3, 0])
     draws = rng.integers(0, v, size=max(0, n - len(corners)), dtype=np.int64)
     return np.unique(np.concatenate([np.asarray(corners, dtype=np.int64), draws]))
+
+
+# ------------------------------------------------------------------ random numbers the cost model draws (passed in as inputs)
+def uniforms(seed: int, n: int) -> np.ndarray:
+    """n float64 uniforms in [0, 1): the draws behind the Glorot initialisation (the scaling is the method's, not done here)."""
+    return np.random.default_rng([int(seed), 11, 0]).random(int(n))
+
+
+def permutations(seed: int, epochs: int, n: int) -> np.ndarray:
+    """int32 [epochs, n]: the order in which the n training rows are visited in each epoch."""
+    rng = np.random.default_rng([int(seed), 12, 0])
+    return np.stack([rng.permutation(int(n)) for _ in range(int(epochs))]).astype(np.int32)
