@@ -41,6 +41,31 @@ def test_library_exports_every_declared_symbol(B):
         assert hasattr(B, name), "binding lacks %s" % name
 
 
+def test_costmodel_header_symbols_are_exported_and_bound(B):
+    """include/advisor_costmodel.h: every declared costmodel_* call is exported by the same library and mirrored by
+    paper_2301_03636_b200/costmodel.py; the size queries need no device."""
+    text = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "advisor_costmodel.h")).read(), flags=re.S)
+    names = sorted(set(re.findall(r"\b(costmodel_[a-z0-9_]+)\s*\(", text)))
+    assert "costmodel_train" in names and "costmodel_predict" in names and len(names) == 10
+    lib = ctypes.CDLL(B.LIB_PATH)
+    from paper_2301_03636_b200 import costmodel as C
+    assert sorted(C.SIGNATURES) == names
+    for name in names:
+        assert hasattr(lib, name) and hasattr(C, name), name
+    # "with 33 input features, have 66, 132, 66, and 33 neurons" (PAPER.md:305)
+    assert C.costmodel_weight_count(33) == 33 * 66 + 66 * 132 + 132 * 66 + 66 * 33 + 33
+    assert C.costmodel_param_count(33) == C.costmodel_weight_count(33) + 66 + 132 + 66 + 33 + 1
+    assert C.costmodel_param_count(0) == 0 and C.costmodel_weight_count(-1) == 0
+    assert C.costmodel_train_smem_bytes(33, 16, 8) < C.costmodel_train_smem_bytes(33, 16, 4) <= 232448
+    assert C.costmodel_train_smem_bytes(33, 16, 5) == 0 and C.costmodel_train_smem_bytes(33, 65, 8) == 0
+    # argument validation precedes CUDA
+    assert C.costmodel_train_status(3, 10, 0, 0, 0, 0, 1, 16, 0.01, 30, 0.1, 1e-4, -1, 1, 0, 0, 0, 0) == B.DSLASH_ERR_NULL
+    assert C.costmodel_train_status(0, 10, 8, 8, 8, 8, 1, 16, 0.01, 30, 0.1, 1e-4, -1, 1, 0, 8, 0, 0) == B.DSLASH_ERR_DIMS
+    assert C.costmodel_train_status(3, 10, 8, 8, 12, 8, 1, 16, 0.01, 30, 0.1, 1e-4, -1, 1, 0, 8, 0, 0) == B.DSLASH_ERR_ALIGN
+    assert C.costmodel_train_status(3, 10, 8, 8, 8, 8, 1, 16, 0.01, 30, 0.1, 1e-4, -1, 1, 3, 8, 0, 0) == B.DSLASH_ERR_UNSUPPORTED
+    assert C.costmodel_launch_count() == 0
+
+
 def test_error_strings(B):
     assert B.dslash_error_string(0) == "DSLASH_OK"
     for code in range(-9, 0):
