@@ -545,6 +545,166 @@ def run_advisor(args):
     return 0
 
 
+# ------------------------------------------------------------------ the Advisor's cost model
+COSTMODEL_LATTICES = [(8, 8, 8, 8), (8, 8, 8, 16), (12, 12, 12, 12), (16, 16, 16, 8), (16, 16, 16, 16), (12, 12, 12, 24),
+                      (24, 24, 24, 12), (16, 16, 16, 32), (24, 24, 24, 24), (32, 32, 32, 16)]
+COSTMODEL_FEATURES = ["parallel_position", "distribute_collapse", "parallel_collapse", "sched_static", "sched_dynamic",
+                      "sched_guided", "log2_league_iterations", "log2_team_iterations", "log2_serial_iterations", "log2_volume",
+                      "log2_L_T", "log2_L_X"]
+
+
+def costmodel_features(dims, x, a, b, sched):
+    """The 12 inputs of this build's cost model for one kernel variant on one lattice.  The paper's 33 features are not
+    published (PAPER.md:305 gives only their number), so these are this build's choice (parity unpinned): the
+    variant parameters of PAPER.md:156-160 and the iteration counts they imply.  Loops outer -> inner = t, z, y, x."""
+    ext = [dims[3], dims[2], dims[1], dims[0]]  # Loop 0..3
+    league = float(np.prod(ext[:a])) if x > 0 else 1.0              # distribute collapse(a) over Loops 0..a-1
+    team = float(np.prod(ext[x:x + b]))                               # parallel for collapse(b) over Loops x..x+b-1
+    serial = float(np.prod(ext)) / (league * team)                    # what one thread runs serially per parallel iteration
+    return [x, a, b, float(sched == 0), float(sched == 1), float(sched == 2), np.log2(league), np.log2(team), np.log2(serial),
+            np.log2(float(np.prod(ext))), np.log2(ext[0]), np.log2(ext[3])]
+
+
+def collect_variant_timings(args, lattices):
+    """Training mode: run every kernel structure x schedule of the paper's space on each lattice, parity-check
+    it against the oracle, time it on the device.  Returns rows (features, runtime in ms, lattice, variant)."""
+    import torch
+    import oracle
+    from paper_2301_03636_b200 import binding as B
+    from paper_2301_03636_b200 import checks, device, inputs
+    rows = []
+    for dims in lattices:
+        g, p = inputs.fields(dims, SEED + 7, "f64", check=False)
+        ref = oracle.dslash(p, g, dims)
+        with device.Lattice(dims, "f64", "soa", False) as lat:
+            gd, pd, od = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
+            seen = set()
+            for i in range(B.dslash_omp_variant_count(4)):
+                x, a, b, sched, _mode = B.dslash_omp_variant_at(4, i)
+                if (x, a, b, sched) in seen:
+                    continue
+                seen.add((x, a, b, sched))
+                B.dslash_set_omp_variant(lat.ctx, x, a, b, sched, 0, args.team_size)
+                od.zero_()
+                lat.apply(od, pd, gd)
+                err = checks.parity_error(lat.download_spinor(od), ref)
+                lat.apply(od, pd, gd)
+                torch.cuda.synchronize()
+                times, budget = [], 0.05
+                while len(times) < 20 and (len(times) < 3 or budget > 0):
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record()
+                    lat.apply(od, pd, gd)
+                    e1.record()
+                    e1.synchronize()
+                    times.append(e0.elapsed_time(e1))
+                    budget -= times[-1] / 1e3
+                rows.append(dict(dims=dims, variant=(x, a, b, sched), ms=float(np.median(times)), parity=err,
+                                 features=costmodel_features(dims, x, a, b, sched)))
+    return rows
+
+
+def run_costmodel(args):
+    """The cost-model half of the Advisor on this build's own measurements: 42 kernel variants x 10 lattices -> runtime;
+    80 % / 20 % split, Z-score, the paper's MLP and optimiser settings, everything on the device through
+    include/advisor_costmodel.h; the NumPy oracle runs the same protocol beside it (parity of the result, CPU baseline)."""
+    import torch
+    from oracle import costmodel as ocm
+    from paper_2301_03636_b200 import costmodel as C
+    from paper_2301_03636_b200 import inputs
+    dev = torch.device("cuda:0")
+    t0 = time.perf_counter()
+    rows = collect_variant_timings(args, COSTMODEL_LATTICES[:args.costmodel_lattices])
+    collect_s = time.perf_counter() - t0
+    f = len(COSTMODEL_FEATURES)
+    n = len(rows)
+    x = np.array([r["features"] for r in rows], dtype=np.float64)
+    y_ms = np.array([r["ms"] for r in rows], dtype=np.float64)
+    order = inputs.permutations(SEED + 8, 1, n)[0]
+    ntr = int(round(0.8 * n))  # "80% for training and 20% for validation" (PAPER.md:311)
+    tr, va = np.sort(order[:ntr]), np.sort(order[ntr:])
+    epochs, batch, m = args.costmodel_epochs, 16, args.costmodel_models
+    nw = C.costmodel_weight_count(f)
+    uni = np.stack([inputs.uniforms(SEED + 100 + k, nw) for k in range(m)])
+    perms = np.stack([inputs.permutations(SEED + 100 + k, epochs, ntr) for k in range(m)])
+    out = {"costmodel": "MLP F-2F-4F-2F-F-1, RMSprop 0.01 x0.1/30 epochs, wd 1e-4, batch 16 (PAPER.md:305-307)",
+           "features": COSTMODEL_FEATURES, "rows": n, "train_rows": ntr, "validation_rows": n - ntr, "epochs": epochs,
+           "lattices": [list(d) for d in COSTMODEL_LATTICES[:args.costmodel_lattices]],
+           "all_variants_parity_ok": bool(max(r["parity"] for r in rows) <= 1e-12), "collect_seconds": collect_s,
+           "runtime_ms_range": [float(y_ms.min()), float(y_ms.max())], "targets": {}}
+    model = C.CostModel(f)
+    xd = torch.from_numpy(x).to(dev)
+    ud, pd = torch.from_numpy(uni).to(dev), torch.from_numpy(perms).to(dev)
+    idx_tr, idx_va = torch.from_numpy(tr).to(dev), torch.from_numpy(va).to(dev)
+    for target, y in (("runtime_ms", y_ms), ("log10_runtime_ms", np.log10(y_ms))):
+        yd = torch.from_numpy(y).to(dev)
+        xtr, ytr, xva, yva = xd[idx_tr].contiguous(), yd[idx_tr].contiguous(), xd[idx_va].contiguous(), yd[idx_va].contiguous()
+        launches0 = C.costmodel_launch_count()
+        model.fit_scaler(xtr, ytr)
+        xs_tr, ys_tr, xs_va, xs_all = model.scale_x(xtr), model.scale_y(ytr), model.scale_x(xva), model.scale_x(xd)
+        model.train(xs_tr, ys_tr, ud, pd, epochs=epochs, batch=batch)  # warm-up launch (module load, clocks)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        params, loss = model.train(xs_tr, ys_tr, ud, pd, epochs=epochs, batch=batch)
+        e1.record()
+        torch.cuda.synchronize()
+        train_ms = e0.elapsed_time(e1)
+        e0.record()
+        model.train(xs_tr, ys_tr, ud[:1], pd[:1], epochs=epochs, batch=batch)
+        e1.record()
+        torch.cuda.synchronize()
+        train1_ms = e0.elapsed_time(e1)
+        pred_va = model.predict(xs_va, params)
+        nrmse = []
+        for k in range(m):
+            pk = model.scale_y(pred_va[k].contiguous(), inverse=True)
+            nrmse.append(float(model.error(pk, yva).cpu().numpy()[1]))
+        pred_all = model.scale_y(model.predict(xs_all, params[:1])[0].contiguous(), inverse=True).cpu().numpy()
+        launches = C.costmodel_launch_count() - launches0
+        # ranking on the largest lattice: measured top-10 vs predicted top-10 of its 42 variants (model 0)
+        big = [i for i, r in enumerate(rows) if r["dims"] == COSTMODEL_LATTICES[args.costmodel_lattices - 1]]
+        top_meas = set(sorted(big, key=lambda i: y[i])[:10])
+        top_pred = set(sorted(big, key=lambda i: pred_all[i])[:10])
+        # the oracle, same protocol, model 0 (CPU baseline and parity of the outcome)
+        t0 = time.perf_counter()
+        mx, sx = ocm.zscore_fit(x[tr])
+        my, sy = ocm.zscore_fit(y[tr])
+        oxs, oys = ocm.zscore_apply(x, mx, sx), ocm.zscore_apply(y, my, sy)
+        oparams, oloss = ocm.train(f, oxs[tr], oys[tr], uni[0], perms[0], epochs=epochs, batch=batch)
+        opred = ocm.predict(oparams, oxs[va]) * sy[0] + my[0]
+        oracle_s = time.perf_counter() - t0
+        onrmse = ocm.nrmse(opred, y[va])
+        steps = epochs * ((ntr + batch - 1) // batch)
+        if target == "runtime_ms":
+            # Sensitivity of the protocol itself: the same training stopped after k updates, CUDA path vs oracle, next to the
+            # oracle vs the oracle with ONE training target moved by one ulp.  Both differences grow at the same exponential
+            # rate until they saturate, which is why whole-run parameters are compared statistically (NRMSE), not digit by digit.
+            oys_p = oys[tr].copy()
+            oys_p[0] = np.nextafter(oys_p[0], np.inf)
+            ks = [k for k in (10, 50, 100, 200, 400, 800, 1600, steps) if k <= steps]
+            grow = {"updates": ks, "cuda_vs_oracle": [], "oracle_vs_oracle_one_ulp": []}
+            for k in ks:
+                pk, _ = model.train(xs_tr, ys_tr, ud[:1], pd[:1], epochs=epochs, batch=batch, max_steps=k)
+                ok = ocm.pack(ocm.train(f, oxs[tr], oys[tr], uni[0], perms[0], epochs=epochs, batch=batch, max_steps=k)[0])
+                op = ocm.pack(ocm.train(f, oxs[tr], oys_p, uni[0], perms[0], epochs=epochs, batch=batch, max_steps=k)[0])
+                grow["cuda_vs_oracle"].append(float(np.abs(pk[0].cpu().numpy() - ok).max()))
+                grow["oracle_vs_oracle_one_ulp"].append(float(np.abs(op - ok).max()))
+            out["trajectory_sensitivity_max_abs_param_diff"] = grow
+        out["targets"][target] = {
+            "nrmse_validation": nrmse[0], "success_nrmse_below_0.1": bool(nrmse[0] < 0.1),
+            "nrmse_models": {"n": m, "mean": float(np.mean(nrmse)), "min": float(np.min(nrmse)), "max": float(np.max(nrmse))},
+            "oracle_nrmse_validation": float(onrmse), "nrmse_rel_diff_vs_oracle": float(abs(nrmse[0] - onrmse) / onrmse),
+            "params_max_abs_diff_vs_oracle": float(np.abs(params[0].cpu().numpy() - ocm.pack(oparams)).max()),
+            "final_epoch_loss": float(loss[0, -1].item()), "oracle_final_epoch_loss": float(oloss[-1]),
+            "top10_overlap_largest_lattice": len(top_meas & top_pred),
+            "train_ms_one_model": train1_ms, "us_per_update_one_model": 1e3 * train1_ms / steps,
+            "train_ms_all_models": train_ms, "model_updates_per_s": m * steps / (train_ms / 1e3),
+            "oracle_seconds_one_model": oracle_s, "oracle_updates_per_s": steps / oracle_s, "gpu_launches": int(launches)}
+    print(json.dumps(out))
+    return 0
+
+
 # ------------------------------------------------------------------ the solver around Dslash
 def run_cg(args):
     """CG on M^dagger M (dslash_cg_solve) on a BASELINE lattice: what "called several times throughout the LQCD
@@ -684,6 +844,10 @@ def main():
     ap.add_argument("--cg-mass", type=float, default=0.2)
     ap.add_argument("--cg-tol", type=float, default=1e-8)
     ap.add_argument("--cg-max-iter", type=int, default=2000)
+    ap.add_argument("--costmodel", action="store_true", help="fit the Advisor's cost model on the variants' measured runtimes")
+    ap.add_argument("--costmodel-lattices", type=int, default=len(COSTMODEL_LATTICES))
+    ap.add_argument("--costmodel-epochs", type=int, default=150)
+    ap.add_argument("--costmodel-models", type=int, default=16, help="independent seeds trained in the same launch")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "cuda" and not args.sweep:
         args.warmup = 3  # timing rule: at least 3 warm-up steps
@@ -691,6 +855,8 @@ def main():
         return run_sweep(args)
     if args.advisor:
         return run_advisor(args)
+    if args.costmodel:
+        return run_costmodel(args)
     if args.cg:
         return run_cg(args)
     if args.eo:

@@ -87,6 +87,11 @@ DSLASH_API int costmodel_zscore_apply(int n, int cols, const double *a, const do
  * NaN if RMSE == 0 as well), over n >= 1 values.  Deterministic. */
 DSLASH_API int costmodel_error(int n, const double *pred, const double *y, double *out, dslash_stream_t stream);
 
+/* Tuning knobs of costmodel_train() (process-wide).  COSTMODEL_OPT_THREADS: threads per block, a multiple of 32 in 32..1024,
+ * 0 = the library's default.  Results do not depend on it bit for bit.  Anything else: DSLASH_ERR_UNSUPPORTED. */
+#define COSTMODEL_OPT_THREADS 1
+DSLASH_API int costmodel_set_option(int option, int value);
+
 /* The cudaError_t of the last failed CUDA call of a costmodel_* function on this host thread's library (0 if none). */
 DSLASH_API int costmodel_last_cuda_error(void);
 

@@ -22,6 +22,7 @@ SIGNATURES = {
     "costmodel_zscore_fit": (_i, [_i, _i, _vp, _vp, _vp, _vp]),
     "costmodel_zscore_apply": (_i, [_i, _i, _vp, _vp, _vp, _i, _vp, _vp]),
     "costmodel_error": (_i, [_i, _vp, _vp, _vp, _vp]),
+    "costmodel_set_option": (_i, [_i, _i]),
     "costmodel_last_cuda_error": (_i, []),
     "costmodel_launch_count": (_ll, []),
 }
@@ -87,6 +88,13 @@ def costmodel_zscore_apply(n, cols, a, mean, std, inverse, out, stream) -> None:
 
 def costmodel_error(n, pred, y, out, stream) -> None:
     _check(_lib.costmodel_error(int(n), _ptr(pred), _ptr(y), _ptr(out), _ptr(stream)), "costmodel_error")
+
+
+COSTMODEL_OPT_THREADS = 1
+
+
+def costmodel_set_option(option: int, value: int) -> None:
+    _check(_lib.costmodel_set_option(int(option), int(value)), "costmodel_set_option")
 
 
 def costmodel_last_cuda_error() -> int:

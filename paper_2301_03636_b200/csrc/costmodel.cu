@@ -30,12 +30,14 @@ namespace {
 constexpr int kLayers = 5;
 constexpr int kMaxBatch = 64;
 constexpr int kMaxLrSteps = 32;
-constexpr int kThreads = 256;
+constexpr int kThreads = 256;       // block size of the small kernels
+constexpr int kTrainMaxThreads = 1024;
 constexpr size_t kMaxSmem = 232448;  // 227 KB opt-in limit of sm_100
 constexpr double kAlpha = 0.99;      // RMSprop smoothing constant (Reading R22)
 constexpr double kEps = 1e-8;        // added to sqrt(v) (Reading R22)
 
 std::atomic<long long> g_launches{0};
+std::atomic<int> g_train_threads{0};  // COSTMODEL_OPT_THREADS (0: default)
 thread_local int g_last_cuda = 0;
 
 inline int cuda_fail(cudaError_t e) {
@@ -124,15 +126,22 @@ struct TrainArgs {
     double weight_decay;
     long long max_steps;
     double lr[kMaxLrSteps];  // lr0 * gamma^k
+    Shape S;                 // in the kernel's constant bank: indexing it by layer costs no local memory (a cluster barrier
+    Plan P;                  // invalidates L1, so a stack copy would be re-fetched from L2 after every barrier)
 };
 
 // z[b][r] = sum_i W[r][i] a[b][i] + bias[r] for the rows r < rows of a weight block and the nb samples of the batch; one
-// work item = one row x four samples (the weight is loaded once for four FMAs).  emit(b, r, z) consumes the result.
+// work item = one row x four samples (the weight is loaded once for four FMAs), shared by KS = 2^k <= 32 adjacent lanes: lane
+// kl sums the terms i = kl, kl + KS, ... and a butterfly of shuffles adds the KS partial sums (the same bits in every lane).
+// emit(b, r, z) consumes the result.  All threads of the block must call it (full-warp shuffles).
 template <class Emit>
 __device__ __forceinline__ void dense_rows(const double* __restrict__ W, int sw, const double* __restrict__ bias, int rows, int n_in,
-                                           const double* __restrict__ a, int sa, int nb, Emit emit) {
-    const int nbq = (nb + 3) >> 2;
-    for (int item = threadIdx.x; item < rows * nbq; item += blockDim.x) {
+                                           const double* __restrict__ a, int sa, int nb, int ks, Emit emit) {
+    const int nbq = (nb + 3) >> 2, nitems = rows * nbq;
+    const int group = threadIdx.x / ks, kl = threadIdx.x - group * ks, ngroups = blockDim.x / ks;
+    for (int base = 0; base < nitems; base += ngroups) {
+        const bool valid = base + group < nitems;
+        const int item = valid ? base + group : nitems - 1;
         const int r = item / nbq, b0 = (item - r * nbq) * 4;
         const double* wr = W + (size_t)r * sw;
         const double* a0 = a + (size_t)b0 * sa;
@@ -140,19 +149,36 @@ __device__ __forceinline__ void dense_rows(const double* __restrict__ W, int sw,
         const double* a2 = a + (size_t)min(b0 + 2, nb - 1) * sa;
         const double* a3 = a + (size_t)min(b0 + 3, nb - 1) * sa;
         double z0 = 0.0, z1 = 0.0, z2 = 0.0, z3 = 0.0;
-        for (int i = 0; i < n_in; ++i) {
+        for (int i = kl; i < n_in; i += ks) {
             const double wv = wr[i];
             z0 = fma(wv, a0[i], z0);
             z1 = fma(wv, a1[i], z1);
             z2 = fma(wv, a2[i], z2);
             z3 = fma(wv, a3[i], z3);
         }
+        for (int m = 1; m < ks; m <<= 1) {
+            z0 += __shfl_xor_sync(0xffffffffu, z0, m);
+            z1 += __shfl_xor_sync(0xffffffffu, z1, m);
+            z2 += __shfl_xor_sync(0xffffffffu, z2, m);
+            z3 += __shfl_xor_sync(0xffffffffu, z3, m);
+        }
+        if (!valid) continue;
         const double bv = bias[r];
-        emit(b0, r, z0 + bv);
-        if (b0 + 1 < nb) emit(b0 + 1, r, z1 + bv);
-        if (b0 + 2 < nb) emit(b0 + 2, r, z2 + bv);
-        if (b0 + 3 < nb) emit(b0 + 3, r, z3 + bv);
+        const int km = ks - 1;  // the four results are emitted by (up to) four different lanes of the group
+        if ((0 & km) == kl) emit(b0, r, z0 + bv);
+        if ((1 & km) == kl && b0 + 1 < nb) emit(b0 + 1, r, z1 + bv);
+        if ((2 & km) == kl && b0 + 2 < nb) emit(b0 + 2, r, z2 + bv);
+        if ((3 & km) == kl && b0 + 3 < nb) emit(b0 + 3, r, z3 + bv);
     }
+}
+
+// Lanes per work item of dense_rows in the training kernel: as many as keep 512 threads busy, at least 4 terms per lane.  A
+// function of the layer and batch alone, NOT of the launch's block size, so that results do not depend on the latter.
+__device__ __forceinline__ int lanes_per_item(int rows, int nb, int n_in) {
+    const int nitems = rows * ((nb + 3) >> 2);
+    int ks = 1;
+    while (ks < 32 && nitems * ks * 2 <= 512 && ks * 8 <= n_in) ks *= 2;
+    return ks;
 }
 
 // One RMSprop update (Reading R22), in the oracle's order of operations: g += wd p; v = 0.99 v + (0.01 g) g;
@@ -163,24 +189,26 @@ __device__ __forceinline__ void rmsprop(double& p, double& v, double g, double l
     p = __dsub_rn(p, __ddiv_rn(__dmul_rn(lr, g), __dadd_rn(__dsqrt_rn(v), kEps)));
 }
 
-__global__ void __launch_bounds__(kThreads, 1) costmodel_train_kernel(const TrainArgs A) {
+__global__ void __launch_bounds__(kTrainMaxThreads, 1) costmodel_train_kernel(const TrainArgs A) {
     extern __shared__ double sm[];
     cg::cluster_group cluster = cg::this_cluster();
     const int C = A.C;
     const int rank = (int)cluster.block_rank();
     const int model = blockIdx.x / C;
     const int tid = threadIdx.x, nthr = blockDim.x;
-    const Shape S = make_shape(A.f);
-    const Plan P = make_plan(S, A.batch, C);
-    int lo[kLayers], rows[kLayers];
-    for (int l = 0; l < kLayers; ++l) {
-        lo[l] = (int)(((long long)S.w[l + 1] * rank) / C);
-        rows[l] = (int)(((long long)S.w[l + 1] * (rank + 1)) / C) - lo[l];
+    const Shape& S = A.S;
+    const Plan& P = A.P;
+    __shared__ int lo[kLayers], rows[kLayers];  // the block's neurons of layer l: [lo, lo + rows)
+    if (tid < kLayers) {
+        lo[tid] = (int)(((long long)S.w[tid + 1] * rank) / C);
+        rows[tid] = (int)(((long long)S.w[tid + 1] * (rank + 1)) / C) - lo[tid];
     }
+    __syncthreads();
     const double* uni = A.uniforms + (size_t)model * S.nweight;
     const int* perms = A.perms + (size_t)model * A.epochs * A.n;
     int* idx = reinterpret_cast<int*>(sm + P.idx);
     const bool owner = rows[kLayers - 1] == 1;  // the block that holds the single output neuron (the last one of the cluster)
+    const bool solo = C == 1;                   // a cluster of one block: block barriers do
 
     // Glorot uniform initialisation (Reading R21), biases and RMSprop accumulators 0
     for (int l = 0; l < kLayers; ++l) {
@@ -230,15 +258,17 @@ __global__ void __launch_bounds__(kThreads, 1) costmodel_train_kernel(const Trai
                 double* out_local = sm + P.act[l + 1];
                 const int lo_l = lo[l];
                 dense_rows(sm + P.wrow[l], odd(S.w[l]), sm + P.brow[l], rows[l], S.w[l], sm + P.act[l], odd(S.w[l]), nb,
+                           lanes_per_item(rows[l], nb, S.w[l]),
                            [&](int b, int r, double z) {
                                const double a = fmax(z, 0.0);  // ReLU (Reading R20)
                                double* dst = out_local + b * sa_out + lo_l + r;
                                for (int c = 0; c < C; ++c) *cluster.map_shared_rank(dst, c) = a;
                            });
-                cluster.sync();
+                if (solo) __syncthreads(); else cluster.sync();
             }
             // ---- output layer (one neuron, owned by one block), loss (Eq. 2) and its derivative (Reading R23)
             dense_rows(sm + P.wrow[4], odd(S.w[4]), sm + P.brow[4], rows[4], S.w[4], sm + P.act[4], odd(S.w[4]), nb,
+                       lanes_per_item(rows[4], nb, S.w[4]),
                        [&](int b, int, double z) { sm[P.pred + b] = z; });
             __syncthreads();
             if (owner && tid < 32) {
@@ -286,11 +316,12 @@ __global__ void __launch_bounds__(kThreads, 1) costmodel_train_kernel(const Trai
                         if (b0 + 3 < nb) part[(b0 + 3) * sa + i] = p3;
                     }
                     __syncthreads();           // every thread has read the old W_l before anyone updates it
-                    cluster.barrier_arrive();  // release: the partial is visible to the peers after their wait
+                    if (!solo) cluster.barrier_arrive();  // release: the partial is visible to the peers after their wait
                 }
                 // gradient of the own rows and RMSprop in place: g[r][i] = sum_b delta_l[b][r] a_l[b][i] (i == n_in: the bias)
                 {
                     const double* al = sm + P.act[l];
+                    double* bl = sm + P.brow[l];
                     for (int k = tid; k < nrow * (n_in + 1); k += nthr) {
                         const int r = k / (n_in + 1), i = k - r * (n_in + 1);
                         double g = 0.0;
@@ -300,13 +331,13 @@ __global__ void __launch_bounds__(kThreads, 1) costmodel_train_kernel(const Trai
                             rmsprop(p[0], p[P.vshift], g, lr, A.weight_decay);
                         } else {
                             for (int b = 0; b < nb; ++b) g += dl[b * P.drow + r];
-                            double* p = sm + P.brow[l] + r;
+                            double* p = bl + r;
                             rmsprop(p[0], p[P.vshift], g, lr, A.weight_decay);
                         }
                     }
                 }
                 if (l > 0) {
-                    cluster.barrier_wait();  // acquire: all partials of this layer are complete
+                    if (solo) __syncthreads(); else cluster.barrier_wait();  // acquire: all partials of this layer are complete
                     // delta of the own neurons of layer l-1: sum of the C partials in block order, times the ReLU mask
                     const double* part = sm + P.part[l & 1];
                     const double* al = sm + P.act[l];
@@ -323,7 +354,7 @@ __global__ void __launch_bounds__(kThreads, 1) costmodel_train_kernel(const Trai
                 }
             }
             ++steps;
-            cluster.sync();  // nobody overwrites activations / partials of this step while a peer still reads them
+            if (solo) __syncthreads(); else cluster.sync();  // nobody overwrites activations / partials of this step while a peer still reads them
         }
         if (owner && tid == 0 && A.epoch_loss_out)
             A.epoch_loss_out[(size_t)model * A.epochs + e] = nloss ? loss_sum / (double)nloss : nan("");
@@ -369,10 +400,10 @@ __global__ void __launch_bounds__(kThreads) costmodel_predict_kernel(int f, int 
             const int n_in = S.w[l], n_out = S.w[l + 1];
             const double* W = P + S.poff[l];
             if (l < kLayers - 1) {
-                dense_rows(W, n_in, W + (size_t)n_in * n_out, n_out, n_in, in, sa, nb,
+                dense_rows(W, n_in, W + (size_t)n_in * n_out, n_out, n_in, in, sa, nb, 1,
                            [&](int b, int r, double z) { out[b * sa + r] = fmax(z, 0.0); });
             } else {
-                dense_rows(W, n_in, W + (size_t)n_in * n_out, n_out, n_in, in, sa, nb,
+                dense_rows(W, n_in, W + (size_t)n_in * n_out, n_out, n_in, in, sa, nb, 1,
                            [&](int b, int, double z) { pred[(size_t)model * n + r0 + b] = z; });
             }
             __syncthreads();
@@ -462,6 +493,13 @@ size_t costmodel_train_smem_bytes(int f, int batch, int cluster_size) {
     return (size_t)make_plan(make_shape(f), batch, cluster_size).total * sizeof(double);
 }
 
+int costmodel_set_option(int option, int value) {
+    if (option != COSTMODEL_OPT_THREADS) return DSLASH_ERR_UNSUPPORTED;
+    if (value != 0 && (value < 32 || value > kTrainMaxThreads || value % 32)) return DSLASH_ERR_UNSUPPORTED;
+    g_train_threads.store(value);
+    return DSLASH_OK;
+}
+
 int costmodel_last_cuda_error(void) { return g_last_cuda; }
 long long costmodel_launch_count(void) { return g_launches.load(); }
 
@@ -477,11 +515,12 @@ int costmodel_train(int f, int n, const double* x, const double* y, const double
         return DSLASH_ERR_UNSUPPORTED;
     const int nlr = (lr_step > 0 && epochs > 0) ? (epochs - 1) / lr_step + 1 : 1;
     if (nlr > kMaxLrSteps) return DSLASH_ERR_UNSUPPORTED;
+    const int threads = g_train_threads.load() > 0 ? g_train_threads.load() : 512;
     int C = cluster_size;
     if (C == 0) {
         // one block while the widest layer gives every thread at most one work item, more blocks as the layers grow
         C = 1;
-        while (C < 8 && (costmodel_train_smem_bytes(f, batch, C) > kMaxSmem || 4 * f * ((batch + 3) / 4) > kThreads * C)) C *= 2;
+        while (C < 8 && (costmodel_train_smem_bytes(f, batch, C) > kMaxSmem || 4 * f * ((batch + 3) / 4) > threads * C)) C *= 2;
     }
     const size_t smem = costmodel_train_smem_bytes(f, batch, C);
     if (smem == 0 || smem > kMaxSmem) return DSLASH_ERR_UNSUPPORTED;
@@ -492,12 +531,14 @@ int costmodel_train(int f, int n, const double* x, const double* y, const double
     A.params_out = params_out; A.epoch_loss_out = epoch_loss_out;
     A.weight_decay = weight_decay; A.max_steps = max_steps;
     for (int k = 0; k < kMaxLrSteps; ++k) A.lr[k] = lr0 * pow(lr_gamma, (double)k);
+    A.S = make_shape(f);
+    A.P = make_plan(A.S, batch, C);
 
     cudaError_t e = cudaFuncSetAttribute(costmodel_train_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return cuda_fail(e);
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)(n_models * C), 1, 1);
-    cfg.blockDim = dim3(kThreads, 1, 1);
+    cfg.blockDim = dim3((unsigned)threads, 1, 1);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = (cudaStream_t)stream;
     cudaLaunchAttribute attr[1];

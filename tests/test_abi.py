@@ -46,7 +46,7 @@ def test_costmodel_header_symbols_are_exported_and_bound(B):
     paper_2301_03636_b200/costmodel.py; the size queries need no device."""
     text = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "advisor_costmodel.h")).read(), flags=re.S)
     names = sorted(set(re.findall(r"\b(costmodel_[a-z0-9_]+)\s*\(", text)))
-    assert "costmodel_train" in names and "costmodel_predict" in names and len(names) == 10
+    assert "costmodel_train" in names and "costmodel_predict" in names and len(names) == 11
     lib = ctypes.CDLL(B.LIB_PATH)
     from paper_2301_03636_b200 import costmodel as C
     assert sorted(C.SIGNATURES) == names
