@@ -217,6 +217,10 @@ def run_cuda(args, cfg):
                 B.dslash_set_option(lat.ctx, B.DSLASH_OPT_X_SHUFFLE, args.x_shuffle)
             if args.t_chunk is not None:
                 B.dslash_set_option(lat.ctx, B.DSLASH_OPT_T_CHUNK, args.t_chunk)
+            if args.pipe_slots is not None:
+                B.dslash_set_option(lat.ctx, B.DSLASH_OPT_PIPE_SLOTS, args.pipe_slots)
+            if args.pipe_warps is not None:
+                B.dslash_set_option(lat.ctx, B.DSLASH_OPT_PIPE_WARPS, args.pipe_warps)
             gd, pd, od = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
             n0 = B.dslash_launch_count(lat.ctx)
             ms, ck = time_applies(torch, lat, od, pd, gd, args.steps, args.warmup, group, local)
@@ -227,7 +231,7 @@ def run_cuda(args, cfg):
                                 gbs=bps * v / (ms / args.steps) / 1e6, bps=bps, recon12=recon12,
                                 tile=list(B.dslash_get_tile(lat.ctx)),
                                 kernel={B.DSLASH_KERNEL_DIRECT: "direct", B.DSLASH_KERNEL_TMA: "tma", B.DSLASH_KERNEL_TMA_LINKS: "tma_links",
-                                        B.DSLASH_KERNEL_RING: "ring"}[B.dslash_get_kernel(lat.ctx)],
+                                        B.DSLASH_KERNEL_RING: "ring", B.DSLASH_KERNEL_WARP_PIPE: "wpipe"}[B.dslash_get_kernel(lat.ctx)],
                                 t_chunk=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_T_CHUNK),
                                 occupancy=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_OCCUPANCY),
                                 x_shuffle=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_X_SHUFFLE))
@@ -821,7 +825,9 @@ def main():
     ap.add_argument("--layout", choices=["soa", "aos"], default="soa")
     ap.add_argument("--tile", type=int, nargs=4, default=None, help="tile of the tuned kernel (x y z t)")
     ap.add_argument("--occupancy", type=int, default=None, help="DSLASH_OPT_OCCUPANCY override")
-    ap.add_argument("--kernel", choices=["auto", "direct", "tma", "tma_links", "ring"], default=None)
+    ap.add_argument("--kernel", choices=["auto", "direct", "tma", "tma_links", "ring", "wpipe"], default=None)
+    ap.add_argument("--pipe-slots", type=int, default=None, help="DSLASH_OPT_PIPE_SLOTS override (wpipe kernel)")
+    ap.add_argument("--pipe-warps", type=int, default=None, help="DSLASH_OPT_PIPE_WARPS override (wpipe kernel)")
     ap.add_argument("--t-chunk", type=int, default=None, help="DSLASH_OPT_T_CHUNK override (ring kernel)")
     ap.add_argument("--x-shuffle", type=int, choices=[0, 1], default=None, help="DSLASH_OPT_X_SHUFFLE override")
     ap.add_argument("--both-recon", action="store_true", default=True, help="also time the other link compression")

@@ -106,6 +106,10 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
 #define DSLASH_KERNEL_RING 4   /* t-marching with the tile's spinor rows of t, t+1, t+2 in a shared-memory ring filled by bulk
                                   async copies one step ahead (blocked SoA, tile 32 x by x bz x 1 that tiles the lattice exactly,
                                   L_X a multiple of 32); bit-identical to DSLASH_KERNEL_DIRECT */
+#define DSLASH_KERNEL_WARP_PIPE 5 /* persistent warps, one 32-site x row per warp; every hop stage (neighbour spinors + links of
+                                  the row: two contiguous runs in the blocked SoA layout) is brought into per-warp shared-memory
+                                  slots by two bulk async copies, DSLASH_OPT_PIPE_SLOTS stages ahead, no block barriers
+                                  (blocked SoA, L_X == 32); bit-identical to DSLASH_KERNEL_DIRECT */
 
 /* options of the tuned kernels, dslash_set_option() */
 #define DSLASH_OPT_OCCUPANCY 2        /* blocks of <= 128 threads: 0 = 168 registers/thread (12 warps/SM), 1 = 128 (16 warps),
@@ -120,6 +124,8 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
                                          for bit */
 
 #define DSLASH_OPT_T_CHUNK 6          /* ring kernel: time slices a block marches through, 1..L_T (0 = library default 8) */
+#define DSLASH_OPT_PIPE_SLOTS 7       /* warp-pipelined kernel: hop stages in flight per warp, 2..4 (0 = library default) */
+#define DSLASH_OPT_PIPE_WARPS 8       /* warp-pipelined kernel: warps per thread block, 1 or 4 (0 = library default) */
 
 /* host<->device mapping modes of dslash_apply_host() (section 4.1.2) */
 #define DSLASH_MAP_MINIMAL 0 /* to: gauge, in;  from: out            (after the Advisor's data analysis) */

@@ -230,6 +230,8 @@ int dslash_create(dslash_ctx** ctx, const int dims[4], int precision, int layout
     c->cfg.l2_policy = 0;
     c->cfg.l1_carveout = -1;
     c->cfg.t_chunk = 0;
+    c->cfg.pipe_slots = 0;
+    c->cfg.pipe_warps = 0;
     c->cfg.x_shuffle = precision == DSLASH_FP64 ? 1 : 0;  // measured: -1.3 % (burst) / -2 % (sustained) in fp64, +0.8 % in fp32
     c->launches = 0;
     c->last_cuda = 0;
@@ -281,6 +283,7 @@ static int resolve_kernel(const dslash_ctx* c) {
     if (c->kernel == DSLASH_KERNEL_DIRECT) return DSLASH_KERNEL_DIRECT;
     if (c->kernel == DSLASH_KERNEL_TMA || c->kernel == DSLASH_KERNEL_TMA_LINKS) return can_tma ? c->kernel : -1;
     if (c->kernel == DSLASH_KERNEL_RING) return ring_eligible(c->layout_base, c->geom, c->tg) ? DSLASH_KERNEL_RING : -1;
+    if (c->kernel == DSLASH_KERNEL_WARP_PIPE) return wpipe_eligible(c->layout_base, c->geom) ? DSLASH_KERNEL_WARP_PIPE : -1;
     return DSLASH_KERNEL_DIRECT;  // AUTO
 }
 
@@ -302,6 +305,7 @@ int dslash_apply(dslash_ctx* c, void* out, const void* in, const void* gauge, ds
         if (k < 0) return DSLASH_ERR_UNSUPPORTED;
         e = (k == DSLASH_KERNEL_DIRECT)   ? launch_tuned(c->precision, c->layout_base, c->recon, a, c->tg, c->cfg)
             : (k == DSLASH_KERNEL_RING)   ? launch_ring(c->precision, c->layout_base, c->recon, a, c->tg, c->cfg)
+            : (k == DSLASH_KERNEL_WARP_PIPE) ? launch_wpipe(c->precision, c->layout_base, c->recon, a, c->tg, c->cfg)
                                           : launch_tma(c->precision, c->recon, a, c->tg, k == DSLASH_KERNEL_TMA_LINKS);
     } else if (!full_time_range(c)) {
         return DSLASH_ERR_UNSUPPORTED;  // the variant kernels always sweep the whole lattice
@@ -680,6 +684,14 @@ int dslash_set_option(dslash_ctx* c, int option, int value) {
             if (value < 0 || value > 1) return DSLASH_ERR_UNSUPPORTED;
             c->cfg.x_shuffle = value;
             return DSLASH_OK;
+        case DSLASH_OPT_PIPE_SLOTS:
+            if (value != 0 && (value < 2 || value > 4)) return DSLASH_ERR_UNSUPPORTED;
+            c->cfg.pipe_slots = value;
+            return DSLASH_OK;
+        case DSLASH_OPT_PIPE_WARPS:
+            if (value != 0 && value != 1 && value != 4) return DSLASH_ERR_UNSUPPORTED;
+            c->cfg.pipe_warps = value;
+            return DSLASH_OK;
         default:
             return DSLASH_ERR_UNSUPPORTED;
     }
@@ -693,6 +705,8 @@ int dslash_get_option(const dslash_ctx* c, int option, int* value) {
         case DSLASH_OPT_L1_CARVEOUT: *value = c->cfg.l1_carveout; return DSLASH_OK;
         case DSLASH_OPT_X_SHUFFLE: *value = c->cfg.x_shuffle; return DSLASH_OK;
         case DSLASH_OPT_T_CHUNK: *value = c->cfg.t_chunk; return DSLASH_OK;
+        case DSLASH_OPT_PIPE_SLOTS: *value = c->cfg.pipe_slots; return DSLASH_OK;
+        case DSLASH_OPT_PIPE_WARPS: *value = c->cfg.pipe_warps; return DSLASH_OK;
         default: return DSLASH_ERR_UNSUPPORTED;
     }
 }
@@ -700,7 +714,7 @@ int dslash_get_option(const dslash_ctx* c, int option, int* value) {
 int dslash_set_kernel(dslash_ctx* c, int kernel) {
     if (!c) return DSLASH_ERR_NULL;
     if (kernel != DSLASH_KERNEL_AUTO && kernel != DSLASH_KERNEL_DIRECT && kernel != DSLASH_KERNEL_TMA &&
-        kernel != DSLASH_KERNEL_TMA_LINKS && kernel != DSLASH_KERNEL_RING)
+        kernel != DSLASH_KERNEL_TMA_LINKS && kernel != DSLASH_KERNEL_RING && kernel != DSLASH_KERNEL_WARP_PIPE)
         return DSLASH_ERR_UNSUPPORTED;
     c->kernel = kernel;
     return DSLASH_OK;

@@ -37,6 +37,8 @@ struct TunedConfig {
     int l2_policy;         // DSLASH_OPT_L2_POLICY bits (0: no cache hints)
     int l1_carveout;       // preferred shared-memory carve-out of the direct kernel in percent (-1: driver default)
     int t_chunk;           // time slices a block of the ring kernel marches through (0: default)
+    int pipe_slots;        // warp-pipelined kernel: stages in flight per warp (2..4; 0: default 2)
+    int pipe_warps;        // warp-pipelined kernel: warps per block (1 or 4; 0: default 1)
     int x_shuffle;         // 1: exchange the x hops inside the warp when the tile allows it (fp64 default), 0: always load them
 };
 bool x_shuffle_eligible(const Geom& g, const TileGeom& tg);
@@ -48,6 +50,10 @@ cudaError_t launch_tuned(int precision, int layout_base, int recon, const Launch
 // t-marching kernel with a shared-memory ring of spinor time slices fed by bulk async copies (dslash_ring.cu).
 bool ring_eligible(int layout_base, const Geom& g, const TileGeom& tg);
 cudaError_t launch_ring(int precision, int layout_base, int recon, const LaunchArgs& a, const TileGeom& tg, const TunedConfig& cfg);
+
+// warp-pipelined kernel: every hop stage of a 32-site row by two bulk async copies into per-warp shared-memory slots (dslash_wpipe.cu).
+bool wpipe_eligible(int layout_base, const Geom& g);
+cudaError_t launch_wpipe(int precision, int layout_base, int recon, const LaunchArgs& a, const TileGeom& tg, const TunedConfig& cfg);
 
 // TMA-staged kernel (SoA only): tile's own spinors + links by cp.async.bulk.tensor into shared memory.
 bool tma_eligible(int precision, int recon, const Geom& g, const TileGeom& tg);
