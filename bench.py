@@ -47,7 +47,11 @@ CONFIGS = {
 NCU_TRAFFIC_BYTES = {
     # profiles/r01_ncu_tuned_kernel.txt, capture r01c: 1.6424 GB read + 0.3903 GB written (mean of 2 launches)
     "32x32x32x64_f64_soa_r18": 2032698000,
+    # profiles/r01f_ncu_wpipe.txt: the warp-pipelined kernel, 1.689388 GB read + 0.391466 GB written
+    "32x32x32x64_f64_soa_r18_wpipe": 2080854000,
 }
+KERNEL_NAMES = {"direct": "dslash_tuned_kernel", "wpipe": "dslash_wpipe_kernel", "ring": "dslash_ring_kernel", "tma": "dslash_tma_kernel",
+                "tma_links": "dslash_tma_kernel"}
 
 
 def bytes_per_site(precision, recon12):
@@ -222,6 +226,9 @@ def run_cuda(args, cfg):
             if args.pipe_warps is not None:
                 B.dslash_set_option(lat.ctx, B.DSLASH_OPT_PIPE_WARPS, args.pipe_warps)
             gd, pd, od = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
+            tuned = None
+            if not args.kernel and not args.no_tune:
+                tuned = lat.tune(od, pd, gd)  # outside the timed region: the library picks its kernel by measurement
             n0 = B.dslash_launch_count(lat.ctx)
             ms, ck = time_applies(torch, lat, od, pd, gd, args.steps, args.warmup, group, local)
             n1 = B.dslash_launch_count(lat.ctx)
@@ -234,7 +241,8 @@ def run_cuda(args, cfg):
                                         B.DSLASH_KERNEL_RING: "ring", B.DSLASH_KERNEL_WARP_PIPE: "wpipe"}[B.dslash_get_kernel(lat.ctx)],
                                 t_chunk=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_T_CHUNK),
                                 occupancy=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_OCCUPANCY),
-                                x_shuffle=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_X_SHUFFLE))
+                                x_shuffle=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_X_SHUFFLE),
+                                tuned_ms=None if tuned is None else tuned[1])
             if tag == "main":
                 clocks, launches = ck, n1 - n0 - args.warmup
                 if args.sustained_steps > 0:
@@ -249,7 +257,8 @@ def run_cuda(args, cfg):
     peak, peak_src = hbm_peak()
     key = "%s_%s_%s_r%d" % ("x".join(map(str, dims)), prec, args.layout, 12 if main["recon12"] else 18)
     roofline = {"bound": "hbm", "achieved": main["gbs"], "peak": peak, "unit": "GB/s", "frac": main["gbs"] / peak,
-                "traffic": NCU_TRAFFIC_BYTES.get(key), "peak_source": peak_src, "kernel": "dslash_tuned_kernel",
+                "traffic": NCU_TRAFFIC_BYTES.get(key if main["kernel"] == "direct" else key + "_" + main["kernel"]),
+                "peak_source": peak_src, "kernel": KERNEL_NAMES.get(main["kernel"], main["kernel"]),
                 "algorithmic_bytes_per_site": main["bps"], "algorithmic_bytes_per_launch": main["bps"] * v,
                 "frac_of_nominal_8TBs": main["gbs"] / 8000.0}
 
@@ -293,7 +302,8 @@ def run_cuda(args, cfg):
             "warmup": args.warmup, "ms_per_step": main["ms_per_step"], "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": prec, "data": "synthetic",
             "config": {"workload": cfg["name"], "dims": list(dims), "layout": args.layout, "recon": 12 if main["recon12"] else 18,
-                       "tile": main["tile"], "kernel": main["kernel"], "occupancy_option": main["occupancy"],
+                       "tile": main["tile"], "kernel": main["kernel"],
+                       "kernel_chosen_by": "dslash_tune (measured before the timed region)" if main["tuned_ms"] is not None else "option", "occupancy_option": main["occupancy"],
                        "x_shuffle_option": main["x_shuffle"], "t_chunk_option": main["t_chunk"], "sites": v, "parallelism": "replicas x%d" % world,
                        "l2": "inputs larger than L2: %.2f GB working set per apply vs 126 MB L2, no flush needed"
                              % (main["bps"] * v / 1e9)},
@@ -826,6 +836,7 @@ def main():
     ap.add_argument("--tile", type=int, nargs=4, default=None, help="tile of the tuned kernel (x y z t)")
     ap.add_argument("--occupancy", type=int, default=None, help="DSLASH_OPT_OCCUPANCY override")
     ap.add_argument("--kernel", choices=["auto", "direct", "tma", "tma_links", "ring", "wpipe"], default=None)
+    ap.add_argument("--no-tune", action="store_true", help="skip dslash_tune (keep the library's static default kernel)")
     ap.add_argument("--pipe-slots", type=int, default=None, help="DSLASH_OPT_PIPE_SLOTS override (wpipe kernel)")
     ap.add_argument("--pipe-warps", type=int, default=None, help="DSLASH_OPT_PIPE_WARPS override (wpipe kernel)")
     ap.add_argument("--t-chunk", type=int, default=None, help="DSLASH_OPT_T_CHUNK override (ring kernel)")

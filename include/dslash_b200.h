@@ -125,7 +125,9 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
 
 #define DSLASH_OPT_T_CHUNK 6          /* ring kernel: time slices a block marches through, 1..L_T (0 = library default 8) */
 #define DSLASH_OPT_PIPE_SLOTS 7       /* warp-pipelined kernel: hop stages in flight per warp, 2..4 (0 = library default) */
-#define DSLASH_OPT_PIPE_WARPS 8       /* warp-pipelined kernel: warps per thread block, 1 or 4 (0 = library default) */
+#define DSLASH_OPT_PIPE_WARPS 8       /* warp-pipelined kernel: warps per thread block, 1, 2 or 4 (0 = library default) */
+#define DSLASH_OPT_PIPE_ZBLOCK 9      /* warp-pipelined kernel: rows are visited y fastest, z inside blocks of this many planes, then t,
+                                         then the z blocks (a divisor of L_Z; 0 = L_Z): shortens the L2 reuse distance of the t hops */
 
 /* host<->device mapping modes of dslash_apply_host() (section 4.1.2) */
 #define DSLASH_MAP_MINIMAL 0 /* to: gauge, in;  from: out            (after the Advisor's data analysis) */
@@ -247,6 +249,17 @@ DSLASH_API int dslash_get_time_range(const dslash_ctx *ctx, int *t_begin, int *t
  */
 DSLASH_API int dslash_set_kernel(dslash_ctx *ctx, int kernel);
 DSLASH_API int dslash_get_kernel(const dslash_ctx *ctx, int *kernel);
+
+/*
+ * Pick the kernel by measurement (the Advisor's own method, applied to the library's kernels): every kernel
+ * that can run this context (DSLASH_KERNEL_DIRECT; DSLASH_KERNEL_WARP_PIPE where eligible) is timed on the caller's buffers
+ * (3 warm-up + 20 timed applications each, two interleaved rounds, CUDA events on `stream`) and the fastest becomes the
+ * context's kernel, as if set by dslash_set_kernel().  out, in, gauge: device pointers as for dslash_apply(); out is left
+ * holding D in.  *chosen (may be NULL) receives the kernel, *ms_per_apply (may be NULL) its time.  This call SYNCHRONISES
+ * with `stream`.  Errors: those of dslash_apply(); DSLASH_ERR_UNSUPPORTED when a sweep variant is selected.
+ */
+DSLASH_API int dslash_tune(dslash_ctx *ctx, void *out, const void *in, const void *gauge, dslash_stream_t stream, int *chosen,
+                           float *ms_per_apply);
 
 /*
  * The operators a caller of Dslash needs next (the paper: D is the "unpreconditioned Dirac operator", and

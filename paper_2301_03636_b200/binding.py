@@ -22,7 +22,7 @@ DSLASH_VARIANT_TUNED = 0
 DSLASH_MAP_MINIMAL, DSLASH_MAP_TOFROM = 0, 1
 DSLASH_KERNEL_AUTO, DSLASH_KERNEL_DIRECT, DSLASH_KERNEL_TMA, DSLASH_KERNEL_TMA_LINKS, DSLASH_KERNEL_RING = 0, 1, 2, 3, 4
 DSLASH_KERNEL_WARP_PIPE = 5
-DSLASH_OPT_PIPE_SLOTS, DSLASH_OPT_PIPE_WARPS = 7, 8
+DSLASH_OPT_PIPE_SLOTS, DSLASH_OPT_PIPE_WARPS, DSLASH_OPT_PIPE_ZBLOCK = 7, 8, 9
 DSLASH_OPT_OCCUPANCY, DSLASH_OPT_L2_POLICY, DSLASH_OPT_L1_CARVEOUT, DSLASH_OPT_X_SHUFFLE, DSLASH_OPT_T_CHUNK = 2, 3, 4, 5, 6
 DSLASH_SCHED_STATIC, DSLASH_SCHED_DYNAMIC, DSLASH_SCHED_GUIDED = 0, 1, 2
 DSLASH_OP_D, DSLASH_OP_D_DAGGER, DSLASH_OP_M, DSLASH_OP_M_DAGGER = 0, 1, 2, 3
@@ -73,6 +73,7 @@ SIGNATURES = {
     "dslash_get_time_range": (ctypes.c_int, [_vp, _c_int_p, _c_int_p]),
     "dslash_set_kernel": (ctypes.c_int, [_vp, ctypes.c_int]),
     "dslash_get_kernel": (ctypes.c_int, [_vp, _c_int_p]),
+    "dslash_tune": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _c_int_p, ctypes.POINTER(ctypes.c_float)]),
     "dslash_set_option": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int]),
     "dslash_get_option": (ctypes.c_int, [_vp, ctypes.c_int, _c_int_p]),
     "dslash_apply_host": (ctypes.c_int, [_vp, _vp, _vp, _vp, ctypes.c_int, _vp, _c_size_p, _c_size_p]),
@@ -312,6 +313,19 @@ def dslash_get_time_range(ctx):
 
 def dslash_set_kernel(ctx, kernel: int) -> None:
     _check(_lib.dslash_set_kernel(_ptr(ctx), int(kernel)), "dslash_set_kernel")
+
+
+def dslash_tune(ctx, out, inp, gauge, stream=None):
+    """Times the eligible kernels on these buffers, keeps the fastest; returns (kernel, ms per application).  Synchronises."""
+    k, ms = ctypes.c_int(0), ctypes.c_float(0.0)
+    _check(_lib.dslash_tune(_ptr(ctx), _ptr(out), _ptr(inp), _ptr(gauge), _ptr(stream), ctypes.byref(k), ctypes.byref(ms)),
+           "dslash_tune")
+    return k.value, ms.value
+
+
+def dslash_tune_status(ctx, out, inp, gauge, stream=None) -> int:
+    """dslash_tune returning the raw status instead of raising (error-path tests)."""
+    return int(_lib.dslash_tune(_ptr(ctx), _ptr(out), _ptr(inp), _ptr(gauge), _ptr(stream), None, None))
 
 
 def dslash_get_kernel(ctx) -> int:

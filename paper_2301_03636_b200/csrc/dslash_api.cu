@@ -232,6 +232,7 @@ int dslash_create(dslash_ctx** ctx, const int dims[4], int precision, int layout
     c->cfg.t_chunk = 0;
     c->cfg.pipe_slots = 0;
     c->cfg.pipe_warps = 0;
+    c->cfg.pipe_zblock = 0;
     c->cfg.x_shuffle = precision == DSLASH_FP64 ? 1 : 0;  // measured: -1.3 % (burst) / -2 % (sustained) in fp64, +0.8 % in fp32
     c->launches = 0;
     c->last_cuda = 0;
@@ -688,8 +689,12 @@ int dslash_set_option(dslash_ctx* c, int option, int value) {
             if (value != 0 && (value < 2 || value > 4)) return DSLASH_ERR_UNSUPPORTED;
             c->cfg.pipe_slots = value;
             return DSLASH_OK;
+        case DSLASH_OPT_PIPE_ZBLOCK:
+            if (value < 0 || value > c->geom.L[2] || (value > 0 && c->geom.L[2] % value)) return DSLASH_ERR_UNSUPPORTED;
+            c->cfg.pipe_zblock = value;
+            return DSLASH_OK;
         case DSLASH_OPT_PIPE_WARPS:
-            if (value != 0 && value != 1 && value != 4) return DSLASH_ERR_UNSUPPORTED;
+            if (value != 0 && value != 1 && value != 2 && value != 4) return DSLASH_ERR_UNSUPPORTED;
             c->cfg.pipe_warps = value;
             return DSLASH_OK;
         default:
@@ -707,6 +712,7 @@ int dslash_get_option(const dslash_ctx* c, int option, int* value) {
         case DSLASH_OPT_T_CHUNK: *value = c->cfg.t_chunk; return DSLASH_OK;
         case DSLASH_OPT_PIPE_SLOTS: *value = c->cfg.pipe_slots; return DSLASH_OK;
         case DSLASH_OPT_PIPE_WARPS: *value = c->cfg.pipe_warps; return DSLASH_OK;
+        case DSLASH_OPT_PIPE_ZBLOCK: *value = c->cfg.pipe_zblock; return DSLASH_OK;
         default: return DSLASH_ERR_UNSUPPORTED;
     }
 }
@@ -725,6 +731,56 @@ int dslash_get_kernel(const dslash_ctx* c, int* kernel) {
     const int k = resolve_kernel(c);
     *kernel = k < 0 ? DSLASH_KERNEL_DIRECT : k;
     return DSLASH_OK;
+}
+
+// Times the kernels that can run this context on the caller's own buffers and keeps the fastest (the Advisor's "execute every
+// variant on the device, rank" -- PAPER.md:82-84 -- applied to the library's own kernels).  out is overwritten with D in by every
+// candidate, so the call leaves the same result as one dslash_apply().
+int dslash_tune(dslash_ctx* c, void* out, const void* in, const void* gauge, dslash_stream_t stream, int* chosen, float* ms_per_apply) {
+    if (!c || !out || !in || !gauge) return DSLASH_ERR_NULL;
+    if (c->var_depth != DSLASH_VARIANT_TUNED) return DSLASH_ERR_UNSUPPORTED;
+    int cand[2], ncand = 0;
+    cand[ncand++] = DSLASH_KERNEL_DIRECT;
+    if (wpipe_eligible(c->layout_base, c->geom)) cand[ncand++] = DSLASH_KERNEL_WARP_PIPE;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    cudaEvent_t e0, e1;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) {
+        c->last_cuda = (int)cudaGetLastError();
+        return DSLASH_ERR_CUDA;
+    }
+    const int keep = c->kernel;
+    int best = DSLASH_KERNEL_DIRECT, rc = DSLASH_OK;
+    float best_ms = 0.f;
+    for (int round = 0; round < 2 && rc == DSLASH_OK; ++round)  // two interleaved rounds: a clock or thermal drift hits both candidates
+        for (int k = 0; k < ncand && rc == DSLASH_OK; ++k) {
+            c->kernel = cand[k];
+            for (int i = 0; i < 3 && rc == DSLASH_OK; ++i) rc = dslash_apply(c, out, in, gauge, stream);
+            if (rc != DSLASH_OK) break;
+            cudaEventRecord(e0, st);
+            const int reps = 20;
+            for (int i = 0; i < reps && rc == DSLASH_OK; ++i) rc = dslash_apply(c, out, in, gauge, stream);
+            cudaEventRecord(e1, st);
+            if (rc != DSLASH_OK) break;
+            float ms = 0.f;
+            if (cudaEventSynchronize(e1) != cudaSuccess || cudaEventElapsedTime(&ms, e0, e1) != cudaSuccess) {
+                c->last_cuda = (int)cudaGetLastError();
+                rc = DSLASH_ERR_CUDA;
+                break;
+            }
+            ms /= reps;
+            if (best_ms == 0.f || ms < best_ms) {
+                best_ms = ms;
+                best = cand[k];
+            }
+        }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    c->kernel = rc == DSLASH_OK ? best : keep;
+    if (rc == DSLASH_OK) {
+        if (chosen) *chosen = best;
+        if (ms_per_apply) *ms_per_apply = best_ms;
+    }
+    return rc;
 }
 
 int dslash_apply_host(dslash_ctx* c, void* out_host, const void* in_host, const void* gauge_host, int map_mode,

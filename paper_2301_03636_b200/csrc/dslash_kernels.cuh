@@ -38,7 +38,8 @@ struct TunedConfig {
     int l1_carveout;       // preferred shared-memory carve-out of the direct kernel in percent (-1: driver default)
     int t_chunk;           // time slices a block of the ring kernel marches through (0: default)
     int pipe_slots;        // warp-pipelined kernel: stages in flight per warp (2..4; 0: default 2)
-    int pipe_warps;        // warp-pipelined kernel: warps per block (1 or 4; 0: default 1)
+    int pipe_warps;        // warp-pipelined kernel: warps per block (1, 2 or 4; 0: default 4)
+    int pipe_zblock;       // warp-pipelined kernel: z planes per block of the row order (0: L_Z, i.e. plain lexicographic)
     int x_shuffle;         // 1: exchange the x hops inside the warp when the tile allows it (fp64 default), 0: always load them
 };
 bool x_shuffle_eligible(const Geom& g, const TileGeom& tg);

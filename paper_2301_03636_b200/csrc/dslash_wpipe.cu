@@ -104,7 +104,10 @@ __device__ __forceinline__ void hop_regs(cplx<Real> (&acc)[12], const cplx<Real>
 struct PipeGeom {
     int LY, LZ, LT;      // rows are indexed v = y + LY * (z + LZ * t); one row = one 32-site vector
     int t_begin;         // first time slice computed
-    unsigned nrows;      // LY * LZ * (t_end - t_begin)
+    int nt;              // time slices computed
+    int zb;              // rows are visited y fastest, then z inside a block of zb planes, then t, then the z blocks: the slice
+                         // spacing of the t-neighbour reuse shrinks from LY*LZ rows to LY*zb rows (L2 capacity)
+    unsigned nrows;      // LY * LZ * nt
 };
 
 }  // namespace
@@ -129,9 +132,11 @@ struct Row {
 __device__ __forceinline__ Row decode_row(const PipeGeom& pg, unsigned r) {
     Row w;
     w.y = (int)(r % (unsigned)pg.LY);
-    const unsigned q = r / (unsigned)pg.LY;
-    w.z = (int)(q % (unsigned)pg.LZ);
-    w.t = pg.t_begin + (int)(q / (unsigned)pg.LZ);
+    unsigned q = r / (unsigned)pg.LY;
+    const unsigned zl = q % (unsigned)pg.zb;
+    q /= (unsigned)pg.zb;
+    w.t = pg.t_begin + (int)(q % (unsigned)pg.nt);
+    w.z = (int)(zl + (q / (unsigned)pg.nt) * (unsigned)pg.zb);
     w.v = (unsigned)w.y + (unsigned)pg.LY * ((unsigned)w.z + (unsigned)pg.LZ * (unsigned)w.t);
     return w;
 }
@@ -255,7 +260,7 @@ bool wpipe_eligible(int layout_base, const Geom& g) { return layout_base == LAYO
 namespace {
 
 template <typename Real, int RECON, int NSLOT, int NW>
-cudaError_t launch_wpipe_k(const LaunchArgs& a, const TileGeom& tg) {
+cudaError_t launch_wpipe_k(const LaunchArgs& a, const TileGeom& tg, int zblock) {
     using PB = PipeBytes<Real, RECON>;
     constexpr size_t smem = kPipeHeader + (size_t)NW * NSLOT * PB::SLOT;
     constexpr int fit = (int)(232448u / (smem + 1024u));  // blocks per SM by shared memory (1 KB reserved per block)
@@ -273,8 +278,9 @@ cudaError_t launch_wpipe_k(const LaunchArgs& a, const TileGeom& tg) {
         if (bps < 1) return cudaErrorInvalidConfiguration;
         blocks_per_sm = bps;
     }
-    PipeGeom pg{a.geom.L[1], a.geom.L[2], a.geom.L[3], tg.t_begin, 0u};
-    pg.nrows = (unsigned)a.geom.L[1] * (unsigned)a.geom.L[2] * (unsigned)(tg.t_end - tg.t_begin);
+    PipeGeom pg{a.geom.L[1], a.geom.L[2], a.geom.L[3], tg.t_begin, tg.t_end - tg.t_begin, a.geom.L[2], 0u};
+    if (zblock > 0 && zblock < a.geom.L[2] && a.geom.L[2] % zblock == 0) pg.zb = zblock;
+    pg.nrows = (unsigned)a.geom.L[1] * (unsigned)a.geom.L[2] * (unsigned)pg.nt;
     if (pg.nrows == 0) return cudaSuccess;
     const unsigned need = (pg.nrows + NW - 1) / NW, resident = (unsigned)(blocks_per_sm * sms);
     kernel<<<need < resident ? need : resident, NW * 32, smem, a.stream>>>(a.out, a.in, a.gauge, a.geom, pg);
@@ -282,15 +288,20 @@ cudaError_t launch_wpipe_k(const LaunchArgs& a, const TileGeom& tg) {
 }
 
 template <typename Real, int RECON>
-cudaError_t launch_wpipe_r(const LaunchArgs& a, const TileGeom& tg, int slots, int warps) {
+cudaError_t launch_wpipe_r(const LaunchArgs& a, const TileGeom& tg, int slots, int warps, int zblock) {
     if (warps == 1) {
-        if (slots == 2) return launch_wpipe_k<Real, RECON, 2, 1>(a, tg);
-        if (slots == 3) return launch_wpipe_k<Real, RECON, 3, 1>(a, tg);
-        return launch_wpipe_k<Real, RECON, 4, 1>(a, tg);
+        if (slots == 2) return launch_wpipe_k<Real, RECON, 2, 1>(a, tg, zblock);
+        if (slots == 3) return launch_wpipe_k<Real, RECON, 3, 1>(a, tg, zblock);
+        return launch_wpipe_k<Real, RECON, 4, 1>(a, tg, zblock);
     }
-    if (slots == 2) return launch_wpipe_k<Real, RECON, 2, 4>(a, tg);
-    if (slots == 3) return launch_wpipe_k<Real, RECON, 3, 4>(a, tg);
-    return launch_wpipe_k<Real, RECON, 4, 4>(a, tg);
+    if (warps == 2) {
+        if (slots == 2) return launch_wpipe_k<Real, RECON, 2, 2>(a, tg, zblock);
+        if (slots == 3) return launch_wpipe_k<Real, RECON, 3, 2>(a, tg, zblock);
+        return launch_wpipe_k<Real, RECON, 4, 2>(a, tg, zblock);
+    }
+    if (slots == 2) return launch_wpipe_k<Real, RECON, 2, 4>(a, tg, zblock);
+    if (slots == 3) return launch_wpipe_k<Real, RECON, 3, 4>(a, tg, zblock);
+    return launch_wpipe_k<Real, RECON, 4, 4>(a, tg, zblock);
 }
 
 }  // namespace
@@ -298,9 +309,10 @@ cudaError_t launch_wpipe_r(const LaunchArgs& a, const TileGeom& tg, int slots, i
 cudaError_t launch_wpipe(int precision, int layout_base, int recon, const LaunchArgs& a, const TileGeom& tg, const TunedConfig& cfg) {
     if (!wpipe_eligible(layout_base, a.geom)) return cudaErrorInvalidConfiguration;
     const int slots = cfg.pipe_slots >= 2 && cfg.pipe_slots <= 4 ? cfg.pipe_slots : 2;
-    const int warps = cfg.pipe_warps == 4 ? 4 : 1;
-    if (precision == 0) return recon == 12 ? launch_wpipe_r<double, 12>(a, tg, slots, warps) : launch_wpipe_r<double, 18>(a, tg, slots, warps);
-    return recon == 12 ? launch_wpipe_r<float, 12>(a, tg, slots, warps) : launch_wpipe_r<float, 18>(a, tg, slots, warps);
+    const int warps = cfg.pipe_warps == 1 ? 1 : (cfg.pipe_warps == 2 ? 2 : 4);  // default 4: 2 blocks x 4 warps x 2 slots per SM
+    const int zblock = cfg.pipe_zblock;
+    if (precision == 0) return recon == 12 ? launch_wpipe_r<double, 12>(a, tg, slots, warps, zblock) : launch_wpipe_r<double, 18>(a, tg, slots, warps, zblock);
+    return recon == 12 ? launch_wpipe_r<float, 12>(a, tg, slots, warps, zblock) : launch_wpipe_r<float, 18>(a, tg, slots, warps, zblock);
 }
 
 }  // namespace dslash

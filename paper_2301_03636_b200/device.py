@@ -90,6 +90,10 @@ class Lattice:
     def apply(self, out, inp, gauge):
         B.dslash_apply(self.ctx, out.data_ptr(), inp.data_ptr(), gauge.data_ptr(), self.stream())
 
+    def tune(self, out, inp, gauge):
+        """dslash_tune: time the eligible kernels on these buffers and keep the fastest; returns (kernel, ms)."""
+        return B.dslash_tune(self.ctx, out.data_ptr(), inp.data_ptr(), gauge.data_ptr(), self.stream())
+
     def apply_op(self, op, mass, out, inp, gauge):
         B.dslash_apply_op(self.ctx, op, mass, out.data_ptr(), inp.data_ptr(), gauge.data_ptr(), self.stream())
 

@@ -220,6 +220,73 @@ def test_ring_kernel_refuses_what_it_cannot_run(env):
                 B.dslash_set_option(lat.ctx, B.DSLASH_OPT_T_CHUNK, dims[3] + 1)
 
 
+# ---------------------------------------------------------------- the warp-pipelined kernel (SoA, L_X = 32), selected explicitly
+@pytest.mark.parametrize("dims", [
+    (32, 4, 4, 8),       # several rows per warp, all wraps
+    (32, 1, 1, 1),       # one row: every neighbour is the row itself
+    (32, 2, 1, 3),       # y+1 == y-1, z neighbour == self
+    (32, 5, 3, 2),       # odd extents, t+1 == t-1
+    (32, 16, 12, 9),     # 1728 rows: more rows than resident warps on any configuration (persistent loop, tail)
+])
+@pytest.mark.parametrize("slots,warps,zblock", [(0, 0, 0), (2, 1, 0), (3, 2, 0), (4, 4, 0), (2, 4, 1), (3, 1, 3)])
+@pytest.mark.parametrize("precision", ["f64", "f32"])
+@pytest.mark.parametrize("recon12", [False, True])
+def test_warp_pipelined_kernel_matches_the_oracle_and_the_direct_kernel_bit_for_bit(env, dims, slots, warps, zblock, precision, recon12):
+    B = env.B
+    if zblock and dims[2] % zblock:
+        pytest.skip("z block does not divide L_Z")
+    g, p, ref, _ = fields_and_ref(env, dims, SEED + 23, precision)
+    with env.device.Lattice(dims, precision, "soa", recon12) as lat:
+        gi, pi, o = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
+        lat.apply(o, pi, gi)
+        direct = lat.download_spinor(o)
+        lat.set_kernel("wpipe")
+        B.dslash_set_option(lat.ctx, B.DSLASH_OPT_PIPE_SLOTS, slots)
+        B.dslash_set_option(lat.ctx, B.DSLASH_OPT_PIPE_WARPS, warps)
+        B.dslash_set_option(lat.ctx, B.DSLASH_OPT_PIPE_ZBLOCK, zblock)
+        assert B.dslash_get_kernel(lat.ctx) == B.DSLASH_KERNEL_WARP_PIPE
+        assert B.dslash_get_option(lat.ctx, B.DSLASH_OPT_PIPE_SLOTS) == slots
+        o.zero_()
+        lat.apply(o, pi, gi)
+        got = lat.download_spinor(o)
+        assert env.checks.parity_error(got, ref) <= TOL[precision]
+        assert np.array_equal(got, direct)  # same arithmetic in the same order
+        if dims[3] >= 4:  # a time range (multi-GPU slab interior): only its slices are written
+            B.dslash_set_time_range(lat.ctx, 1, dims[3] - 1)
+            o.zero_()
+            lat.apply(o, pi, gi)
+            part = lat.download_spinor(o)
+            assert np.array_equal(part[1:-1], direct[1:-1]) and not part[0].any() and not part[-1].any()
+
+
+def test_warp_pipelined_kernel_refuses_what_it_cannot_run_and_tune_picks_a_working_kernel(env):
+    B = env.B
+    for dims, layout in [((32, 4, 4, 4), "aos"), ((16, 4, 4, 4), "soa"), ((64, 4, 2, 2), "soa")]:
+        with env.device.Lattice(dims, "f64", layout, False) as lat:
+            lat.set_kernel("wpipe")
+            o, p, g = lat.new_spinor(), lat.new_spinor(), lat.new_gauge()
+            assert B.dslash_apply_status(lat.ctx, o.data_ptr(), p.data_ptr(), g.data_ptr()) == B.DSLASH_ERR_UNSUPPORTED, (dims, layout)
+    with env.device.Lattice((32, 4, 4, 4), "f64", "soa", False) as lat:
+        for opt, bad in [(B.DSLASH_OPT_PIPE_SLOTS, 1), (B.DSLASH_OPT_PIPE_SLOTS, 5), (B.DSLASH_OPT_PIPE_WARPS, 3), (B.DSLASH_OPT_PIPE_ZBLOCK, 3)]:
+            with pytest.raises(B.DslashError):
+                B.dslash_set_option(lat.ctx, opt, bad)
+    # dslash_tune: times direct (+ wpipe where eligible), keeps one of them, leaves D in in `out`
+    for dims, eligible in [((32, 8, 8, 8), True), ((16, 8, 8, 8), False)]:
+        g, p, ref, _ = fields_and_ref(env, dims, SEED + 24, "f64")
+        with env.device.Lattice(dims, "f64", "soa", False) as lat:
+            gi, pi, o = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
+            kernel, ms = lat.tune(o, pi, gi)
+            assert kernel in ((B.DSLASH_KERNEL_DIRECT, B.DSLASH_KERNEL_WARP_PIPE) if eligible else (B.DSLASH_KERNEL_DIRECT,)) and ms > 0
+            assert B.dslash_get_kernel(lat.ctx) == kernel
+            assert env.checks.parity_error(lat.download_spinor(o), ref) <= TOL["f64"]
+            o.zero_()
+            lat.apply(o, pi, gi)
+            assert env.checks.parity_error(lat.download_spinor(o), ref) <= TOL["f64"]
+            B.dslash_set_variant(lat.ctx, 4, 128, 1)
+            assert B.dslash_tune_status(lat.ctx, o.data_ptr(), pi.data_ptr(), gi.data_ptr()) == B.DSLASH_ERR_UNSUPPORTED
+    assert B.dslash_tune_status(None, 16, 32, 48) == B.DSLASH_ERR_NULL
+
+
 # ---------------------------------------------------------------- config 2: 16^4 FP64
 @pytest.mark.parametrize("layout,recon12", ALL_MODES)
 def test_config2_16x16x16x16(env, layout, recon12):
