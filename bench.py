@@ -229,6 +229,7 @@ def run_cuda(args, cfg):
             tuned = None
             if not args.kernel and not args.no_tune:
                 tuned = lat.tune(od, pd, gd)  # outside the timed region: the library picks its kernel by measurement
+                time.sleep(1.0)               # back to idle: the timed region starts from the same state with or without tuning
             n0 = B.dslash_launch_count(lat.ctx)
             ms, ck = time_applies(torch, lat, od, pd, gd, args.steps, args.warmup, group, local)
             n1 = B.dslash_launch_count(lat.ctx)
@@ -242,6 +243,8 @@ def run_cuda(args, cfg):
                                 t_chunk=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_T_CHUNK),
                                 occupancy=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_OCCUPANCY),
                                 x_shuffle=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_X_SHUFFLE),
+                                pipe_slots=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_PIPE_SLOTS),
+                                pipe_warps=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_PIPE_WARPS),
                                 tuned_ms=None if tuned is None else tuned[1])
             if tag == "main":
                 clocks, launches = ck, n1 - n0 - args.warmup
@@ -304,7 +307,7 @@ def run_cuda(args, cfg):
             "config": {"workload": cfg["name"], "dims": list(dims), "layout": args.layout, "recon": 12 if main["recon12"] else 18,
                        "tile": main["tile"], "kernel": main["kernel"],
                        "kernel_chosen_by": "dslash_tune (measured before the timed region)" if main["tuned_ms"] is not None else "option", "occupancy_option": main["occupancy"],
-                       "x_shuffle_option": main["x_shuffle"], "t_chunk_option": main["t_chunk"], "sites": v, "parallelism": "replicas x%d" % world,
+                       "x_shuffle_option": main["x_shuffle"], "pipe_slots": main["pipe_slots"], "pipe_warps": main["pipe_warps"], "t_chunk_option": main["t_chunk"], "sites": v, "parallelism": "replicas x%d" % world,
                        "l2": "inputs larger than L2: %.2f GB working set per apply vs 126 MB L2, no flush needed"
                              % (main["bps"] * v / 1e9)},
             "hbm_gbs": main["gbs"], "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "clocks": clocks,

@@ -252,9 +252,11 @@ DSLASH_API int dslash_get_kernel(const dslash_ctx *ctx, int *kernel);
 
 /*
  * Pick the kernel by measurement (the Advisor's own method, applied to the library's kernels): every kernel
- * that can run this context (DSLASH_KERNEL_DIRECT; DSLASH_KERNEL_WARP_PIPE where eligible) is timed on the caller's buffers
- * (3 warm-up + 20 timed applications each, two interleaved rounds, CUDA events on `stream`) and the fastest becomes the
- * context's kernel, as if set by dslash_set_kernel().  out, in, gauge: device pointers as for dslash_apply(); out is left
+ * that can run this context (DSLASH_KERNEL_DIRECT; DSLASH_KERNEL_WARP_PIPE in three slot/warp configurations where
+ * eligible) is timed on the caller's buffers
+ * (2 warm-up + 8 timed applications each, CUDA events on `stream`; about 15 ms in all, so that every candidate is
+ * timed inside the board's boost window -- call it on an idle device) and the fastest becomes the
+ * context's kernel, as if set by dslash_set_kernel() (and DSLASH_OPT_PIPE_SLOTS / _WARPS).  out, in, gauge: device pointers as for dslash_apply(); out is left
  * holding D in.  *chosen (may be NULL) receives the kernel, *ms_per_apply (may be NULL) its time.  This call SYNCHRONISES
  * with `stream`.  Errors: those of dslash_apply(); DSLASH_ERR_UNSUPPORTED when a sweep variant is selected.
  */

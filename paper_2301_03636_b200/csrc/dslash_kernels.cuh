@@ -39,6 +39,7 @@ struct TunedConfig {
     int t_chunk;           // time slices a block of the ring kernel marches through (0: default)
     int pipe_slots;        // warp-pipelined kernel: stages in flight per warp (2..4; 0: default 2)
     int pipe_warps;        // warp-pipelined kernel: warps per block (1, 2 or 4; 0: default 4)
+    unsigned* pipe_counters;  // warp-pipelined kernel: {next row, finished warps} of this launch (device memory, zero between launches)
     int pipe_zblock;       // warp-pipelined kernel: z planes per block of the row order (0: L_Z, i.e. plain lexicographic)
     int x_shuffle;         // 1: exchange the x hops inside the warp when the tile allows it (fp64 default), 0: always load them
 };
