@@ -47,8 +47,8 @@ CONFIGS = {
 NCU_TRAFFIC_BYTES = {
     # profiles/r01_ncu_tuned_kernel.txt, capture r01c: 1.6424 GB read + 0.3903 GB written (mean of 2 launches)
     "32x32x32x64_f64_soa_r18": 2032698000,
-    # profiles/r01f_ncu_wpipe.txt: the warp-pipelined kernel, 1.689388 GB read + 0.391466 GB written
-    "32x32x32x64_f64_soa_r18_wpipe": 2080854000,
+    # profiles/r01f_wpipe.md: the warp-pipelined kernel (rows from the counter), 1.660823 GB read + 0.391139 GB written
+    "32x32x32x64_f64_soa_r18_wpipe": 2051962000,
 }
 KERNEL_NAMES = {"direct": "dslash_tuned_kernel", "wpipe": "dslash_wpipe_kernel", "ring": "dslash_ring_kernel", "tma": "dslash_tma_kernel",
                 "tma_links": "dslash_tma_kernel"}
