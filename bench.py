@@ -722,6 +722,49 @@ def run_costmodel(args):
     return 0
 
 
+# ------------------------------------------------------------------ ceilings of the board at hand
+def run_probe(args):
+    """Read / write / copy / 4:1-mix bandwidth over 4 GiB working sets and the FP64 FMA rate, each the best of 5 launches after
+    1 s idle (boost window), with the library's own probe kernels (csrc/dslash_probe.cu)."""
+    import torch
+    from paper_2301_03636_b200 import binding as B
+    dev = torch.device("cuda:0")
+    torch.cuda.set_device(dev)
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    n = 1 << 26  # 16-byte units: 1 GiB per stream
+    src = torch.empty(4 * n * 2, dtype=torch.float64, device=dev).normal_()
+    dst = torch.empty(n * 2, dtype=torch.float64, device=dev)
+    st = torch.cuda.current_stream().cuda_stream
+
+    def best(kind, units, blocks, bytes_moved=None, flops=None):
+        B.dslash_probe_launch(kind, dst.data_ptr(), src.data_ptr(), units, blocks, st)
+        torch.cuda.synchronize()
+        time.sleep(1.0)
+        ts = []
+        for _ in range(5):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            B.dslash_probe_launch(kind, dst.data_ptr(), src.data_ptr(), units, blocks, st)
+            e1.record()
+            e1.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        ms = min(ts)
+        return {"ms": ms, "GB/s": None if bytes_moved is None else bytes_moved / ms / 1e6,
+                "TFLOP/s": None if flops is None else flops / ms / 1e9}
+    blocks = sms * 8
+    iters = 1 << 14
+    peak, peak_src = hbm_peak()
+    out = {"probe": "csrc/dslash_probe.cu, best of 5 launches after 1 s idle", "sms": sms, "blocks": blocks,
+           "read": best(B.DSLASH_PROBE_READ, 4 * n, blocks, bytes_moved=64 * n),
+           "write": best(B.DSLASH_PROBE_WRITE, n, blocks, bytes_moved=16 * n),
+           "copy": best(B.DSLASH_PROBE_COPY, n, blocks, bytes_moved=32 * n),
+           "read4_write1": best(B.DSLASH_PROBE_READ4_WRITE1, n, blocks, bytes_moved=80 * n),
+           "dfma": best(B.DSLASH_PROBE_DFMA, iters, blocks, flops=2.0 * 8 * iters * blocks * 256),
+           "measured_peaks_hbm_gbs": peak, "peak_source": peak_src}
+    print(json.dumps(out))
+    return 0
+
+
 # ------------------------------------------------------------------ the solver around Dslash
 def run_cg(args):
     """CG on M^dagger M (dslash_cg_solve) on a BASELINE lattice: what "called several times throughout the LQCD
@@ -864,6 +907,7 @@ def main():
     ap.add_argument("--cg-mass", type=float, default=0.2)
     ap.add_argument("--cg-tol", type=float, default=1e-8)
     ap.add_argument("--cg-max-iter", type=int, default=2000)
+    ap.add_argument("--probe", action="store_true", help="read/write/copy/4:1-mix bandwidth and FP64 FMA rate of this board")
     ap.add_argument("--costmodel", action="store_true", help="fit the Advisor's cost model on the variants' measured runtimes")
     ap.add_argument("--costmodel-lattices", type=int, default=len(COSTMODEL_LATTICES))
     ap.add_argument("--costmodel-epochs", type=int, default=150)
@@ -875,6 +919,8 @@ def main():
         return run_sweep(args)
     if args.advisor:
         return run_advisor(args)
+    if args.probe:
+        return run_probe(args)
     if args.costmodel:
         return run_costmodel(args)
     if args.cg:

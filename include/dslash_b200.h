@@ -264,6 +264,23 @@ DSLASH_API int dslash_tune(dslash_ctx *ctx, void *out, const void *in, const voi
                            float *ms_per_apply);
 
 /*
+ * Ceilings of the board at hand, measured with trivial kernels of this library (not on the Dslash
+ * path).  Enqueues ONE kernel of `blocks` blocks of 256 threads on `stream`; the caller times it (bench.py --probe).
+ *   DSLASH_PROBE_READ          reads n 16-byte units of src (dst: >= 8 bytes, never written)
+ *   DSLASH_PROBE_WRITE         writes n units of dst
+ *   DSLASH_PROBE_COPY          dst[i] = src[i], n units
+ *   DSLASH_PROBE_READ4_WRITE1  dst[i] = src[i] + src[n+i] + src[2n+i] + src[3n+i]: Dslash's 4 : 1 read : write mix (src: 4n units)
+ *   DSLASH_PROBE_DFMA          n iterations of 8 independent FP64 FMAs per thread in registers (dst: >= 8 bytes, never written)
+ * dst, src: device pointers, 16-byte aligned.  Errors: DSLASH_ERR_NULL, _DIMS (n or blocks < 1), _ALIGN, _UNSUPPORTED, _CUDA.
+ */
+#define DSLASH_PROBE_READ 0
+#define DSLASH_PROBE_WRITE 1
+#define DSLASH_PROBE_COPY 2
+#define DSLASH_PROBE_READ4_WRITE1 3
+#define DSLASH_PROBE_DFMA 4
+DSLASH_API int dslash_probe_launch(int kind, void *dst, const void *src, size_t n, int blocks, dslash_stream_t stream);
+
+/*
  * The operators a caller of Dslash needs next (the paper: D is the "unpreconditioned Dirac operator", and
  * "is called several times throughout the LQCD application").
  * dslash_apply_op: out = OP in with OP one of DSLASH_OP_* (mass is used by _M and _M_DAGGER only); same buffers, layouts,

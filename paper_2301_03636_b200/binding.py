@@ -73,6 +73,7 @@ SIGNATURES = {
     "dslash_get_time_range": (ctypes.c_int, [_vp, _c_int_p, _c_int_p]),
     "dslash_set_kernel": (ctypes.c_int, [_vp, ctypes.c_int]),
     "dslash_get_kernel": (ctypes.c_int, [_vp, _c_int_p]),
+    "dslash_probe_launch": (ctypes.c_int, [ctypes.c_int, _vp, _vp, ctypes.c_size_t, ctypes.c_int, _vp]),
     "dslash_tune": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _c_int_p, ctypes.POINTER(ctypes.c_float)]),
     "dslash_set_option": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int]),
     "dslash_get_option": (ctypes.c_int, [_vp, ctypes.c_int, _c_int_p]),
@@ -321,6 +322,13 @@ def dslash_tune(ctx, out, inp, gauge, stream=None):
     _check(_lib.dslash_tune(_ptr(ctx), _ptr(out), _ptr(inp), _ptr(gauge), _ptr(stream), ctypes.byref(k), ctypes.byref(ms)),
            "dslash_tune")
     return k.value, ms.value
+
+
+DSLASH_PROBE_READ, DSLASH_PROBE_WRITE, DSLASH_PROBE_COPY, DSLASH_PROBE_READ4_WRITE1, DSLASH_PROBE_DFMA = 0, 1, 2, 3, 4
+
+
+def dslash_probe_launch(kind: int, dst, src, n: int, blocks: int, stream=None) -> None:
+    _check(_lib.dslash_probe_launch(int(kind), _ptr(dst), _ptr(src), int(n), int(blocks), _ptr(stream)), "dslash_probe_launch")
 
 
 def dslash_tune_status(ctx, out, inp, gauge, stream=None) -> int:

@@ -1,0 +1,73 @@
+// dslash_probe.cu -- the ceilings the Dslash kernels are judged against, measured with the library's own trivial kernels on
+// the board at hand ("a plain FP64 copy/triad GB/s (the honest ceiling for this access mix)", "FP64
+// DFMA peak").  dslash_probe_launch() enqueues ONE kernel; bench.py --probe times it with CUDA events.  Nothing here is on
+// the Dslash path.
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/dslash_b200.h"
+
+namespace {
+
+constexpr int kThreads = 256;
+
+// 16-byte units, grid-stride, every access a full 512-byte warp transaction
+__global__ void __launch_bounds__(kThreads) probe_read(const double2* __restrict__ src, size_t n, double* __restrict__ sink) {
+    double2 acc = {0.0, 0.0};
+    for (size_t i = blockIdx.x * (size_t)kThreads + threadIdx.x; i < n; i += (size_t)gridDim.x * kThreads) {
+        const double2 v = __ldg(src + i);
+        acc.x += v.x;
+        acc.y += v.y;
+    }
+    if (acc.x == 1.2345e300 && acc.y == 5.4321e300) sink[0] = acc.x;  // never true: keeps the loads alive
+}
+
+__global__ void __launch_bounds__(kThreads) probe_write(double2* __restrict__ dst, size_t n) {
+    const double2 v = {1.0, 2.0};
+    for (size_t i = blockIdx.x * (size_t)kThreads + threadIdx.x; i < n; i += (size_t)gridDim.x * kThreads) dst[i] = v;
+}
+
+__global__ void __launch_bounds__(kThreads) probe_copy(double2* __restrict__ dst, const double2* __restrict__ src, size_t n) {
+    for (size_t i = blockIdx.x * (size_t)kThreads + threadIdx.x; i < n; i += (size_t)gridDim.x * kThreads) dst[i] = __ldg(src + i);
+}
+
+// Dslash's own mix: 4 units read (src[i], src[n+i], src[2n+i], src[3n+i]) for 1 written (768 B in : 192 B out per site)
+__global__ void __launch_bounds__(kThreads) probe_read4_write1(double2* __restrict__ dst, const double2* __restrict__ src, size_t n) {
+    for (size_t i = blockIdx.x * (size_t)kThreads + threadIdx.x; i < n; i += (size_t)gridDim.x * kThreads) {
+        const double2 a = __ldg(src + i), b = __ldg(src + n + i), c = __ldg(src + 2 * n + i), d = __ldg(src + 3 * n + i);
+        dst[i] = {a.x + b.x + c.x + d.x, a.y + b.y + c.y + d.y};
+    }
+}
+
+// register-resident DFMA chains: 8 independent accumulators per thread, iters x 8 FMAs
+__global__ void __launch_bounds__(kThreads) probe_dfma(double* __restrict__ sink, size_t iters) {
+    double a0 = threadIdx.x, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+    const double m = 0.999999, c = 1e-9;
+    for (size_t i = 0; i < iters; ++i) {
+        a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+        a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+    }
+    const double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+    if (s == 1.2345e300) sink[0] = s;
+}
+
+}  // namespace
+
+extern "C" int dslash_probe_launch(int kind, void* dst, const void* src, size_t n, int blocks, dslash_stream_t stream) {
+    if (blocks < 1 || n < 1) return DSLASH_ERR_DIMS;
+    if (kind != DSLASH_PROBE_DFMA && kind != DSLASH_PROBE_WRITE && !src) return DSLASH_ERR_NULL;
+    if (!dst) return DSLASH_ERR_NULL;
+    if ((reinterpret_cast<uintptr_t>(dst) | reinterpret_cast<uintptr_t>(src)) & 15u) return DSLASH_ERR_ALIGN;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    switch (kind) {
+        case DSLASH_PROBE_READ: probe_read<<<blocks, kThreads, 0, st>>>(static_cast<const double2*>(src), n, static_cast<double*>(dst)); break;
+        case DSLASH_PROBE_WRITE: probe_write<<<blocks, kThreads, 0, st>>>(static_cast<double2*>(dst), n); break;
+        case DSLASH_PROBE_COPY: probe_copy<<<blocks, kThreads, 0, st>>>(static_cast<double2*>(dst), static_cast<const double2*>(src), n); break;
+        case DSLASH_PROBE_READ4_WRITE1:
+            probe_read4_write1<<<blocks, kThreads, 0, st>>>(static_cast<double2*>(dst), static_cast<const double2*>(src), n);
+            break;
+        case DSLASH_PROBE_DFMA: probe_dfma<<<blocks, kThreads, 0, st>>>(static_cast<double*>(dst), n); break;
+        default: return DSLASH_ERR_UNSUPPORTED;
+    }
+    return cudaGetLastError() == cudaSuccess ? DSLASH_OK : DSLASH_ERR_CUDA;
+}

@@ -98,6 +98,13 @@ def test_argument_validation_precedes_cuda(B):
     with pytest.raises(B.DslashError) as e:
         B.dslash_set_variant(None, 1, 64, 1)
     assert e.value.status == B.DSLASH_ERR_NULL
+    assert B.dslash_tune_status(None, 16, 32, 48) == B.DSLASH_ERR_NULL
+    for kind, dst, src, n, blocks, want in [(B.DSLASH_PROBE_COPY, 16, 0, 4, 1, B.DSLASH_ERR_NULL), (B.DSLASH_PROBE_COPY, 0, 16, 4, 1, B.DSLASH_ERR_NULL),
+                                            (B.DSLASH_PROBE_COPY, 16, 32, 0, 1, B.DSLASH_ERR_DIMS), (B.DSLASH_PROBE_COPY, 16, 32, 4, 0, B.DSLASH_ERR_DIMS),
+                                            (B.DSLASH_PROBE_COPY, 16, 40, 4, 1, B.DSLASH_ERR_ALIGN), (9, 16, 32, 4, 1, B.DSLASH_ERR_UNSUPPORTED)]:
+        with pytest.raises(B.DslashError) as e:
+            B.dslash_probe_launch(kind, dst, src, n, blocks)
+        assert e.value.status == want, (kind, dst, src, n, blocks)
 
 
 def test_variant_enumeration_is_the_120_of_config_5(B):

@@ -628,3 +628,25 @@ def test_apply_host_matches_oracle_and_counts_bytes(env, layout, recon12):
         # PAPER.md:265 (Fig. 4): 1.5 GB without data analysis -> 0.75 GB with it, exactly 2:1
         assert h2d2 + d2h2 == 2 * (h2d + d2h)
         assert np.array_equal(gh.numpy(), g) and np.array_equal(ph.numpy(), p)
+
+
+# ---------------------------------------------------------------- the probe kernels (bench.py --probe) do what they say
+def test_probe_kernels_move_the_bytes_they_claim(env):
+    B, torch = env.B, env.torch
+    dev = torch.device("cuda:0")
+    n = 100003  # 16-byte units, not a multiple of anything
+    src = torch.randn(4 * n * 2, dtype=torch.float64, device=dev)
+    dst = torch.zeros(n * 2, dtype=torch.float64, device=dev)
+    st = torch.cuda.current_stream().cuda_stream
+    B.dslash_probe_launch(B.DSLASH_PROBE_COPY, dst.data_ptr(), src.data_ptr(), n, 37, st)
+    assert torch.equal(dst, src[:2 * n])
+    B.dslash_probe_launch(B.DSLASH_PROBE_READ4_WRITE1, dst.data_ptr(), src.data_ptr(), n, 37, st)
+    want = ((src[:2 * n] + src[2 * n:4 * n]) + src[4 * n:6 * n]) + src[6 * n:]
+    assert torch.equal(dst, want)
+    B.dslash_probe_launch(B.DSLASH_PROBE_WRITE, dst.data_ptr(), 0, n, 37, st)
+    assert torch.equal(dst.view(n, 2), torch.tensor([1.0, 2.0], dtype=torch.float64, device=dev).expand(n, 2))
+    keep = dst.clone()
+    B.dslash_probe_launch(B.DSLASH_PROBE_READ, dst.data_ptr(), src.data_ptr(), 4 * n, 37, st)
+    B.dslash_probe_launch(B.DSLASH_PROBE_DFMA, dst.data_ptr(), 0, 100, 37, st)
+    torch.cuda.synchronize()
+    assert torch.equal(dst, keep)  # the read and FMA probes never write
