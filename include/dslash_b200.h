@@ -128,6 +128,10 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
 #define DSLASH_OPT_PIPE_WARPS 8       /* warp-pipelined kernel: warps per thread block, 1, 2 or 4 (0 = library default) */
 #define DSLASH_OPT_PIPE_ZBLOCK 9      /* warp-pipelined kernel: rows are visited y fastest, z inside blocks of this many planes, then t,
                                          then the z blocks (a divisor of L_Z; 0 = L_Z): shortens the L2 reuse distance of the t hops */
+#define DSLASH_OPT_TUNE_MODE 10       /* what dslash_tune() optimises: DSLASH_TUNE_BURST (default; the first ~35 ms after idle, board at its
+                                         boost clock) or DSLASH_TUNE_SUSTAINED (continuous load, board at its power-capped clock) */
+#define DSLASH_TUNE_BURST 0
+#define DSLASH_TUNE_SUSTAINED 1
 
 /* host<->device mapping modes of dslash_apply_host() (section 4.1.2) */
 #define DSLASH_MAP_MINIMAL 0 /* to: gauge, in;  from: out            (after the Advisor's data analysis) */
@@ -255,7 +259,8 @@ DSLASH_API int dslash_get_kernel(const dslash_ctx *ctx, int *kernel);
  * that can run this context (DSLASH_KERNEL_DIRECT; DSLASH_KERNEL_WARP_PIPE in three slot/warp configurations where
  * eligible) is timed on the caller's buffers
  * (2 warm-up + 8 timed applications each, CUDA events on `stream`; about 15 ms in all, so that every candidate is
- * timed inside the board's boost window -- call it on an idle device) and the fastest becomes the
+ * timed inside the board's boost window -- call it on an idle device; with DSLASH_OPT_TUNE_MODE = DSLASH_TUNE_SUSTAINED:
+ * 150 applications to leave the boost window, then two interleaved rounds of 3 + 20 applications each, ~0.15 s in all) and the fastest becomes the
  * context's kernel, as if set by dslash_set_kernel() (and DSLASH_OPT_PIPE_SLOTS / _WARPS).  out, in, gauge: device pointers as for dslash_apply(); out is left
  * holding D in.  *chosen (may be NULL) receives the kernel, *ms_per_apply (may be NULL) its time.  This call SYNCHRONISES
  * with `stream`.  Errors: those of dslash_apply(); DSLASH_ERR_UNSUPPORTED when a sweep variant is selected.

@@ -22,7 +22,8 @@ DSLASH_VARIANT_TUNED = 0
 DSLASH_MAP_MINIMAL, DSLASH_MAP_TOFROM = 0, 1
 DSLASH_KERNEL_AUTO, DSLASH_KERNEL_DIRECT, DSLASH_KERNEL_TMA, DSLASH_KERNEL_TMA_LINKS, DSLASH_KERNEL_RING = 0, 1, 2, 3, 4
 DSLASH_KERNEL_WARP_PIPE = 5
-DSLASH_OPT_PIPE_SLOTS, DSLASH_OPT_PIPE_WARPS, DSLASH_OPT_PIPE_ZBLOCK = 7, 8, 9
+DSLASH_OPT_PIPE_SLOTS, DSLASH_OPT_PIPE_WARPS, DSLASH_OPT_PIPE_ZBLOCK, DSLASH_OPT_TUNE_MODE = 7, 8, 9, 10
+DSLASH_TUNE_BURST, DSLASH_TUNE_SUSTAINED = 0, 1
 DSLASH_OPT_OCCUPANCY, DSLASH_OPT_L2_POLICY, DSLASH_OPT_L1_CARVEOUT, DSLASH_OPT_X_SHUFFLE, DSLASH_OPT_T_CHUNK = 2, 3, 4, 5, 6
 DSLASH_SCHED_STATIC, DSLASH_SCHED_DYNAMIC, DSLASH_SCHED_GUIDED = 0, 1, 2
 DSLASH_OP_D, DSLASH_OP_D_DAGGER, DSLASH_OP_M, DSLASH_OP_M_DAGGER = 0, 1, 2, 3

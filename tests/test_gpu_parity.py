@@ -282,6 +282,13 @@ def test_warp_pipelined_kernel_refuses_what_it_cannot_run_and_tune_picks_a_worki
             o.zero_()
             lat.apply(o, pi, gi)
             assert env.checks.parity_error(lat.download_spinor(o), ref) <= TOL["f64"]
+            B.dslash_set_option(lat.ctx, B.DSLASH_OPT_TUNE_MODE, B.DSLASH_TUNE_SUSTAINED)
+            assert B.dslash_get_option(lat.ctx, B.DSLASH_OPT_TUNE_MODE) == B.DSLASH_TUNE_SUSTAINED
+            kernel, ms = lat.tune(o, pi, gi)
+            assert kernel in (B.DSLASH_KERNEL_DIRECT, B.DSLASH_KERNEL_WARP_PIPE) and ms > 0
+            assert env.checks.parity_error(lat.download_spinor(o), ref) <= TOL["f64"]
+            with pytest.raises(B.DslashError):
+                B.dslash_set_option(lat.ctx, B.DSLASH_OPT_TUNE_MODE, 2)
             B.dslash_set_variant(lat.ctx, 4, 128, 1)
             assert B.dslash_tune_status(lat.ctx, o.data_ptr(), pi.data_ptr(), gi.data_ptr()) == B.DSLASH_ERR_UNSUPPORTED
     assert B.dslash_tune_status(None, 16, 32, 48) == B.DSLASH_ERR_NULL
