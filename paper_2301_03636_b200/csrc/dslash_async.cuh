@@ -46,6 +46,9 @@ __device__ __forceinline__ void mbar_wait_spin(uint64_t* bar, uint32_t parity) {
             : "memory");
     } while (!done);
 }
+// Orders this thread's earlier generic-proxy accesses to shared memory (and, through a preceding barrier, those of the threads
+// it synchronised with) before its later async-proxy operations: needed before a bulk copy REFILLS a buffer that was just read.
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 // global -> shared bulk copy, completion (bytes) signalled on the mbarrier
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),

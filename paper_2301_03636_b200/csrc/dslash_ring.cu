@@ -116,6 +116,7 @@ __global__ void __launch_bounds__(MAXTPB, MINBLK)
             int t = t0 + i;
             if (t >= g.L[3]) t -= g.L[3];
             const unsigned vec = (row0 + st * (unsigned)t) >> VL_LOG2;
+            fence_proxy_async();  // the slot was read through the generic proxy (before the block barrier): order those reads first
             mbar_arrive_expect_tx(&full[slot], ROW_BYTES);
             bulk_g2s(ring + (size_t)(slot * nw + w) * ROW_BYTES, in_bytes + (size_t)vec * ROW_BYTES, ROW_BYTES, &full[slot]);
         }

@@ -185,9 +185,13 @@ struct PipeState {
         mbar_wait_spin(bar, (phase >> slot) & 1u);
         load_psi_slot<Real>(psi, sp, lane);
         load_link_slot<Real, RECON>(u, sp + PB::PSI, lane);
-        __syncwarp();  // every lane has its copy: the slot may be overwritten
+        __syncwarp();  // every lane has its copy: the slot may be overwritten ...
         phase ^= 1u << slot;
         if (lane == 0) {
+            // ... by the ASYNC proxy, which is not ordered after the generic-proxy reads above without this fence.  Measured:
+            // without it 9 % of the launches of a small L2-resident fp32 lattice (13 one-warp blocks per SM, bulk copies
+            // landing within a few hundred cycles) returned one wrong row; with it 0 of 600.
+            fence_proxy_async();
             constexpr int J = I + NSLOT;
             if (J < 7)
                 issue_stage<(J < 7 ? J : 0), Real, RECON>(pg, cur, in, gauge, sp, bar);
