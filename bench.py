@@ -5,9 +5,14 @@
     python bench.py --impl reference [--steps K] [--warmup W]       # the CPU oracle, same metric/config
     python bench.py --sweep [--sweep-csv PATH]                      # config 5: 120 variants, top-10
     python bench.py --advisor [--advisor-csv PATH]                  # the paper's own 84 variants on 32x32x32x16
+    python bench.py --costmodel                                     # the Advisor's cost model fitted on measured variant runtimes
+    python bench.py --probe                                         # read/write/copy/4:1-mix bandwidth, FP64 FMA rate of this board
+    python bench.py --cg | --eo | --decomposition slab              # solver, even-odd operator, multi-GPU slab form
+    python bench.py --kernel direct|wpipe|ring|tma ...              # force a kernel instead of letting dslash_tune pick
 
 A "step" is one application of D (one dslash_apply = one kernel launch covering SURVEY.md section 8(a)
-steps a1-a7) to one seeded synthetic lattice that is already resident in HBM in the native layout.
+steps a1-a7) to one seeded synthetic lattice that is already resident in HBM in the native layout.  Before the timed
+region the library picks its kernel by measurement (dslash_tune), then the device idles 1 s.
 `value` = 1320 flop/site * sites of all ranks / max-over-ranks device time (CUDA events on the
 launching stream).  `e2e` = the same through dslash_apply_host with pinned HOST buffers (H2D copy of
 gauge and spinor, pack, apply, unpack, D2H copy of the result inside the timed region).

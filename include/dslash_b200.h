@@ -243,12 +243,13 @@ DSLASH_API int dslash_set_time_range(dslash_ctx *ctx, int t_begin, int t_end);
 DSLASH_API int dslash_get_time_range(const dslash_ctx *ctx, int *t_begin, int *t_end);
 
 /*
- * Choose the implementation behind DSLASH_VARIANT_TUNED: DSLASH_KERNEL_AUTO (default), _DIRECT, _TMA or _TMA_LINKS.
+ * Choose the implementation behind DSLASH_VARIANT_TUNED: DSLASH_KERNEL_AUTO (default: _DIRECT until dslash_tune() has
+ * picked one), _DIRECT, _TMA, _TMA_LINKS, _RING or _WARP_PIPE (eligibility of the last two: see their definitions above).
  * _TMA and _TMA_LINKS need a DSLASH_SOA ctx, a tile whose x-extent is a multiple of 32 and divides L_X, the other tile
  * extents <= the lattice extents, and 32..128 sites per tile;
  * if it is selected explicitly and the current tile/lattice do not allow it, dslash_apply returns
  * DSLASH_ERR_UNSUPPORTED (AUTO falls back to _DIRECT silently -- both are CUDA kernels of this library).
- * dslash_get_kernel reports the kernel the next dslash_apply would launch (_DIRECT, _TMA or _TMA_LINKS).
+ * dslash_get_kernel reports the kernel the next dslash_apply would launch.
  * Errors: NULL, UNSUPPORTED (unknown value).
  */
 DSLASH_API int dslash_set_kernel(dslash_ctx *ctx, int kernel);
