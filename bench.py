@@ -688,6 +688,22 @@ def run_costmodel(args):
         e1.record()
         torch.cuda.synchronize()
         train1_ms = e0.elapsed_time(e1)
+        fill_ms = None
+        if target == "runtime_ms":
+            # the axis along which the GPU is filled: one model (seed) per SM in the same launch
+            sms = torch.cuda.get_device_properties(dev).multi_processor_count
+            uf = torch.from_numpy(np.stack([inputs.uniforms(SEED + 1000 + k, nw) for k in range(sms)])).to(dev)
+            pf = torch.from_numpy(np.stack([inputs.permutations(SEED + 1000 + k, epochs, ntr) for k in range(sms)])).to(dev)
+            model.train(xs_tr, ys_tr, uf, pf, epochs=epochs, batch=batch)
+            torch.cuda.synchronize()
+            e0.record()
+            model.train(xs_tr, ys_tr, uf, pf, epochs=epochs, batch=batch)
+            e1.record()
+            torch.cuda.synchronize()
+            fill_ms = e0.elapsed_time(e1)
+            out["one_model_per_sm"] = {"models": sms, "train_ms": fill_ms,
+                                       "model_updates_per_s": sms * epochs * ((ntr + batch - 1) // batch) / (fill_ms / 1e3)}
+            del uf, pf
         pred_va = model.predict(xs_va, params)
         nrmse = []
         for k in range(m):
