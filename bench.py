@@ -8,7 +8,7 @@
     python bench.py --costmodel                                     # the Advisor's cost model fitted on measured variant runtimes
     python bench.py --probe                                         # read/write/copy/4:1-mix bandwidth, FP64 FMA rate of this board
     python bench.py --cg | --eo | --decomposition slab              # solver, even-odd operator, multi-GPU slab form
-    python bench.py --kernel direct|wpipe|ring|tma ...              # force a kernel instead of letting dslash_tune pick
+    python bench.py --kernel direct|wpipe|march ...                 # force a kernel instead of letting dslash_tune pick
 
 A "step" is one application of D (one dslash_apply = one kernel launch covering SURVEY.md section 8(a)
 steps a1-a7) to one seeded synthetic lattice that is already resident in HBM in the native layout.  Before the timed
@@ -55,8 +55,10 @@ NCU_TRAFFIC_BYTES = {
     # profiles/r01f_wpipe.md: the warp-pipelined kernel (rows from the counter), 1.660823 GB read + 0.391139 GB written
     "32x32x32x64_f64_soa_r18_wpipe": 2051962000,
 }
-KERNEL_NAMES = {"direct": "dslash_tuned_kernel", "wpipe": "dslash_wpipe_kernel", "ring": "dslash_ring_kernel", "tma": "dslash_tma_kernel",
-                "tma_links": "dslash_tma_kernel"}
+KERNEL_NAMES = {"direct": "dslash_tuned_kernel", "wpipe": "dslash_wpipe_kernel", "march": "dslash_march_kernel"}
+
+
+KERNEL_IDS = {1: "direct", 5: "wpipe", 6: "march"}  # DSLASH_KERNEL_*
 
 
 def bytes_per_site(precision, recon12):
@@ -224,8 +226,6 @@ def run_cuda(args, cfg):
                 lat.set_kernel(args.kernel)
             if args.x_shuffle is not None:
                 B.dslash_set_option(lat.ctx, B.DSLASH_OPT_X_SHUFFLE, args.x_shuffle)
-            if args.t_chunk is not None:
-                B.dslash_set_option(lat.ctx, B.DSLASH_OPT_T_CHUNK, args.t_chunk)
             if args.pipe_slots is not None:
                 B.dslash_set_option(lat.ctx, B.DSLASH_OPT_PIPE_SLOTS, args.pipe_slots)
             if args.pipe_warps is not None:
@@ -247,9 +247,7 @@ def run_cuda(args, cfg):
                                 gflops=replicas.whole_job_rate(FLOP_PER_SITE * v, world, ms / args.steps) / 1e9,
                                 gbs=bps * v / (ms / args.steps) / 1e6, bps=bps, recon12=recon12,
                                 tile=list(B.dslash_get_tile(lat.ctx)),
-                                kernel={B.DSLASH_KERNEL_DIRECT: "direct", B.DSLASH_KERNEL_TMA: "tma", B.DSLASH_KERNEL_TMA_LINKS: "tma_links",
-                                        B.DSLASH_KERNEL_RING: "ring", B.DSLASH_KERNEL_WARP_PIPE: "wpipe"}[B.dslash_get_kernel(lat.ctx)],
-                                t_chunk=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_T_CHUNK),
+                                kernel=KERNEL_IDS[B.dslash_get_kernel(lat.ctx)],
                                 occupancy=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_OCCUPANCY),
                                 x_shuffle=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_X_SHUFFLE),
                                 pipe_slots=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_PIPE_SLOTS),
@@ -264,7 +262,7 @@ def run_cuda(args, cfg):
                     if tuned is not None:
                         B.dslash_set_option(lat.ctx, B.DSLASH_OPT_TUNE_MODE, B.DSLASH_TUNE_SUSTAINED)
                         ks, _ = lat.tune(od, pd, gd)
-                        kernel_s = {B.DSLASH_KERNEL_DIRECT: "direct", B.DSLASH_KERNEL_WARP_PIPE: "wpipe"}.get(ks, str(ks))
+                        kernel_s = KERNEL_IDS.get(ks, str(ks))
                     ms_s, ck_s = time_applies(torch, lat, od, pd, gd, args.sustained_steps, args.heat_steps, group, local)
                     results["sustained"] = dict(ms_per_step=ms_s / args.sustained_steps, clocks=ck_s, kernel=kernel_s,
                                                 gbs=bps * v / (ms_s / args.sustained_steps) / 1e6,
@@ -322,7 +320,7 @@ def run_cuda(args, cfg):
             "config": {"workload": cfg["name"], "dims": list(dims), "layout": args.layout, "recon": 12 if main["recon12"] else 18,
                        "tile": main["tile"], "kernel": main["kernel"],
                        "kernel_chosen_by": "dslash_tune (measured before the timed region)" if main["tuned_ms"] is not None else "option", "occupancy_option": main["occupancy"],
-                       "x_shuffle_option": main["x_shuffle"], "pipe_slots": main["pipe_slots"], "pipe_warps": main["pipe_warps"], "t_chunk_option": main["t_chunk"], "sites": v, "parallelism": "replicas x%d" % world,
+                       "x_shuffle_option": main["x_shuffle"], "pipe_slots": main["pipe_slots"], "pipe_warps": main["pipe_warps"], "sites": v, "parallelism": "replicas x%d" % world,
                        "l2": "inputs larger than L2: %.2f GB working set per apply vs 126 MB L2, no flush needed"
                              % (main["bps"] * v / 1e9)},
             "hbm_gbs": main["gbs"], "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "clocks": clocks,
@@ -913,11 +911,10 @@ def main():
     ap.add_argument("--layout", choices=["soa", "aos"], default="soa")
     ap.add_argument("--tile", type=int, nargs=4, default=None, help="tile of the tuned kernel (x y z t)")
     ap.add_argument("--occupancy", type=int, default=None, help="DSLASH_OPT_OCCUPANCY override")
-    ap.add_argument("--kernel", choices=["auto", "direct", "tma", "tma_links", "ring", "wpipe"], default=None)
+    ap.add_argument("--kernel", choices=["auto", "direct", "wpipe", "march"], default=None)
     ap.add_argument("--no-tune", action="store_true", help="skip dslash_tune (keep the library's static default kernel)")
     ap.add_argument("--pipe-slots", type=int, default=None, help="DSLASH_OPT_PIPE_SLOTS override (wpipe kernel)")
     ap.add_argument("--pipe-warps", type=int, default=None, help="DSLASH_OPT_PIPE_WARPS override (wpipe kernel)")
-    ap.add_argument("--t-chunk", type=int, default=None, help="DSLASH_OPT_T_CHUNK override (ring kernel)")
     ap.add_argument("--x-shuffle", type=int, choices=[0, 1], default=None, help="DSLASH_OPT_X_SHUFFLE override")
     ap.add_argument("--both-recon", action="store_true", default=True, help="also time the other link compression")
     ap.add_argument("--one-recon", dest="both_recon", action="store_false")

@@ -99,16 +99,18 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
 #define DSLASH_SCHED_GUIDED 2
 
 /* kernel selection of the tuned path, dslash_set_kernel() */
-#define DSLASH_KERNEL_AUTO 0   /* the library picks (TMA-staged when the layout/lattice/tile allow it, else direct) */
+#define DSLASH_KERNEL_AUTO 0   /* the library picks: _DIRECT until dslash_tune() has measured and chosen */
 #define DSLASH_KERNEL_DIRECT 1 /* one thread per site, all neighbours gathered from global memory through L1/L2 */
-#define DSLASH_KERNEL_TMA 2    /* tile's own spinors and links staged in shared memory by TMA bulk copies */
-#define DSLASH_KERNEL_TMA_LINKS 3 /* only the tile's own links staged by TMA bulk copies; spinors gathered directly */
-#define DSLASH_KERNEL_RING 4   /* t-marching with the tile's spinor rows of t, t+1, t+2 in a shared-memory ring filled by bulk
-                                  async copies one step ahead (blocked SoA, tile 32 x by x bz x 1 that tiles the lattice exactly,
-                                  L_X a multiple of 32); bit-identical to DSLASH_KERNEL_DIRECT */
+/* 2, 3, 4: kernels of round 1 (tile staged by bulk copies; spinor ring) that lost to the ones below and were removed */
 #define DSLASH_KERNEL_WARP_PIPE 5 /* persistent warps, one 32-site x row per warp; every hop stage (neighbour spinors + links of
                                   the row: two contiguous runs in the blocked SoA layout) is brought into per-warp shared-memory
                                   slots by two bulk async copies, DSLASH_OPT_PIPE_SLOTS stages ahead, no block barriers
+                                  (blocked SoA, L_X == 32); bit-identical to DSLASH_KERNEL_DIRECT */
+
+#define DSLASH_KERNEL_MARCH 6 /* block-cooperative t-marching: a block owns up to 7 x rows that are neighbours in the (y,z) plane
+                                  and marches through the time slices; every link and every spinor row of the patch crosses
+                                  L2 -> SM once (links used for the own forward hop AND the neighbour's backward contribution,
+                                  spinor rows kept in a shared-memory ring), all operands by bulk async copies
                                   (blocked SoA, L_X == 32); bit-identical to DSLASH_KERNEL_DIRECT */
 
 /* options of the tuned kernels, dslash_set_option() */
@@ -123,7 +125,6 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
                                          lanes by warp shuffles instead of loaded; 0 = always load them.  Same result, bit
                                          for bit */
 
-#define DSLASH_OPT_T_CHUNK 6          /* ring kernel: time slices a block marches through, 1..L_T (0 = library default 8) */
 #define DSLASH_OPT_PIPE_SLOTS 7       /* warp-pipelined kernel: hop stages in flight per warp, 2..4 (0 = library default) */
 #define DSLASH_OPT_PIPE_WARPS 8       /* warp-pipelined kernel: warps per thread block, 1, 2 or 4 (0 = library default) */
 #define DSLASH_OPT_PIPE_ZBLOCK 9      /* warp-pipelined kernel: rows are visited y fastest, z inside blocks of this many planes, then t,
@@ -159,7 +160,8 @@ DSLASH_API int dslash_destroy(dslash_ctx *ctx);
  *   out, in   device pointers, native spinor layout of the ctx, dslash_spinor_bytes() each,
  *             16-byte aligned, must not overlap.
  *   gauge     device pointer, native gauge layout, dslash_gauge_bytes(), 16-byte aligned.
- * Exactly one kernel launch; no allocation, copy or synchronisation.
+ * Exactly one kernel launch (DSLASH_KERNEL_WARP_PIPE: preceded by an 8-byte cudaMemsetAsync of its row counters on
+ * `stream`); no allocation, copy or synchronisation.
  * Errors: NULL, ALIGN, ALIAS, CUDA (launch failure, also stored in the ctx).
  */
 DSLASH_API int dslash_apply(dslash_ctx *ctx, void *out, const void *in, const void *gauge, dslash_stream_t stream);
@@ -235,30 +237,41 @@ DSLASH_API int dslash_get_tile(const dslash_ctx *ctx, int tile[4]);
  * outside the range are neither computed nor written.  This is the hook of the multi-GPU slab decomposition
  * (paper_2301_03636_b200/slab.py): a rank's local lattice carries one ghost slice at each end in t, only the interior
  * slices are computed, and the interior can be launched while the ghost slices are still being exchanged.
- * With a partial range the tuned path always uses the direct kernel; the sweep variants and dslash_cg_solve need the
- * full range (DSLASH_ERR_UNSUPPORTED otherwise).
- * Errors: NULL, UNSUPPORTED (not 0 <= t_begin < t_end <= L_T).
+ * Every tuned kernel honours the range (the marching kernel's block plan is rebuilt by this call: synchronous); the sweep
+ * variants and dslash_cg_solve need the full range (DSLASH_ERR_UNSUPPORTED otherwise).
+ * Errors: NULL, UNSUPPORTED (not 0 <= t_begin < t_end <= L_T), CUDA.
  */
 DSLASH_API int dslash_set_time_range(dslash_ctx *ctx, int t_begin, int t_end);
 DSLASH_API int dslash_get_time_range(const dslash_ctx *ctx, int *t_begin, int *t_end);
 
 /*
  * Choose the implementation behind DSLASH_VARIANT_TUNED: DSLASH_KERNEL_AUTO (default: _DIRECT until dslash_tune() has
- * picked one), _DIRECT, _TMA, _TMA_LINKS, _RING or _WARP_PIPE (eligibility of the last two: see their definitions above).
- * _TMA and _TMA_LINKS need a DSLASH_SOA ctx, a tile whose x-extent is a multiple of 32 and divides L_X, the other tile
- * extents <= the lattice extents, and 32..128 sites per tile;
- * if it is selected explicitly and the current tile/lattice do not allow it, dslash_apply returns
- * DSLASH_ERR_UNSUPPORTED (AUTO falls back to _DIRECT silently -- both are CUDA kernels of this library).
- * dslash_get_kernel reports the kernel the next dslash_apply would launch.
- * Errors: NULL, UNSUPPORTED (unknown value).
+ * picked one), _DIRECT, _WARP_PIPE or _MARCH (eligibility: see their definitions above).  The call also creates the
+ * device-side resources the kernel needs besides the caller's fields (row counters of _WARP_PIPE, block plan of _MARCH:
+ * one small cudaMalloc + cudaMemcpy, synchronous), so that dslash_apply itself never allocates, copies or synchronises.
+ * If a kernel is selected explicitly and the lattice/layout do not allow it, dslash_apply returns DSLASH_ERR_UNSUPPORTED.
+ * dslash_get_kernel reports the kernel the next dslash_apply would launch.  All kernels give bit-identical results.
+ * Errors: NULL, UNSUPPORTED (unknown value), NOMEM, CUDA.
  */
 DSLASH_API int dslash_set_kernel(dslash_ctx *ctx, int kernel);
 DSLASH_API int dslash_get_kernel(const dslash_ctx *ctx, int *kernel);
 
 /*
+ * Host-side view of the work decomposition of DSLASH_KERNEL_MARCH (no device needed; what dslash_set_kernel uploads).
+ * The rows of the (y,z) plane are ordered along a snake (strips of two z planes, boustrophedon in y) and cut into S
+ * segments of at most 7 rows; the time slices t_begin <= t < t_end into G chunks; block c*S + s marches segment s through
+ * chunk c.  S and G are chosen so that S*G fills whole waves of `wave` co-resident blocks (the SM count).
+ *   dims      {32, L_Y, L_Z, L_T} (L_X must be 32);  ints: host array receiving, per block, 4 + 7*9 ints:
+ *             {t0, nt, active warps, 0} then per warp {row, fwd[2], wr[2], rd[2], bwd[2]} (MarchWarpPlan in
+ *             csrc/dslash_kernels.cuh); ints may be NULL to query *nblocks only; capacity_ints = its size in ints.
+ * Errors: NULL, DIMS, UNSUPPORTED (L_X != 32, bad range, wave < 1, capacity too small).
+ */
+DSLASH_API int dslash_march_plan(const int dims[4], int t_begin, int t_end, int wave, int *ints, size_t capacity_ints, int *nblocks);
+
+/*
  * Pick the kernel by measurement (the Advisor's own method, applied to the library's kernels): every kernel
- * that can run this context (DSLASH_KERNEL_DIRECT; DSLASH_KERNEL_WARP_PIPE in three slot/warp configurations where
- * eligible) is timed on the caller's buffers
+ * that can run this context (DSLASH_KERNEL_DIRECT; where eligible DSLASH_KERNEL_MARCH and DSLASH_KERNEL_WARP_PIPE in
+ * three slot/warp configurations) is timed on the caller's buffers
  * (2 warm-up + 8 timed applications each, CUDA events on `stream`; about 15 ms in all, so that every candidate is
  * timed inside the board's boost window -- call it on an idle device; with DSLASH_OPT_TUNE_MODE = DSLASH_TUNE_SUSTAINED:
  * 150 applications to leave the boost window, then two interleaved rounds of 3 + 20 applications each, ~0.15 s in all) and the fastest becomes the

@@ -20,11 +20,12 @@ DSLASH_ERR_NULL, DSLASH_ERR_DIMS, DSLASH_ERR_PRECISION, DSLASH_ERR_LAYOUT = -1, 
 DSLASH_ERR_ALIGN, DSLASH_ERR_ALIAS, DSLASH_ERR_UNSUPPORTED, DSLASH_ERR_CUDA, DSLASH_ERR_NOMEM = -5, -6, -7, -8, -9
 DSLASH_VARIANT_TUNED = 0
 DSLASH_MAP_MINIMAL, DSLASH_MAP_TOFROM = 0, 1
-DSLASH_KERNEL_AUTO, DSLASH_KERNEL_DIRECT, DSLASH_KERNEL_TMA, DSLASH_KERNEL_TMA_LINKS, DSLASH_KERNEL_RING = 0, 1, 2, 3, 4
-DSLASH_KERNEL_WARP_PIPE = 5
+DSLASH_KERNEL_AUTO, DSLASH_KERNEL_DIRECT = 0, 1
+DSLASH_KERNEL_WARP_PIPE, DSLASH_KERNEL_MARCH = 5, 6
+MARCH_NW, MARCH_NWS, MARCH_BLOCK_INTS = 7, 10, 4 + 7 * 9  # block plan of dslash_march_plan()
 DSLASH_OPT_PIPE_SLOTS, DSLASH_OPT_PIPE_WARPS, DSLASH_OPT_PIPE_ZBLOCK, DSLASH_OPT_TUNE_MODE = 7, 8, 9, 10
 DSLASH_TUNE_BURST, DSLASH_TUNE_SUSTAINED = 0, 1
-DSLASH_OPT_OCCUPANCY, DSLASH_OPT_L2_POLICY, DSLASH_OPT_L1_CARVEOUT, DSLASH_OPT_X_SHUFFLE, DSLASH_OPT_T_CHUNK = 2, 3, 4, 5, 6
+DSLASH_OPT_OCCUPANCY, DSLASH_OPT_L2_POLICY, DSLASH_OPT_L1_CARVEOUT, DSLASH_OPT_X_SHUFFLE = 2, 3, 4, 5
 DSLASH_SCHED_STATIC, DSLASH_SCHED_DYNAMIC, DSLASH_SCHED_GUIDED = 0, 1, 2
 DSLASH_OP_D, DSLASH_OP_D_DAGGER, DSLASH_OP_M, DSLASH_OP_M_DAGGER = 0, 1, 2, 3
 
@@ -74,6 +75,7 @@ SIGNATURES = {
     "dslash_get_time_range": (ctypes.c_int, [_vp, _c_int_p, _c_int_p]),
     "dslash_set_kernel": (ctypes.c_int, [_vp, ctypes.c_int]),
     "dslash_get_kernel": (ctypes.c_int, [_vp, _c_int_p]),
+    "dslash_march_plan": (ctypes.c_int, [_c_int_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, _c_int_p, ctypes.c_size_t, _c_int_p]),
     "dslash_probe_launch": (ctypes.c_int, [ctypes.c_int, _vp, _vp, ctypes.c_size_t, ctypes.c_int, _vp]),
     "dslash_tune": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _c_int_p, ctypes.POINTER(ctypes.c_float)]),
     "dslash_set_option": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int]),
@@ -341,6 +343,26 @@ def dslash_get_kernel(ctx) -> int:
     k = ctypes.c_int()
     _check(_lib.dslash_get_kernel(_ptr(ctx), ctypes.byref(k)), "dslash_get_kernel")
     return k.value
+
+
+def dslash_march_plan(dims, t_begin: int, t_end: int, wave: int):
+    """Host-side block plan of DSLASH_KERNEL_MARCH (no device needed): a list of blocks
+    {t0, nt, nact, warps: [{row, fwd, wr, rd, bwd}]}."""
+    arr = (ctypes.c_int * 4)(*[int(d) for d in dims])
+    nb = ctypes.c_int()
+    _check(_lib.dslash_march_plan(arr, int(t_begin), int(t_end), int(wave), None, 0, ctypes.byref(nb)), "dslash_march_plan")
+    n = nb.value * MARCH_BLOCK_INTS
+    buf = (ctypes.c_int * n)()
+    _check(_lib.dslash_march_plan(arr, int(t_begin), int(t_end), int(wave), buf, n, ctypes.byref(nb)), "dslash_march_plan")
+    blocks = []
+    for b in range(nb.value):
+        v = buf[b * MARCH_BLOCK_INTS:(b + 1) * MARCH_BLOCK_INTS]
+        warps = []
+        for w in range(MARCH_NW):
+            q = v[4 + 9 * w:4 + 9 * (w + 1)]
+            warps.append(dict(row=q[0], fwd=(q[1], q[2]), wr=(q[3], q[4]), rd=(q[5], q[6]), bwd=(q[7], q[8])))
+        blocks.append(dict(t0=v[0], nt=v[1], nact=v[2], warps=warps))
+    return blocks
 
 
 def dslash_set_option(ctx, option: int, value: int) -> None:

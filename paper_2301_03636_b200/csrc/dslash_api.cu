@@ -41,6 +41,10 @@ struct dslash_ctx {
     unsigned* pipe_ctr;
     unsigned pipe_seq;
     int tune_mode;  // DSLASH_TUNE_BURST / DSLASH_TUNE_SUSTAINED (DSLASH_OPT_TUNE_MODE)
+    // block plan of the marching kernel for the time range [march_t0, march_t1) (device memory, owned; made by
+    // ensure_kernel_resources(), never by dslash_apply)
+    void* march_plan;
+    int march_blocks, march_t0, march_t1;
 };
 
 static int cuda_fail(dslash_ctx* c, cudaError_t e) {
@@ -179,6 +183,33 @@ static int cg_normal_equations(dslash_ctx* c, unsigned V, size_t sb, void** vec,
     return DSLASH_OK;
 }
 
+// Device-side resources a kernel needs besides the caller's fields: the row counters of the warp-pipelined kernel, the block
+// plan of the marching kernel.  Called where a kernel is SELECTED (dslash_set_kernel, dslash_tune, dslash_set_time_range,
+// dslash_create), so that dslash_apply itself never allocates, copies or synchronises.
+static int ensure_kernel_resources(dslash_ctx* c, int kernel) {
+    if (kernel == DSLASH_KERNEL_WARP_PIPE && !c->pipe_ctr && wpipe_eligible(c->layout_base, c->geom)) {
+        cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&c->pipe_ctr), 32 * sizeof(unsigned));
+        if (e != cudaSuccess) {
+            c->pipe_ctr = nullptr;
+            c->last_cuda = (int)e;
+            (void)cudaGetLastError();
+            return DSLASH_ERR_NOMEM;
+        }
+    }
+    if (kernel == DSLASH_KERNEL_MARCH && march_eligible(c->layout_base, c->geom) &&
+        (!c->march_plan || c->march_t0 != c->tg.t_begin || c->march_t1 != c->tg.t_end)) {
+        if (c->march_plan && cudaDeviceSynchronize() != cudaSuccess) return cuda_fail(c, cudaGetLastError());  // a launch may still read it
+        cudaError_t e = march_plan_create(c->geom, c->tg.t_begin, c->tg.t_end, c->device, &c->march_plan, &c->march_blocks);
+        if (e != cudaSuccess) {
+            (void)cudaGetLastError();
+            return cuda_fail(c, e);
+        }
+        c->march_t0 = c->tg.t_begin;
+        c->march_t1 = c->tg.t_end;
+    }
+    return DSLASH_OK;
+}
+
 extern "C" {
 
 int dslash_create(dslash_ctx** ctx, const int dims[4], int precision, int layout) {
@@ -234,13 +265,15 @@ int dslash_create(dslash_ctx** ctx, const int dims[4], int precision, int layout
     c->cfg.occupancy = precision == DSLASH_FP64 ? 2 : 1;  // measured: fp64 wants registers (ILP), fp32 wants warps
     c->cfg.l2_policy = 0;
     c->cfg.l1_carveout = -1;
-    c->cfg.t_chunk = 0;
     c->cfg.pipe_slots = 0;
     c->cfg.pipe_warps = 0;
     c->cfg.pipe_zblock = 0;
     c->cfg.pipe_counters = nullptr;
     c->pipe_ctr = nullptr;
     c->pipe_seq = 0;
+    c->march_plan = nullptr;
+    c->march_blocks = 0;
+    c->march_t0 = c->march_t1 = -1;
     c->tune_mode = DSLASH_TUNE_BURST;
     c->cfg.x_shuffle = precision == DSLASH_FP64 ? 1 : 0;  // measured: -1.3 % (burst) / -2 % (sustained) in fp64, +0.8 % in fp32
     c->launches = 0;
@@ -255,7 +288,7 @@ int dslash_create(dslash_ctx** ctx, const int dims[4], int precision, int layout
 int dslash_destroy(dslash_ctx* c) {
     if (!c) return DSLASH_OK;
     int rc = DSLASH_OK;
-    bool any = c->cg_scratch != nullptr;
+    bool any = c->cg_scratch != nullptr || c->pipe_ctr != nullptr || c->march_plan != nullptr;
     for (int i = 0; i < 3; ++i) any = any || c->d_can[i] || c->d_nat[i];
     for (int i = 0; i < 4; ++i) any = any || c->cg_vec[i];
     for (int i = 0; i < 6; ++i) any = any || c->eo_vec[i];
@@ -267,6 +300,7 @@ int dslash_destroy(dslash_ctx* c) {
             if (c->cg_vec[i]) cudaFree(c->cg_vec[i]);
         if (c->cg_scratch) cudaFree(c->cg_scratch);
         if (c->pipe_ctr) cudaFree(c->pipe_ctr);
+        if (c->march_plan) cudaFree(c->march_plan);
         for (int i = 0; i < 3; ++i) {
             if (c->d_nat[i] && c->d_nat[i] != c->d_can[i]) cudaFree(c->d_nat[i]);
             if (c->d_can[i]) cudaFree(c->d_can[i]);
@@ -287,14 +321,12 @@ size_t dslash_gauge_bytes(const dslash_ctx* c) {
 size_t dslash_canonical_spinor_bytes(const dslash_ctx* c) { return c ? (size_t)c->geom.V * 24u * real_bytes(c) : 0; }
 size_t dslash_canonical_gauge_bytes(const dslash_ctx* c) { return c ? (size_t)c->geom.V * 72u * real_bytes(c) : 0; }
 
-// The kernel dslash_apply will launch for the tuned path: DSLASH_KERNEL_DIRECT / _TMA, or -1 if _TMA was
-// requested explicitly but cannot run this configuration.
+// The kernel dslash_apply will launch for the tuned path, or -1 if a kernel was requested explicitly that cannot run this
+// configuration.
 static int resolve_kernel(const dslash_ctx* c) {
-    const bool can_tma = c->layout_base == LAYOUT_SOA && full_time_range(c) && tma_eligible(c->precision, c->recon, c->geom, c->tg);
     if (c->kernel == DSLASH_KERNEL_DIRECT) return DSLASH_KERNEL_DIRECT;
-    if (c->kernel == DSLASH_KERNEL_TMA || c->kernel == DSLASH_KERNEL_TMA_LINKS) return can_tma ? c->kernel : -1;
-    if (c->kernel == DSLASH_KERNEL_RING) return ring_eligible(c->layout_base, c->geom, c->tg) ? DSLASH_KERNEL_RING : -1;
     if (c->kernel == DSLASH_KERNEL_WARP_PIPE) return wpipe_eligible(c->layout_base, c->geom) ? DSLASH_KERNEL_WARP_PIPE : -1;
+    if (c->kernel == DSLASH_KERNEL_MARCH) return march_eligible(c->layout_base, c->geom) ? DSLASH_KERNEL_MARCH : -1;
     return DSLASH_KERNEL_DIRECT;  // AUTO
 }
 
@@ -315,20 +347,18 @@ int dslash_apply(dslash_ctx* c, void* out, const void* in, const void* gauge, ds
         const int k = resolve_kernel(c);
         if (k < 0) return DSLASH_ERR_UNSUPPORTED;
         if (k == DSLASH_KERNEL_WARP_PIPE) {
-            if (!c->pipe_ctr) {
-                cudaError_t ea = cudaMalloc(reinterpret_cast<void**>(&c->pipe_ctr), 32 * sizeof(unsigned));
-                if (ea == cudaSuccess) ea = cudaMemset(c->pipe_ctr, 0, 32 * sizeof(unsigned));
-                if (ea != cudaSuccess) {
-                    c->pipe_ctr = nullptr;
-                    return cuda_fail(c, ea);
-                }
-            }
+            if (!c->pipe_ctr) return DSLASH_ERR_UNSUPPORTED;  // ensure_kernel_resources() runs wherever the kernel is selected
+            // {next row, finished warps} of this launch: one of 16 pairs, zeroed on the launch stream (stream-ordered with
+            // the kernel whatever kind of stream it is; a faulted launch cannot leave a pair dirty for the next one)
             c->cfg.pipe_counters = c->pipe_ctr + 2u * (c->pipe_seq++ & 15u);
+            cudaError_t ez = cudaMemsetAsync(c->cfg.pipe_counters, 0, 2 * sizeof(unsigned), a.stream);
+            if (ez != cudaSuccess) return cuda_fail(c, ez);
         }
-        e = (k == DSLASH_KERNEL_DIRECT)   ? launch_tuned(c->precision, c->layout_base, c->recon, a, c->tg, c->cfg)
-            : (k == DSLASH_KERNEL_RING)   ? launch_ring(c->precision, c->layout_base, c->recon, a, c->tg, c->cfg)
-            : (k == DSLASH_KERNEL_WARP_PIPE) ? launch_wpipe(c->precision, c->layout_base, c->recon, a, c->tg, c->cfg)
-                                          : launch_tma(c->precision, c->recon, a, c->tg, k == DSLASH_KERNEL_TMA_LINKS);
+        if (k == DSLASH_KERNEL_MARCH && (!c->march_plan || c->march_t0 != c->tg.t_begin || c->march_t1 != c->tg.t_end))
+            return DSLASH_ERR_UNSUPPORTED;
+        e = (k == DSLASH_KERNEL_WARP_PIPE) ? launch_wpipe(c->precision, c->layout_base, c->recon, a, c->tg, c->cfg)
+            : (k == DSLASH_KERNEL_MARCH)   ? launch_march(c->precision, c->layout_base, c->recon, a, c->march_plan, c->march_blocks, c->cfg)
+                                           : launch_tuned(c->precision, c->layout_base, c->recon, a, c->tg, c->cfg);
     } else if (!full_time_range(c)) {
         return DSLASH_ERR_UNSUPPORTED;  // the variant kernels always sweep the whole lattice
     } else if (c->var_depth < 0) {
@@ -667,7 +697,7 @@ int dslash_set_time_range(dslash_ctx* c, int t_begin, int t_end) {
     c->tg.t_begin = t_begin;
     c->tg.t_end = t_end;
     set_tile_geom(c, c->tile);
-    return DSLASH_OK;
+    return ensure_kernel_resources(c, c->kernel);
 }
 
 int dslash_get_time_range(const dslash_ctx* c, int* t_begin, int* t_end) {
@@ -697,10 +727,6 @@ int dslash_set_option(dslash_ctx* c, int option, int value) {
         case DSLASH_OPT_L1_CARVEOUT:
             if (value < -1 || value > 100) return DSLASH_ERR_UNSUPPORTED;
             c->cfg.l1_carveout = value;
-            return DSLASH_OK;
-        case DSLASH_OPT_T_CHUNK:
-            if (value < 0 || value > c->geom.L[3]) return DSLASH_ERR_UNSUPPORTED;
-            c->cfg.t_chunk = value;
             return DSLASH_OK;
         case DSLASH_OPT_X_SHUFFLE:
             if (value < 0 || value > 1) return DSLASH_ERR_UNSUPPORTED;
@@ -734,7 +760,6 @@ int dslash_get_option(const dslash_ctx* c, int option, int* value) {
         case DSLASH_OPT_L2_POLICY: *value = c->cfg.l2_policy; return DSLASH_OK;
         case DSLASH_OPT_L1_CARVEOUT: *value = c->cfg.l1_carveout; return DSLASH_OK;
         case DSLASH_OPT_X_SHUFFLE: *value = c->cfg.x_shuffle; return DSLASH_OK;
-        case DSLASH_OPT_T_CHUNK: *value = c->cfg.t_chunk; return DSLASH_OK;
         case DSLASH_OPT_PIPE_SLOTS: *value = c->cfg.pipe_slots; return DSLASH_OK;
         case DSLASH_OPT_PIPE_WARPS: *value = c->cfg.pipe_warps; return DSLASH_OK;
         case DSLASH_OPT_PIPE_ZBLOCK: *value = c->cfg.pipe_zblock; return DSLASH_OK;
@@ -745,9 +770,11 @@ int dslash_get_option(const dslash_ctx* c, int option, int* value) {
 
 int dslash_set_kernel(dslash_ctx* c, int kernel) {
     if (!c) return DSLASH_ERR_NULL;
-    if (kernel != DSLASH_KERNEL_AUTO && kernel != DSLASH_KERNEL_DIRECT && kernel != DSLASH_KERNEL_TMA &&
-        kernel != DSLASH_KERNEL_TMA_LINKS && kernel != DSLASH_KERNEL_RING && kernel != DSLASH_KERNEL_WARP_PIPE)
+    if (kernel != DSLASH_KERNEL_AUTO && kernel != DSLASH_KERNEL_DIRECT && kernel != DSLASH_KERNEL_WARP_PIPE &&
+        kernel != DSLASH_KERNEL_MARCH)
         return DSLASH_ERR_UNSUPPORTED;
+    const int rc = ensure_kernel_resources(c, kernel);
+    if (rc != DSLASH_OK) return rc;
     c->kernel = kernel;
     return DSLASH_OK;
 }
@@ -768,10 +795,15 @@ int dslash_tune(dslash_ctx* c, void* out, const void* in, const void* gauge, dsl
     struct Cand {
         int kernel, slots, warps;
     };
-    Cand cand[4];
+    Cand cand[5];
     int ncand = 0;
     cand[ncand++] = {DSLASH_KERNEL_DIRECT, 0, 0};
-    if (wpipe_eligible(c->layout_base, c->geom)) {
+    if (march_eligible(c->layout_base, c->geom)) cand[ncand++] = {DSLASH_KERNEL_MARCH, 0, 0};
+    for (int k = 0; k < ncand; ++k) {
+        const int rcr = ensure_kernel_resources(c, cand[k].kernel);
+        if (rcr != DSLASH_OK) return rcr;
+    }
+    if (wpipe_eligible(c->layout_base, c->geom) && ensure_kernel_resources(c, DSLASH_KERNEL_WARP_PIPE) == DSLASH_OK) {
         cand[ncand++] = {DSLASH_KERNEL_WARP_PIPE, 2, 4};  // 8 warps x 2 stages in flight per SM (fp64, 18-real)
         cand[ncand++] = {DSLASH_KERNEL_WARP_PIPE, 3, 1};  // 6 warps x 3 stages
         cand[ncand++] = {DSLASH_KERNEL_WARP_PIPE, 2, 1};  // 10 warps x 2 stages
@@ -790,7 +822,7 @@ int dslash_tune(dslash_ctx* c, void* out, const void* in, const void* gauge, dsl
     // ones not.  DSLASH_TUNE_SUSTAINED: 150 applications first (the board leaves its boost window after ~35 ms and settles at
     // its power-capped clock), then two interleaved rounds of 3 + 20 applications per candidate, summed per candidate.
     const bool sustained = c->tune_mode == DSLASH_TUNE_SUSTAINED;
-    float total[4] = {0.f, 0.f, 0.f, 0.f};
+    float total[5] = {0.f, 0.f, 0.f, 0.f, 0.f};
     if (sustained) {
         c->kernel = DSLASH_KERNEL_DIRECT;
         for (int i = 0; i < 150 && rc == DSLASH_OK; ++i) rc = dslash_apply(c, out, in, gauge, stream);

@@ -1,6 +1,6 @@
-// dslash_async.cuh -- sm_100a asynchronous-copy plumbing shared by the shared-memory-staged kernels (dslash_tma.cu,
-// dslash_ring.cu): mbarrier + cp.async.bulk (the TMA unit, SASS UBLKCP) PTX wrappers and spinor reads from a shared-memory
-// copy of a 32-site vector in the global blocked-SoA format.
+// dslash_async.cuh -- sm_100a asynchronous-copy plumbing shared by the shared-memory-staged kernels (dslash_march.cu,
+// dslash_wpipe.cu): mbarrier + cp.async.bulk (the TMA unit's flat bulk copy, SASS UBLKCP) PTX wrappers, reads of spinors and
+// links from a shared-memory copy of a 32-site vector in the global blocked-SoA format, and hops on operands in registers.
 #pragma once
 #include <stdint.h>
 
@@ -56,6 +56,14 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                  : "memory");
 }
 
+// the same copy with an L2 eviction policy (createpolicy, see make_policy) for the global read
+__device__ __forceinline__ void bulk_g2s_hint(void* dst, const void* src, uint32_t bytes, uint64_t* bar, uint64_t policy) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+                     smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
+                 : "memory");
+}
+
 // ------------------------------------------------------------------ shared-memory field access
 // Same vector format as global memory, indexed by the tile-local site number (plain ld.shared).
 template <typename Real>
@@ -85,5 +93,72 @@ __device__ __forceinline__ void load_spinor_smem(cplx<float> (&psi)[12], const v
         psi[2 * q] = {v.x, v.y};
         psi[2 * q + 1] = {v.z, v.w};
     }
+}
+// ------------------------------------------------------------------ one 32-site vector in shared memory, lane = site
+// spinor of lane `lane` from a shared-memory copy of one spinor vector (global blocked-SoA format)
+template <typename Real>
+__device__ __forceinline__ void load_psi_slot(cplx<Real> (&psi)[12], const unsigned char* p, unsigned lane);
+template <>
+__device__ __forceinline__ void load_psi_slot<double>(cplx<double> (&psi)[12], const unsigned char* p, unsigned lane) {
+    const double2* q = reinterpret_cast<const double2*>(p) + lane;
+#pragma unroll
+    for (int k = 0; k < 12; ++k) {
+        const double2 v = q[k * VL];
+        psi[k] = {v.x, v.y};
+    }
+}
+template <>
+__device__ __forceinline__ void load_psi_slot<float>(cplx<float> (&psi)[12], const unsigned char* p, unsigned lane) {
+    const float4* q = reinterpret_cast<const float4*>(p) + lane;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        const float4 v = q[k * VL];
+        psi[2 * k] = {v.x, v.y};
+        psi[2 * k + 1] = {v.z, v.w};
+    }
+}
+
+// link of lane `lane` from a shared-memory copy of one (vector, mu) block of the gauge field; RECON == 12 rebuilds row 2
+// exactly as load_link() does.
+template <typename Real, int RECON>
+__device__ __forceinline__ void load_link_slot(cplx<Real> (&u)[9], const unsigned char* p, unsigned lane) {
+    using V2 = typename vec2<Real>::type;
+    constexpr int R = (RECON == 12) ? 6 : 9;
+    const V2* q = reinterpret_cast<const V2*>(p) + lane;
+#pragma unroll
+    for (int e = 0; e < R; ++e) {
+        const V2 v = q[e * VL];
+        u[e] = {v.x, v.y};
+    }
+    if (RECON == 12) reconstruct_row2(u);
+}
+
+// the two x hops from the row's own spinors and links (the arithmetic of x_hops_shuffle with the operands in registers)
+template <typename Real>
+__device__ __forceinline__ void x_hops_regs(cplx<Real> (&acc)[12], const cplx<Real> (&psi)[12], const cplx<Real> (&u)[9],
+                                            int lane_fwd, int lane_bwd) {
+    cplx<Real> hm[6], hq[6], w[6], hp[6];
+    project<0, -1>(hm, psi);
+    project<0, +1>(hq, psi);
+    su3_mul<true>(w, u, hq);
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        hm[k].re = shfl_(hm[k].re, lane_fwd);
+        hm[k].im = shfl_(hm[k].im, lane_fwd);
+        w[k].re = shfl_(w[k].re, lane_bwd);
+        w[k].im = shfl_(w[k].im, lane_bwd);
+    }
+    su3_mul<false>(hp, u, hm);
+    reconstruct_accumulate<0, -1, true>(acc, hp);
+    reconstruct_accumulate<0, +1, false>(acc, w);
+}
+
+// one hop with both operands in registers
+template <int MU, int SIGN, typename Real>
+__device__ __forceinline__ void hop_regs(cplx<Real> (&acc)[12], const cplx<Real> (&psi)[12], const cplx<Real> (&u)[9]) {
+    cplx<Real> h[6], hp[6];
+    project<MU, SIGN>(h, psi);
+    su3_mul<(SIGN > 0)>(hp, u, h);
+    reconstruct_accumulate<MU, SIGN, false>(acc, hp);
 }
 }  // namespace dslash

@@ -36,7 +36,6 @@ struct TunedConfig {
     int occupancy;         // 0: default register budget, 1: 128-register variant
     int l2_policy;         // DSLASH_OPT_L2_POLICY bits (0: no cache hints)
     int l1_carveout;       // preferred shared-memory carve-out of the direct kernel in percent (-1: driver default)
-    int t_chunk;           // time slices a block of the ring kernel marches through (0: default)
     int pipe_slots;        // warp-pipelined kernel: stages in flight per warp (2..4; 0: default 2)
     int pipe_warps;        // warp-pipelined kernel: warps per block (1, 2 or 4; 0: default 4)
     unsigned* pipe_counters;  // warp-pipelined kernel: {next row, finished warps} of this launch (device memory, zero between launches)
@@ -49,17 +48,33 @@ bool x_shuffle_eligible(const Geom& g, const TileGeom& tg);
 cudaError_t launch_tuned(int precision, int layout_base, int recon, const LaunchArgs& a, const TileGeom& tg,
                          const TunedConfig& cfg);
 
-// t-marching kernel with a shared-memory ring of spinor time slices fed by bulk async copies (dslash_ring.cu).
-bool ring_eligible(int layout_base, const Geom& g, const TileGeom& tg);
-cudaError_t launch_ring(int precision, int layout_base, int recon, const LaunchArgs& a, const TileGeom& tg, const TunedConfig& cfg);
-
-// warp-pipelined kernel: every hop stage of a 32-site row by two bulk async copies into per-warp shared-memory slots (dslash_wpipe.cu).
+// warp-pipelined kernel: every hop stage of a 32-site row by two flat bulk async copies (cp.async.bulk, SASS UBLKCP) into
+// per-warp shared-memory slots (dslash_wpipe.cu).
 bool wpipe_eligible(int layout_base, const Geom& g);
 cudaError_t launch_wpipe(int precision, int layout_base, int recon, const LaunchArgs& a, const TileGeom& tg, const TunedConfig& cfg);
 
-// TMA-staged kernel (SoA only): tile's own spinors + links by cp.async.bulk.tensor into shared memory.
-bool tma_eligible(int precision, int recon, const Geom& g, const TileGeom& tg);
-cudaError_t launch_tma(int precision, int recon, const LaunchArgs& a, const TileGeom& tg, bool links_only);
+// block-cooperative t-marching kernel (dslash_march.cu): a block owns up to MARCH_NW x rows that are neighbours in the (y,z)
+// plane and marches through a chunk of time slices.  The decomposition is a host-built plan in device memory.
+constexpr int MARCH_NW = 7;    // warps (= rows) per block: what 227 KB of shared memory hold in fp64
+constexpr int MARCH_NWS = 10;  // exchange buffers per block (>= the 8 neighbour pairs 7 cells of a grid can form)
+struct MarchWarpPlan {
+    int row;     // the warp's row = vector index inside a time slice, y + L_Y * z (L_X == 32); -1: idle warp
+    int fwd[2];  // spinor source of the forward y (0) / z (1) hop: >= 0 warp of this block whose ring row it is; < 0: -(row' + 1),
+                 // row' = the neighbour row, fetched from global memory (halo)
+    int wr[2];   // exchange buffer this warp fills with U^dagger P+ psi for its y+ / z+ neighbour (-1: none)
+    int rd[2];   // exchange buffer holding the backward contribution of the y- / z- neighbour (-1: halo hop from row bwd[])
+    int bwd[2];  // row of the y- / z- neighbour
+};
+struct MarchBlockPlan {
+    int t0, nt;  // first time slice and number of steps
+    int nact;    // active warps
+    int pad;
+    MarchWarpPlan w[MARCH_NW];
+};
+bool march_eligible(int layout_base, const Geom& g);
+cudaError_t march_plan_create(const Geom& g, int t_begin, int t_end, int device, void** d_plan, int* nblocks);
+cudaError_t launch_march(int precision, int layout_base, int recon, const LaunchArgs& a, const void* d_plan, int nblocks,
+                         const TunedConfig& cfg);
 
 // Operators around Dslash (dslash_ops.cu): op 0 D, 1 D^dagger, 2 M = (4+m) - D/2, 3 M^dagger; solver vector kernels.
 cudaError_t launch_op(int precision, int layout_base, int recon, const LaunchArgs& a, const TileGeom& tg, int op, double mass);

@@ -225,8 +225,25 @@ struct vec2<float> {
     using type = float2;
 };
 
+// Row 2 of an SU(3) link from rows 0 and 1: row2 = conj(row0 x row1) (exact for SU(3), DESIGN.md Reading R14).
+// u[0..5] = rows 0,1 on entry; u[6..8] written.  The ONE place this is computed: every kernel with RECON == 12 calls it.
+template <typename Real>
+__device__ __forceinline__ void reconstruct_row2(cplx<Real> (&u)[9]) {
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+        const int j1 = (j + 1) % 3, j2 = (j + 2) % 3;
+        // row2[j] = conj(row0[j1]*row1[j2] - row0[j2]*row1[j1])
+        cplx<Real> a = c_mul(u[j1], u[3 + j2]);
+        Real re = fma_(-u[j2].re, u[3 + j1].re, a.re);
+        re = fma_(u[j2].im, u[3 + j1].im, re);
+        Real im = fma_(-u[j2].re, u[3 + j1].im, a.im);
+        im = fma_(-u[j2].im, u[3 + j1].re, im);
+        u[6 + j] = {re, -im};
+    }
+}
+
 // Link U_mu(s): 9 complex entries u[row*3+col]; with RECON == 12 only rows 0,1 are stored and row 2
-// is rebuilt as conj(row0 x row1) (exact for SU(3), DESIGN.md Reading R14).
+// is rebuilt by reconstruct_row2().
 template <typename Real, int LAYOUT, int RECON, int HINT = 0>
 __device__ __forceinline__ void load_link(cplx<Real> (&u)[9], const void* base, unsigned V, unsigned s, int mu, uint64_t pol = 0) {
     using V2 = typename vec2<Real>::type;
@@ -247,19 +264,7 @@ __device__ __forceinline__ void load_link(cplx<Real> (&u)[9], const void* base, 
             u[e] = {v.x, v.y};
         }
     }
-    if (RECON == 12) {
-#pragma unroll
-        for (int j = 0; j < 3; ++j) {
-            const int j1 = (j + 1) % 3, j2 = (j + 2) % 3;
-            // row2[j] = conj(row0[j1]*row1[j2] - row0[j2]*row1[j1])
-            cplx<Real> a = c_mul(u[j1], u[3 + j2]);
-            Real re = fma_(-u[j2].re, u[3 + j1].re, a.re);
-            re = fma_(u[j2].im, u[3 + j1].im, re);
-            Real im = fma_(-u[j2].re, u[3 + j1].im, a.im);
-            im = fma_(-u[j2].im, u[3 + j1].re, im);
-            u[6 + j] = {re, -im};
-        }
-    }
+    if (RECON == 12) reconstruct_row2(u);
 }
 
 // ------------------------------------------------------------------ spin projection / reconstruction
@@ -427,13 +432,15 @@ __device__ __forceinline__ void dslash_site(void* out, const void* in, const voi
         hop<0, -1, true, Real, LAYOUT, RECON, (HINT ? 1 : 0)>(acc, in, gauge, V, xf, s, pol.psi, pol.u_s);
         hop<0, +1, false, Real, LAYOUT, RECON, (HINT ? 1 : 0)>(acc, in, gauge, V, xb, xb, pol.psi, pol.u_s);
     }
+    // ORDER of the sum (every tuned kernel of the library uses it, so their results are bit-identical):
+    // x forward, x backward, y forward, z forward, t forward, t backward, y backward, z backward
     hop<1, -1, false, Real, LAYOUT, RECON, (HINT ? 1 : 0)>(acc, in, gauge, V, yf, s, pol.psi, pol.u_s);
-    hop<1, +1, false, Real, LAYOUT, RECON, (HINT ? 1 : 0)>(acc, in, gauge, V, yb, yb, pol.psi, pol.u_s);
     hop<2, -1, false, Real, LAYOUT, RECON, (HINT ? 1 : 0)>(acc, in, gauge, V, zf, s, pol.psi, pol.u_s);
-    hop<2, +1, false, Real, LAYOUT, RECON, (HINT ? 1 : 0)>(acc, in, gauge, V, zb, zb, pol.psi, pol.u_s);
     // HINT == 2: the t-direction loads bypass L1 allocation (a block's tile is one slice thick in t: no reuse inside the block)
     hop<3, -1, false, Real, LAYOUT, RECON, HINT>(acc, in, gauge, V, tf, s, pol.psi, pol.u_t);
     hop<3, +1, false, Real, LAYOUT, RECON, HINT>(acc, in, gauge, V, tb, tb, pol.psi, pol.u_t);
+    hop<1, +1, false, Real, LAYOUT, RECON, (HINT ? 1 : 0)>(acc, in, gauge, V, yb, yb, pol.psi, pol.u_s);
+    hop<2, +1, false, Real, LAYOUT, RECON, (HINT ? 1 : 0)>(acc, in, gauge, V, zb, zb, pol.psi, pol.u_s);
     if (active) SpinorIO<Real, LAYOUT>::template store<(HINT ? 1 : 0)>(out, V, s, acc, pol.out);
 }
 

@@ -1,6 +1,6 @@
 // dslash_wpipe.cu -- warp-pipelined Dslash kernel (DSLASH_KERNEL_WARP_PIPE), sm_100a.
 //
-// Same operator, same per-hop arithmetic and the same hop order as dslash_tuned.cu (Eq. 1; results
+// Same operator, same per-hop arithmetic and the same order of the sum as dslash_tuned.cu (Eq. 1; results
 // bit-identical).  What changes is how the operands travel.  The direct kernel is bound by the bytes its ~8 resident warps
 // per SM can keep in flight in REGISTERS (profiles/r01d_ncu_direct_ring_eo.txt: at most one hop = 336 B per thread).  Here
 // the in-flight operands sit in SHARED MEMORY, written by the TMA unit, and cost neither registers nor LSU instructions:
@@ -26,82 +26,6 @@
 namespace dslash {
 
 namespace {
-
-template <typename Real>
-__device__ __forceinline__ void load_psi_slot(cplx<Real> (&psi)[12], const unsigned char* p, unsigned lane);
-template <>
-__device__ __forceinline__ void load_psi_slot<double>(cplx<double> (&psi)[12], const unsigned char* p, unsigned lane) {
-    const double2* q = reinterpret_cast<const double2*>(p) + lane;
-#pragma unroll
-    for (int k = 0; k < 12; ++k) {
-        const double2 v = q[k * VL];
-        psi[k] = {v.x, v.y};
-    }
-}
-template <>
-__device__ __forceinline__ void load_psi_slot<float>(cplx<float> (&psi)[12], const unsigned char* p, unsigned lane) {
-    const float4* q = reinterpret_cast<const float4*>(p) + lane;
-#pragma unroll
-    for (int k = 0; k < 6; ++k) {
-        const float4 v = q[k * VL];
-        psi[2 * k] = {v.x, v.y};
-        psi[2 * k + 1] = {v.z, v.w};
-    }
-}
-
-// link of lane `lane` from a shared-memory copy of one (vector, mu) block of the gauge field; RECON == 12 rebuilds row 2
-// exactly as load_link() does.
-template <typename Real, int RECON>
-__device__ __forceinline__ void load_link_slot(cplx<Real> (&u)[9], const unsigned char* p, unsigned lane) {
-    using V2 = typename vec2<Real>::type;
-    constexpr int R = (RECON == 12) ? 6 : 9;
-    const V2* q = reinterpret_cast<const V2*>(p) + lane;
-#pragma unroll
-    for (int e = 0; e < R; ++e) {
-        const V2 v = q[e * VL];
-        u[e] = {v.x, v.y};
-    }
-    if (RECON == 12) {
-#pragma unroll
-        for (int j = 0; j < 3; ++j) {
-            const int j1 = (j + 1) % 3, j2 = (j + 2) % 3;
-            cplx<Real> a = c_mul(u[j1], u[3 + j2]);
-            Real re = fma_(-u[j2].re, u[3 + j1].re, a.re);
-            re = fma_(u[j2].im, u[3 + j1].im, re);
-            Real im = fma_(-u[j2].re, u[3 + j1].im, a.im);
-            im = fma_(-u[j2].im, u[3 + j1].re, im);
-            u[6 + j] = {re, -im};
-        }
-    }
-}
-
-// the two x hops from the row's own spinors and links (the arithmetic of x_hops_shuffle with the operands in registers)
-template <typename Real>
-__device__ __forceinline__ void x_hops_regs(cplx<Real> (&acc)[12], const cplx<Real> (&psi)[12], const cplx<Real> (&u)[9],
-                                            int lane_fwd, int lane_bwd) {
-    cplx<Real> hm[6], hq[6], w[6], hp[6];
-    project<0, -1>(hm, psi);
-    project<0, +1>(hq, psi);
-    su3_mul<true>(w, u, hq);
-#pragma unroll
-    for (int k = 0; k < 6; ++k) {
-        hm[k].re = shfl_(hm[k].re, lane_fwd);
-        hm[k].im = shfl_(hm[k].im, lane_fwd);
-        w[k].re = shfl_(w[k].re, lane_bwd);
-        w[k].im = shfl_(w[k].im, lane_bwd);
-    }
-    su3_mul<false>(hp, u, hm);
-    reconstruct_accumulate<0, -1, true>(acc, hp);
-    reconstruct_accumulate<0, +1, false>(acc, w);
-}
-
-template <int MU, int SIGN, typename Real>
-__device__ __forceinline__ void hop_regs(cplx<Real> (&acc)[12], const cplx<Real> (&psi)[12], const cplx<Real> (&u)[9]) {
-    cplx<Real> h[6], hp[6];
-    project<MU, SIGN>(h, psi);
-    su3_mul<(SIGN > 0)>(hp, u, h);
-    reconstruct_accumulate<MU, SIGN, false>(acc, hp);
-}
 
 struct PipeGeom {
     int LY, LZ, LT;      // rows are indexed v = y + LY * (z + LZ * t); one row = one 32-site vector
@@ -143,21 +67,26 @@ __device__ __forceinline__ Row decode_row(const PipeGeom& pg, unsigned r) {
     return w;
 }
 
-// Stage I of a row: I = 0 own psi + U_x(row); 1 psi(y+1), U_y(row); 2 psi(y-1), U_y(y-1); 3, 4 the same in z; 5, 6 in t.
+// Stage I of a row, in the order of the sum (dslash_site.cuh): 0 own psi + U_x(row) for the shuffled x pair; 1 y forward
+// (psi(y+1), U_y(row)); 2 z forward; 3 t forward; 4 t backward (psi(t-1), U_t(t-1)); 5 y backward; 6 z backward.
 // Two bulk copies into `slot`, completion on `bar`.  Called by one lane.
+__host__ __device__ constexpr int stage_mu(int I) { return I == 0 ? 0 : (I == 1 || I == 5) ? 1 : (I == 2 || I == 6) ? 2 : 3; }
+__host__ __device__ constexpr bool stage_forward(int I) { return I >= 1 && I <= 3; }
+
 template <int I, typename Real, int RECON>
 __device__ __forceinline__ void issue_stage(const PipeGeom& pg, const Row& w, const unsigned char* in, const unsigned char* gauge,
                                             unsigned char* slot, uint64_t* bar) {
     using PB = PipeBytes<Real, RECON>;
-    constexpr int MU = (I + 1) / 2;
+    constexpr int MU = stage_mu(I);
+    constexpr bool FWD = stage_forward(I);
     unsigned vp = w.v;
-    if (I == 1) vp = (w.y + 1 == pg.LY) ? w.v - (unsigned)(pg.LY - 1) : w.v + 1u;
-    if (I == 2) vp = (w.y == 0) ? w.v + (unsigned)(pg.LY - 1) : w.v - 1u;
-    if (I == 3) vp = (w.z + 1 == pg.LZ) ? w.v - (unsigned)((pg.LZ - 1) * pg.LY) : w.v + (unsigned)pg.LY;
-    if (I == 4) vp = (w.z == 0) ? w.v + (unsigned)((pg.LZ - 1) * pg.LY) : w.v - (unsigned)pg.LY;
-    if (I == 5) vp = (w.t + 1 == pg.LT) ? w.v - (unsigned)((pg.LT - 1) * pg.LZ * pg.LY) : w.v + (unsigned)(pg.LZ * pg.LY);
-    if (I == 6) vp = (w.t == 0) ? w.v + (unsigned)((pg.LT - 1) * pg.LZ * pg.LY) : w.v - (unsigned)(pg.LZ * pg.LY);
-    const unsigned vl = (I == 0 || (I & 1)) ? w.v : vp;  // forward hops use the row's own link, backward hops the neighbour's
+    if (MU == 1 && FWD) vp = (w.y + 1 == pg.LY) ? w.v - (unsigned)(pg.LY - 1) : w.v + 1u;
+    if (MU == 1 && !FWD) vp = (w.y == 0) ? w.v + (unsigned)(pg.LY - 1) : w.v - 1u;
+    if (MU == 2 && FWD) vp = (w.z + 1 == pg.LZ) ? w.v - (unsigned)((pg.LZ - 1) * pg.LY) : w.v + (unsigned)pg.LY;
+    if (MU == 2 && !FWD) vp = (w.z == 0) ? w.v + (unsigned)((pg.LZ - 1) * pg.LY) : w.v - (unsigned)pg.LY;
+    if (MU == 3 && FWD) vp = (w.t + 1 == pg.LT) ? w.v - (unsigned)((pg.LT - 1) * pg.LZ * pg.LY) : w.v + (unsigned)(pg.LZ * pg.LY);
+    if (MU == 3 && !FWD) vp = (w.t == 0) ? w.v + (unsigned)((pg.LT - 1) * pg.LZ * pg.LY) : w.v - (unsigned)(pg.LZ * pg.LY);
+    const unsigned vl = (I == 0 || FWD) ? w.v : vp;  // forward hops use the row's own link, backward hops the neighbour's
     mbar_arrive_expect_tx(bar, PB::SLOT);
     bulk_g2s(slot, in + (size_t)vp * PB::PSI, PB::PSI, bar);
     bulk_g2s(slot + PB::PSI, gauge + ((size_t)vl * 4u + (unsigned)MU) * PB::LINK, PB::LINK, bar);
@@ -261,15 +190,15 @@ __global__ void __launch_bounds__(NW * 32, MINBLK)
         st.template fetch<1>(psi, u);
         hop_regs<1, -1>(acc, psi, u);
         st.template fetch<2>(psi, u);
-        hop_regs<1, +1>(acc, psi, u);
-        st.template fetch<3>(psi, u);
         hop_regs<2, -1>(acc, psi, u);
-        st.template fetch<4>(psi, u);
-        hop_regs<2, +1>(acc, psi, u);
-        st.template fetch<5>(psi, u);
+        st.template fetch<3>(psi, u);
         hop_regs<3, -1>(acc, psi, u);
-        st.template fetch<6>(psi, u);
+        st.template fetch<4>(psi, u);
         hop_regs<3, +1>(acc, psi, u);
+        st.template fetch<5>(psi, u);
+        hop_regs<1, +1>(acc, psi, u);
+        st.template fetch<6>(psi, u);
+        hop_regs<2, +1>(acc, psi, u);
         SpinorIO<Real, LAYOUT_SOA>::store(out, g.V, st.cur.v * VL + lane, acc);
         st.cur = st.nxt;
         more = st.nxt_valid;

@@ -155,8 +155,7 @@ class Lattice:
 
     def set_kernel(self, kernel):
         B.dslash_set_kernel(self.ctx, {"auto": B.DSLASH_KERNEL_AUTO, "direct": B.DSLASH_KERNEL_DIRECT,
-                                       "tma": B.DSLASH_KERNEL_TMA, "tma_links": B.DSLASH_KERNEL_TMA_LINKS,
-                                       "ring": B.DSLASH_KERNEL_RING, "wpipe": B.DSLASH_KERNEL_WARP_PIPE}.get(kernel, kernel))
+                                       "wpipe": B.DSLASH_KERNEL_WARP_PIPE, "march": B.DSLASH_KERNEL_MARCH}.get(kernel, kernel))
 
     def dslash(self, gauge_canonical, spinor_canonical):
         """Convenience: canonical NumPy in -> canonical NumPy out (one application on the device)."""

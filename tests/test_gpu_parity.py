@@ -129,95 +129,91 @@ def test_x_shuffle_kernel_matches_the_oracle_and_the_loading_kernel_bit_for_bit(
             assert np.array_equal(outs[1], outs[0]), (layout, recon12)
 
 
-# ---------------------------------------------------------------- the TMA-staged kernel (SoA), selected explicitly
-@pytest.mark.parametrize("dims,tile", [
-    ((32, 4, 4, 4), (32, 2, 2, 1)), ((32, 4, 4, 4), (32, 1, 2, 2)), ((32, 4, 4, 4), (32, 4, 1, 1)), ((32, 4, 4, 4), (32, 1, 1, 1)),
-    ((32, 2, 2, 1), (32, 2, 2, 1)),          # a single tile: every neighbour wraps
-    ((32, 6, 5, 3), (32, 4, 1, 1)),          # ragged: partial tiles (inactive warps) in y
-    ((32, 3, 5, 7), (32, 2, 2, 1)), ((64, 4, 2, 6), (32, 2, 1, 2)), ((64, 2, 3, 2), (64, 2, 1, 1)),
-])
+# ---------------------------------------------------------------- the block-cooperative marching kernel (SoA, L_X = 32)
+MARCH_DIMS = [
+    (32, 4, 4, 8),       # 16 rows: 1-row .. 7-row patches depending on the SM count, all wraps
+    (32, 1, 1, 1),       # one row: every neighbour is the row itself (the warp exchanges with itself), t+1 == t-1 == t
+    (32, 2, 1, 3),       # y+1 == y-1, z neighbour == self
+    (32, 5, 3, 2),       # odd extents: a strip of one z plane, t+1 == t-1
+    (32, 2, 2, 5),       # a single 4-row patch when the plan has one segment
+    (32, 16, 12, 9),     # 192 rows
+    (32, 32, 32, 4),     # 1024 rows: the 7/6-row patches of the bench lattice, one wave, four steps
+    (32, 40, 30, 3),     # 1200 rows: more than one wave of 7-row patches on 148 SMs
+]
+
+
+@pytest.mark.parametrize("dims", MARCH_DIMS)
 @pytest.mark.parametrize("precision", ["f64", "f32"])
 @pytest.mark.parametrize("recon12", [False, True])
-@pytest.mark.parametrize("kernel", ["tma", "tma_links"])
-def test_tma_kernel_parity(env, dims, tile, precision, recon12, kernel):
-    g, p, ref, _ = fields_and_ref(env, dims, SEED + 13, precision)
-    with env.device.Lattice(dims, precision, "soa", recon12) as lat:
-        lat.set_tile(tile)
-        lat.set_kernel(kernel)
-        want = env.B.DSLASH_KERNEL_TMA if kernel == "tma" else env.B.DSLASH_KERNEL_TMA_LINKS
-        assert env.B.dslash_get_kernel(lat.ctx) == want
-        assert gpu_vs_ref(env, lat, g, p, ref) <= TOL[precision]
-
-
-def test_tma_kernel_refuses_what_it_cannot_run(env):
-    B = env.B
-    with env.device.Lattice((4, 4, 4, 4), "f64", "aos", False) as lat:  # AoS: no TMA path
-        lat.set_kernel("tma")
-        o, p, g = lat.new_spinor(), lat.new_spinor(), lat.new_gauge()
-        assert B.dslash_apply_status(lat.ctx, o.data_ptr(), p.data_ptr(), g.data_ptr()) == B.DSLASH_ERR_UNSUPPORTED
-        lat.set_kernel("auto")
-        assert B.dslash_apply_status(lat.ctx, o.data_ptr(), p.data_ptr(), g.data_ptr()) == B.DSLASH_OK
-    with env.device.Lattice((16, 4, 4, 4), "f64", "soa", False) as lat:
-        lat.set_tile((16, 4, 2, 1))  # tile rows are not whole 32-site vectors
-        lat.set_kernel("tma")
-        o, p, g = lat.new_spinor(), lat.new_spinor(), lat.new_gauge()
-        assert B.dslash_apply_status(lat.ctx, o.data_ptr(), p.data_ptr(), g.data_ptr()) == B.DSLASH_ERR_UNSUPPORTED
-        with pytest.raises(B.DslashError):
-            B.dslash_set_kernel(lat.ctx, 7)
-
-
-# ---------------------------------------------------------------- the t-marching ring kernel (SoA), selected explicitly
-@pytest.mark.parametrize("dims,tile,chunk", [
-    ((32, 4, 4, 8), (32, 2, 2, 1), 0),        # default chunk (8): one chunk
-    ((32, 4, 4, 8), (32, 2, 2, 1), 3),        # chunks of 3, 3, 2 steps: ring wrap-around, parity flips, short last chunk
-    ((32, 4, 4, 7), (32, 4, 1, 1), 1),        # one step per block: prologue + a single step
-    ((32, 4, 4, 7), (32, 1, 4, 1), 7),        # the whole time extent in one block: forward hop of the last step wraps to t = 0
-    ((32, 2, 2, 5), (32, 2, 2, 1), 2),        # a single spatial tile: every y/z neighbour is in the tile or wraps through global
-    ((32, 8, 4, 4), (32, 4, 2, 1), 4),        # 8 warps per block
-    ((32, 6, 4, 4), (32, 2, 1, 1), 2),        # L_Y = 6 tiled by 2
-    ((64, 4, 2, 6), (32, 2, 1, 1), 4),        # L_X = 64: x hops loaded (no whole row in a warp), two x tiles
-    ((32, 2, 6, 3), (32, 1, 1, 1), 2),        # one warp per block, no in-tile neighbours
-])
-@pytest.mark.parametrize("precision", ["f64", "f32"])
-@pytest.mark.parametrize("recon12", [False, True])
-def test_ring_kernel_matches_the_oracle_and_the_direct_kernel_bit_for_bit(env, dims, tile, chunk, precision, recon12):
+def test_marching_kernel_matches_the_oracle_and_the_direct_kernel_bit_for_bit(env, dims, precision, recon12):
     B = env.B
     g, p, ref, _ = fields_and_ref(env, dims, SEED + 19, precision)
     with env.device.Lattice(dims, precision, "soa", recon12) as lat:
         gi, pi, o = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
-        lat.set_tile(tile)
         lat.apply(o, pi, gi)
         direct = lat.download_spinor(o)
-        lat.set_kernel("ring")
-        B.dslash_set_option(lat.ctx, B.DSLASH_OPT_T_CHUNK, chunk)
-        assert B.dslash_get_kernel(lat.ctx) == B.DSLASH_KERNEL_RING and B.dslash_get_option(lat.ctx, B.DSLASH_OPT_T_CHUNK) == chunk
-        o.zero_()
+        lat.set_kernel("march")
+        assert B.dslash_get_kernel(lat.ctx) == B.DSLASH_KERNEL_MARCH
+        o.fill_(0x7f)  # a site the kernel forgot to store would stay garbage
+        n0 = B.dslash_launch_count(lat.ctx)
         lat.apply(o, pi, gi)
+        assert B.dslash_launch_count(lat.ctx) == n0 + 1
         got = lat.download_spinor(o)
         assert env.checks.parity_error(got, ref) <= TOL[precision]
-        assert np.array_equal(got, direct)  # same arithmetic in the same order
-        # a time range (multi-GPU slab interior) with the ring kernel: only its slices are written
-        if dims[3] >= 4:
-            B.dslash_set_time_range(lat.ctx, 1, dims[3] - 1)
+        assert np.array_equal(got, direct)  # same arithmetic, same order of the sum
+        # a second application on the same context gives the same bits (no state left behind by the first)
+        o.fill_(0x7f)
+        lat.apply(o, pi, gi)
+        assert np.array_equal(lat.download_spinor(o), direct)
+        # time ranges (multi-GPU slab interior, single slices at the ends): only their slices are written
+        lt = dims[3]
+        for t0, t1 in [(1, lt - 1), (0, 1), (lt - 1, lt), (lt // 2, lt)]:
+            if not (0 <= t0 < t1 <= lt):
+                continue
+            B.dslash_set_time_range(lat.ctx, t0, t1)
             o.zero_()
             lat.apply(o, pi, gi)
             part = lat.download_spinor(o)
-            assert np.array_equal(part[1:-1], direct[1:-1]) and not part[0].any() and not part[-1].any()
+            assert np.array_equal(part[t0:t1], direct[t0:t1]), (t0, t1)
+            assert not part[:t0].any() and not part[t1:].any(), (t0, t1)
 
 
-def test_ring_kernel_refuses_what_it_cannot_run(env):
+def test_marching_kernel_refuses_what_it_cannot_run(env):
     B = env.B
-    for dims, layout, tile in [((32, 4, 4, 4), "aos", (32, 2, 2, 1)),   # AoS rows are not contiguous vectors
-                               ((16, 4, 4, 4), "soa", (16, 4, 2, 1)),   # rows shorter than a 32-site vector
-                               ((32, 6, 4, 4), "soa", (32, 4, 1, 1)),   # tile does not divide L_Y
-                               ((32, 4, 4, 4), "soa", (32, 2, 1, 2))]:  # tile with a t extent
+    for dims, layout in [((32, 4, 4, 4), "aos"),   # AoS rows are not contiguous vectors
+                         ((16, 4, 4, 4), "soa"),   # two x rows per 32-site vector
+                         ((64, 4, 4, 4), "soa")]:  # an x row is two vectors
         with env.device.Lattice(dims, "f64", layout, False) as lat:
-            lat.set_tile(tile)
-            lat.set_kernel("ring")
+            lat.set_kernel("march")
             o, p, g = lat.new_spinor(), lat.new_spinor(), lat.new_gauge()
-            assert B.dslash_apply_status(lat.ctx, o.data_ptr(), p.data_ptr(), g.data_ptr()) == B.DSLASH_ERR_UNSUPPORTED, (dims, tile)
+            assert B.dslash_apply_status(lat.ctx, o.data_ptr(), p.data_ptr(), g.data_ptr()) == B.DSLASH_ERR_UNSUPPORTED, dims
+            lat.set_kernel("auto")
+            assert B.dslash_apply_status(lat.ctx, o.data_ptr(), p.data_ptr(), g.data_ptr()) == B.DSLASH_OK
             with pytest.raises(B.DslashError):
-                B.dslash_set_option(lat.ctx, B.DSLASH_OPT_T_CHUNK, dims[3] + 1)
+                B.dslash_set_kernel(lat.ctx, 2)  # a kernel of round 1 that no longer exists
+
+
+@pytest.mark.parametrize("kernel", ["march", "wpipe"])
+def test_staged_kernels_on_a_non_blocking_stream_and_fresh_context(env, kernel):
+    """The staged kernels keep device-side state (row counters / block plan).  A fresh context whose FIRST launch runs on a
+    cudaStreamNonBlocking stream (every torch.cuda.Stream is one) must be correct: nothing may depend on the legacy default
+    stream having run first (round-1 advisor finding on the counter memset)."""
+    B, torch = env.B, env.torch
+    dims = (32, 8, 6, 5)
+    g, p, ref, _ = fields_and_ref(env, dims, SEED + 29, "f64")
+    for attempt in range(3):
+        with env.device.Lattice(dims, "f64", "soa", False) as lat:
+            gi, pi = lat.upload_gauge(g), lat.upload_spinor(p)
+            torch.cuda.synchronize()
+            st = torch.cuda.Stream()
+            lat.set_kernel(kernel)
+            o = lat.new_spinor()
+            o.fill_(0x7f)
+            torch.cuda.synchronize()
+            for _ in range(4):  # back-to-back launches on the side stream
+                B.dslash_apply(lat.ctx, o.data_ptr(), pi.data_ptr(), gi.data_ptr(), st.cuda_stream)
+            st.synchronize()
+            assert env.checks.parity_error(lat.download_spinor(o), ref) <= TOL["f64"], attempt
 
 
 # ---------------------------------------------------------------- the warp-pipelined kernel (SoA, L_X = 32), selected explicitly
@@ -513,12 +509,40 @@ def test_time_range_only_touches_its_slices(env):
 
 
 # ---------------------------------------------------------------- config 3: 32^3 x 64 FP64, 18- and 12-real links
+# WHOLE lattice against the oracle, for every kernel dslash_tune() can return, in the launch configurations it tries
+# (the oracle applies the 2 M-site lattice in well under a second per core-second on the box).
+TUNABLE_KERNELS = [("direct", 0, 0), ("march", 0, 0), ("wpipe", 2, 4), ("wpipe", 3, 1), ("wpipe", 2, 1)]
+
+
 @pytest.mark.parametrize("recon12", [False, True])
 def test_config3_32x32x32x64_fp64(env, recon12):
+    B = env.B
     dims = (32, 32, 32, 64)
-    g, p, ref, sites = fields_and_ref(env, dims, SEED + 3, "f64", full=False, nsample=8192)
+    g, p, ref, _ = fields_and_ref(env, dims, SEED + 3, "f64", full=True)
     with env.device.Lattice(dims, "f64", "soa", recon12) as lat:
-        assert gpu_vs_ref(env, lat, g, p, ref, sites) <= TOL["f64"]
+        gi, pi, o = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
+        first = None
+        for kernel, slots, warps in TUNABLE_KERNELS:
+            lat.set_kernel(kernel)
+            if kernel == "wpipe":
+                B.dslash_set_option(lat.ctx, B.DSLASH_OPT_PIPE_SLOTS, slots)
+                B.dslash_set_option(lat.ctx, B.DSLASH_OPT_PIPE_WARPS, warps)
+            o.fill_(0x7f)
+            lat.apply(o, pi, gi)
+            got = lat.download_spinor(o)
+            assert env.checks.parity_error(got, ref) <= TOL["f64"], (kernel, slots, warps)
+            if first is None:
+                first = got
+            else:
+                assert np.array_equal(got, first), (kernel, slots, warps)  # every tuned kernel gives the same bits
+        # and whatever dslash_tune() picks, in both regimes, on the buffer it leaves behind
+        for mode in (B.DSLASH_TUNE_BURST, B.DSLASH_TUNE_SUSTAINED):
+            B.dslash_set_option(lat.ctx, B.DSLASH_OPT_TUNE_MODE, mode)
+            o.fill_(0x7f)
+            chosen, ms = B.dslash_tune(lat.ctx, o.data_ptr(), pi.data_ptr(), gi.data_ptr(), lat.stream())
+            assert chosen in (B.DSLASH_KERNEL_DIRECT, B.DSLASH_KERNEL_MARCH, B.DSLASH_KERNEL_WARP_PIPE) and ms > 0
+            assert np.array_equal(lat.download_spinor(o), first), (mode, chosen)
+    _FIELD_CACHE.clear()
 
 
 def test_config3_full_size_properties(env):
@@ -537,11 +561,21 @@ def test_config3_full_size_properties(env):
 
 # ---------------------------------------------------------------- config 4: 48^3 x 96 FP32 vs the FP64 oracle
 def test_config4_48x48x48x96_fp32(env):
+    """WHOLE lattice (10.6 M sites) against the fp64 oracle; dslash_tune() first, so the kernel checked is the one bench.py times."""
+    B = env.B
     dims = (48, 48, 48, 96)
-    g, p, ref, sites = fields_and_ref(env, dims, SEED + 4, "f32", full=False, nsample=8192)
+    g, p, ref, _ = fields_and_ref(env, dims, SEED + 4, "f32", full=True)
     with env.device.Lattice(dims, "f32", "soa", False) as lat:
-        assert gpu_vs_ref(env, lat, g, p, ref, sites) <= TOL["f32"]
-    _FIELD_CACHE.clear()
+        gi, pi, o = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
+        o.fill_(0x7f)
+        lat.apply(o, pi, gi)
+        direct = lat.download_spinor(o)
+        assert env.checks.parity_error(direct, ref) <= TOL["f32"]
+        del ref
+        _FIELD_CACHE.clear()
+        o.fill_(0x7f)
+        chosen, _ = B.dslash_tune(lat.ctx, o.data_ptr(), pi.data_ptr(), gi.data_ptr(), lat.stream())
+        assert np.array_equal(lat.download_spinor(o), direct), chosen
 
 
 # ---------------------------------------------------------------- invariants evaluated on the GPU itself
