@@ -226,6 +226,10 @@ def run_cuda(args, cfg):
                 lat.set_kernel(args.kernel)
             if args.x_shuffle is not None:
                 B.dslash_set_option(lat.ctx, B.DSLASH_OPT_X_SHUFFLE, args.x_shuffle)
+            if args.l2_policy is not None:
+                B.dslash_set_option(lat.ctx, B.DSLASH_OPT_L2_POLICY, args.l2_policy)
+            if args.march_lead is not None:
+                B.dslash_set_option(lat.ctx, B.DSLASH_OPT_MARCH_LEAD, args.march_lead)
             if args.pipe_slots is not None:
                 B.dslash_set_option(lat.ctx, B.DSLASH_OPT_PIPE_SLOTS, args.pipe_slots)
             if args.pipe_warps is not None:
@@ -912,6 +916,8 @@ def main():
     ap.add_argument("--tile", type=int, nargs=4, default=None, help="tile of the tuned kernel (x y z t)")
     ap.add_argument("--occupancy", type=int, default=None, help="DSLASH_OPT_OCCUPANCY override")
     ap.add_argument("--kernel", choices=["auto", "direct", "wpipe", "march"], default=None)
+    ap.add_argument("--l2-policy", type=int, default=None, help="DSLASH_OPT_L2_POLICY bits")
+    ap.add_argument("--march-lead", type=int, default=None, help="DSLASH_OPT_MARCH_LEAD")
     ap.add_argument("--no-tune", action="store_true", help="skip dslash_tune (keep the library's static default kernel)")
     ap.add_argument("--pipe-slots", type=int, default=None, help="DSLASH_OPT_PIPE_SLOTS override (wpipe kernel)")
     ap.add_argument("--pipe-warps", type=int, default=None, help="DSLASH_OPT_PIPE_WARPS override (wpipe kernel)")

@@ -131,6 +131,8 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
                                          then the z blocks (a divisor of L_Z; 0 = L_Z): shortens the L2 reuse distance of the t hops */
 #define DSLASH_OPT_TUNE_MODE 10       /* what dslash_tune() optimises: DSLASH_TUNE_BURST (default; the first ~35 ms after idle, board at its
                                          boost clock) or DSLASH_TUNE_SUSTAINED (continuous load, board at its power-capped clock) */
+#define DSLASH_OPT_MARCH_LEAD 11      /* marching kernel: steps a block may run ahead of the slowest block of its chunk, 0..16
+                                         (0 = unbounded).  Blocks that stay close share their halo rows through L2 */
 #define DSLASH_TUNE_BURST 0
 #define DSLASH_TUNE_SUSTAINED 1
 
@@ -267,6 +269,15 @@ DSLASH_API int dslash_get_kernel(const dslash_ctx *ctx, int *kernel);
  * Errors: NULL, DIMS, UNSUPPORTED (L_X != 32, bad range, wave < 1, capacity too small).
  */
 DSLASH_API int dslash_march_plan(const int dims[4], int t_begin, int t_end, int wave, int *ints, size_t capacity_ints, int *nblocks);
+
+/*
+ * Where and how fast the blocks of the LAST DSLASH_KERNEL_MARCH launch of this ctx ran (a measurement aid: the kernel's work is
+ * split statically, one block per SM, so the slowest SM sets the time).  stats (host, may be NULL to query *nblocks)
+ * receives per block {SM id, SM clock cycles from block start to the last store of its first compute warp, low word of
+ * %globaltimer (ns) when that warp began the middle step of its march}; capacity = its size in unsigned (>= 3 * *nblocks).
+ * SYNCHRONISES the device.  Errors: NULL, UNSUPPORTED (capacity), CUDA.
+ */
+DSLASH_API int dslash_march_stats(dslash_ctx *ctx, unsigned *stats, size_t capacity, int *nblocks);
 
 /*
  * Pick the kernel by measurement (the Advisor's own method, applied to the library's kernels): every kernel

@@ -22,8 +22,9 @@ DSLASH_VARIANT_TUNED = 0
 DSLASH_MAP_MINIMAL, DSLASH_MAP_TOFROM = 0, 1
 DSLASH_KERNEL_AUTO, DSLASH_KERNEL_DIRECT = 0, 1
 DSLASH_KERNEL_WARP_PIPE, DSLASH_KERNEL_MARCH = 5, 6
-MARCH_NW, MARCH_NWS, MARCH_BLOCK_INTS = 7, 10, 4 + 7 * 9  # block plan of dslash_march_plan()
-DSLASH_OPT_PIPE_SLOTS, DSLASH_OPT_PIPE_WARPS, DSLASH_OPT_PIPE_ZBLOCK, DSLASH_OPT_TUNE_MODE = 7, 8, 9, 10
+MARCH_NW, MARCH_NWS, MARCH_WARP_INTS = 7, 9, 9
+MARCH_BLOCK_INTS = 4 + MARCH_NW * MARCH_WARP_INTS  # block plan of dslash_march_plan()
+DSLASH_OPT_PIPE_SLOTS, DSLASH_OPT_PIPE_WARPS, DSLASH_OPT_PIPE_ZBLOCK, DSLASH_OPT_TUNE_MODE, DSLASH_OPT_MARCH_LEAD = 7, 8, 9, 10, 11
 DSLASH_TUNE_BURST, DSLASH_TUNE_SUSTAINED = 0, 1
 DSLASH_OPT_OCCUPANCY, DSLASH_OPT_L2_POLICY, DSLASH_OPT_L1_CARVEOUT, DSLASH_OPT_X_SHUFFLE = 2, 3, 4, 5
 DSLASH_SCHED_STATIC, DSLASH_SCHED_DYNAMIC, DSLASH_SCHED_GUIDED = 0, 1, 2
@@ -75,6 +76,7 @@ SIGNATURES = {
     "dslash_get_time_range": (ctypes.c_int, [_vp, _c_int_p, _c_int_p]),
     "dslash_set_kernel": (ctypes.c_int, [_vp, ctypes.c_int]),
     "dslash_get_kernel": (ctypes.c_int, [_vp, _c_int_p]),
+    "dslash_march_stats": (ctypes.c_int, [_vp, ctypes.POINTER(ctypes.c_uint), ctypes.c_size_t, _c_int_p]),
     "dslash_march_plan": (ctypes.c_int, [_c_int_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, _c_int_p, ctypes.c_size_t, _c_int_p]),
     "dslash_probe_launch": (ctypes.c_int, [ctypes.c_int, _vp, _vp, ctypes.c_size_t, ctypes.c_int, _vp]),
     "dslash_tune": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _c_int_p, ctypes.POINTER(ctypes.c_float)]),
@@ -359,10 +361,21 @@ def dslash_march_plan(dims, t_begin: int, t_end: int, wave: int):
         v = buf[b * MARCH_BLOCK_INTS:(b + 1) * MARCH_BLOCK_INTS]
         warps = []
         for w in range(MARCH_NW):
-            q = v[4 + 9 * w:4 + 9 * (w + 1)]
+            q = v[4 + MARCH_WARP_INTS * w:4 + MARCH_WARP_INTS * (w + 1)]
             warps.append(dict(row=q[0], fwd=(q[1], q[2]), wr=(q[3], q[4]), rd=(q[5], q[6]), bwd=(q[7], q[8])))
         blocks.append(dict(t0=v[0], nt=v[1], nact=v[2], warps=warps))
     return blocks
+
+
+def dslash_march_stats(ctx):
+    """[(sm_id, cycles, ns_at_mid_march)] per block of the last DSLASH_KERNEL_MARCH launch of this ctx (synchronises)."""
+    nb = ctypes.c_int()
+    _check(_lib.dslash_march_stats(_ptr(ctx), None, 0, ctypes.byref(nb)), "dslash_march_stats")
+    if nb.value == 0:
+        return []
+    buf = (ctypes.c_uint * (3 * nb.value))()
+    _check(_lib.dslash_march_stats(_ptr(ctx), buf, 3 * nb.value, ctypes.byref(nb)), "dslash_march_stats")
+    return [(buf[3 * i], buf[3 * i + 1], buf[3 * i + 2]) for i in range(nb.value)]
 
 
 def dslash_set_option(ctx, option: int, value: int) -> None:

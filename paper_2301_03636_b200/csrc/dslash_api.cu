@@ -45,6 +45,7 @@ struct dslash_ctx {
     // ensure_kernel_resources(), never by dslash_apply)
     void* march_plan;
     int march_blocks, march_t0, march_t1;
+    unsigned march_epoch;  // launches on the current plan (its progress counters accumulate)
 };
 
 static int cuda_fail(dslash_ctx* c, cudaError_t e) {
@@ -206,6 +207,7 @@ static int ensure_kernel_resources(dslash_ctx* c, int kernel) {
         }
         c->march_t0 = c->tg.t_begin;
         c->march_t1 = c->tg.t_end;
+        c->march_epoch = 0;
     }
     return DSLASH_OK;
 }
@@ -274,6 +276,8 @@ int dslash_create(dslash_ctx** ctx, const int dims[4], int precision, int layout
     c->march_plan = nullptr;
     c->march_blocks = 0;
     c->march_t0 = c->march_t1 = -1;
+    c->march_epoch = 0;
+    c->cfg.march_lead = 0;
     c->tune_mode = DSLASH_TUNE_BURST;
     c->cfg.x_shuffle = precision == DSLASH_FP64 ? 1 : 0;  // measured: -1.3 % (burst) / -2 % (sustained) in fp64, +0.8 % in fp32
     c->launches = 0;
@@ -357,7 +361,7 @@ int dslash_apply(dslash_ctx* c, void* out, const void* in, const void* gauge, ds
         if (k == DSLASH_KERNEL_MARCH && (!c->march_plan || c->march_t0 != c->tg.t_begin || c->march_t1 != c->tg.t_end))
             return DSLASH_ERR_UNSUPPORTED;
         e = (k == DSLASH_KERNEL_WARP_PIPE) ? launch_wpipe(c->precision, c->layout_base, c->recon, a, c->tg, c->cfg)
-            : (k == DSLASH_KERNEL_MARCH)   ? launch_march(c->precision, c->layout_base, c->recon, a, c->march_plan, c->march_blocks, c->cfg)
+            : (k == DSLASH_KERNEL_MARCH)   ? launch_march(c->precision, c->layout_base, c->recon, a, c->march_plan, c->march_blocks, c->cfg, ++c->march_epoch)
                                            : launch_tuned(c->precision, c->layout_base, c->recon, a, c->tg, c->cfg);
     } else if (!full_time_range(c)) {
         return DSLASH_ERR_UNSUPPORTED;  // the variant kernels always sweep the whole lattice
@@ -366,7 +370,10 @@ int dslash_apply(dslash_ctx* c, void* out, const void* in, const void* gauge, ds
                                c->omp_team_size);
     } else
         e = launch_variant(c->precision, c->layout_base, c->recon, a, c->var_depth, c->var_tpb, c->var_spt);
-    if (e != cudaSuccess) return cuda_fail(c, e);
+    if (e != cudaSuccess) {
+        if (c->var_depth == DSLASH_VARIANT_TUNED && resolve_kernel(c) == DSLASH_KERNEL_MARCH) --c->march_epoch;  // nothing was counted
+        return cuda_fail(c, e);
+    }
     c->launches += 1;
     return DSLASH_OK;
 }
@@ -748,6 +755,10 @@ int dslash_set_option(dslash_ctx* c, int option, int value) {
             if (value != 0 && value != 1 && value != 2 && value != 4) return DSLASH_ERR_UNSUPPORTED;
             c->cfg.pipe_warps = value;
             return DSLASH_OK;
+        case DSLASH_OPT_MARCH_LEAD:
+            if (value < 0 || value > 16) return DSLASH_ERR_UNSUPPORTED;
+            c->cfg.march_lead = value;
+            return DSLASH_OK;
         default:
             return DSLASH_ERR_UNSUPPORTED;
     }
@@ -762,6 +773,7 @@ int dslash_get_option(const dslash_ctx* c, int option, int* value) {
         case DSLASH_OPT_X_SHUFFLE: *value = c->cfg.x_shuffle; return DSLASH_OK;
         case DSLASH_OPT_PIPE_SLOTS: *value = c->cfg.pipe_slots; return DSLASH_OK;
         case DSLASH_OPT_PIPE_WARPS: *value = c->cfg.pipe_warps; return DSLASH_OK;
+        case DSLASH_OPT_MARCH_LEAD: *value = c->cfg.march_lead; return DSLASH_OK;
         case DSLASH_OPT_PIPE_ZBLOCK: *value = c->cfg.pipe_zblock; return DSLASH_OK;
         case DSLASH_OPT_TUNE_MODE: *value = c->tune_mode; return DSLASH_OK;
         default: return DSLASH_ERR_UNSUPPORTED;
@@ -931,6 +943,18 @@ int dslash_apply_host(dslash_ctx* c, void* out_host, const void* in_host, const 
     if (h2d_bytes) *h2d_bytes = h2d;
     if (d2h_bytes) *d2h_bytes = d2h;
     return DSLASH_OK;
+}
+
+int dslash_march_stats(dslash_ctx* c, unsigned* stats, size_t capacity, int* nblocks) {
+    if (!c || !nblocks) return DSLASH_ERR_NULL;
+    *nblocks = c->march_plan ? c->march_blocks : 0;
+    if (!stats || !c->march_plan) return DSLASH_OK;
+    if (capacity < 3u * (size_t)c->march_blocks) return DSLASH_ERR_UNSUPPORTED;
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e == cudaSuccess)
+        e = cudaMemcpy(stats, static_cast<const MarchBlockPlan*>(c->march_plan) + c->march_blocks,
+                       3u * (size_t)c->march_blocks * sizeof(unsigned), cudaMemcpyDeviceToHost);
+    return e == cudaSuccess ? DSLASH_OK : cuda_fail(c, e);
 }
 
 long long dslash_launch_count(const dslash_ctx* c) { return c ? c->launches : 0; }

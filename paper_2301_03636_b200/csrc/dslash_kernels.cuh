@@ -40,6 +40,7 @@ struct TunedConfig {
     int pipe_warps;        // warp-pipelined kernel: warps per block (1, 2 or 4; 0: default 4)
     unsigned* pipe_counters;  // warp-pipelined kernel: {next row, finished warps} of this launch (device memory, zero between launches)
     int pipe_zblock;       // warp-pipelined kernel: z planes per block of the row order (0: L_Z, i.e. plain lexicographic)
+    int march_lead;        // marching kernel: steps a block may run ahead of the slowest block of its chunk (0: unbounded)
     int x_shuffle;         // 1: exchange the x hops inside the warp when the tile allows it (fp64 default), 0: always load them
 };
 bool x_shuffle_eligible(const Geom& g, const TileGeom& tg);
@@ -55,8 +56,8 @@ cudaError_t launch_wpipe(int precision, int layout_base, int recon, const Launch
 
 // block-cooperative t-marching kernel (dslash_march.cu): a block owns up to MARCH_NW x rows that are neighbours in the (y,z)
 // plane and marches through a chunk of time slices.  The decomposition is a host-built plan in device memory.
-constexpr int MARCH_NW = 7;    // warps (= rows) per block: what 227 KB of shared memory hold in fp64
-constexpr int MARCH_NWS = 10;  // exchange buffers per block (>= the 8 neighbour pairs 7 cells of a grid can form)
+constexpr int MARCH_NW = 7;    // compute warps (= rows) per block: what 227 KB of shared memory hold in fp64; four more warps feed them
+constexpr int MARCH_NWS = 9;   // exchange buffers per block (>= the 8 neighbour pairs 7 cells of a grid can form)
 struct MarchWarpPlan {
     int row;     // the warp's row = vector index inside a time slice, y + L_Y * z (L_X == 32); -1: idle warp
     int fwd[2];  // spinor source of the forward y (0) / z (1) hop: >= 0 warp of this block whose ring row it is; < 0: -(row' + 1),
@@ -68,13 +69,15 @@ struct MarchWarpPlan {
 struct MarchBlockPlan {
     int t0, nt;  // first time slice and number of steps
     int nact;    // active warps
-    int pad;
+    int chunk;   // which chunk of the time range (blocks of one chunk march together)
     MarchWarpPlan w[MARCH_NW];
 };
+constexpr int MARCH_MAX_CHUNKS = 64;
 bool march_eligible(int layout_base, const Geom& g);
 cudaError_t march_plan_create(const Geom& g, int t_begin, int t_end, int device, void** d_plan, int* nblocks);
+// epoch = number of this launch on this plan (1, 2, ...): the progress counters behind the plan accumulate across launches
 cudaError_t launch_march(int precision, int layout_base, int recon, const LaunchArgs& a, const void* d_plan, int nblocks,
-                         const TunedConfig& cfg);
+                         const TunedConfig& cfg, unsigned epoch);
 
 // Operators around Dslash (dslash_ops.cu): op 0 D, 1 D^dagger, 2 M = (4+m) - D/2, 3 M^dagger; solver vector kernels.
 cudaError_t launch_op(int precision, int layout_base, int recon, const LaunchArgs& a, const TileGeom& tg, int op, double mass);
