@@ -14,10 +14,13 @@ A "step" is one application of D (one dslash_apply = one kernel launch covering 
 steps a1-a7) to one seeded synthetic lattice that is already resident in HBM in the native layout.  Before the timed
 region the library picks its kernel by measurement (dslash_tune), then the device idles 1 s.
 `value` = 1320 flop/site * sites of all ranks / max-over-ranks device time (CUDA events on the
-launching stream).  `e2e` = the same through dslash_apply_host with pinned HOST buffers (H2D copy of
-gauge and spinor, pack, apply, unpack, D2H copy of the result inside the timed region).
-Multi-GPU: the path has no exchange step in this build ("replicas only"): under torchrun
-every rank runs its own lattice; value is the sum (weak scaling).
+launching stream) of the K timed steps; `repeats` = the same region four more times (median, min); `sustained` = the same
+after ~0.6 s of continuous load, when the board runs against its power cap (what a solver sees); `parity` = the buffer the
+timed region wrote, compared with the oracle on the whole lattice (outside the timed region).
+`e2e` = the same metric through dslash_apply_host with pinned HOST buffers (H2D copy of gauge and spinor, pack, apply, unpack,
+D2H copy of the result inside the timed region).
+Multi-GPU: default = replicas (every rank its own lattice, weak scaling, no collective: north_star keeps the path on one
+GPU); --decomposition slab = one lattice cut along t with a halo exchange per application (strong scaling).
 """
 import argparse
 import json
@@ -47,13 +50,12 @@ CONFIGS = {
     "5": dict(dims=(24, 24, 24, 24), precision="f64", recon12=False, name="configs[4]: 24^4 FP64 (sweep lattice)"),
 }
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` capture (profiles/); None until captured for that workload.
-NCU_TRAFFIC_BYTES = {
-    # profiles/r01_ncu_tuned_kernel.txt, capture r01c: 1.6424 GB read + 0.3903 GB written (mean of 2 launches)
-    "32x32x32x64_f64_soa_r18": 2032698000,
-    # profiles/r01f_wpipe.md: the warp-pipelined kernel (rows from the counter), 1.660823 GB read + 0.391139 GB written
-    "32x32x32x64_f64_soa_r18_wpipe": 2051962000,
+# dram__bytes_read.sum + dram__bytes_write.sum per launch and the FP64-pipe utilisation of the dominant kernel, copied from
+# the committed `ncu --set full` captures (profiles/); None until captured for that workload and kernel.
+NCU_FIGURES = {
+    "32x32x32x64_f64_soa_r18_direct": dict(traffic=2032698000, fp64_pipe_pct=31.0, source="profiles/r01_ncu_tuned_kernel.txt"),
+    "32x32x32x64_f64_soa_r18_wpipe": dict(traffic=2051962000, fp64_pipe_pct=None, source="profiles/r01f_wpipe.md"),
+    "32x32x32x64_f64_soa_r18_march": dict(traffic=1995707392, fp64_pipe_pct=30.4, source="profiles/r02_march.md"),
 }
 KERNEL_NAMES = {"direct": "dslash_tuned_kernel", "wpipe": "dslash_wpipe_kernel", "march": "dslash_march_kernel"}
 
@@ -131,26 +133,28 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------ CPU oracle legs
-def oracle_timing(dims, g64, p64, nsites, steps, warmup):
-    """Time the oracle as it stands on `nsites` seeded sample sites per step; returns (GFLOP/s, s/step, cores)."""
+def oracle_timing(dims, g64, p64, nsites, steps, warmup, nthreads=0):
+    """Time the oracle as it stands on `nsites` seeded sample sites per step (the whole lattice if nsites >= V);
+    returns (GFLOP/s, s/step, threads, sites, last output)."""
     import oracle
     from paper_2301_03636_b200 import inputs
     v = inputs.volume(dims)
-    cores = oracle.max_threads()
+    cores = oracle.max_threads() if nthreads <= 0 else nthreads
     if nsites >= v:
-        fn = lambda: oracle.dslash(p64, g64, dims)
+        fn = lambda: oracle.dslash(p64, g64, dims, nthreads)
         n = v
     else:
         sites = np.sort(np.random.default_rng([SEED, 77]).choice(v, size=nsites, replace=False)).astype(np.int64)
-        fn = lambda: oracle.dslash_sites(p64, g64, dims, sites)
+        fn = lambda: oracle.dslash_sites(p64, g64, dims, sites, nthreads)
         n = nsites
+    out = None
     for _ in range(warmup):
-        fn()
+        out = fn()
     t0 = time.perf_counter()
     for _ in range(steps):
-        fn()
+        out = fn()
     dt = (time.perf_counter() - t0) / max(steps, 1)
-    return FLOP_PER_SITE * n / dt / 1e9, dt, cores, n
+    return FLOP_PER_SITE * n / dt / 1e9, dt, cores, n, out
 
 
 def run_reference(args, cfg):
@@ -162,15 +166,17 @@ def run_reference(args, cfg):
     dims = cfg["dims"]
     g, p = inputs.fields(dims, SEED + 3, cfg["precision"], check=False)
     g64, p64 = inputs.promote(g), inputs.promote(p)
-    nsites = min(inputs.volume(dims), args.ref_sites)
-    gflops, dt, cores, n = oracle_timing(dims, g64, p64, nsites, args.steps, args.warmup)
-    sample = "%d seeded sample sites of the %s lattice per step (oracle_dslash_sites)" % (n, "x".join(map(str, dims)))
+    v = inputs.volume(dims)
+    nsites = v if args.ref_sites <= 0 else min(v, args.ref_sites)
+    gflops, dt, cores, n, _ = oracle_timing(dims, g64, p64, nsites, args.steps, args.warmup)
+    sample = ("the whole %s lattice per step (oracle_dslash)" % "x".join(map(str, dims)) if n == v else
+              "%d seeded sample sites of the %s lattice per step (oracle_dslash_sites)" % (n, "x".join(map(str, dims))))
     line = {
         "impl": "reference", "metric": METRIC, "value": gflops, "unit": "GFLOP/s", "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": cfg["name"], "dims": list(dims), "sample": sample},
-        "cpu_baseline": {"value": gflops, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "config": {"workload": cfg["name"], "dims": list(dims), "sample": sample, "sites_per_step": int(n)},
+        "cpu_baseline": {"value": gflops, "unit": "GFLOP/s", "cores": cores, "nproc": os.cpu_count(), "kind": "oracle", "sample": sample},
         "e2e": {"value": gflops, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -197,10 +203,29 @@ def time_applies(torch, lat, out, inp, gauge, steps, warmup, group, sampler_inde
     return ms, cs.summary()
 
 
+def lattice_options(B, lat, args):
+    if args.tile:
+        lat.set_tile(args.tile)
+    if args.occupancy is not None:
+        B.dslash_set_option(lat.ctx, B.DSLASH_OPT_OCCUPANCY, args.occupancy)
+    if args.kernel:
+        lat.set_kernel(args.kernel)
+    if args.x_shuffle is not None:
+        B.dslash_set_option(lat.ctx, B.DSLASH_OPT_X_SHUFFLE, args.x_shuffle)
+    if args.l2_policy is not None:
+        B.dslash_set_option(lat.ctx, B.DSLASH_OPT_L2_POLICY, args.l2_policy)
+    if args.march_lead is not None:
+        B.dslash_set_option(lat.ctx, B.DSLASH_OPT_MARCH_LEAD, args.march_lead)
+    if args.pipe_slots is not None:
+        B.dslash_set_option(lat.ctx, B.DSLASH_OPT_PIPE_SLOTS, args.pipe_slots)
+    if args.pipe_warps is not None:
+        B.dslash_set_option(lat.ctx, B.DSLASH_OPT_PIPE_WARPS, args.pipe_warps)
+
+
 def run_cuda(args, cfg):
     import torch
     from paper_2301_03636_b200 import binding as B
-    from paper_2301_03636_b200 import device, inputs, replicas
+    from paper_2301_03636_b200 import checks, device, inputs, replicas
 
     rank, world, local = replicas.env_ranks()
     if not torch.cuda.is_available():
@@ -214,26 +239,12 @@ def run_cuda(args, cfg):
     results = {}
     clocks = None
     launches = 0
+    timed_out = None  # the buffer the main timed region wrote, canonical layout, host
     for tag, recon12 in (("main", cfg["recon12"]), ("other_recon", not cfg["recon12"])):
         if tag == "other_recon" and not args.both_recon:
             continue
         with device.Lattice(dims, prec, args.layout, recon12, device="cuda:%d" % local) as lat:
-            if args.tile:
-                lat.set_tile(args.tile)
-            if args.occupancy is not None:
-                B.dslash_set_option(lat.ctx, B.DSLASH_OPT_OCCUPANCY, args.occupancy)
-            if args.kernel:
-                lat.set_kernel(args.kernel)
-            if args.x_shuffle is not None:
-                B.dslash_set_option(lat.ctx, B.DSLASH_OPT_X_SHUFFLE, args.x_shuffle)
-            if args.l2_policy is not None:
-                B.dslash_set_option(lat.ctx, B.DSLASH_OPT_L2_POLICY, args.l2_policy)
-            if args.march_lead is not None:
-                B.dslash_set_option(lat.ctx, B.DSLASH_OPT_MARCH_LEAD, args.march_lead)
-            if args.pipe_slots is not None:
-                B.dslash_set_option(lat.ctx, B.DSLASH_OPT_PIPE_SLOTS, args.pipe_slots)
-            if args.pipe_warps is not None:
-                B.dslash_set_option(lat.ctx, B.DSLASH_OPT_PIPE_WARPS, args.pipe_warps)
+            lattice_options(B, lat, args)
             gd, pd, od = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
             tuned = None
             if not args.kernel and not args.no_tune:
@@ -243,6 +254,7 @@ def run_cuda(args, cfg):
                 B.dslash_set_option(lat.ctx, B.DSLASH_OPT_TUNE_MODE, B.DSLASH_TUNE_SUSTAINED if long_run else B.DSLASH_TUNE_BURST)
                 tuned = lat.tune(od, pd, gd)
                 time.sleep(1.0)               # back to idle: the timed region starts from the same state with or without tuning
+            od.fill_(0x7f)                    # whatever the timed region leaves behind is what `parity` looks at
             n0 = B.dslash_launch_count(lat.ctx)
             ms, ck = time_applies(torch, lat, od, pd, gd, args.steps, args.warmup, group, local)
             n1 = B.dslash_launch_count(lat.ctx)
@@ -254,11 +266,21 @@ def run_cuda(args, cfg):
                                 kernel=KERNEL_IDS[B.dslash_get_kernel(lat.ctx)],
                                 occupancy=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_OCCUPANCY),
                                 x_shuffle=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_X_SHUFFLE),
+                                l2_policy=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_L2_POLICY),
                                 pipe_slots=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_PIPE_SLOTS),
                                 pipe_warps=B.dslash_get_option(lat.ctx, B.DSLASH_OPT_PIPE_WARPS),
                                 tuned_ms=None if tuned is None else tuned[1])
             if tag == "main":
                 clocks, launches = ck, n1 - n0 - args.warmup
+                if not args.no_parity and rank == 0:
+                    timed_out = lat.download_spinor(od)
+                # "x5 repeats, median and min" -- four more regions of the same K steps, each from idle
+                reps = [ms / args.steps]
+                for _ in range(max(0, args.repeats - 1)):
+                    time.sleep(0.5)
+                    ms_r, _ = time_applies(torch, lat, od, pd, gd, args.steps, args.warmup, group, local)
+                    reps.append(ms_r / args.steps)
+                results["repeats"] = reps
                 if args.sustained_steps > 0:
                     # ~0.6 s of continuous load, when the board runs against its power cap; the library re-picks its kernel for
                     # that regime (DSLASH_TUNE_SUSTAINED), again outside the timed region
@@ -275,17 +297,33 @@ def run_cuda(args, cfg):
 
     main = results["main"]
     peak, peak_src = hbm_peak()
-    key = "%s_%s_%s_r%d" % ("x".join(map(str, dims)), prec, args.layout, 12 if main["recon12"] else 18)
-    roofline = {"bound": "hbm", "achieved": main["gbs"], "peak": peak, "unit": "GB/s", "frac": main["gbs"] / peak,
-                "traffic": NCU_TRAFFIC_BYTES.get(key if main["kernel"] == "direct" else key + "_" + main["kernel"]),
-                "peak_source": peak_src, "kernel": KERNEL_NAMES.get(main["kernel"], main["kernel"]),
-                "algorithmic_bytes_per_site": main["bps"], "algorithmic_bytes_per_launch": main["bps"] * v,
-                "frac_of_nominal_8TBs": main["gbs"] / 8000.0}
+    key = "%s_%s_%s_r%d_%s" % ("x".join(map(str, dims)), prec, args.layout, 12 if main["recon12"] else 18, main["kernel"])
+    ncu = NCU_FIGURES.get(key, {})
+    working_set = main["bps"] * v
+    l2_resident = working_set < 126e6  # the whole working set of an application fits the 126 MB L2: repeated applies never reach HBM
+    if l2_resident:
+        # report it, but never as an HBM fraction
+        roofline = {"bound": "l2", "achieved": main["gbs"], "peak": None, "unit": "GB/s", "frac": None, "traffic": None,
+                    "note": "working set %.1f MB fits the 126 MB L2: algorithmic GB/s served from L2, no HBM roofline applies"
+                            % (working_set / 1e6),
+                    "kernel": KERNEL_NAMES.get(main["kernel"], main["kernel"]),
+                    "algorithmic_bytes_per_site": main["bps"], "algorithmic_bytes_per_launch": working_set}
+    else:
+        roofline = {"bound": "hbm", "achieved": main["gbs"], "peak": peak, "unit": "GB/s", "frac": main["gbs"] / peak,
+                    "traffic": ncu.get("traffic"), "traffic_source": ncu.get("source"),
+                    "fp64_pipe_pct": ncu.get("fp64_pipe_pct"), "fp64_pipe_source": ncu.get("source"),
+                    "peak_source": peak_src, "kernel": KERNEL_NAMES.get(main["kernel"], main["kernel"]),
+                    "algorithmic_bytes_per_site": main["bps"], "algorithmic_bytes_per_launch": working_set,
+                    "frac_of_nominal_8TBs": main["gbs"] / 8000.0,
+                    "regime": "burst: K steps from idle (board at its boost clock); see `sustained` for the power-capped regime"}
+        if "sustained" in results:
+            roofline["sustained_frac"] = results["sustained"]["gbs"] / peak
 
     # end to end through the C ABI with pinned HOST buffers (H2D + pack + apply + unpack + D2H per step)
     e2e = None
     if not args.no_e2e:
         with device.Lattice(dims, prec, args.layout, cfg["recon12"], device="cuda:%d" % local) as lat:
+            lattice_options(B, lat, args)
             gh = torch.from_numpy(np.ascontiguousarray(g)).pin_memory()
             ph = torch.from_numpy(np.ascontiguousarray(p)).pin_memory()
             oh = torch.empty(ph.shape, dtype=ph.dtype).pin_memory()
@@ -305,18 +343,34 @@ def run_cuda(args, cfg):
             ms_e = group.max_over_ranks(e0.elapsed_time(e1))
             e2e = {"value": replicas.whole_job_rate(FLOP_PER_SITE * v, world, ms_e / n_e2e) / 1e9, "unit": "GFLOP/s", "h2d_bytes_per_step": int(h2d),
                    "d2h_bytes_per_step": int(d2h), "ms_per_step": ms_e / n_e2e, "steps": n_e2e,
-                   "path": "dslash_apply_host(DSLASH_MAP_MINIMAL), pinned host buffers, canonical layout"}
+                   "gb_per_s_h2d": h2d / (ms_e / n_e2e) / 1e6,
+                   "path": "dslash_apply_host(DSLASH_MAP_MINIMAL), pinned host buffers, canonical layout; t-slabs pipelined over three streams"}
+            if timed_out is not None:  # the end-to-end path must give the same field as the device-resident one
+                e2e["max_abs_diff_vs_timed_buffer"] = float(np.abs(oh.numpy().reshape(timed_out.shape) - timed_out).max())
             del gh, ph, oh
 
     cpu_baseline = None
+    parity = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         g64, p64 = inputs.promote(g), inputs.promote(p)
-        gf, dt, cores, n = oracle_timing(dims, g64, p64, min(v, args.cpu_sites), 3, 1)
-        cpu_baseline = {"value": gf, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "seconds_per_application": dt,
+        nsite = min(v, args.cpu_sites)
+        gf, dt, cores, n, ref = oracle_timing(dims, g64, p64, nsite, 3, 1)
+        # the same oracle on ONE thread, on a sample an eighth as large (SURVEY.md section 8(d) asks for both)
+        gf1, dt1, _, n1s, _ = oracle_timing(dims, g64, p64, max(1, min(v, args.cpu_sites) // 8), 1, 0, nthreads=1)
+        cpu_baseline = {"value": gf, "unit": "GFLOP/s", "cores": cores, "nproc": os.cpu_count(), "kind": "oracle",
+                        "seconds_per_application": dt,
+                        "single_thread": {"value": gf1, "unit": "GFLOP/s", "seconds": dt1, "sites": int(n1s)},
                         "sample": "mean of 3 applications (after 1 warm-up) to %d of %d sites (%s)"
                                   % (n, v, "whole lattice" if n == v else "seeded sample")}
+        if timed_out is not None and n == v:
+            # parity of the buffer the timed region wrote, against the oracle's whole-lattice result (DESIGN.md Reading R10)
+            e = float(checks.parity_error(timed_out, ref))
+            parity = {"e": e, "sites": int(v), "kernel": main["kernel"], "tolerance": 1e-12 if prec == "f64" else 1e-5,
+                      "ok": bool(e <= (1e-12 if prec == "f64" else 1e-5)),
+                      "metric": "max_k |g_k - r_k| / max(|r_k|, rms(r)) over complex components, whole lattice, oracle = oracle_dslash"}
 
     if rank == 0:
+        reps = results["repeats"]
         line = {
             "metric": METRIC, "value": main["gflops"], "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": main["ms_per_step"], "higher_is_better": True, "scaling": "weak",
@@ -324,23 +378,26 @@ def run_cuda(args, cfg):
             "config": {"workload": cfg["name"], "dims": list(dims), "layout": args.layout, "recon": 12 if main["recon12"] else 18,
                        "tile": main["tile"], "kernel": main["kernel"],
                        "kernel_chosen_by": "dslash_tune (measured before the timed region)" if main["tuned_ms"] is not None else "option", "occupancy_option": main["occupancy"],
-                       "x_shuffle_option": main["x_shuffle"], "pipe_slots": main["pipe_slots"], "pipe_warps": main["pipe_warps"], "sites": v, "parallelism": "replicas x%d" % world,
-                       "l2": "inputs larger than L2: %.2f GB working set per apply vs 126 MB L2, no flush needed"
-                             % (main["bps"] * v / 1e9)},
-            "hbm_gbs": main["gbs"], "roofline": roofline, "cpu_baseline": cpu_baseline, "e2e": e2e, "clocks": clocks,
+                       "x_shuffle_option": main["x_shuffle"], "l2_policy_option": main["l2_policy"], "pipe_slots": main["pipe_slots"], "pipe_warps": main["pipe_warps"], "sites": v, "parallelism": "replicas x%d" % world,
+                       "l2": ("working set %.1f MB fits L2: L2-resident by design of this config" % (working_set / 1e6)) if l2_resident else
+                             ("inputs larger than L2: %.2f GB working set per apply vs 126 MB L2, no flush needed" % (working_set / 1e9))},
+            "hbm_gbs": None if l2_resident else main["gbs"], "roofline": roofline, "parity": parity,
+            "repeats": {"n": len(reps), "ms_per_step": reps, "median": float(np.median(reps)), "min": float(np.min(reps)),
+                        "note": "the K-step region repeated, each after 0.5 s idle; the first entry is `ms_per_step`"},
+            "cpu_baseline": cpu_baseline, "e2e": e2e, "clocks": clocks,
             "gpu_launches": int(launches),
         }
         if "sustained" in results:
             su = results["sustained"]
             line["sustained"] = {"value": su["gflops"], "ms_per_step": su["ms_per_step"], "hbm_gbs": su["gbs"],
-                                 "roofline_frac": su["gbs"] / peak, "steps": args.sustained_steps, "heat_steps": args.heat_steps,
+                                 "roofline_frac": None if l2_resident else su["gbs"] / peak, "steps": args.sustained_steps, "heat_steps": args.heat_steps,
                                  "clocks": su["clocks"], "kernel": su["kernel"],
                                  "note": "after heat_steps back-to-back applies (SM clock under the power cap); kernel re-picked by "
                                          "dslash_tune in DSLASH_TUNE_SUSTAINED mode unless --kernel / --no-tune"}
         if "other_recon" in results:
             o = results["other_recon"]
             line["also"] = {"recon": 12 if o["recon12"] else 18, "value": o["gflops"], "ms_per_step": o["ms_per_step"],
-                            "hbm_gbs": o["gbs"], "roofline_frac": o["gbs"] / peak}
+                            "hbm_gbs": o["gbs"], "roofline_frac": None if l2_resident else o["gbs"] / peak, "kernel": o["kernel"]}
         print(json.dumps(line))
     group.close()
     return 0
@@ -927,8 +984,10 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-parity", action="store_true", help="skip the whole-lattice parity check of the timed buffer")
+    ap.add_argument("--repeats", type=int, default=5, help="K-step regions timed in all (median and min reported)")
     ap.add_argument("--cpu-sites", type=int, default=1 << 21, help="sites the cpu_baseline oracle run covers")
-    ap.add_argument("--ref-sites", type=int, default=1 << 14, help="sample sites per step of --impl reference")
+    ap.add_argument("--ref-sites", type=int, default=0, help="sites per step of --impl reference (0: the whole lattice)")
     ap.add_argument("--decomposition", choices=["replicas", "slab"], default="replicas",
                     help="multi-GPU mode: independent lattices per rank (default) or one lattice cut into T-slabs")
     ap.add_argument("--sweep", action="store_true")

@@ -88,7 +88,8 @@ DSLASH_API int costmodel_zscore_apply(int n, int cols, const double *a, const do
 DSLASH_API int costmodel_error(int n, const double *pred, const double *y, double *out, dslash_stream_t stream);
 
 /* Tuning knobs of costmodel_train() (process-wide).  COSTMODEL_OPT_THREADS: threads per block, a multiple of 32 in 32..1024,
- * 0 = the library's default.  Results do not depend on it bit for bit.  Anything else: DSLASH_ERR_UNSUPPORTED. */
+ * 0 = the library's default.  Results do not depend on it bit for bit.  Anything else: DSLASH_ERR_UNSUPPORTED.
+ * costmodel_train() returns DSLASH_ERR_UNSUPPORTED when it is smaller than the mini-batch size. */
 #define COSTMODEL_OPT_THREADS 1
 DSLASH_API int costmodel_set_option(int option, int value);
 

@@ -116,9 +116,13 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
 /* options of the tuned kernels, dslash_set_option() */
 #define DSLASH_OPT_OCCUPANCY 2        /* blocks of <= 128 threads: 0 = 168 registers/thread (12 warps/SM), 1 = 128 (16 warps),
                                          2 = 255 (8 warps, deeper load hoisting) */
-#define DSLASH_OPT_L2_POLICY 3        /* bit mask of L2 eviction hints: 1 spinor loads evict_last, 2 U_t loads evict_last,
-                                         4 U_x/U_y/U_z loads evict_first, 8 stores of `out` evict_first,
-                                         16 t-direction loads bypass L1 allocation (0: none) */
+#define DSLASH_OPT_L2_POLICY 3        /* bit mask of L2 hints, -1 (default) = each kernel's own default.
+                                         Direct kernel (default 0): 1 spinor loads evict_last, 2 U_t loads evict_last,
+                                         4 U_x/U_y/U_z loads evict_first, 8 stores of `out` evict_first, 16 t-direction loads
+                                         bypass L1 allocation.
+                                         Marching kernel (default 4|8|16): 1 data other blocks read too evict_last, 4 links
+                                         read once per application evict_first, 8 stores evict_first, 16 a ring row is
+                                         fetched late, about one step before its first use instead of two */
 #define DSLASH_OPT_L1_CARVEOUT 4      /* direct kernel: preferred shared-memory carve-out in percent, -1 = driver default */
 #define DSLASH_OPT_X_SHUFFLE 5        /* direct kernel: 1 (default for FP64; FP32 defaults to 0) = when a whole x row sits inside one warp
                                          (tile x-extent == L_X, a power of two <= 32) the two x hops are exchanged between
@@ -164,7 +168,8 @@ DSLASH_API int dslash_destroy(dslash_ctx *ctx);
  *   gauge     device pointer, native gauge layout, dslash_gauge_bytes(), 16-byte aligned.
  * Exactly one kernel launch (DSLASH_KERNEL_WARP_PIPE: preceded by an 8-byte cudaMemsetAsync of its row counters on
  * `stream`); no allocation, copy or synchronisation.
- * Errors: NULL, ALIGN, ALIAS, CUDA (launch failure, also stored in the ctx).
+ * Errors: NULL, ALIGN, ALIAS, UNSUPPORTED (the current CUDA device is not the one the ctx was created on; an explicitly
+ * selected kernel cannot run this lattice), CUDA (launch failure, also stored in the ctx).
  */
 DSLASH_API int dslash_apply(dslash_ctx *ctx, void *out, const void *in, const void *gauge, dslash_stream_t stream);
 
@@ -386,13 +391,18 @@ DSLASH_API int dslash_get_option(const dslash_ctx *ctx, int option, int *value);
 /*
  * End-to-end application from HOST buffers in the canonical layout at the ctx's precision
  * (the path of PAPER.md:138-148: map to the device, run the kernel, map back):
- *   H2D copy of gauge and in -> pack -> dslash_apply -> unpack -> D2H copy of out, then the stream is
- *   synchronised.  With DSLASH_MAP_TOFROM all three fields travel both ways (what an offload without
+ *   H2D copy of gauge and in -> pack -> apply -> unpack -> D2H copy of out, then `stream` is synchronised.
+ *   The lattice is cut into up to 16 slabs of whole time slices and the three phases run on three internal streams (ordered
+ *   after the caller's earlier work on `stream`): slab k+1 travels to the device while slab k is packed, applied (direct
+ *   kernel on the slab's time range) and unpacked and slab k-1 of `out` travels back, so both directions of the host link
+ *   are busy.  Every byte crosses the link exactly once.  (A blocked-SoA lattice whose time slice is not a whole number of
+ *   32-site vectors, or a ctx with a partial time range, runs as one slab.)
+ *   With DSLASH_MAP_TOFROM all three fields travel both ways (what an offload without
  *   data analysis does); with DSLASH_MAP_MINIMAL only gauge,in go to the device and only out comes back.
  *   out_host, in_host, gauge_host   host pointers (pinned memory makes the copies asynchronous and
  *   faster; pageable memory works).  DSLASH_MAP_TOFROM reads out_host and rewrites in_host/gauge_host
  *   with the identical values.
- * The ctx owns the device staging buffers (allocated on first use, freed by dslash_destroy).
+ * The ctx owns the device staging buffers, streams and events (created on first use, freed by dslash_destroy).
  * h2d_bytes / d2h_bytes (optional, may be NULL) receive the bytes copied in each direction.
  * Errors: NULL, UNSUPPORTED (map_mode), NOMEM, CUDA.
  */

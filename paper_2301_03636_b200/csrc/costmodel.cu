@@ -516,6 +516,7 @@ int costmodel_train(int f, int n, const double* x, const double* y, const double
     const int nlr = (lr_step > 0 && epochs > 0) ? (epochs - 1) / lr_step + 1 : 1;
     if (nlr > kMaxLrSteps) return DSLASH_ERR_UNSUPPORTED;
     const int threads = g_train_threads.load() > 0 ? g_train_threads.load() : 512;
+    if (threads < batch) return DSLASH_ERR_UNSUPPORTED;  // the training kernel loads one mini-batch index per thread
     int C = cluster_size;
     if (C == 0) {
         // one block while the widest layer gives every thread at most one work item, more blocks as the layers grow

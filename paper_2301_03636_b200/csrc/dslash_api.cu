@@ -27,6 +27,9 @@ struct dslash_ctx {
     // staging buffers of dslash_apply_host (device memory, owned)
     void* d_can[3];  // canonical gauge, in, out
     void* d_nat[3];  // native gauge, in, out (alias d_can when the native layout is the canonical one)
+    // dslash_apply_host pipelines t-slabs over three streams: host->device copies, pack + apply + unpack, device->host copies
+    cudaStream_t host_stream[3];
+    cudaEvent_t host_event[2 * 16 + 2];  // [k]: slab k is on the device; [16 + k]: slab k of `out` is ready; [32], [33]: entry / exit
     // workspace of dslash_cg_solve (device memory, owned): r, p, t, q spinors; reduction scratch; one result
     void* cg_vec[4];
     double* cg_scratch;
@@ -265,7 +268,7 @@ int dslash_create(dslash_ctx** ctx, const int dims[4], int precision, int layout
     for (int i = 0; i < 6; ++i) c->eo_vec[i] = nullptr;
     c->kernel = DSLASH_KERNEL_AUTO;
     c->cfg.occupancy = precision == DSLASH_FP64 ? 2 : 1;  // measured: fp64 wants registers (ILP), fp32 wants warps
-    c->cfg.l2_policy = 0;
+    c->cfg.l2_policy = -1;  // each kernel's own default
     c->cfg.l1_carveout = -1;
     c->cfg.pipe_slots = 0;
     c->cfg.pipe_warps = 0;
@@ -283,6 +286,8 @@ int dslash_create(dslash_ctx** ctx, const int dims[4], int precision, int layout
     c->launches = 0;
     c->last_cuda = 0;
     for (int i = 0; i < 3; ++i) c->d_can[i] = c->d_nat[i] = nullptr;
+    for (int i = 0; i < 3; ++i) c->host_stream[i] = nullptr;
+    for (int i = 0; i < 34; ++i) c->host_event[i] = nullptr;
     for (int i = 0; i < 4; ++i) c->cg_vec[i] = nullptr;
     c->cg_scratch = nullptr;
     *ctx = c;
@@ -305,6 +310,10 @@ int dslash_destroy(dslash_ctx* c) {
         if (c->cg_scratch) cudaFree(c->cg_scratch);
         if (c->pipe_ctr) cudaFree(c->pipe_ctr);
         if (c->march_plan) cudaFree(c->march_plan);
+        for (int i = 0; i < 34; ++i)
+            if (c->host_event[i]) cudaEventDestroy(c->host_event[i]);
+        for (int i = 0; i < 3; ++i)
+            if (c->host_stream[i]) cudaStreamDestroy(c->host_stream[i]);
         for (int i = 0; i < 3; ++i) {
             if (c->d_nat[i] && c->d_nat[i] != c->d_can[i]) cudaFree(c->d_nat[i]);
             if (c->d_can[i]) cudaFree(c->d_can[i]);
@@ -347,6 +356,8 @@ int dslash_apply(dslash_ctx* c, void* out, const void* in, const void* gauge, ds
     if (overlap(out, sb, in, sb)) return DSLASH_ERR_ALIAS;
     LaunchArgs a{out, in, gauge, c->geom, static_cast<cudaStream_t>(stream)};
     cudaError_t e;
+    int cur_dev = -1;
+    if (cudaGetDevice(&cur_dev) != cudaSuccess || cur_dev != c->device) return DSLASH_ERR_UNSUPPORTED;  // the ctx belongs to its device
     if (c->var_depth == DSLASH_VARIANT_TUNED) {
         const int k = resolve_kernel(c);
         if (k < 0) return DSLASH_ERR_UNSUPPORTED;
@@ -728,7 +739,7 @@ int dslash_set_option(dslash_ctx* c, int option, int value) {
             c->cfg.occupancy = value;
             return DSLASH_OK;
         case DSLASH_OPT_L2_POLICY:
-            if (value < 0 || value > 31) return DSLASH_ERR_UNSUPPORTED;
+            if (value < -1 || value > 31) return DSLASH_ERR_UNSUPPORTED;
             c->cfg.l2_policy = value;
             return DSLASH_OK;
         case DSLASH_OPT_L1_CARVEOUT:
@@ -910,36 +921,114 @@ int dslash_apply_host(dslash_ctx* c, void* out_host, const void* in_host, const 
             }
         }
     }
-    size_t h2d = 0, d2h = 0;
     cudaError_t e;
-    // map(to: gauge, in) [+ map(tofrom: out) copies out in as well]
-    e = cudaMemcpyAsync(c->d_can[0], gauge_host, can_bytes[0], cudaMemcpyHostToDevice, stream);
-    if (e != cudaSuccess) return cuda_fail(c, e);
-    e = cudaMemcpyAsync(c->d_can[1], in_host, can_bytes[1], cudaMemcpyHostToDevice, stream);
-    if (e != cudaSuccess) return cuda_fail(c, e);
-    h2d += can_bytes[0] + can_bytes[1];
-    if (map_mode == DSLASH_MAP_TOFROM) {
-        e = cudaMemcpyAsync(c->d_can[2], out_host, can_bytes[2], cudaMemcpyHostToDevice, stream);
-        if (e != cudaSuccess) return cuda_fail(c, e);
-        h2d += can_bytes[2];
+    for (int i = 0; i < 3; ++i)
+        if (!c->host_stream[i] && (e = cudaStreamCreateWithFlags(&c->host_stream[i], cudaStreamNonBlocking)) != cudaSuccess) {
+            c->host_stream[i] = nullptr;
+            return cuda_fail(c, e);
+        }
+    for (int i = 0; i < 34; ++i)
+        if (!c->host_event[i] && (e = cudaEventCreateWithFlags(&c->host_event[i], cudaEventDisableTiming)) != cudaSuccess) {
+            c->host_event[i] = nullptr;
+            return cuda_fail(c, e);
+        }
+    // The lattice is cut into NS slabs of whole time slices (contiguous byte ranges of every field in every layout, provided a
+    // slice is a whole number of 32-site vectors).  Three streams: slab k+1 travels to the device while slab k is packed, applied
+    // and unpacked and slab k-1 of `out` travels back, so both directions of the host link are busy.  An application of slab k
+    // reads the spinors of slabs k-1 and k+1 too (periodic in t), so it runs once those are on the device: slabs 1 .. NS-2 in
+    // step with the copies, then NS-1 and 0.  Every byte crosses the link once: the byte counts are those of the serial path.
+    const int LT = c->geom.L[3];
+    const size_t slice = (size_t)c->geom.L[0] * c->geom.L[1] * c->geom.L[2];
+    int NS = LT < 16 ? LT : 16;
+    if (c->layout_base == LAYOUT_SOA && slice % VL != 0) NS = 1;  // slabs would not start on a vector boundary
+    if (NS < 2 || !full_time_range(c)) NS = 1;
+    const size_t rb = real_bytes(c), links = c->recon == 12 ? 12u : 18u;
+    auto slab_t0 = [&](int k) { return (int)((long long)k * LT / NS); };
+    cudaStream_t s_up = c->host_stream[0], s_run = c->host_stream[1], s_down = c->host_stream[2];
+    cudaEvent_t ev_entry = c->host_event[32], ev_exit = c->host_event[33];
+#define HOST_TRY(call)                                           \
+    do {                                                         \
+        if ((e = (call)) != cudaSuccess) return cuda_fail(c, e); \
+    } while (0)
+    HOST_TRY(cudaEventRecord(ev_entry, stream));  // everything here is ordered after the caller's earlier work on `stream`
+    HOST_TRY(cudaStreamWaitEvent(s_up, ev_entry, 0));
+    HOST_TRY(cudaStreamWaitEvent(s_run, ev_entry, 0));
+    HOST_TRY(cudaStreamWaitEvent(s_down, ev_entry, 0));
+    size_t h2d = 0, d2h = 0;
+    char *dcg = static_cast<char*>(c->d_can[0]), *dci = static_cast<char*>(c->d_can[1]), *dco = static_cast<char*>(c->d_can[2]);
+    char *dng = static_cast<char*>(c->d_nat[0]), *dni = static_cast<char*>(c->d_nat[1]), *dno = static_cast<char*>(c->d_nat[2]);
+    const char *hg = static_cast<const char*>(gauge_host), *hi = static_cast<const char*>(in_host);
+    char* ho = static_cast<char*>(out_host);
+    // map(to: gauge, in) [+ map(tofrom: out) copies out in as well], slab by slab, followed by the pack kernels of the slab
+    for (int k = 0; k < NS; ++k) {
+        const size_t s0 = (size_t)slab_t0(k) * slice, s1 = (size_t)slab_t0(k + 1) * slice, ns = s1 - s0;
+        const size_t go = s0 * 72u * rb, gn = ns * 72u * rb, so = s0 * 24u * rb, sn = ns * 24u * rb;
+        HOST_TRY(cudaMemcpyAsync(dcg + go, hg + go, gn, cudaMemcpyHostToDevice, s_up));
+        HOST_TRY(cudaMemcpyAsync(dci + so, hi + so, sn, cudaMemcpyHostToDevice, s_up));
+        h2d += gn + sn;
+        if (map_mode == DSLASH_MAP_TOFROM) {
+            HOST_TRY(cudaMemcpyAsync(dco + so, ho + so, sn, cudaMemcpyHostToDevice, s_up));
+            h2d += sn;
+        }
+        HOST_TRY(cudaEventRecord(c->host_event[k], s_up));
+        HOST_TRY(cudaStreamWaitEvent(s_run, c->host_event[k], 0));
+        if (!native_is_canonical[0]) {
+            HOST_TRY(launch_pack_gauge(c->precision, c->layout_base, c->recon, dng + s0 * 4u * links * rb, dcg + go, (unsigned)ns, s_run));
+            c->launches += 1;
+        }
+        if (!native_is_canonical[1]) {
+            HOST_TRY(launch_convert_spinor(c->precision, c->layout_base, dni + so, dci + so, (unsigned)ns, 0, s_run));
+            c->launches += 1;
+        }
+        // slabs whose neighbours are both packed by now: k - 1 (its forward neighbour k has just been packed)
+        auto run_slab = [&](int j) -> cudaError_t {
+            const size_t j0 = (size_t)slab_t0(j) * slice, jn = (size_t)slab_t0(j + 1) * slice - j0, jo = j0 * 24u * rb;
+            cudaError_t er;
+            if (NS == 1) {
+                LaunchArgs a{dno, dni, dng, c->geom, s_run};
+                er = launch_tuned(c->precision, c->layout_base, c->recon, a, c->tg, c->cfg);
+            } else {
+                TileGeom tg = c->tg;  // the direct kernel on the slices of this slab only
+                tg.t_begin = slab_t0(j);
+                tg.t_end = slab_t0(j + 1);
+                tg.nt[3] = (tg.t_end - tg.t_begin + c->tile[3] - 1) / c->tile[3];
+                LaunchArgs a{dno, dni, dng, c->geom, s_run};
+                er = launch_tuned(c->precision, c->layout_base, c->recon, a, tg, c->cfg);
+            }
+            if (er != cudaSuccess) return er;
+            c->launches += 1;
+            if (!native_is_canonical[2]) {
+                if ((er = launch_convert_spinor(c->precision, c->layout_base, dco + jo, dno + jo, (unsigned)jn, 1, s_run)) != cudaSuccess) return er;
+                c->launches += 1;
+            }
+            if ((er = cudaEventRecord(c->host_event[16 + j], s_run)) != cudaSuccess) return er;
+            if ((er = cudaStreamWaitEvent(s_down, c->host_event[16 + j], 0)) != cudaSuccess) return er;
+            if ((er = cudaMemcpyAsync(ho + jo, dco + jo, jn * 24u * rb, cudaMemcpyDeviceToHost, s_down)) != cudaSuccess) return er;
+            d2h += jn * 24u * rb;
+            return cudaSuccess;
+        };
+        if (NS == 1) {
+            HOST_TRY(run_slab(0));
+        } else {
+            if (k >= 2) HOST_TRY(run_slab(k - 1));
+            if (k == NS - 1) {
+                HOST_TRY(run_slab(NS - 1));
+                HOST_TRY(run_slab(0));
+            }
+        }
     }
-    int rc;
-    if (!native_is_canonical[0] && (rc = dslash_pack_gauge(c, c->d_nat[0], c->d_can[0], stream)) != DSLASH_OK) return rc;
-    if (!native_is_canonical[1] && (rc = dslash_pack_spinor(c, c->d_nat[1], c->d_can[1], stream)) != DSLASH_OK) return rc;
-    if ((rc = dslash_apply(c, c->d_nat[2], c->d_nat[1], c->d_nat[0], stream)) != DSLASH_OK) return rc;
-    if (!native_is_canonical[2] && (rc = dslash_unpack_spinor(c, c->d_can[2], c->d_nat[2], stream)) != DSLASH_OK) return rc;
-    e = cudaMemcpyAsync(out_host, c->d_can[2], can_bytes[2], cudaMemcpyDeviceToHost, stream);
-    if (e != cudaSuccess) return cuda_fail(c, e);
-    d2h += can_bytes[2];
-    if (map_mode == DSLASH_MAP_TOFROM) {
-        e = cudaMemcpyAsync(const_cast<void*>(gauge_host), c->d_can[0], can_bytes[0], cudaMemcpyDeviceToHost, stream);
-        if (e != cudaSuccess) return cuda_fail(c, e);
-        e = cudaMemcpyAsync(const_cast<void*>(in_host), c->d_can[1], can_bytes[1], cudaMemcpyDeviceToHost, stream);
-        if (e != cudaSuccess) return cuda_fail(c, e);
+    if (map_mode == DSLASH_MAP_TOFROM) {  // map(tofrom:): the unmodified inputs travel back as well
+        HOST_TRY(cudaMemcpyAsync(const_cast<void*>(gauge_host), c->d_can[0], can_bytes[0], cudaMemcpyDeviceToHost, s_down));
+        HOST_TRY(cudaMemcpyAsync(const_cast<void*>(in_host), c->d_can[1], can_bytes[1], cudaMemcpyDeviceToHost, s_down));
         d2h += can_bytes[0] + can_bytes[1];
     }
-    e = cudaStreamSynchronize(stream);
-    if (e != cudaSuccess) return cuda_fail(c, e);
+    // the caller's stream continues after all three; then, as documented, the call synchronises
+    for (int i = 0; i < 3; ++i) {
+        HOST_TRY(cudaEventRecord(ev_exit, c->host_stream[i]));
+        HOST_TRY(cudaStreamWaitEvent(stream, ev_exit, 0));
+    }
+    HOST_TRY(cudaStreamSynchronize(stream));
+#undef HOST_TRY
     if (h2d_bytes) *h2d_bytes = h2d;
     if (d2h_bytes) *d2h_bytes = d2h;
     return DSLASH_OK;

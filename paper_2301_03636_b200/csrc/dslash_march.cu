@@ -250,10 +250,11 @@ __device__ __forceinline__ void march_producer(unsigned char* smem, const unsign
             }
         }
     }
-    // L2 eviction policies (DSLASH_OPT_L2_POLICY bits).  1: what ANOTHER block reads too is evict_last -- every spinor row (a
-    // halo of up to four other blocks, whenever they get there) and the links a halo hop of another block needs (U_y / U_z of a
-    // row whose y+ / z+ neighbour is outside the block, and the halo links themselves).  4: what is read exactly once per
-    // application is evict_first -- U_x, U_t, and U_y / U_z of rows whose forward neighbour is in the block.
+    // L2 eviction policies (DSLASH_OPT_L2_POLICY bits).  4: what is read exactly once per application is evict_first -- U_x, U_t,
+    // and U_y / U_z of rows whose forward neighbour is in the block (with bits 8 and 16: HBM reads 1.80 -> 1.63 GB on 32^3x64,
+    // 1.011 x compulsory).  1: what ANOTHER block reads too is evict_last -- every spinor row and the links a halo hop of another
+    // block needs (U_y / U_z of a row whose y+ / z+ neighbour is outside the block, the halo links themselves); measured
+    // harmful (1.77 GB with 4, 8, 16 also set), so it is not part of the default.
     const uint64_t pol_shared = (hints & 1) ? make_policy(POLICY_EVICT_LAST) : 0ull;
     const uint64_t pol_stream = (hints & 4) ? make_policy(POLICY_EVICT_FIRST) : 0ull;
     unsigned shared_stage = ~0u;  // bit k: stage k of this queue is read by another block as well
@@ -561,7 +562,9 @@ cudaError_t launch_march(int precision, int layout_base, int recon, const Launch
     const MarchBlockPlan* p = static_cast<const MarchBlockPlan*>(d_plan);
     unsigned* st = reinterpret_cast<unsigned*>(const_cast<MarchBlockPlan*>(p + nblocks));
     unsigned* pr = st + 3u * (unsigned)nblocks;
-    const int h = cfg.l2_policy;
+    // default policy of this kernel (measured, profiles/r02_march.md): 4 read-once links evict_first, 8 stores evict_first,
+    // 16 late ring fill; 1 (shared data evict_last) is harmful
+    const int h = cfg.l2_policy >= 0 ? cfg.l2_policy : (4 | 8 | 16);
     // the throttle needs every block of a chunk resident at the same time: single-wave plans only
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) sms = 0;

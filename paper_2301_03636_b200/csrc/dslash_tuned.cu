@@ -2,7 +2,7 @@
 //
 // One thread per site; the thread block covers a 4-D tile of sites (x fastest inside the tile).  Tiles are
 // numbered x fastest, so blocks that run at the same time touch adjacent memory and the halos they share
-// stay in the 126 MB L2; HBM sees each field about once per application (profiles/: 1.11x).
+// stay in the 126 MB L2; HBM sees each field about once per application (profiles/r01_ncu_tuned_kernel.txt: 1.01x).
 // With the blocked SoA layout the 12 (9) loads of a spinor (link) share one base address, which took the
 // kernel from ~2100 to ~1500 SASS instructions per site -- that matters because under sustained load the
 // B200 runs this kernel against its 1 kW power cap (SM clock ~1.4 GHz), not against a fixed clock.
@@ -78,14 +78,16 @@ template <typename Real, int LAYOUT, int RECON, int HINT, bool XSHFL>
 static cudaError_t launch_tuned_s(const LaunchArgs& a, const TileGeom& tg, const TunedConfig& cfg) {
     const int tpb = 1 << (tg.lb[0] + tg.lb[1] + tg.lb[2] + tg.lb[3]);
     const unsigned grid = (unsigned)tg.nt[0] * (unsigned)tg.nt[1] * (unsigned)tg.nt[2] * (unsigned)tg.nt[3];
-    TunedOpts o{cfg.l2_policy};
+    TunedOpts o{cfg.l2_policy > 0 ? cfg.l2_policy : 0};
 #define DSLASH_LAUNCH(MAXTPB, MINBLK)                                                                                        \
     do {                                                                                                                     \
-        static int carve_set = -1;                                                                                           \
-        if (carve_set != cfg.l1_carveout) {                                                                                  \
+        static int carve_set[64]; /* per device; value + 2 so that 0 means "never set" */                                    \
+        int dev_ = 0;                                                                                                        \
+        cudaGetDevice(&dev_);                                                                                                \
+        if (carve_set[dev_ & 63] != cfg.l1_carveout + 2) {                                                                   \
             cudaFuncSetAttribute(dslash_tuned_kernel<Real, LAYOUT, RECON, MAXTPB, MINBLK, HINT, XSHFL>,                           \
                                  cudaFuncAttributePreferredSharedMemoryCarveout, cfg.l1_carveout);                          \
-            carve_set = cfg.l1_carveout;                                                                                     \
+            carve_set[dev_ & 63] = cfg.l1_carveout + 2;                                                                      \
         }                                                                                                                    \
         dslash_tuned_kernel<Real, LAYOUT, RECON, MAXTPB, MINBLK, HINT, XSHFL><<<grid, tpb, 0, a.stream>>>(a.out, a.in,        \
                                                                                                           a.gauge, a.geom, \
@@ -110,8 +112,8 @@ static cudaError_t launch_tuned_s(const LaunchArgs& a, const TileGeom& tg, const
 
 template <typename Real, int LAYOUT, int RECON>
 static cudaError_t launch_tuned_t(const LaunchArgs& a, const TileGeom& tg, const TunedConfig& cfg) {
-    if (cfg.l2_policy & 16) return launch_tuned_s<Real, LAYOUT, RECON, 2, false>(a, tg, cfg);
-    if (cfg.l2_policy) return launch_tuned_s<Real, LAYOUT, RECON, 1, false>(a, tg, cfg);
+    if (cfg.l2_policy > 0 && (cfg.l2_policy & 16)) return launch_tuned_s<Real, LAYOUT, RECON, 2, false>(a, tg, cfg);
+    if (cfg.l2_policy > 0) return launch_tuned_s<Real, LAYOUT, RECON, 1, false>(a, tg, cfg);
     // x hops by warp shuffle when a whole x row sits inside one warp (see x_hops_shuffle in dslash_site.cuh)
     if (cfg.x_shuffle && x_shuffle_eligible(a.geom, tg)) return launch_tuned_s<Real, LAYOUT, RECON, 0, true>(a, tg, cfg);
     return launch_tuned_s<Real, LAYOUT, RECON, 0, false>(a, tg, cfg);

@@ -227,17 +227,22 @@ cudaError_t launch_wpipe_k(const LaunchArgs& a, const TileGeom& tg, int zblock, 
     constexpr int cap = 16 / NW > 0 ? 16 / NW : 1;        // no more than 16 warps per SM: keep >= 128 registers per thread
     constexpr int MINBLK = fit < 1 ? 1 : (fit < cap ? fit : cap);
     auto kernel = dslash_wpipe_kernel<Real, RECON, NSLOT, NW, MINBLK>;
-    static int blocks_per_sm = 0, sms = 0;
-    if (blocks_per_sm == 0) {
-        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        int dev = 0, bps = 0;
-        if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
-        if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+    // occupancy and the dynamic shared-memory attribute are per DEVICE: cached per device id, not per process
+    static int blocks_per_sm_of[64] = {0}, sms_of[64] = {0};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const int di = dev & 63;
+    if (blocks_per_sm_of[di] == 0) {
+        if ((e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+        int bps = 0, nsm = 0;
+        if ((e = cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
         if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kernel, NW * 32, smem)) != cudaSuccess) return e;
         if (bps < 1) return cudaErrorInvalidConfiguration;
-        blocks_per_sm = bps;
+        sms_of[di] = nsm;
+        blocks_per_sm_of[di] = bps;
     }
+    const int blocks_per_sm = blocks_per_sm_of[di], sms = sms_of[di];
     PipeGeom pg{a.geom.L[1], a.geom.L[2], a.geom.L[3], tg.t_begin, tg.t_end - tg.t_begin, a.geom.L[2], 0u};
     if (zblock > 0 && zblock < a.geom.L[2] && a.geom.L[2] % zblock == 0) pg.zb = zblock;
     pg.nrows = (unsigned)a.geom.L[1] * (unsigned)a.geom.L[2] * (unsigned)pg.nt;

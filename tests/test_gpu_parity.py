@@ -672,20 +672,35 @@ def test_error_paths_on_device(env):
 
 # ---------------------------------------------------------------- host entry point (e2e path) and its byte accounting
 @pytest.mark.parametrize("layout,recon12", [("soa", False), ("soa", True), ("aos", False)])
-def test_apply_host_matches_oracle_and_counts_bytes(env, layout, recon12):
-    dims = (8, 6, 4, 10)
-    g, p, ref, _ = fields_and_ref(env, dims, SEED + 41, "f64")
+@pytest.mark.parametrize("dims,precision", [
+    ((8, 6, 4, 10), "f64"),   # 10 slabs of one time slice (192 sites = 6 vectors) pipelined over three streams
+    ((32, 4, 4, 40), "f64"),  # 16 slabs of 2-3 slices
+    ((32, 4, 4, 40), "f32"),
+    ((6, 3, 5, 4), "f64"),    # a slice of 90 sites is not a whole number of vectors: blocked SoA runs as one slab, AoS as 4
+    ((4, 4, 4, 2), "f64"),    # two slabs: each one's neighbours in t are both the other one
+    ((4, 4, 2, 1), "f64"),    # a single time slice
+])
+def test_apply_host_matches_oracle_and_counts_bytes(env, layout, recon12, dims, precision):
+    g, p, ref, _ = fields_and_ref(env, dims, SEED + 41, precision)
     torch, B = env.torch, env.B
     gh = torch.from_numpy(g.copy()).pin_memory()
     ph = torch.from_numpy(p.copy()).pin_memory()
-    oh = torch.zeros(p.shape, dtype=torch.float64).pin_memory()
-    with env.device.Lattice(dims, "f64", layout, recon12) as lat:
+    oh = torch.zeros(p.shape, dtype=ph.dtype).pin_memory()
+    with env.device.Lattice(dims, precision, layout, recon12) as lat:
         h2d, d2h = B.dslash_apply_host(lat.ctx, oh.data_ptr(), ph.data_ptr(), gh.data_ptr(), B.DSLASH_MAP_MINIMAL, lat.stream())
-        assert env.checks.parity_error(oh.numpy(), ref) <= TOL["f64"]
-        assert (h2d, d2h) == (g.nbytes + p.nbytes, p.nbytes)
+        assert env.checks.parity_error(oh.numpy(), ref) <= TOL[precision]
+        assert (h2d, d2h) == (g.nbytes + p.nbytes, p.nbytes)  # every byte crosses the host link once
+        # the same field, bit for bit, as the device-resident path
+        assert np.array_equal(oh.numpy(), lat.dslash(g, p))
+        # on a side stream, twice in a row (the internal streams are ordered after the caller's stream)
+        st = torch.cuda.Stream()
+        oh.zero_()
+        B.dslash_apply_host(lat.ctx, oh.data_ptr(), ph.data_ptr(), gh.data_ptr(), B.DSLASH_MAP_MINIMAL, st.cuda_stream)
+        B.dslash_apply_host(lat.ctx, oh.data_ptr(), ph.data_ptr(), gh.data_ptr(), B.DSLASH_MAP_MINIMAL, st.cuda_stream)
+        assert env.checks.parity_error(oh.numpy(), ref) <= TOL[precision]
         oh.zero_()
         h2d2, d2h2 = B.dslash_apply_host(lat.ctx, oh.data_ptr(), ph.data_ptr(), gh.data_ptr(), B.DSLASH_MAP_TOFROM, lat.stream())
-        assert env.checks.parity_error(oh.numpy(), ref) <= TOL["f64"]
+        assert env.checks.parity_error(oh.numpy(), ref) <= TOL[precision]
         # PAPER.md:265 (Fig. 4): 1.5 GB without data analysis -> 0.75 GB with it, exactly 2:1
         assert h2d2 + d2h2 == 2 * (h2d + d2h)
         assert np.array_equal(gh.numpy(), g) and np.array_equal(ph.numpy(), p)
