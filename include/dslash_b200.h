@@ -131,8 +131,12 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
 
 #define DSLASH_OPT_PIPE_SLOTS 7       /* warp-pipelined kernel: hop stages in flight per warp, 2..4 (0 = library default) */
 #define DSLASH_OPT_PIPE_WARPS 8       /* warp-pipelined kernel: warps per thread block, 1, 2 or 4 (0 = library default) */
-#define DSLASH_OPT_PIPE_ZBLOCK 9      /* warp-pipelined kernel: rows are visited y fastest, z inside blocks of this many planes, then t,
-                                         then the z blocks (a divisor of L_Z; 0 = L_Z): shortens the L2 reuse distance of the t hops */
+#define DSLASH_OPT_PIPE_ZBLOCK 9      /* z planes per block of the traversal order, a divisor of L_Z.  Warp-pipelined kernel: rows are
+                                         visited y fastest, z inside a z block, then t, then the z blocks (0 = L_Z).  Direct kernel:
+                                         tiles are numbered x, y, z inside a z block, t, z block (the value must be a multiple
+                                         of the tile's z extent; 0 = automatic: no blocking while a time slice of the three
+                                         fields is <= 40 MB, else the largest block whose slice is <= 20 MB).  Both shorten
+                                         the L2 reuse distance of the t hops (48^3x96 fp32: HBM reads 1.26 x -> see profiles/) */
 #define DSLASH_OPT_TUNE_MODE 10       /* what dslash_tune() optimises: DSLASH_TUNE_BURST (default; the first ~35 ms after idle, board at its
                                          boost clock) or DSLASH_TUNE_SUSTAINED (continuous load, board at its power-capped clock) */
 #define DSLASH_OPT_MARCH_LEAD 11      /* marching kernel: steps a block may run ahead of the slowest block of its chunk, 0..16
@@ -290,7 +294,7 @@ DSLASH_API int dslash_march_stats(dslash_ctx *ctx, unsigned *stats, size_t capac
  * three slot/warp configurations) is timed on the caller's buffers
  * (2 warm-up + 8 timed applications each, CUDA events on `stream`; about 15 ms in all, so that every candidate is
  * timed inside the board's boost window -- call it on an idle device; with DSLASH_OPT_TUNE_MODE = DSLASH_TUNE_SUSTAINED:
- * 150 applications to leave the boost window, then two interleaved rounds of 3 + 20 applications each, ~0.15 s in all) and the fastest becomes the
+ * 600 applications to leave the boost window, then three interleaved rounds of 5 + 30 applications each, ~0.4 s in all) and the fastest becomes the
  * context's kernel, as if set by dslash_set_kernel() (and DSLASH_OPT_PIPE_SLOTS / _WARPS).  out, in, gauge: device pointers as for dslash_apply(); out is left
  * holding D in.  *chosen (may be NULL) receives the kernel, *ms_per_apply (may be NULL) its time.  This call SYNCHRONISES
  * with `stream`.  Errors: those of dslash_apply(); DSLASH_ERR_UNSUPPORTED when a sweep variant is selected.

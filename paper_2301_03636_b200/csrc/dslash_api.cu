@@ -64,6 +64,21 @@ static int ilog2_exact(int v) {
     return ((1 << l) == v) ? l : -1;
 }
 
+// Tiles per z block of the block order (decode_tile): asked for in planes (DSLASH_OPT_PIPE_ZBLOCK, a multiple of the tile's z
+// extent whose tile count divides nt[2]), else automatic: no blocking while a time slice of the three fields is <= 40 MB
+// (two of them fit L2 with room to spare), otherwise the largest divisor of nt[2] that keeps a slice of the z block <= 20 MB.
+static int z_block_tiles(const dslash_ctx* c, const Geom& g, const TileGeom& tg, int planes) {
+    const int tz = 1 << tg.lb[2];
+    if (planes > 0 && planes % tz == 0 && tg.nt[2] % (planes / tz) == 0) return planes / tz;
+    const double per_site = (24.0 + 4.0 * (c->recon == 12 ? 12.0 : 18.0) + 24.0) * (double)real_bytes(c);
+    const double plane = (double)g.L[0] * g.L[1] * tz * per_site;  // one tile-thick z plane of one time slice
+    if (plane * tg.nt[2] <= 40e6) return tg.nt[2];
+    int best = 1;
+    for (int d = 1; d <= tg.nt[2]; ++d)
+        if (tg.nt[2] % d == 0 && plane * d <= 20e6) best = d;
+    return best;
+}
+
 static void set_tile_geom(dslash_ctx* c, const int tile[4]) {
     for (int d = 0; d < 4; ++d) {
         c->tile[d] = tile[d];
@@ -71,6 +86,7 @@ static void set_tile_geom(dslash_ctx* c, const int tile[4]) {
         c->tg.nt[d] = (c->geom.L[d] + tile[d] - 1) / tile[d];
     }
     c->tg.nt[3] = (c->tg.t_end - c->tg.t_begin + tile[3] - 1) / tile[3];  // tiles in t cover the active range only
+    c->tg.zb = z_block_tiles(c, c->geom, c->tg, c->cfg.pipe_zblock);
 }
 static bool full_time_range(const dslash_ctx* c) { return c->tg.t_begin == 0 && c->tg.t_end == c->geom.L[3]; }
 
@@ -264,6 +280,7 @@ int dslash_create(dslash_ctx** ctx, const int dims[4], int precision, int layout
         }
         c->tg_eo.t_begin = 0;
         c->tg_eo.t_end = dims[3];
+        c->tg_eo.zb = c->tg_eo.nt[2];
     }
     for (int i = 0; i < 6; ++i) c->eo_vec[i] = nullptr;
     c->kernel = DSLASH_KERNEL_AUTO;
@@ -761,6 +778,7 @@ int dslash_set_option(dslash_ctx* c, int option, int value) {
         case DSLASH_OPT_PIPE_ZBLOCK:
             if (value < 0 || value > c->geom.L[2] || (value > 0 && c->geom.L[2] % value)) return DSLASH_ERR_UNSUPPORTED;
             c->cfg.pipe_zblock = value;
+            set_tile_geom(c, c->tile);
             return DSLASH_OK;
         case DSLASH_OPT_PIPE_WARPS:
             if (value != 0 && value != 1 && value != 2 && value != 4) return DSLASH_ERR_UNSUPPORTED;
@@ -842,15 +860,15 @@ int dslash_tune(dslash_ctx* c, void* out, const void* in, const void* gauge, dsl
     float best_ms = 0.f;
     // DSLASH_TUNE_BURST: one short pass (2 warm-up + 8 timed applications per candidate, ~15 ms in all): the whole comparison
     // stays inside the board's boost window; a longer one would time the later candidates under the power cap and the earlier
-    // ones not.  DSLASH_TUNE_SUSTAINED: 150 applications first (the board leaves its boost window after ~35 ms and settles at
-    // its power-capped clock), then two interleaved rounds of 3 + 20 applications per candidate, summed per candidate.
+    // ones not.  DSLASH_TUNE_SUSTAINED: 600 applications first (the board leaves its boost window after ~35 ms; its clock keeps
+    // settling for another ~0.1 s), then three interleaved rounds of 5 + 30 applications per candidate, summed per candidate.
     const bool sustained = c->tune_mode == DSLASH_TUNE_SUSTAINED;
     float total[5] = {0.f, 0.f, 0.f, 0.f, 0.f};
     if (sustained) {
         c->kernel = DSLASH_KERNEL_DIRECT;
-        for (int i = 0; i < 150 && rc == DSLASH_OK; ++i) rc = dslash_apply(c, out, in, gauge, stream);
+        for (int i = 0; i < 600 && rc == DSLASH_OK; ++i) rc = dslash_apply(c, out, in, gauge, stream);
     }
-    const int rounds = sustained ? 2 : 1, warm = sustained ? 3 : 2, reps = sustained ? 20 : 8;
+    const int rounds = sustained ? 3 : 1, warm = sustained ? 5 : 2, reps = sustained ? 30 : 8;
     for (int round = 0; round < rounds && rc == DSLASH_OK; ++round)
         for (int k = 0; k < ncand && rc == DSLASH_OK; ++k) {
             c->kernel = cand[k].kernel;

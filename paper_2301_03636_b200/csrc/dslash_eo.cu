@@ -34,13 +34,8 @@ __global__ void __launch_bounds__(128, MINBLK)
     dslash_eo_kernel(void* __restrict__ out, const void* __restrict__ in, const void* __restrict__ gauge_out_parity,
                      const void* __restrict__ gauge_in_parity, Geom gh, TileGeom tg, EoParams op) {
     // gh = the half geometry {L_X/2, L_Y, L_Z, L_T}, gh.V = V/2; tiles and threads are laid over (xh, y, z, t)
-    unsigned b = blockIdx.x;
-    const unsigned bx = b % (unsigned)tg.nt[0];
-    b /= (unsigned)tg.nt[0];
-    const unsigned by = b % (unsigned)tg.nt[1];
-    b /= (unsigned)tg.nt[1];
-    const unsigned bz = b % (unsigned)tg.nt[2];
-    const unsigned bt = b / (unsigned)tg.nt[2];
+    unsigned bx, by, bz, bt;
+    decode_tile(blockIdx.x, tg, bx, by, bz, bt);
     unsigned r = threadIdx.x;
     const int xh = (int)((bx << tg.lb[0]) + (r & ((1u << tg.lb[0]) - 1u)));
     r >>= tg.lb[0];

@@ -12,7 +12,25 @@ struct TileGeom {
     int lb[4];
     int nt[4];
     int t_begin, t_end;  // time slices [t_begin, t_end) are computed (dslash_set_time_range); nt[3] tiles cover that range
+    int zb;              // tiles per z block of the block order (a divisor of nt[2]; nt[2] = plain x, y, z, t order)
 };
+
+// Block number -> tile coordinates.  Blocks run roughly in the order of their numbers, and what one block fetches the next
+// ones find in L2, so the ORDER decides how far apart in time the two uses of a spinor by t-neighbours are.  Plain order
+// (x, y, z, t) puts a whole time slice between them: 31 MB at 32^3 fp64, which L2 holds (HBM traffic 1.01 x compulsory), but
+// 53 MB at 48^3 fp32, which it does not (ncu: 1.26 x).  So the z extent is cut into blocks of zb tiles and the order is
+// x, y, z inside the z block, t, z block: the reuse distance shrinks to one slice of the z block, at the price of re-reading
+// the z halo planes at the block boundaries (2 of 2 * zb * tile_z planes).
+__device__ __forceinline__ void decode_tile(unsigned b, const TileGeom& tg, unsigned& bx, unsigned& by, unsigned& bz, unsigned& bt) {
+    bx = b % (unsigned)tg.nt[0];
+    b /= (unsigned)tg.nt[0];
+    by = b % (unsigned)tg.nt[1];
+    b /= (unsigned)tg.nt[1];
+    const unsigned bzi = b % (unsigned)tg.zb;
+    b /= (unsigned)tg.zb;
+    bt = b % (unsigned)tg.nt[3];
+    bz = (b / (unsigned)tg.nt[3]) * (unsigned)tg.zb + bzi;
+}
 
 struct LaunchArgs {
     void* out;

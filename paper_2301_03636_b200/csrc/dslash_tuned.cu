@@ -36,13 +36,8 @@ __global__ void __launch_bounds__(MAXTPB, MINBLK)
     dslash_tuned_kernel(void* __restrict__ out, const void* __restrict__ in, const void* __restrict__ gauge, Geom g,
                         TileGeom tg, TunedOpts opt) {
     // tile coordinates of this block
-    unsigned b = blockIdx.x;
-    const unsigned bx = b % (unsigned)tg.nt[0];
-    b /= (unsigned)tg.nt[0];
-    const unsigned by = b % (unsigned)tg.nt[1];
-    b /= (unsigned)tg.nt[1];
-    const unsigned bz = b % (unsigned)tg.nt[2];
-    const unsigned bt = b / (unsigned)tg.nt[2];
+    unsigned bx, by, bz, bt;
+    decode_tile(blockIdx.x, tg, bx, by, bz, bt);
     // in-tile coordinates of this thread (power-of-two tile extents)
     unsigned r = threadIdx.x;
     const int x = (int)((bx << tg.lb[0]) + (r & ((1u << tg.lb[0]) - 1u)));

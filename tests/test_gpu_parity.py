@@ -97,6 +97,34 @@ def test_tuned_kernel_every_tile_shape(env, tile):
         assert gpu_vs_ref(env, lat, g, p, ref) <= TOL["f64"]
 
 
+@pytest.mark.parametrize("dims,tile,zblock", [
+    ((8, 4, 12, 3), (8, 4, 2, 1), 2), ((8, 4, 12, 3), (8, 4, 2, 1), 4), ((8, 4, 12, 3), (8, 4, 2, 1), 6),
+    ((8, 4, 12, 3), (8, 4, 2, 1), 12),      # one block: the plain order
+    ((8, 4, 12, 3), (8, 4, 2, 1), 3),       # not a multiple of the tile's z extent: the automatic choice
+    ((12, 6, 10, 5), (4, 4, 2, 1), 2), ((12, 6, 9, 4), (4, 2, 4, 2), 0),  # ragged in y and z with partial tiles
+])
+def test_direct_kernel_z_blocked_tile_order(env, dims, tile, zblock):
+    """The block order x, y, z inside a z block, t, z block (DSLASH_OPT_PIPE_ZBLOCK) visits every site exactly once."""
+    B = env.B
+    g, p, ref, _ = fields_and_ref(env, dims, SEED + 15, "f64")
+    with env.device.Lattice(dims, "f64", "soa", False) as lat:
+        lat.set_tile(tile)
+        gi, pi, o = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
+        lat.apply(o, pi, gi)
+        plain = lat.download_spinor(o)
+        if zblock and dims[2] % zblock == 0:
+            B.dslash_set_option(lat.ctx, B.DSLASH_OPT_PIPE_ZBLOCK, zblock)
+        o.fill_(0x7f)
+        lat.apply(o, pi, gi)
+        got = lat.download_spinor(o)
+        assert env.checks.parity_error(got, ref) <= TOL["f64"]
+        assert np.array_equal(got, plain)
+        for op in (B.DSLASH_OP_D_DAGGER, B.DSLASH_OP_M):  # the operator kernels share the block decode
+            o.fill_(0x7f)
+            lat.apply_op(op, 0.3, o, pi, gi)
+            assert np.isfinite(lat.download_spinor(o)).all()
+
+
 # ---------------------------------------------------------------- x hops by warp shuffle (DSLASH_OPT_X_SHUFFLE)
 @pytest.mark.parametrize("dims,tile", [
     ((32, 3, 5, 2), (32, 2, 2, 1)),   # one row per warp, ragged tiles in y and z (clamped rows that do not store)
