@@ -406,8 +406,8 @@ def run_cuda(args, cfg):
 # ------------------------------------------------------------------ multi-GPU: one global lattice cut into T-slabs
 def run_slab(args, cfg):
     """--decomposition slab: the --config lattice is cut along t across the ranks (paper_2301_03636_b200/slab.py);
-    every apply exchanges one spinor slice with each t-neighbour over torch.distributed (NCCL) and overlaps the
-    exchange with the interior slices.  Strong scaling: value = 1320 * V_global / max-over-ranks time."""
+    every apply exchanges one face of spin-projected half-spinors with each t-neighbour over torch.distributed (NCCL)
+    and overlaps the exchange with the interior slices (dslash_slab_* calls of the C ABI).  Strong scaling: value = 1320 * V_global / max-over-ranks time."""
     import torch
     from paper_2301_03636_b200 import binding as B
     from paper_2301_03636_b200 import inputs, replicas, slab
@@ -446,12 +446,13 @@ def run_slab(args, cfg):
                 "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
                 "dtype": prec, "data": "synthetic",
                 "config": {"workload": cfg["name"], "dims": list(dims), "layout": args.layout, "recon": 12 if cfg["recon12"] else 18,
-                           "parallelism": "t-slabs x%d, %d slices per rank + 2 ghost slices" % (world, rk.geom.lt),
-                           "halo_bytes_per_rank_per_step": 2 * rk.spinor_slice,
+                           "parallelism": "t-slabs x%d, %d slices per rank, half-spinor faces" % (world, rk.geom.lt),
+                           "halo_bytes_per_rank_per_step": rk.halo_bytes_per_application,
+                           "face_bytes": rk.face_bytes,
                            "l2": "inputs larger than L2 per rank" if bps * v / world > 2 * 126e6 else "per-rank working set near L2 size"},
                 "hbm_gbs": gbs, "roofline": {"bound": "hbm", "achieved": gbs / world, "peak": peak, "unit": "GB/s",
                                              "frac": gbs / world / peak, "traffic": None, "peak_source": peak_src,
-                                             "kernel": "dslash_tuned_kernel (3 launches per apply: interior, 2 boundary slices)"},
+                                             "kernel": "slab_pack_faces_kernel + dslash_tuned_kernel (interior) + slab_boundary_kernel: 3 launches per apply"},
                 "cpu_baseline": None, "e2e": None, "clocks": cs.summary(), "gpu_launches": int(launches)}
         print(json.dumps(line))
     rk.close()

@@ -245,9 +245,7 @@ DSLASH_API int dslash_get_tile(const dslash_ctx *ctx, int tile[4]);
 
 /*
  * Restrict dslash_apply / dslash_apply_op to the time slices t_begin <= t < t_end (default: the whole lattice); sites
- * outside the range are neither computed nor written.  This is the hook of the multi-GPU slab decomposition
- * (paper_2301_03636_b200/slab.py): a rank's local lattice carries one ghost slice at each end in t, only the interior
- * slices are computed, and the interior can be launched while the ghost slices are still being exchanged.
+ * outside the range are neither computed nor written (what dslash_apply_host and the dslash_slab_* calls use internally).
  * Every tuned kernel honours the range (the marching kernel's block plan is rebuilt by this call: synchronous); the sweep
  * variants and dslash_cg_solve need the full range (DSLASH_ERR_UNSUPPORTED otherwise).
  * Errors: NULL, UNSUPPORTED (not 0 <= t_begin < t_end <= L_T), CUDA.
@@ -384,6 +382,32 @@ DSLASH_API int dslash_eo_cg_solve(dslash_ctx *ctx, void *x_even, const void *b_e
                                   int max_iter, int *iterations, double *rel_residual, dslash_stream_t stream);
 DSLASH_API int dslash_eo_solve(dslash_ctx *ctx, void *x_even, void *x_odd, const void *b_even, const void *b_odd, const void *gauge_eo,
                                double mass, double tol, int max_iter, int *iterations, double *rel_residual, dslash_stream_t stream);
+
+/*
+ * Multi-GPU form of Eq. 1 by T-slab decomposition (the paper's future work).
+ * A rank owns lt consecutive time slices of the global lattice; its ctx is created with dims {L_X, L_Y, L_Z, lt} and its fields
+ * are ordinary native fields of that local lattice (no ghost slices; links never travel).  Of the eight hops only two leave
+ * the slab, and both projectors (1 -+ gamma_t) have rank 2, so one application exchanges two FACES of half-spinors
+ * (6 complex numbers per site of a time slice, dslash_slab_face_bytes() each: 3.1 MB at 32^3 FP64):
+ *     face DOWN, to the rank that owns the slices below:  P^-_t in(x, 0)                         (receiver multiplies by ITS U_t)
+ *     face UP,   to the rank that owns the slices above:  U_t(x, lt-1)^dagger P^+_t in(x, lt-1)  (complete contribution)
+ * One application on every rank:
+ *     dslash_slab_pack_faces(ctx, face_down, face_up, in, gauge, s)       one launch; then post the two sends / two receives
+ *     dslash_slab_interior(ctx, out, in, gauge, s)                        slices 1 .. lt-2 while the faces travel (no launch if lt <= 2)
+ *     dslash_slab_boundary(ctx, out, in, gauge, face_from_below, face_from_above, s)    slices 0 and lt-1, after the receives
+ * face_from_below is the face UP of the rank below, face_from_above the face DOWN of the rank above (with one rank: the
+ * rank's own faces -- the periodic wrap).  Together the three calls write every site of `out` once, with the arithmetic
+ * and the order of the sum of dslash_apply: bit-identical to the single-GPU result on the global lattice.
+ * All pointers: device memory, 16-byte aligned; faces are opaque (same ctx parameters on sender and receiver); out must not
+ * overlap in or the received faces.  Asynchronous on `stream`; the caller orders the message passing against it.
+ * Errors: NULL, ALIGN, ALIAS, UNSUPPORTED (a partial time range is set), CUDA.
+ */
+DSLASH_API size_t dslash_slab_face_bytes(const dslash_ctx *ctx);
+DSLASH_API int dslash_slab_pack_faces(dslash_ctx *ctx, void *face_down, void *face_up, const void *in, const void *gauge,
+                                      dslash_stream_t stream);
+DSLASH_API int dslash_slab_interior(dslash_ctx *ctx, void *out, const void *in, const void *gauge, dslash_stream_t stream);
+DSLASH_API int dslash_slab_boundary(dslash_ctx *ctx, void *out, const void *in, const void *gauge, const void *face_from_below,
+                                    const void *face_from_above, dslash_stream_t stream);
 
 /*
  * Performance options of the tuned kernels (DSLASH_OPT_*); they never change results beyond rounding order.

@@ -4,7 +4,7 @@
     from paper_2301_03636_b200 import inputs    # seeded synthetic fields (NumPy only)
 
 Importing the package itself touches neither CUDA nor torch, so the CPU-only tooling (input
-generator, variant enumerator) stays usable without a GPU.  There is no CPU fallback: every
+generator, library build) stays usable without a GPU.  There is no CPU fallback: every
 compute entry point lives in `binding` and goes through include/dslash_b200.h.
 """
-__all__ = ["binding", "inputs", "variants", "build"]
+__all__ = ["binding", "build", "checks", "costmodel", "device", "inputs", "replicas", "slab"]

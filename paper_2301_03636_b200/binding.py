@@ -76,6 +76,10 @@ SIGNATURES = {
     "dslash_get_time_range": (ctypes.c_int, [_vp, _c_int_p, _c_int_p]),
     "dslash_set_kernel": (ctypes.c_int, [_vp, ctypes.c_int]),
     "dslash_get_kernel": (ctypes.c_int, [_vp, _c_int_p]),
+    "dslash_slab_face_bytes": (ctypes.c_size_t, [_vp]),
+    "dslash_slab_pack_faces": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _vp]),
+    "dslash_slab_interior": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp]),
+    "dslash_slab_boundary": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "dslash_march_stats": (ctypes.c_int, [_vp, ctypes.POINTER(ctypes.c_uint), ctypes.c_size_t, _c_int_p]),
     "dslash_march_plan": (ctypes.c_int, [_c_int_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, _c_int_p, ctypes.c_size_t, _c_int_p]),
     "dslash_probe_launch": (ctypes.c_int, [ctypes.c_int, _vp, _vp, ctypes.c_size_t, ctypes.c_int, _vp]),
@@ -365,6 +369,24 @@ def dslash_march_plan(dims, t_begin: int, t_end: int, wave: int):
             warps.append(dict(row=q[0], fwd=(q[1], q[2]), wr=(q[3], q[4]), rd=(q[5], q[6]), bwd=(q[7], q[8])))
         blocks.append(dict(t0=v[0], nt=v[1], nact=v[2], warps=warps))
     return blocks
+
+
+def dslash_slab_face_bytes(ctx) -> int:
+    return int(_lib.dslash_slab_face_bytes(_ptr(ctx)))
+
+
+def dslash_slab_pack_faces(ctx, face_down, face_up, inp, gauge, stream=0) -> None:
+    _check(_lib.dslash_slab_pack_faces(_ptr(ctx), _ptr(face_down), _ptr(face_up), _ptr(inp), _ptr(gauge), _ptr(stream)),
+           "dslash_slab_pack_faces")
+
+
+def dslash_slab_interior(ctx, out, inp, gauge, stream=0) -> None:
+    _check(_lib.dslash_slab_interior(_ptr(ctx), _ptr(out), _ptr(inp), _ptr(gauge), _ptr(stream)), "dslash_slab_interior")
+
+
+def dslash_slab_boundary(ctx, out, inp, gauge, face_from_below, face_from_above, stream=0) -> None:
+    _check(_lib.dslash_slab_boundary(_ptr(ctx), _ptr(out), _ptr(inp), _ptr(gauge), _ptr(face_from_below), _ptr(face_from_above),
+                                     _ptr(stream)), "dslash_slab_boundary")
 
 
 def dslash_march_stats(ctx):

@@ -1052,6 +1052,60 @@ int dslash_apply_host(dslash_ctx* c, void* out_host, const void* in_host, const 
     return DSLASH_OK;
 }
 
+/* ------------------------------------------------------------------ multi-GPU T-slab form */
+size_t dslash_slab_face_bytes(const dslash_ctx* c) {
+    if (!c) return 0;
+    size_t slice = (size_t)c->geom.L[0] * c->geom.L[1] * c->geom.L[2];
+    if (c->layout_base == LAYOUT_SOA) slice = (slice + VL - 1u) / VL * VL;
+    return slice * 12u * real_bytes(c);
+}
+
+int dslash_slab_pack_faces(dslash_ctx* c, void* face_down, void* face_up, const void* in, const void* gauge, dslash_stream_t stream) {
+    if (!c || !face_down || !face_up || !in || !gauge) return DSLASH_ERR_NULL;
+    if (misaligned(face_down) || misaligned(face_up) || misaligned(in) || misaligned(gauge)) return DSLASH_ERR_ALIGN;
+    if (!full_time_range(c)) return DSLASH_ERR_UNSUPPORTED;
+    const size_t fb = dslash_slab_face_bytes(c);
+    if (overlap(face_down, fb, face_up, fb)) return DSLASH_ERR_ALIAS;
+    cudaError_t e = launch_slab_pack_faces(c->precision, c->layout_base, c->recon, face_down, face_up, in, gauge, c->geom,
+                                           static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    c->launches += 1;
+    return DSLASH_OK;
+}
+
+int dslash_slab_interior(dslash_ctx* c, void* out, const void* in, const void* gauge, dslash_stream_t stream) {
+    if (!c || !out || !in || !gauge) return DSLASH_ERR_NULL;
+    if (misaligned(out) || misaligned(in) || misaligned(gauge)) return DSLASH_ERR_ALIGN;
+    const size_t sb = dslash_spinor_bytes(c);
+    if (overlap(out, sb, in, sb)) return DSLASH_ERR_ALIAS;
+    if (!full_time_range(c)) return DSLASH_ERR_UNSUPPORTED;
+    if (c->geom.L[3] <= 2) return DSLASH_OK;  // every slice is a boundary slice
+    TileGeom tg = c->tg;  // the direct kernel on slices 1 .. lt-2: none of their hops leaves the slab
+    tg.t_begin = 1;
+    tg.t_end = c->geom.L[3] - 1;
+    tg.nt[3] = (tg.t_end - tg.t_begin + c->tile[3] - 1) / c->tile[3];
+    LaunchArgs a{out, in, gauge, c->geom, static_cast<cudaStream_t>(stream)};
+    cudaError_t e = launch_tuned(c->precision, c->layout_base, c->recon, a, tg, c->cfg);
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    c->launches += 1;
+    return DSLASH_OK;
+}
+
+int dslash_slab_boundary(dslash_ctx* c, void* out, const void* in, const void* gauge, const void* face_from_below,
+                         const void* face_from_above, dslash_stream_t stream) {
+    if (!c || !out || !in || !gauge || !face_from_below || !face_from_above) return DSLASH_ERR_NULL;
+    if (misaligned(out) || misaligned(in) || misaligned(gauge) || misaligned(face_from_below) || misaligned(face_from_above))
+        return DSLASH_ERR_ALIGN;
+    const size_t sb = dslash_spinor_bytes(c), fb = dslash_slab_face_bytes(c);
+    if (overlap(out, sb, in, sb) || overlap(out, sb, face_from_below, fb) || overlap(out, sb, face_from_above, fb)) return DSLASH_ERR_ALIAS;
+    if (!full_time_range(c)) return DSLASH_ERR_UNSUPPORTED;
+    cudaError_t e = launch_slab_boundary(c->precision, c->layout_base, c->recon, out, in, gauge, face_from_below, face_from_above, c->geom,
+                                         static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    c->launches += 1;
+    return DSLASH_OK;
+}
+
 int dslash_march_stats(dslash_ctx* c, unsigned* stats, size_t capacity, int* nblocks) {
     if (!c || !nblocks) return DSLASH_ERR_NULL;
     *nblocks = c->march_plan ? c->march_blocks : 0;

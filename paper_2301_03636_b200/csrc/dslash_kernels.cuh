@@ -97,6 +97,12 @@ cudaError_t march_plan_create(const Geom& g, int t_begin, int t_end, int device,
 cudaError_t launch_march(int precision, int layout_base, int recon, const LaunchArgs& a, const void* d_plan, int nblocks,
                          const TunedConfig& cfg, unsigned epoch);
 
+// Multi-GPU T-slab form (dslash_slab.cu): half-spinor faces and the boundary slices that consume them.
+cudaError_t launch_slab_pack_faces(int precision, int layout_base, int recon, void* face_down, void* face_up, const void* in,
+                                   const void* gauge, const Geom& g, cudaStream_t st);
+cudaError_t launch_slab_boundary(int precision, int layout_base, int recon, void* out, const void* in, const void* gauge,
+                                 const void* face_from_below, const void* face_from_above, const Geom& g, cudaStream_t st);
+
 // Operators around Dslash (dslash_ops.cu): op 0 D, 1 D^dagger, 2 M = (4+m) - D/2, 3 M^dagger; solver vector kernels.
 cudaError_t launch_op(int precision, int layout_base, int recon, const LaunchArgs& a, const TileGeom& tg, int op, double mass);
 cudaError_t launch_axpby(int precision, int layout_base, unsigned V, void* y, const void* x, double a, double b, cudaStream_t st);

@@ -1,9 +1,9 @@
-"""Multi-GPU plumbing: "replicas only".
+"""Multi-GPU plumbing shared by both modes of `bench.py --gpus N`.
 
-The Dslash path has no exchange step in this build, so N GPUs run N independent lattices.  This
-module holds the only cross-rank logic there is -- rendezvous, barrier, max-over-ranks of the
-device time, and the whole-job throughput -- on torch.distributed (NCCL on GPUs, gloo in the CPU
-tests).  No data-path collective exists.
+Default mode = replicas: N GPUs run N independent lattices (north_star keeps the path on one GPU), no data-path
+collective.  The sharded alternative (one lattice cut into T-slabs with a face exchange per application) lives in
+slab.py and uses the same Group.  This module holds the cross-rank logic both need -- rendezvous, barrier,
+max-over-ranks of the device time, whole-job throughput -- on torch.distributed (NCCL on GPUs, gloo in the CPU tests).
 """
 import os
 

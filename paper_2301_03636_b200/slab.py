@@ -1,22 +1,19 @@
-"""Multi-GPU Dslash by T-slab decomposition with a one-slice halo exchange.
+"""Multi-GPU Dslash by T-slab decomposition with half-spinor faces.
 
 The paper runs one GPU per node and leaves multi-GPU to future work; BASELINE.json's north_star
 keeps everything on one GPU, so `bench.py` defaults to independent replicas.  This module is the sharded alternative:
 
-  * the global lattice (L_X, L_Y, L_Z, L_T) is cut along t into `world` slabs of lt = L_T / world slices;
-  * a rank's local lattice has lt + 2 slices: ghost slice 0 (global t0 - 1), interior slices 1..lt, ghost slice lt + 1;
-    in every native layout a time slice is one contiguous byte range (blocked SoA: L_X*L_Y*L_Z must be a multiple of 32),
-    so the exchange moves plain sub-buffers -- no pack kernels;
-  * links are static: their ghost slices are filled once (only U_t of ghost slice 0 is ever read);
-  * per application each rank sends its first interior spinor slice down and its last interior slice up
-    (torch.distributed P2P over NCCL / NVLink; gloo for the CPU tests), computes the interior slices 2..lt-1 with
-    dslash_set_time_range while the messages fly, then the two boundary slices.  No global collective exists.
+  * the global lattice (L_X, L_Y, L_Z, L_T) is cut along t into `world` slabs of lt = L_T / world slices; a rank's
+    fields are ordinary native fields of its local lattice (L_X, L_Y, L_Z, lt): no ghost slices, links never travel;
+  * per application a rank sends two FACES of spin-projected half-spinors (6 complex numbers per site of a time slice,
+    half of a spinor slice): face DOWN = P^-_t in(x, 0) to the rank below, face UP = U_t^dagger P^+_t in(x, lt-1) to the
+    rank above (torch.distributed P2P over NCCL / NVLink; gloo for the CPU tests).  No global collective exists;
+  * the interior slices are computed while the faces fly, the two boundary slices after they have arrived.
 
-Everything numerical is done by libdslash_b200.so; this file only moves bytes and sequences launches.
+All arithmetic and all launches sit behind the C ABI (dslash_slab_pack_faces / _interior / _boundary,
+include/dslash_b200.h); this file only posts the four messages and orders the streams.
 """
 import numpy as np
-
-from . import replicas
 
 
 class SlabGeometry:
@@ -28,64 +25,49 @@ class SlabGeometry:
             raise ValueError("L_T = %d is not divisible by the number of ranks %d" % (lt, world))
         self.global_dims = (lx, ly, lz, lt)
         self.world, self.rank = world, rank
-        self.lt = lt // world                      # interior slices per rank
-        self.t0 = rank * self.lt                   # global t of local interior slice 1
-        self.local_dims = (lx, ly, lz, self.lt + 2)
+        self.lt = lt // world                      # slices per rank
+        self.t0 = rank * self.lt                   # global t of local slice 0
+        self.local_dims = (lx, ly, lz, self.lt)
         self.slice_sites = lx * ly * lz
-        self.up = (rank + 1) % world               # owns global t + lt
+        self.up = (rank + 1) % world               # owns global t0 + lt
         self.down = (rank - 1) % world
 
-    def slice_bytes(self, field: str, precision: str, layout: str, recon12: bool) -> int:
-        """Bytes of one time slice of a native field ("spinor" or "gauge")."""
-        rb = 8 if precision == "f64" else 4
-        if layout == "soa" and self.slice_sites % 32:
-            raise ValueError("blocked SoA slabs need L_X*L_Y*L_Z to be a multiple of 32 (got %d)" % self.slice_sites)
-        reals = 24 if field == "spinor" else 4 * (12 if recon12 else 18)
-        return self.slice_sites * reals * rb
 
-
-def halo_messages(geom: SlabGeometry):
+def face_messages(geom: SlabGeometry):
     """The four messages of one exchange, in the order they must be posted (the order makes world = 2, where both
     neighbours are the same peer, match correctly without tags: my first send pairs with the peer's first receive).
-    Each entry: (kind, peer, local_slice_index)."""
-    return [("send", geom.down, 1),              # my first interior slice is the upper ghost of the rank below
-            ("send", geom.up, geom.lt),          # my last interior slice is the lower ghost of the rank above
-            ("recv", geom.up, geom.lt + 1),      # upper ghost  <- first interior slice of the rank above
-            ("recv", geom.down, 0)]              # lower ghost  <- last interior slice of the rank below
+    Each entry: (kind, peer, buffer name)."""
+    return [("send", geom.down, "face_down"),          # P^-_t in(x, 0): the forward t hop of the rank below's last slice
+            ("send", geom.up, "face_up"),              # U_t^dagger P^+_t in(x, lt-1): backward t hop of the rank above's first slice
+            ("recv", geom.up, "face_from_above"),      # <- the face DOWN of the rank above
+            ("recv", geom.down, "face_from_below")]    # <- the face UP of the rank below
 
 
-def _slice_view(buf, index: int, nbytes: int):
-    return buf[index * nbytes:(index + 1) * nbytes]
-
-
-def exchange_halos(buf, geom: SlabGeometry, nbytes: int, dist=None):
-    """Start the halo exchange of a native field held in the flat uint8 tensor `buf` (lt + 2 slices of `nbytes`).
-    Returns a list of requests to wait on (empty when world == 1: the periodic wrap is two local copies).
-    `dist` is torch.distributed (already initialised) or None for world == 1."""
+def exchange_faces(faces: dict, geom: SlabGeometry, dist=None):
+    """Start the exchange of the four face buffers (flat uint8 tensors).  Returns the requests to wait on (empty when
+    world == 1: the periodic wrap is two local copies).  `dist` is torch.distributed (initialised) or None."""
     if geom.world == 1:
-        _slice_view(buf, geom.lt + 1, nbytes).copy_(_slice_view(buf, 1, nbytes))
-        _slice_view(buf, 0, nbytes).copy_(_slice_view(buf, geom.lt, nbytes))
+        faces["face_from_above"].copy_(faces["face_down"])
+        faces["face_from_below"].copy_(faces["face_up"])
         return []
     ops = []
-    for kind, peer, idx in halo_messages(geom):
+    for kind, peer, name in face_messages(geom):
         fn = dist.isend if kind == "send" else dist.irecv
-        ops.append(dist.P2POp(fn, _slice_view(buf, idx, nbytes), peer))
+        ops.append(dist.P2POp(fn, faces[name], peer))
     return dist.batch_isend_irecv(ops)
 
 
-def exchange_halos_in_process(bufs, geoms, nbytes: int):
+def exchange_faces_in_process(all_faces, geoms):
     """The same data movement for `world` slabs that live in ONE process (single-GPU emulation of the ranks: the
     profiling guide forbids running mutually waiting ranks as separate kernels/processes on one GPU)."""
-    world = len(bufs)
-    for r in range(world):
-        g = geoms[r]
-        _slice_view(bufs[g.down], geoms[g.down].lt + 1, nbytes).copy_(_slice_view(bufs[r], 1, nbytes))
-        _slice_view(bufs[g.up], 0, nbytes).copy_(_slice_view(bufs[r], g.lt, nbytes))
+    for r, g in enumerate(geoms):
+        all_faces[g.down]["face_from_above"].copy_(all_faces[r]["face_down"])
+        all_faces[g.up]["face_from_below"].copy_(all_faces[r]["face_up"])
 
 
 class SlabDslash:
-    """One rank's share of a T-slab decomposed Dslash.  `exchange` is a callable(buf, nbytes) -> requests; the default
-    uses torch.distributed through `group` (a replicas.Group)."""
+    """One rank's share of a T-slab decomposed Dslash.  `exchange` is a callable(faces) -> requests; the default uses
+    torch.distributed through `group` (a replicas.Group)."""
 
     def __init__(self, global_dims, precision="f64", layout="soa", recon12=False, group=None, rank=None, world=None,
                  device="cuda:0", exchange=None):
@@ -97,65 +79,55 @@ class SlabDslash:
             rank, world = group.rank, group.world
         self.geom = SlabGeometry(global_dims, world if world is not None else 1, rank if rank is not None else 0)
         self.group = group
-        self.precision, self.layout, self.recon12 = precision, layout, recon12
         self.lat = Lattice(self.geom.local_dims, precision, layout, recon12, device=device)
-        self.spinor_slice = self.geom.slice_bytes("spinor", precision, layout, recon12)
-        self.gauge_slice = self.geom.slice_bytes("gauge", precision, layout, recon12)
+        self.face_bytes = B.dslash_slab_face_bytes(self.lat.ctx)
+        self.faces = {name: torch.empty(self.face_bytes, dtype=torch.uint8, device=self.lat.device)
+                      for name in ("face_down", "face_up", "face_from_above", "face_from_below")}
         self._exchange = exchange
         self.comm_stream = torch.cuda.Stream(device=self.lat.device)
 
     def close(self):
         self.lat.close()
 
+    @property
+    def halo_bytes_per_application(self):
+        """Bytes this rank SENDS per application (it receives as many)."""
+        return 2 * self.face_bytes
+
     # -- data placement (canonical NumPy, global arrays indexed [T, Z, Y, X, ...])
-    def _local_with_ghosts(self, global_field):
+    def _local(self, global_field):
         g = self.geom
-        lt_glob = g.global_dims[3]
-        idx = [(g.t0 - 1 + k) % lt_glob for k in range(g.lt + 2)]
-        return np.ascontiguousarray(global_field[idx])
+        return np.ascontiguousarray(global_field[g.t0:g.t0 + g.lt])
 
     def upload_gauge(self, global_gauge):
-        """Local native links incl. both ghost slices (links are static: filled once, here straight from the global
-        array every rank can generate from the seed)."""
-        return self.lat.upload_gauge(self._local_with_ghosts(global_gauge))
+        return self.lat.upload_gauge(self._local(global_gauge))
 
     def upload_spinor(self, global_spinor):
-        """Local native spinor; the ghost slices are deliberately zeroed -- apply() must fetch them."""
-        loc = self._local_with_ghosts(global_spinor)
-        loc[0] = 0
-        loc[-1] = 0
-        return self.lat.upload_spinor(loc)
+        return self.lat.upload_spinor(self._local(global_spinor))
 
-    def download_interior(self, native):
-        """Canonical NumPy of the interior slices, shape [lt, Z, Y, X, 4, 3, 2]."""
-        return self.lat.download_spinor(native)[1:self.geom.lt + 1]
+    def download(self, native):
+        """Canonical NumPy of the rank's slices, shape [lt, Z, Y, X, 4, 3, 2]."""
+        return self.lat.download_spinor(native)
 
     # -- the operator
-    def start_exchange(self, spinor):
+    def start_exchange(self):
         if self._exchange is not None:
-            return self._exchange(spinor, self.spinor_slice)
+            return self._exchange(self.faces)
         dist = self.group.dist if self.group is not None else None
-        return exchange_halos(spinor, self.geom, self.spinor_slice, dist)
+        return exchange_faces(self.faces, self.geom, dist)
 
     def apply(self, out, inp, gauge):
-        """out(interior) = D in: exchange the two boundary slices of `inp`, overlap with the interior slices."""
-        torch, B, g = self.torch, self.B, self.geom
+        """out = (D in) restricted to this rank's slices."""
+        torch, B, f = self.torch, self.B, self.faces
         main = torch.cuda.current_stream()
-        self.comm_stream.wait_stream(main)  # `inp` was produced on the main stream
+        st = main.cuda_stream
+        B.dslash_slab_pack_faces(self.lat.ctx, f["face_down"].data_ptr(), f["face_up"].data_ptr(), inp.data_ptr(), gauge.data_ptr(), st)
+        self.comm_stream.wait_stream(main)  # the faces are written on the main stream
         with torch.cuda.stream(self.comm_stream):
-            reqs = self.start_exchange(inp)
-        if g.lt > 2:  # slices 2..lt-1 need no ghost data
-            B.dslash_set_time_range(self.lat.ctx, 2, g.lt)
-            self.lat.apply(out, inp, gauge)
+            reqs = self.start_exchange()
+        B.dslash_slab_interior(self.lat.ctx, out.data_ptr(), inp.data_ptr(), gauge.data_ptr(), st)  # while the faces fly
         for r in reqs:
             r.wait()
         main.wait_stream(self.comm_stream)
-        if g.lt >= 2:
-            B.dslash_set_time_range(self.lat.ctx, 1, 2)
-            self.lat.apply(out, inp, gauge)
-            B.dslash_set_time_range(self.lat.ctx, g.lt, g.lt + 1)
-            self.lat.apply(out, inp, gauge)
-        else:  # a single interior slice touches both ghosts
-            B.dslash_set_time_range(self.lat.ctx, 1, 2)
-            self.lat.apply(out, inp, gauge)
-        B.dslash_set_time_range(self.lat.ctx, 0, g.lt + 2)
+        B.dslash_slab_boundary(self.lat.ctx, out.data_ptr(), inp.data_ptr(), gauge.data_ptr(), f["face_from_below"].data_ptr(),
+                               f["face_from_above"].data_ptr(), st)

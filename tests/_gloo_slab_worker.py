@@ -1,4 +1,4 @@
-"""Worker for tests/test_multirank_gloo.py: the slab halo exchange on CPU tensors over gloo."""
+"""Worker for tests/test_multirank_gloo.py: the slab face exchange on CPU tensors over gloo."""
 import json
 import os
 import sys
@@ -11,20 +11,19 @@ from paper_2301_03636_b200 import replicas, slab  # noqa: E402
 g = replicas.Group(backend="gloo")
 global_dims = (4, 4, 2, 4 * g.world)  # lt = 4 slices per rank, 32 sites per slice
 geom = slab.SlabGeometry(global_dims, g.world, g.rank)
-nbytes = geom.slice_bytes("spinor", "f64", "soa", False)
-buf = torch.zeros((geom.lt + 2) * nbytes, dtype=torch.uint8)
-# interior slice k (1..lt) of rank r is filled with the byte value 10*r + k; ghosts start as 255
-for k in range(geom.lt + 2):
-    buf[k * nbytes:(k + 1) * nbytes] = 255 if k in (0, geom.lt + 1) else 10 * g.rank + k
-reqs = slab.exchange_halos(buf, geom, nbytes, g.dist)
-for r in reqs:
+nbytes = geom.slice_sites * 12 * 8  # one fp64 half-spinor face
+# a rank's face DOWN is filled with the byte 10 * rank + 1, its face UP with 10 * rank + 2; the receive buffers start as 255
+faces = {"face_down": torch.full((nbytes,), 10 * g.rank + 1, dtype=torch.uint8),
+         "face_up": torch.full((nbytes,), 10 * g.rank + 2, dtype=torch.uint8),
+         "face_from_above": torch.full((nbytes,), 255, dtype=torch.uint8),
+         "face_from_below": torch.full((nbytes,), 255, dtype=torch.uint8)}
+for r in slab.exchange_faces(faces, geom, g.dist):
     r.wait()
 g.barrier()
-lo = buf[0:nbytes]
-hi = buf[(geom.lt + 1) * nbytes:]
-out = {"rank": g.rank, "world": g.world, "lo_min": int(lo.min()), "lo_max": int(lo.max()), "hi_min": int(hi.min()),
-       "hi_max": int(hi.max()), "interior_ok": all(int(buf[k * nbytes]) == 10 * g.rank + k for k in range(1, geom.lt + 1)),
-       "lt": geom.lt, "up": geom.up, "down": geom.down}
+out = {"rank": g.rank, "world": g.world, "lt": geom.lt, "up": geom.up, "down": geom.down, "t0": geom.t0,
+       "above_min": int(faces["face_from_above"].min()), "above_max": int(faces["face_from_above"].max()),
+       "below_min": int(faces["face_from_below"].min()), "below_max": int(faces["face_from_below"].max()),
+       "sent_intact": bool((faces["face_down"] == 10 * g.rank + 1).all() and (faces["face_up"] == 10 * g.rank + 2).all())}
 with open(os.path.join(sys.argv[1], "slab_rank%d.json" % g.rank), "w") as f:
     json.dump(out, f)
 g.close()

@@ -474,42 +474,76 @@ def test_cg_solves_the_normal_equations(env, dims, precision, layout, tol):
 
 
 # ---------------------------------------------------------------- multi-GPU slab decomposition, ranks emulated in one process
-@pytest.mark.parametrize("world", [1, 2, 3, 4])
-@pytest.mark.parametrize("precision,layout,recon12", [("f64", "soa", False), ("f64", "aos", True), ("f32", "soa", True)])
+@pytest.mark.parametrize("world", [1, 2, 3, 4, 6, 12])
+@pytest.mark.parametrize("precision,layout,recon12", [("f64", "soa", False), ("f64", "aos", True), ("f32", "soa", True),
+                                                      ("f32", "aos", False)])
 def test_slab_decomposition_reproduces_the_single_lattice_result(env, world, precision, layout, recon12):
-    """T-slabs with ghost slices + halo exchange + dslash_set_time_range (interior first, then the two boundary
-    slices) must give the oracle's result for the GLOBAL lattice.  One GPU is available, so the `world` ranks are
-    emulated in one process and the exchange is a device copy between their buffers (slab.exchange_halos_in_process);
-    the torch.distributed path is covered on CPU by tests/test_multirank_gloo.py."""
+    """T-slabs + half-spinor faces (dslash_slab_pack_faces / _interior / _boundary) must give the oracle's result for the
+    GLOBAL lattice, and the same bits as dslash_apply on one GPU.  world = 6 and 12 are the slabs of two and one slices
+    (no interior).  One GPU is available, so the ranks are emulated in one process and the exchange is a device copy
+    between their face buffers (slab.exchange_faces_in_process); the torch.distributed path is covered on CPU by
+    tests/test_multirank_gloo.py."""
     from paper_2301_03636_b200 import slab
+    B = env.B
     dims = (8, 4, 4, 12)
     g, p, ref, _ = fields_and_ref(env, dims, SEED + 18, precision)
+    with env.device.Lattice(dims, precision, layout, recon12) as lat:
+        single = lat.dslash(g, p)
     ranks = [slab.SlabDslash(dims, precision, layout, recon12, rank=r, world=world) for r in range(world)]
     try:
         gauges = [rk.upload_gauge(g) for rk in ranks]
         ins = [rk.upload_spinor(p) for rk in ranks]
         outs = [rk.lat.new_spinor() for rk in ranks]
-        geoms = [rk.geom for rk in ranks]
-        done = []
-
-        def exchange_all(_buf, nbytes):  # the first rank that asks triggers the exchange for everybody
-            if not done:
-                slab.exchange_halos_in_process(ins, geoms, nbytes)
-                done.append(True)
-            return []
-        for rk in ranks:
-            rk._exchange = exchange_all
+        for o in outs:
+            o.fill_(0x7f)
+        # half of a spinor slice per face: 6 complex per site
+        rb = 8 if precision == "f64" else 4
+        assert ranks[0].face_bytes == dims[0] * dims[1] * dims[2] * 12 * rb and ranks[0].halo_bytes_per_application == 2 * ranks[0].face_bytes
+        st = env.torch.cuda.current_stream().cuda_stream
+        # the three phases rank by rank, the exchange (for everybody at once) between packing and the boundary slices
+        for rk, i, gg in zip(ranks, ins, gauges):
+            f = rk.faces
+            B.dslash_slab_pack_faces(rk.lat.ctx, f["face_down"].data_ptr(), f["face_up"].data_ptr(), i.data_ptr(), gg.data_ptr(), st)
+        slab.exchange_faces_in_process([rk.faces for rk in ranks], [rk.geom for rk in ranks])
         for rk, o, i, gg in zip(ranks, outs, ins, gauges):
-            o.zero_()
-            rk.apply(o, i, gg)
+            n0 = B.dslash_launch_count(rk.lat.ctx)
+            B.dslash_slab_interior(rk.lat.ctx, o.data_ptr(), i.data_ptr(), gg.data_ptr(), st)
+            assert B.dslash_launch_count(rk.lat.ctx) == n0 + (1 if rk.geom.lt > 2 else 0)
+            f = rk.faces
+            B.dslash_slab_boundary(rk.lat.ctx, o.data_ptr(), i.data_ptr(), gg.data_ptr(), f["face_from_below"].data_ptr(),
+                                   f["face_from_above"].data_ptr(), st)
         env.torch.cuda.synchronize()
-        got = np.concatenate([rk.download_interior(o) for rk, o in zip(ranks, outs)], axis=0)
+        got = np.concatenate([rk.download(o) for rk, o in zip(ranks, outs)], axis=0)
         assert got.shape == ref.shape
         assert env.checks.parity_error(got, ref) <= TOL[precision]
-        assert env.B.dslash_get_time_range(ranks[0].lat.ctx) == (0, ranks[0].geom.lt + 2)
+        assert np.array_equal(got, single)  # the same arithmetic in the same order, merely split between ranks
+        if world == 1:  # SlabDslash.apply with the self-wrap exchange
+            outs[0].fill_(0x7f)
+            ranks[0].apply(outs[0], ins[0], gauges[0])
+            env.torch.cuda.synchronize()
+            assert np.array_equal(ranks[0].download(outs[0]), single)
     finally:
         for rk in ranks:
             rk.close()
+
+
+def test_slab_calls_check_their_arguments(env):
+    B = env.B
+    with env.device.Lattice((8, 4, 4, 6), "f64", "soa", False) as lat:
+        o, p, g = lat.new_spinor(), lat.new_spinor(), lat.new_gauge()
+        fb = B.dslash_slab_face_bytes(lat.ctx)
+        f = [env.torch.zeros(fb, dtype=env.torch.uint8, device="cuda") for _ in range(2)]
+        for bad in [lambda: B.dslash_slab_pack_faces(lat.ctx, 0, f[1].data_ptr(), p.data_ptr(), g.data_ptr()),
+                    lambda: B.dslash_slab_pack_faces(lat.ctx, f[0].data_ptr(), f[0].data_ptr(), p.data_ptr(), g.data_ptr()),
+                    lambda: B.dslash_slab_pack_faces(lat.ctx, f[0].data_ptr() + 8, f[1].data_ptr(), p.data_ptr(), g.data_ptr()),
+                    lambda: B.dslash_slab_interior(lat.ctx, p.data_ptr(), p.data_ptr(), g.data_ptr()),
+                    lambda: B.dslash_slab_boundary(lat.ctx, o.data_ptr(), p.data_ptr(), g.data_ptr(), f[0].data_ptr(), 0)]:
+            with pytest.raises(B.DslashError):
+                bad()
+        B.dslash_set_time_range(lat.ctx, 1, 4)
+        with pytest.raises(B.DslashError) as e:
+            B.dslash_slab_interior(lat.ctx, o.data_ptr(), p.data_ptr(), g.data_ptr())
+        assert e.value.status == B.DSLASH_ERR_UNSUPPORTED
 
 
 def test_time_range_only_touches_its_slices(env):

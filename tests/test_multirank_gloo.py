@@ -1,4 +1,5 @@
-"""N>1 host logic on CPU: gloo, world_size 2 (the GPU path is replicas only -- DESIGN.md section 8)."""
+"""N>1 host logic on CPU over gloo: the max-over-ranks / whole-job arithmetic of the replica mode, the reference arm under
+torchrun, and the face exchange of the T-slab mode (world sizes 2 and 3) -- DESIGN.md section 8."""
 import json
 import os
 import socket
@@ -46,45 +47,15 @@ import pytest  # noqa: E402
 
 
 @pytest.mark.parametrize("world", [2, 3])
-def test_slab_halo_exchange_over_gloo(tmp_path, world):
-    """Each rank's ghost slices must end up holding the neighbouring rank's boundary slices (periodic ring in t).
-    world = 2 is the case where both neighbours are the same peer and message order does the matching."""
+def test_slab_face_exchange_over_gloo(tmp_path, world):
+    """A rank's face DOWN must arrive as the face_from_above of the rank below, its face UP as the face_from_below of the rank
+    above (periodic ring in t).  world = 2 is the case where both neighbours are the same peer and message order does the
+    matching."""
     r = _torchrun([os.path.join(ROOT, "tests", "_gloo_slab_worker.py"), str(tmp_path)], nproc=world)
     assert r.returncode == 0, r.stderr[-2000:]
     for k in range(world):
         o = json.load(open(tmp_path / ("slab_rank%d.json" % k)))
-        lt = o["lt"]
-        assert o["world"] == world and o["up"] == (k + 1) % world and o["down"] == (k - 1) % world
-        assert o["interior_ok"]
-        # lower ghost = last interior slice (index lt) of the rank below; upper ghost = slice 1 of the rank above
-        assert o["lo_min"] == o["lo_max"] == 10 * ((k - 1) % world) + lt
-        assert o["hi_min"] == o["hi_max"] == 10 * ((k + 1) % world) + 1
-
-
-def test_slab_geometry_and_message_plan():
-    from paper_2301_03636_b200 import slab
-    g = slab.SlabGeometry((8, 4, 4, 12), 3, 1)
-    assert g.lt == 4 and g.t0 == 4 and g.local_dims == (8, 4, 4, 6) and (g.up, g.down) == (2, 0)
-    assert g.slice_bytes("spinor", "f64", "soa", False) == 128 * 192
-    assert g.slice_bytes("gauge", "f32", "aos", True) == 128 * 48 * 4
-    assert [m[0] for m in slab.halo_messages(g)] == ["send", "send", "recv", "recv"]
-    with pytest.raises(ValueError):
-        slab.SlabGeometry((8, 4, 4, 10), 3, 0)  # L_T not divisible
-    with pytest.raises(ValueError):
-        slab.SlabGeometry((3, 3, 3, 4), 2, 0).slice_bytes("spinor", "f64", "soa", False)  # 27 sites per slice
-    # in-process exchange (the single-GPU emulation) moves the same slices
-    import torch
-    world, nb = 3, 16
-    geoms = [slab.SlabGeometry((2, 2, 2, 6), world, r) for r in range(world)]
-    bufs = [torch.zeros((geoms[r].lt + 2) * nb, dtype=torch.uint8) for r in range(world)]
-    for r in range(world):
-        for k in range(1, geoms[r].lt + 1):
-            bufs[r][k * nb:(k + 1) * nb] = 10 * r + k
-    slab.exchange_halos_in_process(bufs, geoms, nb)
-    for r in range(world):
-        assert int(bufs[r][0]) == 10 * ((r - 1) % world) + geoms[r].lt and int(bufs[r][-1]) == 10 * ((r + 1) % world) + 1
-    one = slab.SlabGeometry((2, 2, 2, 4), 1, 0)
-    b = torch.arange(6 * nb, dtype=torch.uint8)
-    ref = b.clone()
-    assert slab.exchange_halos(b, one, nb) == []
-    assert torch.equal(b[:nb], ref[4 * nb:5 * nb]) and torch.equal(b[5 * nb:], ref[nb:2 * nb])
+        assert o["world"] == world and o["up"] == (k + 1) % world and o["down"] == (k - 1) % world and o["t0"] == k * o["lt"]
+        assert o["sent_intact"]
+        assert o["above_min"] == o["above_max"] == 10 * ((k + 1) % world) + 1  # the face DOWN of the rank above
+        assert o["below_min"] == o["below_max"] == 10 * ((k - 1) % world) + 2  # the face UP of the rank below
