@@ -353,10 +353,10 @@ def run_cuda(args, cfg):
     parity = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         g64, p64 = inputs.promote(g), inputs.promote(p)
-        nsite = min(v, args.cpu_sites)
+        nsite = v if args.cpu_sites <= 0 else min(v, args.cpu_sites)
         gf, dt, cores, n, ref = oracle_timing(dims, g64, p64, nsite, 3, 1)
         # the same oracle on ONE thread, on a sample an eighth as large (SURVEY.md section 8(d) asks for both)
-        gf1, dt1, _, n1s, _ = oracle_timing(dims, g64, p64, max(1, min(v, args.cpu_sites) // 8), 1, 0, nthreads=1)
+        gf1, dt1, _, n1s, _ = oracle_timing(dims, g64, p64, max(1, min(v, 1 << 21) // 8), 1, 0, nthreads=1)
         cpu_baseline = {"value": gf, "unit": "GFLOP/s", "cores": cores, "nproc": os.cpu_count(), "kind": "oracle",
                         "seconds_per_application": dt,
                         "single_thread": {"value": gf1, "unit": "GFLOP/s", "seconds": dt1, "sites": int(n1s)},
@@ -697,6 +697,35 @@ def collect_variant_timings(args, lattices):
     return rows
 
 
+def run_costmodel_profile_one(args):
+    """--costmodel --profile-one: ONE costmodel_train launch of the paper's network size on seeded random data (F = 33,
+    n = 400 rows, 4 epochs of batch 16 = 100 updates, one model, cluster of 8) -- the command the ncu figures of
+    profiles/r01e_costmodel.md are taken from.  Prints the launch's time per update."""
+    import torch
+    from paper_2301_03636_b200 import costmodel as C
+    from paper_2301_03636_b200 import inputs
+    dev = torch.device("cuda:0")
+    f, n, epochs, batch = 33, 400, 4, 16
+    rng = np.random.default_rng([SEED, 33])
+    xs = torch.from_numpy(rng.standard_normal((n, f))).to(dev)
+    ys = torch.from_numpy(rng.standard_normal(n)).to(dev)
+    uni = torch.from_numpy(inputs.uniforms(SEED + 100, C.costmodel_weight_count(f))[None]).to(dev)
+    perms = torch.from_numpy(inputs.permutations(SEED + 100, epochs, n)[None]).to(dev)
+    model = C.CostModel(f)
+    updates = epochs * ((n + batch - 1) // batch)
+    ms = []
+    for _ in range(3):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        model.train(xs, ys, uni, perms, epochs=epochs, batch=batch, cluster_size=8)
+        e1.record()
+        torch.cuda.synchronize()
+        ms.append(e0.elapsed_time(e1))
+    print(json.dumps({"costmodel_profile_one": True, "f": f, "rows": n, "epochs": epochs, "batch": batch, "cluster": 8,
+                      "updates": updates, "ms_per_launch": ms, "us_per_update": min(ms) * 1e3 / updates}))
+    return 0
+
+
 def run_costmodel(args):
     """The cost-model half of the Advisor on this build's own measurements: 42 kernel variants x 10 lattices -> runtime;
     80 % / 20 % split, Z-score, the paper's MLP and optimiser settings, everything on the device through
@@ -987,7 +1016,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-parity", action="store_true", help="skip the whole-lattice parity check of the timed buffer")
     ap.add_argument("--repeats", type=int, default=5, help="K-step regions timed in all (median and min reported)")
-    ap.add_argument("--cpu-sites", type=int, default=1 << 21, help="sites the cpu_baseline oracle run covers")
+    ap.add_argument("--cpu-sites", type=int, default=0, help="sites the cpu_baseline oracle run covers (0: the whole lattice, which "
+                                                             "is also what the parity object needs)")
     ap.add_argument("--ref-sites", type=int, default=0, help="sites per step of --impl reference (0: the whole lattice)")
     ap.add_argument("--decomposition", choices=["replicas", "slab"], default="replicas",
                     help="multi-GPU mode: independent lattices per rank (default) or one lattice cut into T-slabs")
@@ -1004,6 +1034,7 @@ def main():
     ap.add_argument("--cg-max-iter", type=int, default=2000)
     ap.add_argument("--probe", action="store_true", help="read/write/copy/4:1-mix bandwidth and FP64 FMA rate of this board")
     ap.add_argument("--costmodel", action="store_true", help="fit the Advisor's cost model on the variants' measured runtimes")
+    ap.add_argument("--profile-one", action="store_true", help="with --costmodel: one training launch of the paper's network size")
     ap.add_argument("--costmodel-lattices", type=int, default=len(COSTMODEL_LATTICES))
     ap.add_argument("--costmodel-epochs", type=int, default=150)
     ap.add_argument("--costmodel-models", type=int, default=16, help="independent seeds trained in the same launch")
@@ -1017,7 +1048,7 @@ def main():
     if args.probe:
         return run_probe(args)
     if args.costmodel:
-        return run_costmodel(args)
+        return run_costmodel_profile_one(args) if args.profile_one else run_costmodel(args)
     if args.cg:
         return run_cg(args)
     if args.eo:

@@ -860,15 +860,13 @@ int dslash_tune(dslash_ctx* c, void* out, const void* in, const void* gauge, dsl
     float best_ms = 0.f;
     // DSLASH_TUNE_BURST: one short pass (2 warm-up + 8 timed applications per candidate, ~15 ms in all): the whole comparison
     // stays inside the board's boost window; a longer one would time the later candidates under the power cap and the earlier
-    // ones not.  DSLASH_TUNE_SUSTAINED: 600 applications first (the board leaves its boost window after ~35 ms; its clock keeps
-    // settling for another ~0.1 s), then three interleaved rounds of 5 + 30 applications per candidate, summed per candidate.
+    // ones not.  DSLASH_TUNE_SUSTAINED: every candidate is brought to ITS OWN steady state -- 300 applications of it (the board
+    // leaves its boost window after ~35 ms and its clock settles within ~0.1 s to the value that kernel's power draw allows),
+    // then 100 timed ones.  (Interleaving short windows of the candidates instead makes each inherit the clock the previous one
+    // left behind: measured, it picked the direct kernel at 0.400 ms where the marching kernel sustains 0.366 ms.)
     const bool sustained = c->tune_mode == DSLASH_TUNE_SUSTAINED;
     float total[5] = {0.f, 0.f, 0.f, 0.f, 0.f};
-    if (sustained) {
-        c->kernel = DSLASH_KERNEL_DIRECT;
-        for (int i = 0; i < 600 && rc == DSLASH_OK; ++i) rc = dslash_apply(c, out, in, gauge, stream);
-    }
-    const int rounds = sustained ? 3 : 1, warm = sustained ? 5 : 2, reps = sustained ? 30 : 8;
+    const int rounds = 1, warm = sustained ? 300 : 2, reps = sustained ? 100 : 8;
     for (int round = 0; round < rounds && rc == DSLASH_OK; ++round)
         for (int k = 0; k < ncand && rc == DSLASH_OK; ++k) {
             c->kernel = cand[k].kernel;
