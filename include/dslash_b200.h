@@ -420,7 +420,7 @@ DSLASH_API int dslash_get_option(const dslash_ctx *ctx, int option, int *value);
  * End-to-end application from HOST buffers in the canonical layout at the ctx's precision
  * (the path of PAPER.md:138-148: map to the device, run the kernel, map back):
  *   H2D copy of gauge and in -> pack -> apply -> unpack -> D2H copy of out, then `stream` is synchronised.
- *   The lattice is cut into up to 16 slabs of whole time slices and the three phases run on three internal streams (ordered
+ *   The lattice is cut into up to 32 slabs of whole time slices and the three phases run on three internal streams (ordered
  *   after the caller's earlier work on `stream`): slab k+1 travels to the device while slab k is packed, applied (direct
  *   kernel on the slab's time range) and unpacked and slab k-1 of `out` travels back, so both directions of the host link
  *   are busy.  Every byte crosses the link exactly once.  (A blocked-SoA lattice whose time slice is not a whole number of

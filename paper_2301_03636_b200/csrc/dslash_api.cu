@@ -29,7 +29,7 @@ struct dslash_ctx {
     void* d_nat[3];  // native gauge, in, out (alias d_can when the native layout is the canonical one)
     // dslash_apply_host pipelines t-slabs over three streams: host->device copies, pack + apply + unpack, device->host copies
     cudaStream_t host_stream[3];
-    cudaEvent_t host_event[2 * 16 + 2];  // [k]: slab k is on the device; [16 + k]: slab k of `out` is ready; [32], [33]: entry / exit
+    cudaEvent_t host_event[2 * 32 + 2];  // [k]: slab k is on the device; [32 + k]: slab k of `out` is ready; [64], [65]: entry / exit
     // workspace of dslash_cg_solve (device memory, owned): r, p, t, q spinors; reduction scratch; one result
     void* cg_vec[4];
     double* cg_scratch;
@@ -304,7 +304,7 @@ int dslash_create(dslash_ctx** ctx, const int dims[4], int precision, int layout
     c->last_cuda = 0;
     for (int i = 0; i < 3; ++i) c->d_can[i] = c->d_nat[i] = nullptr;
     for (int i = 0; i < 3; ++i) c->host_stream[i] = nullptr;
-    for (int i = 0; i < 34; ++i) c->host_event[i] = nullptr;
+    for (int i = 0; i < 66; ++i) c->host_event[i] = nullptr;
     for (int i = 0; i < 4; ++i) c->cg_vec[i] = nullptr;
     c->cg_scratch = nullptr;
     *ctx = c;
@@ -327,7 +327,7 @@ int dslash_destroy(dslash_ctx* c) {
         if (c->cg_scratch) cudaFree(c->cg_scratch);
         if (c->pipe_ctr) cudaFree(c->pipe_ctr);
         if (c->march_plan) cudaFree(c->march_plan);
-        for (int i = 0; i < 34; ++i)
+        for (int i = 0; i < 66; ++i)
             if (c->host_event[i]) cudaEventDestroy(c->host_event[i]);
         for (int i = 0; i < 3; ++i)
             if (c->host_stream[i]) cudaStreamDestroy(c->host_stream[i]);
@@ -943,7 +943,7 @@ int dslash_apply_host(dslash_ctx* c, void* out_host, const void* in_host, const 
             c->host_stream[i] = nullptr;
             return cuda_fail(c, e);
         }
-    for (int i = 0; i < 34; ++i)
+    for (int i = 0; i < 66; ++i)
         if (!c->host_event[i] && (e = cudaEventCreateWithFlags(&c->host_event[i], cudaEventDisableTiming)) != cudaSuccess) {
             c->host_event[i] = nullptr;
             return cuda_fail(c, e);
@@ -955,13 +955,13 @@ int dslash_apply_host(dslash_ctx* c, void* out_host, const void* in_host, const 
     // step with the copies, then NS-1 and 0.  Every byte crosses the link once: the byte counts are those of the serial path.
     const int LT = c->geom.L[3];
     const size_t slice = (size_t)c->geom.L[0] * c->geom.L[1] * c->geom.L[2];
-    int NS = LT < 16 ? LT : 16;
+    int NS = LT < 32 ? LT : 32;  // small slabs keep the tail short: the last two slabs of `out` travel back after everything else
     if (c->layout_base == LAYOUT_SOA && slice % VL != 0) NS = 1;  // slabs would not start on a vector boundary
     if (NS < 2 || !full_time_range(c)) NS = 1;
     const size_t rb = real_bytes(c), links = c->recon == 12 ? 12u : 18u;
     auto slab_t0 = [&](int k) { return (int)((long long)k * LT / NS); };
     cudaStream_t s_up = c->host_stream[0], s_run = c->host_stream[1], s_down = c->host_stream[2];
-    cudaEvent_t ev_entry = c->host_event[32], ev_exit = c->host_event[33];
+    cudaEvent_t ev_entry = c->host_event[64], ev_exit = c->host_event[65];
 #define HOST_TRY(call)                                           \
     do {                                                         \
         if ((e = (call)) != cudaSuccess) return cuda_fail(c, e); \
@@ -1017,8 +1017,8 @@ int dslash_apply_host(dslash_ctx* c, void* out_host, const void* in_host, const 
                 if ((er = launch_convert_spinor(c->precision, c->layout_base, dco + jo, dno + jo, (unsigned)jn, 1, s_run)) != cudaSuccess) return er;
                 c->launches += 1;
             }
-            if ((er = cudaEventRecord(c->host_event[16 + j], s_run)) != cudaSuccess) return er;
-            if ((er = cudaStreamWaitEvent(s_down, c->host_event[16 + j], 0)) != cudaSuccess) return er;
+            if ((er = cudaEventRecord(c->host_event[32 + j], s_run)) != cudaSuccess) return er;
+            if ((er = cudaStreamWaitEvent(s_down, c->host_event[32 + j], 0)) != cudaSuccess) return er;
             if ((er = cudaMemcpyAsync(ho + jo, dco + jo, jn * 24u * rb, cudaMemcpyDeviceToHost, s_down)) != cudaSuccess) return er;
             d2h += jn * 24u * rb;
             return cudaSuccess;

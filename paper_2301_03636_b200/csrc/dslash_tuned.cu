@@ -95,8 +95,13 @@ static cudaError_t launch_tuned_s(const LaunchArgs& a, const TileGeom& tg, const
             DSLASH_LAUNCH(128, 2);
         else
             DSLASH_LAUNCH(128, 3);
-    } else if (tpb <= 256)
-        DSLASH_LAUNCH(256, 1);
+    } else if (tpb <= 256) {
+        // fp32 fits 128 registers: two 256-thread blocks per SM (a bigger tile has less halo per site); fp64 needs the registers
+        if (sizeof(Real) == 4 && cfg.occupancy == 1)
+            DSLASH_LAUNCH(256, 2);
+        else
+            DSLASH_LAUNCH(256, 1);
+    }
     else if (tpb <= 512)
         DSLASH_LAUNCH(512, 1);
     else

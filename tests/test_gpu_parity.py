@@ -736,7 +736,7 @@ def test_error_paths_on_device(env):
 @pytest.mark.parametrize("layout,recon12", [("soa", False), ("soa", True), ("aos", False)])
 @pytest.mark.parametrize("dims,precision", [
     ((8, 6, 4, 10), "f64"),   # 10 slabs of one time slice (192 sites = 6 vectors) pipelined over three streams
-    ((32, 4, 4, 40), "f64"),  # 16 slabs of 2-3 slices
+    ((32, 4, 4, 40), "f64"),  # 32 slabs of 1-2 slices
     ((32, 4, 4, 40), "f32"),
     ((6, 3, 5, 4), "f64"),    # a slice of 90 sites is not a whole number of vectors: blocked SoA runs as one slab, AoS as 4
     ((4, 4, 4, 2), "f64"),    # two slabs: each one's neighbours in t are both the other one
