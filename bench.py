@@ -8,7 +8,7 @@
     python bench.py --costmodel                                     # the Advisor's cost model fitted on measured variant runtimes
     python bench.py --probe                                         # read/write/copy/4:1-mix bandwidth, FP64 FMA rate of this board
     python bench.py --cg | --eo | --decomposition slab              # solver, even-odd operator, multi-GPU slab form
-    python bench.py --kernel direct|wpipe|march ...                 # force a kernel instead of letting dslash_tune pick
+    python bench.py --kernel direct|wpipe|march|gmarch ...                 # force a kernel instead of letting dslash_tune pick
 
 A "step" is one application of D (one dslash_apply = one kernel launch covering SURVEY.md section 8(a)
 steps a1-a7) to one seeded synthetic lattice that is already resident in HBM in the native layout.  Before the timed
@@ -57,10 +57,11 @@ NCU_FIGURES = {
     "32x32x32x64_f64_soa_r18_wpipe": dict(traffic=2051962000, fp64_pipe_pct=None, source="profiles/r01f_wpipe.md"),
     "32x32x32x64_f64_soa_r18_march": dict(traffic=1995707392, fp64_pipe_pct=30.4, source="profiles/r02_march.md"),
 }
-KERNEL_NAMES = {"direct": "dslash_tuned_kernel", "wpipe": "dslash_wpipe_kernel", "march": "dslash_march_kernel"}
+KERNEL_NAMES = {"direct": "dslash_tuned_kernel", "wpipe": "dslash_wpipe_kernel", "march": "dslash_march_kernel",
+                "gmarch": "dslash_gmarch_kernel"}
 
 
-KERNEL_IDS = {1: "direct", 5: "wpipe", 6: "march"}  # DSLASH_KERNEL_*
+KERNEL_IDS = {1: "direct", 5: "wpipe", 6: "march", 7: "gmarch"}  # DSLASH_KERNEL_*
 
 
 def bytes_per_site(precision, recon12):
@@ -1002,7 +1003,7 @@ def main():
     ap.add_argument("--layout", choices=["soa", "aos"], default="soa")
     ap.add_argument("--tile", type=int, nargs=4, default=None, help="tile of the tuned kernel (x y z t)")
     ap.add_argument("--occupancy", type=int, default=None, help="DSLASH_OPT_OCCUPANCY override")
-    ap.add_argument("--kernel", choices=["auto", "direct", "wpipe", "march"], default=None)
+    ap.add_argument("--kernel", choices=["auto", "direct", "wpipe", "march", "gmarch"], default=None)
     ap.add_argument("--l2-policy", type=int, default=None, help="DSLASH_OPT_L2_POLICY bits")
     ap.add_argument("--march-lead", type=int, default=None, help="DSLASH_OPT_MARCH_LEAD")
     ap.add_argument("--no-tune", action="store_true", help="skip dslash_tune (keep the library's static default kernel)")

@@ -49,6 +49,10 @@ struct dslash_ctx {
     void* march_plan;
     int march_blocks, march_t0, march_t1;
     unsigned march_epoch;  // launches on the current plan (its progress counters accumulate)
+    // the same for the generalised marching kernel (any L_X): plan, its shape (warps, slots, shared-memory size), time range
+    void* gm_plan;
+    int gm_blocks, gm_t0, gm_t1;
+    GmShape gm_shape;
 };
 
 static int cuda_fail(dslash_ctx* c, cudaError_t e) {
@@ -228,6 +232,23 @@ static int ensure_kernel_resources(dslash_ctx* c, int kernel) {
         c->march_t1 = c->tg.t_end;
         c->march_epoch = 0;
     }
+    if (kernel == DSLASH_KERNEL_GMARCH && gmarch_eligible(c->precision, c->layout_base, c->recon, c->geom) &&
+        (!c->gm_plan || c->gm_t0 != c->tg.t_begin || c->gm_t1 != c->tg.t_end)) {
+        if (c->gm_plan && cudaDeviceSynchronize() != cudaSuccess) return cuda_fail(c, cudaGetLastError());  // a launch may still read it
+        cudaError_t e = gmarch_plan_create(c->precision, c->recon, c->geom, c->tg.t_begin, c->tg.t_end, c->device, &c->gm_plan, &c->gm_blocks,
+                                           &c->gm_shape);
+        if (e == cudaErrorInvalidValue) {  // no decomposition fits the shared memory of a block: the kernel cannot run this lattice
+            (void)cudaGetLastError();
+            c->gm_t0 = c->gm_t1 = -1;
+            return DSLASH_ERR_UNSUPPORTED;
+        }
+        if (e != cudaSuccess) {
+            (void)cudaGetLastError();
+            return cuda_fail(c, e);
+        }
+        c->gm_t0 = c->tg.t_begin;
+        c->gm_t1 = c->tg.t_end;
+    }
     return DSLASH_OK;
 }
 
@@ -297,6 +318,10 @@ int dslash_create(dslash_ctx** ctx, const int dims[4], int precision, int layout
     c->march_blocks = 0;
     c->march_t0 = c->march_t1 = -1;
     c->march_epoch = 0;
+    c->gm_plan = nullptr;
+    c->gm_blocks = 0;
+    c->gm_t0 = c->gm_t1 = -1;
+    c->gm_shape = GmShape{};
     c->cfg.march_lead = 0;
     c->tune_mode = DSLASH_TUNE_BURST;
     c->cfg.x_shuffle = precision == DSLASH_FP64 ? 1 : 0;  // measured: -1.3 % (burst) / -2 % (sustained) in fp64, +0.8 % in fp32
@@ -314,7 +339,7 @@ int dslash_create(dslash_ctx** ctx, const int dims[4], int precision, int layout
 int dslash_destroy(dslash_ctx* c) {
     if (!c) return DSLASH_OK;
     int rc = DSLASH_OK;
-    bool any = c->cg_scratch != nullptr || c->pipe_ctr != nullptr || c->march_plan != nullptr;
+    bool any = c->cg_scratch != nullptr || c->pipe_ctr != nullptr || c->march_plan != nullptr || c->gm_plan != nullptr;
     for (int i = 0; i < 3; ++i) any = any || c->d_can[i] || c->d_nat[i];
     for (int i = 0; i < 4; ++i) any = any || c->cg_vec[i];
     for (int i = 0; i < 6; ++i) any = any || c->eo_vec[i];
@@ -327,6 +352,7 @@ int dslash_destroy(dslash_ctx* c) {
         if (c->cg_scratch) cudaFree(c->cg_scratch);
         if (c->pipe_ctr) cudaFree(c->pipe_ctr);
         if (c->march_plan) cudaFree(c->march_plan);
+        if (c->gm_plan) cudaFree(c->gm_plan);
         for (int i = 0; i < 66; ++i)
             if (c->host_event[i]) cudaEventDestroy(c->host_event[i]);
         for (int i = 0; i < 3; ++i)
@@ -357,6 +383,8 @@ static int resolve_kernel(const dslash_ctx* c) {
     if (c->kernel == DSLASH_KERNEL_DIRECT) return DSLASH_KERNEL_DIRECT;
     if (c->kernel == DSLASH_KERNEL_WARP_PIPE) return wpipe_eligible(c->layout_base, c->geom) ? DSLASH_KERNEL_WARP_PIPE : -1;
     if (c->kernel == DSLASH_KERNEL_MARCH) return march_eligible(c->layout_base, c->geom) ? DSLASH_KERNEL_MARCH : -1;
+    if (c->kernel == DSLASH_KERNEL_GMARCH)
+        return gmarch_eligible(c->precision, c->layout_base, c->recon, c->geom) ? DSLASH_KERNEL_GMARCH : -1;
     return DSLASH_KERNEL_DIRECT;  // AUTO
 }
 
@@ -388,8 +416,10 @@ int dslash_apply(dslash_ctx* c, void* out, const void* in, const void* gauge, ds
         }
         if (k == DSLASH_KERNEL_MARCH && (!c->march_plan || c->march_t0 != c->tg.t_begin || c->march_t1 != c->tg.t_end))
             return DSLASH_ERR_UNSUPPORTED;
+        if (k == DSLASH_KERNEL_GMARCH && (!c->gm_plan || c->gm_t0 != c->tg.t_begin || c->gm_t1 != c->tg.t_end)) return DSLASH_ERR_UNSUPPORTED;
         e = (k == DSLASH_KERNEL_WARP_PIPE) ? launch_wpipe(c->precision, c->layout_base, c->recon, a, c->tg, c->cfg)
             : (k == DSLASH_KERNEL_MARCH)   ? launch_march(c->precision, c->layout_base, c->recon, a, c->march_plan, c->march_blocks, c->cfg, ++c->march_epoch)
+            : (k == DSLASH_KERNEL_GMARCH)  ? launch_gmarch(c->precision, c->layout_base, c->recon, a, c->gm_plan, c->gm_blocks, c->gm_shape, c->cfg)
                                            : launch_tuned(c->precision, c->layout_base, c->recon, a, c->tg, c->cfg);
     } else if (!full_time_range(c)) {
         return DSLASH_ERR_UNSUPPORTED;  // the variant kernels always sweep the whole lattice
@@ -812,7 +842,7 @@ int dslash_get_option(const dslash_ctx* c, int option, int* value) {
 int dslash_set_kernel(dslash_ctx* c, int kernel) {
     if (!c) return DSLASH_ERR_NULL;
     if (kernel != DSLASH_KERNEL_AUTO && kernel != DSLASH_KERNEL_DIRECT && kernel != DSLASH_KERNEL_WARP_PIPE &&
-        kernel != DSLASH_KERNEL_MARCH)
+        kernel != DSLASH_KERNEL_MARCH && kernel != DSLASH_KERNEL_GMARCH)
         return DSLASH_ERR_UNSUPPORTED;
     const int rc = ensure_kernel_resources(c, kernel);
     if (rc != DSLASH_OK) return rc;
@@ -843,6 +873,14 @@ int dslash_tune(dslash_ctx* c, void* out, const void* in, const void* gauge, dsl
     for (int k = 0; k < ncand; ++k) {
         const int rcr = ensure_kernel_resources(c, cand[k].kernel);
         if (rcr != DSLASH_OK) return rcr;
+    }
+    // lattices the L_X == 32 kernels cannot run: the generalised marching kernel, where a decomposition fits a block
+    if (!march_eligible(c->layout_base, c->geom) && gmarch_eligible(c->precision, c->layout_base, c->recon, c->geom)) {
+        const int rcr = ensure_kernel_resources(c, DSLASH_KERNEL_GMARCH);
+        if (rcr == DSLASH_OK)
+            cand[ncand++] = {DSLASH_KERNEL_GMARCH, 0, 0};
+        else if (rcr != DSLASH_ERR_UNSUPPORTED)
+            return rcr;
     }
     if (wpipe_eligible(c->layout_base, c->geom) && ensure_kernel_resources(c, DSLASH_KERNEL_WARP_PIPE) == DSLASH_OK) {
         cand[ncand++] = {DSLASH_KERNEL_WARP_PIPE, 2, 4};  // 8 warps x 2 stages in flight per SM (fp64, 18-real)

@@ -151,6 +151,31 @@ __device__ __forceinline__ void load_link_slot(cplx<Real> (&u)[9], const unsigne
     if (RECON == 12) reconstruct_row2(u);
 }
 
+// a 32-site vector of half-spinors (6 complex per site, component-major like the fields): the exchange buffers of the
+// marching kernels
+template <typename Real>
+__device__ __forceinline__ void store_half(unsigned char* p, unsigned lane, const cplx<Real> (&h)[6]) {
+    using V2 = typename vec2<Real>::type;
+    V2* q = reinterpret_cast<V2*>(p) + lane;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        V2 v;
+        v.x = h[k].re;
+        v.y = h[k].im;
+        q[k * VL] = v;
+    }
+}
+template <typename Real>
+__device__ __forceinline__ void load_half(cplx<Real> (&h)[6], const unsigned char* p, unsigned lane) {
+    using V2 = typename vec2<Real>::type;
+    const V2* q = reinterpret_cast<const V2*>(p) + lane;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        const V2 v = q[k * VL];
+        h[k] = {v.x, v.y};
+    }
+}
+
 // the two x hops from the row's own spinors and links (the arithmetic of x_hops_shuffle with the operands in registers)
 template <typename Real>
 __device__ __forceinline__ void x_hops_regs(cplx<Real> (&acc)[12], const cplx<Real> (&psi)[12], const cplx<Real> (&u)[9],

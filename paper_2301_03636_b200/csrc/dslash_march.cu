@@ -77,29 +77,6 @@ struct MarchSmem {
     static_assert(PSI % 256u == 0 && LINK % 256u == 0, "stage tables hold offsets in units of 256 bytes");
 };
 
-template <typename Real>
-__device__ __forceinline__ void store_half(unsigned char* p, unsigned lane, const cplx<Real> (&h)[6]) {
-    using V2 = typename vec2<Real>::type;
-    V2* q = reinterpret_cast<V2*>(p) + lane;
-#pragma unroll
-    for (int k = 0; k < 6; ++k) {
-        V2 v;
-        v.x = h[k].re;
-        v.y = h[k].im;
-        q[k * VL] = v;
-    }
-}
-template <typename Real>
-__device__ __forceinline__ void load_half(cplx<Real> (&h)[6], const unsigned char* p, unsigned lane) {
-    using V2 = typename vec2<Real>::type;
-    const V2* q = reinterpret_cast<const V2*>(p) + lane;
-#pragma unroll
-    for (int k = 0; k < 6; ++k) {
-        const V2 v = q[k * VL];
-        h[k] = {v.x, v.y};
-    }
-}
-
 // State of one compute warp.  Every member is warp-uniform except `lane`.
 template <typename Real, int RECON, int NLS>
 struct MarchWarp {

@@ -1,0 +1,143 @@
+"""GPU parity of the generalised marching kernel (DSLASH_KERNEL_GMARCH, csrc/dslash_gmarch.cu): any x extent whose rows tile
+whole 32-site vectors.  Every case is compared with the CPU oracle element by element (FP64 1e-12, FP32 1e-5, BASELINE.json
+north_star) AND bit for bit with the direct kernel (same per-hop arithmetic, same order of the sum: a race or a wrong source
+lane shows up as differing bits)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f64": 1e-12, "f32": 1e-5}
+SEED = 230103636
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    import oracle
+    from paper_2301_03636_b200 import binding, checks, device, inputs
+    assert torch.cuda.is_available()
+
+    class E:
+        pass
+    e = E()
+    e.torch, e.oracle, e.B, e.checks, e.device, e.inputs = torch, oracle, binding, checks, device, inputs
+    return e
+
+
+_CACHE = {}
+
+
+def fields_and_ref(env, dims, seed, precision):
+    key = (tuple(dims), seed, precision)
+    if key not in _CACHE:
+        _CACHE.clear()
+        g, p = env.inputs.fields(dims, seed, precision)
+        ref = env.oracle.dslash(env.inputs.promote(p), env.inputs.promote(g), dims)
+        _CACHE[key] = (g, p, ref)
+    return _CACHE[key]
+
+
+GM_DIMS = [
+    (16, 4, 2, 4),       # two rows per vector: half of the y neighbours sit in the warp's own vector
+    (16, 16, 16, 16),    # BASELINE.json configs[1]
+    (8, 8, 4, 3),        # four rows per vector
+    (4, 8, 1, 3),        # eight rows per vector, L_Z = 1 (a vector is its own z neighbour)
+    (2, 16, 3, 2),       # L_X = 2: x+1 == x-1
+    (48, 4, 2, 3),       # a vector is 2/3 of a row: x and y neighbours spread over three / two vectors; y wraps inside two units
+    (48, 8, 6, 4),
+    (24, 8, 4, 5),       # a vector is 4/3 of a row (units of 4 rows)
+    (24, 24, 24, 4),     # the plane of BASELINE.json configs[4]
+    (64, 4, 4, 3),       # a row is two vectors
+    (40, 8, 4, 4),       # lcm(40, 32) = 160: units of five vectors
+    (32, 4, 4, 8),       # L_X = 32: the case of DSLASH_KERNEL_MARCH, here with x hops through shared memory
+    (32, 16, 12, 9),
+    (96, 2, 2, 2),       # a row is three vectors, y+1 == y-1, z+1 == z-1
+]
+
+
+@pytest.mark.parametrize("dims", GM_DIMS)
+@pytest.mark.parametrize("precision", ["f64", "f32"])
+@pytest.mark.parametrize("recon12", [False, True])
+def test_gmarch_matches_the_oracle_and_the_direct_kernel_bit_for_bit(env, dims, precision, recon12):
+    B = env.B
+    g, p, ref = fields_and_ref(env, dims, SEED + 37, precision)
+    with env.device.Lattice(dims, precision, "soa", recon12) as lat:
+        gi, pi, o = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
+        lat.apply(o, pi, gi)
+        direct = lat.download_spinor(o)
+        lat.set_kernel("gmarch")
+        assert B.dslash_get_kernel(lat.ctx) == B.DSLASH_KERNEL_GMARCH
+        o.fill_(0x7f)  # a site the kernel forgot to store would stay garbage
+        n0 = B.dslash_launch_count(lat.ctx)
+        lat.apply(o, pi, gi)
+        assert B.dslash_launch_count(lat.ctx) == n0 + 1
+        got = lat.download_spinor(o)
+        assert env.checks.parity_error(got, ref) <= TOL[precision]
+        assert np.array_equal(got, direct)
+        for _ in range(3):  # repeated applications on the same context give the same bits
+            o.fill_(0x7f)
+            lat.apply(o, pi, gi)
+            assert np.array_equal(lat.download_spinor(o), direct)
+        lt = dims[3]
+        for t0, t1 in [(1, lt - 1), (0, 1), (lt - 1, lt), (lt // 2, lt)]:  # time ranges: only their slices are written
+            if not (0 <= t0 < t1 <= lt):
+                continue
+            B.dslash_set_time_range(lat.ctx, t0, t1)
+            o.zero_()
+            lat.apply(o, pi, gi)
+            part = lat.download_spinor(o)
+            assert np.array_equal(part[t0:t1], direct[t0:t1]), (t0, t1)
+            assert not part[:t0].any() and not part[t1:].any(), (t0, t1)
+
+
+def test_gmarch_refuses_what_it_cannot_run(env):
+    B = env.B
+    for dims, layout in [((48, 4, 4, 4), "aos"),   # AoS has no contiguous vectors
+                         ((48, 3, 4, 4), "soa"),   # L_X * L_Y is not a multiple of 32: vectors straddle z planes
+                         ((33, 32, 2, 2), "soa")]:  # lcm(33, 32): a unit of 33 vectors
+        with env.device.Lattice(dims, "f32", layout, False) as lat:
+            lat.set_kernel("gmarch")
+            o, p, g = lat.new_spinor(), lat.new_spinor(), lat.new_gauge()
+            assert B.dslash_apply_status(lat.ctx, o.data_ptr(), p.data_ptr(), g.data_ptr()) == B.DSLASH_ERR_UNSUPPORTED, dims
+            lat.set_kernel("auto")
+            assert B.dslash_apply_status(lat.ctx, o.data_ptr(), p.data_ptr(), g.data_ptr()) == B.DSLASH_OK
+
+
+def test_gmarch_many_launches_on_a_side_stream_are_bit_stable(env):
+    """200 back-to-back launches on a non-blocking stream, every result compared bit for bit (the kind of test that found the
+    async-proxy refill race of round 1)."""
+    B, torch = env.B, env.torch
+    dims = (48, 8, 6, 6)
+    g, p, ref = fields_and_ref(env, dims, SEED + 41, "f32")
+    with env.device.Lattice(dims, "f32", "soa", False) as lat:
+        gi, pi = lat.upload_gauge(g), lat.upload_spinor(p)
+        o0 = lat.new_spinor()
+        lat.apply(o0, pi, gi)
+        torch.cuda.synchronize()
+        lat.set_kernel("gmarch")
+        st = torch.cuda.Stream()
+        outs = [lat.new_spinor() for _ in range(8)]
+        bad = 0
+        for rep in range(25):
+            for o in outs:
+                B.dslash_apply(lat.ctx, o.data_ptr(), pi.data_ptr(), gi.data_ptr(), st.cuda_stream)
+            st.synchronize()
+            bad += sum(0 if torch.equal(o, o0) else 1 for o in outs)
+        assert bad == 0
+        assert env.checks.parity_error(lat.download_spinor(outs[0]), ref) <= TOL["f32"]
+
+
+def test_tune_considers_gmarch_when_lx_is_not_32(env):
+    B = env.B
+    dims = (48, 8, 8, 8)
+    g, p, ref = fields_and_ref(env, dims, SEED + 43, "f32")
+    with env.device.Lattice(dims, "f32", "soa", False) as lat:
+        gi, pi, o = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
+        chosen, ms = B.dslash_tune(lat.ctx, o.data_ptr(), pi.data_ptr(), gi.data_ptr(), lat.stream())
+        assert ms > 0
+        assert chosen in (B.DSLASH_KERNEL_DIRECT, B.DSLASH_KERNEL_GMARCH)
+        assert env.checks.parity_error(lat.download_spinor(o), ref) <= TOL["f32"]
+        o.fill_(0x7f)
+        lat.apply(o, pi, gi)
+        assert env.checks.parity_error(lat.download_spinor(o), ref) <= TOL["f32"]
