@@ -217,6 +217,8 @@ def lattice_options(B, lat, args):
         B.dslash_set_option(lat.ctx, B.DSLASH_OPT_L2_POLICY, args.l2_policy)
     if args.march_lead is not None:
         B.dslash_set_option(lat.ctx, B.DSLASH_OPT_MARCH_LEAD, args.march_lead)
+    if args.march_units is not None:
+        B.dslash_set_option(lat.ctx, B.DSLASH_OPT_MARCH_UNITS, args.march_units)
     if args.pipe_slots is not None:
         B.dslash_set_option(lat.ctx, B.DSLASH_OPT_PIPE_SLOTS, args.pipe_slots)
     if args.pipe_warps is not None:
@@ -1000,12 +1002,16 @@ def main():
     ap.add_argument("--heat-steps", type=int, default=1500)
     ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
     ap.add_argument("--config", choices=sorted(CONFIGS), default="3")
+    ap.add_argument("--dims", type=int, nargs=4, default=None, help="override the lattice of --config (x y z t): an off-contract "
+                                                                    "workload for kernel comparisons, named as such in the line")
+    ap.add_argument("--precision", choices=["f64", "f32"], default=None, help="override the precision of --config (same remark)")
     ap.add_argument("--layout", choices=["soa", "aos"], default="soa")
     ap.add_argument("--tile", type=int, nargs=4, default=None, help="tile of the tuned kernel (x y z t)")
     ap.add_argument("--occupancy", type=int, default=None, help="DSLASH_OPT_OCCUPANCY override")
     ap.add_argument("--kernel", choices=["auto", "direct", "wpipe", "march", "gmarch"], default=None)
     ap.add_argument("--l2-policy", type=int, default=None, help="DSLASH_OPT_L2_POLICY bits")
     ap.add_argument("--march-lead", type=int, default=None, help="DSLASH_OPT_MARCH_LEAD")
+    ap.add_argument("--march-units", type=int, default=None, help="DSLASH_OPT_MARCH_UNITS (gmarch kernel: cap on the units per block)")
     ap.add_argument("--no-tune", action="store_true", help="skip dslash_tune (keep the library's static default kernel)")
     ap.add_argument("--pipe-slots", type=int, default=None, help="DSLASH_OPT_PIPE_SLOTS override (wpipe kernel)")
     ap.add_argument("--pipe-warps", type=int, default=None, help="DSLASH_OPT_PIPE_WARPS override (wpipe kernel)")
@@ -1054,7 +1060,11 @@ def main():
         return run_cg(args)
     if args.eo:
         return run_eo(args)
-    cfg = CONFIGS[args.config]
+    cfg = dict(CONFIGS[args.config])
+    if args.dims or args.precision:
+        cfg["dims"] = tuple(args.dims) if args.dims else cfg["dims"]
+        cfg["precision"] = args.precision or cfg["precision"]
+        cfg["name"] = "off-contract: %s %s (--dims / --precision override of config %s)" % ("x".join(map(str, cfg["dims"])), cfg["precision"], args.config)
     if args.impl == "reference":
         return run_reference(args, cfg)
     if args.decomposition == "slab":

@@ -117,8 +117,9 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
                                   vectors) that are neighbours in the (y,z) plane; x and y neighbours are lane-shifted and spread
                                   over up to three vectors, so every hop is resolved through a host-built plan (source vectors
                                   + lane masks) and x hops go through shared memory like y and z hops
-                                  (blocked SoA, L_X * L_Y a multiple of 32, a unit of <= 12 (FP32) / <= 6 (FP64) vectors);
-                                  bit-identical to DSLASH_KERNEL_DIRECT */
+                                  (blocked SoA, L_X * L_Y a multiple of 32, a unit of <= 12 (FP32) / <= 8 (FP64) vectors);
+                                  bit-identical to DSLASH_KERNEL_DIRECT.  Opt-in only: measured 2.4-2.9 x slower than _DIRECT
+                                  (profiles/r02b_gmarch.md), dslash_tune() does not consider it */
 
 /* options of the tuned kernels, dslash_set_option() */
 #define DSLASH_OPT_OCCUPANCY 2        /* blocks of <= 128 threads: 0 = 168 registers/thread (12 warps/SM), 1 = 128 (16 warps),
@@ -146,6 +147,9 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
                                          the L2 reuse distance of the t hops (48^3x96 fp32: HBM reads 1.26 x -> see profiles/) */
 #define DSLASH_OPT_TUNE_MODE 10       /* what dslash_tune() optimises: DSLASH_TUNE_BURST (default; the first ~35 ms after idle, board at its
                                          boost clock) or DSLASH_TUNE_SUSTAINED (continuous load, board at its power-capped clock) */
+#define DSLASH_OPT_MARCH_UNITS 12     /* generalised marching kernel: most units (of lcm(L_X, 32) sites) a block may own, 0 (default) = as
+                                         many as fit; fewer units leave shared memory for more link / halo slots per warp.  The block
+                                         plan is rebuilt by the call (synchronous) when DSLASH_KERNEL_GMARCH is selected */
 #define DSLASH_OPT_MARCH_LEAD 11      /* marching kernel: steps a block may run ahead of the slowest block of its chunk, 0..16
                                          (0 = unbounded).  Blocks that stay close share their halo rows through L2 */
 #define DSLASH_TUNE_BURST 0
@@ -321,7 +325,7 @@ DSLASH_API int dslash_march_stats(dslash_ctx *ctx, unsigned *stats, size_t capac
 /*
  * Pick the kernel by measurement (the Advisor's own method, applied to the library's kernels): every kernel
  * that can run this context (DSLASH_KERNEL_DIRECT; where eligible DSLASH_KERNEL_MARCH and DSLASH_KERNEL_WARP_PIPE in
- * three slot/warp configurations, or DSLASH_KERNEL_GMARCH when L_X != 32) is timed on the caller's buffers
+ * three slot/warp configurations; not DSLASH_KERNEL_GMARCH, which loses to _DIRECT on every lattice measured) is timed on the caller's buffers
  * (2 warm-up + 8 timed applications each, CUDA events on `stream`; about 15 ms in all, so that every candidate is
  * timed inside the board's boost window -- call it on an idle device; with DSLASH_OPT_TUNE_MODE = DSLASH_TUNE_SUSTAINED:
  * every candidate runs 300 applications to reach its own power-capped steady state, then 100 timed ones, ~0.8 s in all) and the fastest becomes the

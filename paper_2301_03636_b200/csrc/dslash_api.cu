@@ -235,8 +235,8 @@ static int ensure_kernel_resources(dslash_ctx* c, int kernel) {
     if (kernel == DSLASH_KERNEL_GMARCH && gmarch_eligible(c->precision, c->layout_base, c->recon, c->geom) &&
         (!c->gm_plan || c->gm_t0 != c->tg.t_begin || c->gm_t1 != c->tg.t_end)) {
         if (c->gm_plan && cudaDeviceSynchronize() != cudaSuccess) return cuda_fail(c, cudaGetLastError());  // a launch may still read it
-        cudaError_t e = gmarch_plan_create(c->precision, c->recon, c->geom, c->tg.t_begin, c->tg.t_end, c->device, &c->gm_plan, &c->gm_blocks,
-                                           &c->gm_shape);
+        cudaError_t e = gmarch_plan_create(c->precision, c->recon, c->geom, c->tg.t_begin, c->tg.t_end, c->device, c->cfg.march_units,
+                                           &c->gm_plan, &c->gm_blocks, &c->gm_shape);
         if (e == cudaErrorInvalidValue) {  // no decomposition fits the shared memory of a block: the kernel cannot run this lattice
             (void)cudaGetLastError();
             c->gm_t0 = c->gm_t1 = -1;
@@ -323,6 +323,7 @@ int dslash_create(dslash_ctx** ctx, const int dims[4], int precision, int layout
     c->gm_t0 = c->gm_t1 = -1;
     c->gm_shape = GmShape{};
     c->cfg.march_lead = 0;
+    c->cfg.march_units = 0;
     c->tune_mode = DSLASH_TUNE_BURST;
     c->cfg.x_shuffle = precision == DSLASH_FP64 ? 1 : 0;  // measured: -1.3 % (burst) / -2 % (sustained) in fp64, +0.8 % in fp32
     c->launches = 0;
@@ -814,6 +815,14 @@ int dslash_set_option(dslash_ctx* c, int option, int value) {
             if (value != 0 && value != 1 && value != 2 && value != 4) return DSLASH_ERR_UNSUPPORTED;
             c->cfg.pipe_warps = value;
             return DSLASH_OK;
+        case DSLASH_OPT_MARCH_UNITS:
+            if (value < 0 || value > GM_NW_MAX) return DSLASH_ERR_UNSUPPORTED;
+            if (value != c->cfg.march_units) {
+                c->cfg.march_units = value;
+                c->gm_t0 = c->gm_t1 = -1;  // the plan no longer matches: rebuilt now if the kernel is selected, else when it is
+                if (c->kernel == DSLASH_KERNEL_GMARCH) return ensure_kernel_resources(c, c->kernel);
+            }
+            return DSLASH_OK;
         case DSLASH_OPT_MARCH_LEAD:
             if (value < 0 || value > 16) return DSLASH_ERR_UNSUPPORTED;
             c->cfg.march_lead = value;
@@ -833,6 +842,7 @@ int dslash_get_option(const dslash_ctx* c, int option, int* value) {
         case DSLASH_OPT_PIPE_SLOTS: *value = c->cfg.pipe_slots; return DSLASH_OK;
         case DSLASH_OPT_PIPE_WARPS: *value = c->cfg.pipe_warps; return DSLASH_OK;
         case DSLASH_OPT_MARCH_LEAD: *value = c->cfg.march_lead; return DSLASH_OK;
+        case DSLASH_OPT_MARCH_UNITS: *value = c->cfg.march_units; return DSLASH_OK;
         case DSLASH_OPT_PIPE_ZBLOCK: *value = c->cfg.pipe_zblock; return DSLASH_OK;
         case DSLASH_OPT_TUNE_MODE: *value = c->tune_mode; return DSLASH_OK;
         default: return DSLASH_ERR_UNSUPPORTED;
@@ -874,14 +884,9 @@ int dslash_tune(dslash_ctx* c, void* out, const void* in, const void* gauge, dsl
         const int rcr = ensure_kernel_resources(c, cand[k].kernel);
         if (rcr != DSLASH_OK) return rcr;
     }
-    // lattices the L_X == 32 kernels cannot run: the generalised marching kernel, where a decomposition fits a block
-    if (!march_eligible(c->layout_base, c->geom) && gmarch_eligible(c->precision, c->layout_base, c->recon, c->geom)) {
-        const int rcr = ensure_kernel_resources(c, DSLASH_KERNEL_GMARCH);
-        if (rcr == DSLASH_OK)
-            cand[ncand++] = {DSLASH_KERNEL_GMARCH, 0, 0};
-        else if (rcr != DSLASH_ERR_UNSUPPORTED)
-            return rcr;
-    }
+    // DSLASH_KERNEL_GMARCH is NOT a candidate: measured on every lattice it can run (profiles/r02b_gmarch.md: 48^3x96 fp32
+    // 2.36 ms against 0.91 ms, 24^4 fp64 0.148 against 0.062 ms) it is 2.4-2.9 x slower than the direct kernel, and timing it
+    // here would only heat the board before the caller's own measurement.  It stays selectable with dslash_set_kernel().
     if (wpipe_eligible(c->layout_base, c->geom) && ensure_kernel_resources(c, DSLASH_KERNEL_WARP_PIPE) == DSLASH_OK) {
         cand[ncand++] = {DSLASH_KERNEL_WARP_PIPE, 2, 4};  // 8 warps x 2 stages in flight per SM (fp64, 18-real)
         cand[ncand++] = {DSLASH_KERNEL_WARP_PIPE, 3, 1};  // 6 warps x 3 stages

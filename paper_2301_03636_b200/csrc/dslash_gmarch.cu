@@ -35,6 +35,9 @@ namespace dslash {
 namespace {
 
 constexpr unsigned GM_TAB = 12u;  // stage-table entries per copy queue
+#ifndef GM_IDLE_NS
+#define GM_IDLE_NS 200
+#endif
 
 // Shared-memory map of a block (all run-time: NW, NLS, NHS, NWB depend on the lattice).  Barrier fields are indices into the
 // uint64 array at offset 0, the others byte offsets.
@@ -97,6 +100,7 @@ struct GmWarp {
     const GmLayout* L;     // the kernel parameter (constant bank)
     const GmWarpPlan* wp;  // this warp's plan (shared memory)
     unsigned lane, w;
+    bool late;             // late ring fill (DSLASH_OPT_L2_POLICY bit 16): see read_own()
     int step;              // current step i
     int lslot, hslot;      // slot of the next link / halo stage to consume
     unsigned lphase, hphase;  // parity of the next completion, bit s = slot s
@@ -140,7 +144,7 @@ struct GmWarp {
             const int id = wp->f[D][e].id;
             const bool pred = (wp->f[D][e].mask >> lane) & 1u;
             if (id >= 0)
-                read_ring(psi, (unsigned)(id & 0xff), 0, ((id >> 8) & 1) != 0, ln, pred);
+                read_ring(psi, (unsigned)(id & 0xff), 0, ((id >> 8) & 1) != 0 && (late || (unsigned)(id & 0xff) != w), ln, pred);
             else
                 fetch_halo(psi, ln, pred);
         }
@@ -171,9 +175,13 @@ struct GmWarp {
         }
     }
     // The warp's own spinors of the current slice.  They are NOT kept in registers across the step (48 registers in fp64) but
-    // re-read from the ring row where needed.  The row may already have been handed back by then (`done`, at the warp's last
-    // FORWARD read): its slot is refilled with slice step + 2, and that fill is issued only after every reader of slice
-    // step + 1 -- this warp among them, during the NEXT step -- is done (gm_producer), so the row outlives the step.
+    // re-read from the ring row where needed, the last time in the t phase.  Two ways to hand the row back:
+    //   late fill (bit 16 of DSLASH_OPT_L2_POLICY, default): at the warp's last FORWARD read, as in dslash_march.cu.  The slot
+    //     is refilled with slice step + 2, and that fill is issued only after every reader of slice step + 1 -- this warp
+    //     among them, during the NEXT step -- is done (gm_producer), so the row outlives the step although it was handed back;
+    //   early fill: at the t-phase read, the warp's last read of the row; the refill may then start a whole step before it
+    //     is needed (more time for the copy, but the owner's fetch and the neighbouring blocks' halo fetches of the same
+    //     vector drift a step apart in L2).
     __device__ __forceinline__ void read_own(cplx<Real> (&own)[12], bool done) const { read_ring(own, w, 0, done, lane, true); }
     // w_MU of the warp's own sites for the neighbours that sit in this block
     template <int MU>
@@ -281,10 +289,11 @@ __device__ __forceinline__ void gm_producer(unsigned char* smem, const unsigned 
     while (__any_sync(0xffffffffu, q < total)) {
         bool ready = false;
         if (q < total) ready = round == 0 || mbar_test(bars + bar_empty + (unsigned)slot * bar_stride, ((unsigned)round - 1u) & 1u);
-        // late ring fill (dslash_march.cu's bit 16; here ALWAYS): hold the fill of slice q back until the readers of slice q - 1
-        // are done, so that the owner's fetch and the neighbouring blocks' halo fetches of the same vector are about one step
-        // apart -- and so that the slot it overwrites (slice q - 2) is no longer re-read by its owner (GmWarp::read_own)
-        if (ready && kind == 2u && q >= 2)
+        // late ring fill (bit 16, dslash_march.cu): hold the fill of slice q back until the readers of slice q - 1 are done, so
+        // that the owner's fetch and the neighbouring blocks' halo fetches of the same vector are about one step apart -- and
+        // so that the slot it overwrites (slice q - 2), handed back early in this mode, is no longer re-read by its owner
+        // (GmWarp::read_own)
+        if (ready && kind == 2u && (hints & 16) && q >= 2)
             ready = mbar_test(bars + bar_empty + (unsigned)(slot ^ 1) * bar_stride, (((unsigned)q - 1u) >> 1) & 1u);
         if (ready) {
             int ts = t0 + i;
@@ -309,7 +318,9 @@ __device__ __forceinline__ void gm_producer(unsigned char* smem, const unsigned 
                 ++round;
             }
         }
-        if (!__any_sync(0xffffffffu, ready)) __nanosleep(32);
+        // nothing to issue: sleep.  ncu on 48^3x96 fp32: with 32 ns the four producer warps executed 40 % of the block's
+        // instructions, and the compute warps (three per scheduler) are bound by instruction issue
+        if (!__any_sync(0xffffffffu, ready)) __nanosleep(GM_IDLE_NS);
     }
 }
 
@@ -363,6 +374,7 @@ __global__ void __launch_bounds__(128 * (1 + CWG), 1)
     m.wp = &bp.w[w];
     m.lane = lane;
     m.w = w;
+    m.late = (hints & 16) != 0;
     m.lslot = 0;
     m.hslot = 0;
     m.lphase = 0u;
@@ -397,7 +409,7 @@ __global__ void __launch_bounds__(128 * (1 + CWG), 1)
         {
             cplx<Real> u[9], psi[12], h[6], hp[6];
             m.fetch_link(u, lane);
-            m.template publish<0>(u, m.wp->own_done != 0);
+            m.template publish<0>(u, m.wp->own_done != 0 && m.late);
             m.template gather_fwd<0>(psi, lane_xf);
             project<0, -1>(h, psi);
             su3_mul<false>(hp, u, h);
@@ -420,7 +432,7 @@ __global__ void __launch_bounds__(128 * (1 + CWG), 1)
             reconstruct_accumulate<3, +1, false>(acc, wt);
             {
                 cplx<Real> own[12];
-                m.read_own(own, false);
+                m.read_own(own, !m.late);
                 project<3, +1>(h, own);
             }
             su3_mul<true>(wt, u, h);
@@ -656,11 +668,11 @@ bool gmarch_eligible(int precision, int layout_base, int recon, const Geom& g) {
     if ((g.L[0] * g.L[1]) % (int)VL != 0) return false;
     const GmGeom q = gm_geom(g);
     // a unit must fit the compute warps of a block: 8 at 232 registers (fp64), 12 at 152 (fp32)
-    return q.nvu <= (precision == 0 ? 6 : GM_NW_MAX);
+    return q.nvu <= (precision == 0 ? 8 : GM_NW_MAX);
 }
 
-int gmarch_plan_build(int precision, int recon, const Geom& g, int t_begin, int t_end, int wave, GmShape* shape, GmBlockPlan* plan_out,
-                      size_t capacity_blocks) {
+int gmarch_plan_build(int precision, int recon, const Geom& g, int t_begin, int t_end, int wave, int max_units, GmShape* shape,
+                      GmBlockPlan* plan_out, size_t capacity_blocks) {
     const int NT = t_end - t_begin;
     if (NT < 1 || wave < 1 || !gmarch_eligible(precision, LAYOUT_SOA, recon, g)) return 0;
     const GmGeom q = gm_geom(g);
@@ -670,7 +682,9 @@ int gmarch_plan_build(int precision, int recon, const Geom& g, int t_begin, int 
     double best = 0.0;
     GmShape bs{};
     std::vector<GmBlockPlan> best_plan, plan;
-    for (int ub = nw_cap / q.nvu; ub >= 1; --ub) {
+    int ub_max = nw_cap / q.nvu;
+    if (max_units > 0) ub_max = std::min(ub_max, max_units);
+    for (int ub = ub_max; ub >= 1; --ub) {
         int S = 0, G = 1;
         const double cost = gm_shape(q.NU, q.nvu, NT, ub, wave, &S, &G);
         if (best != 0.0 && cost >= best * 0.999) continue;
@@ -680,9 +694,9 @@ int gmarch_plan_build(int precision, int recon, const Geom& g, int t_begin, int 
         GmLayout L = gm_layout(precision, recon, NW, 2, 1, nwb);
         if (L.total > GM_SMEM_MAX) continue;
         int NLS = 2, NHS = 1;
-        // more data in flight while shared memory lasts: third link slot, second halo slot, fourth link slot
-        const int try_l[3] = {3, 3, 4}, try_h[3] = {1, 2, 2};
-        for (int k = 0; k < 3; ++k) {
+        // more data in flight while shared memory lasts: third link slot, second halo slot, fourth link slot, third halo slot
+        const int try_l[4] = {3, 3, 4, 4}, try_h[4] = {1, 2, 2, 3};
+        for (int k = 0; k < 4; ++k) {
             L = gm_layout(precision, recon, NW, try_l[k], try_h[k], nwb);
             if (L.total > GM_SMEM_MAX) break;
             NLS = try_l[k];
@@ -710,8 +724,8 @@ int gmarch_plan_build(int precision, int recon, const Geom& g, int t_begin, int 
     return (int)best_plan.size();
 }
 
-cudaError_t gmarch_plan_create(int precision, int recon, const Geom& g, int t_begin, int t_end, int device, void** d_plan, int* nblocks,
-                               GmShape* shape) {
+cudaError_t gmarch_plan_create(int precision, int recon, const Geom& g, int t_begin, int t_end, int device, int max_units, void** d_plan,
+                               int* nblocks, GmShape* shape) {
     int sms = 0;
     cudaError_t e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
     if (e != cudaSuccess) return e;
@@ -720,10 +734,10 @@ cudaError_t gmarch_plan_create(int precision, int recon, const Geom& g, int t_be
         *d_plan = nullptr;
     }
     *nblocks = 0;
-    const int nb = gmarch_plan_build(precision, recon, g, t_begin, t_end, sms, shape, nullptr, 0);
+    const int nb = gmarch_plan_build(precision, recon, g, t_begin, t_end, sms, max_units, shape, nullptr, 0);
     if (nb < 1) return cudaErrorInvalidValue;
     std::vector<GmBlockPlan> plan((size_t)nb);
-    if (gmarch_plan_build(precision, recon, g, t_begin, t_end, sms, shape, plan.data(), plan.size()) != nb) return cudaErrorInvalidValue;
+    if (gmarch_plan_build(precision, recon, g, t_begin, t_end, sms, max_units, shape, plan.data(), plan.size()) != nb) return cudaErrorInvalidValue;
     if ((e = cudaMalloc(d_plan, plan.size() * sizeof(GmBlockPlan))) != cudaSuccess) {
         *d_plan = nullptr;
         return e;
@@ -781,7 +795,7 @@ extern "C" int dslash_gmarch_plan(const int dims[4], int precision, int recon, i
     if (t_begin < 0 || t_end > dims[3] || t_begin >= t_end || wave < 1) return DSLASH_ERR_UNSUPPORTED;
     if (!dslash::gmarch_eligible(precision, dslash::LAYOUT_SOA, recon, g)) return DSLASH_ERR_UNSUPPORTED;
     dslash::GmShape sh{};
-    const int nb = dslash::gmarch_plan_build(precision, recon, g, t_begin, t_end, wave, &sh, nullptr, 0);
+    const int nb = dslash::gmarch_plan_build(precision, recon, g, t_begin, t_end, wave, 0, &sh, nullptr, 0);
     if (nb < 1) return DSLASH_ERR_UNSUPPORTED;
     *nblocks = nb;
     if (shape) {
@@ -792,7 +806,7 @@ extern "C" int dslash_gmarch_plan(const int dims[4], int precision, int recon, i
         const size_t per = sizeof(dslash::GmBlockPlan) / sizeof(int);
         if (capacity_ints < per * (size_t)nb) return DSLASH_ERR_UNSUPPORTED;
         std::vector<dslash::GmBlockPlan> plan((size_t)nb);
-        if (dslash::gmarch_plan_build(precision, recon, g, t_begin, t_end, wave, &sh, plan.data(), plan.size()) != nb) return DSLASH_ERR_UNSUPPORTED;
+        if (dslash::gmarch_plan_build(precision, recon, g, t_begin, t_end, wave, 0, &sh, plan.data(), plan.size()) != nb) return DSLASH_ERR_UNSUPPORTED;
         std::copy(reinterpret_cast<const int*>(plan.data()), reinterpret_cast<const int*>(plan.data()) + per * (size_t)nb, ints);
     }
     return DSLASH_OK;

@@ -58,6 +58,7 @@ struct TunedConfig {
     int pipe_warps;        // warp-pipelined kernel: warps per block (1, 2 or 4; 0: default 4)
     unsigned* pipe_counters;  // warp-pipelined kernel: {next row, finished warps} of this launch (device memory, zero between launches)
     int pipe_zblock;       // warp-pipelined kernel: z planes per block of the row order (0: L_Z, i.e. plain lexicographic)
+    int march_units;       // generalised marching kernel: cap on the units per block (0: none)
     int march_lead;        // marching kernel: steps a block may run ahead of the slowest block of its chunk (0: unbounded)
     int x_shuffle;         // 1: exchange the x hops inside the warp when the tile allows it (fp64 default), 0: always load them
 };
@@ -135,10 +136,11 @@ struct GmShape {
 };
 bool gmarch_eligible(int precision, int layout_base, int recon, const Geom& g);
 // host only: decomposition and plan for [t_begin, t_end) with `wave` co-resident blocks; returns the number of blocks (0: none)
-int gmarch_plan_build(int precision, int recon, const Geom& g, int t_begin, int t_end, int wave, GmShape* shape,
+// max_units > 0 caps the units per block
+int gmarch_plan_build(int precision, int recon, const Geom& g, int t_begin, int t_end, int wave, int max_units, GmShape* shape,
                       GmBlockPlan* plan_out, size_t capacity_blocks);
-cudaError_t gmarch_plan_create(int precision, int recon, const Geom& g, int t_begin, int t_end, int device, void** d_plan, int* nblocks,
-                               GmShape* shape);
+cudaError_t gmarch_plan_create(int precision, int recon, const Geom& g, int t_begin, int t_end, int device, int max_units, void** d_plan,
+                               int* nblocks, GmShape* shape);
 cudaError_t launch_gmarch(int precision, int layout_base, int recon, const LaunchArgs& a, const void* d_plan, int nblocks,
                           const GmShape& shape, const TunedConfig& cfg);
 

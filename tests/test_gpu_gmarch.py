@@ -128,16 +128,26 @@ def test_gmarch_many_launches_on_a_side_stream_are_bit_stable(env):
         assert env.checks.parity_error(lat.download_spinor(outs[0]), ref) <= TOL["f32"]
 
 
-def test_tune_considers_gmarch_when_lx_is_not_32(env):
+def test_units_option_rebuilds_the_plan_and_tune_leaves_gmarch_alone(env):
     B = env.B
     dims = (48, 8, 8, 8)
     g, p, ref = fields_and_ref(env, dims, SEED + 43, "f32")
     with env.device.Lattice(dims, "f32", "soa", False) as lat:
         gi, pi, o = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
-        chosen, ms = B.dslash_tune(lat.ctx, o.data_ptr(), pi.data_ptr(), gi.data_ptr(), lat.stream())
-        assert ms > 0
-        assert chosen in (B.DSLASH_KERNEL_DIRECT, B.DSLASH_KERNEL_GMARCH)
-        assert env.checks.parity_error(lat.download_spinor(o), ref) <= TOL["f32"]
-        o.fill_(0x7f)
         lat.apply(o, pi, gi)
+        direct = lat.download_spinor(o)
+        lat.set_kernel("gmarch")
+        for units in (1, 2, 3, 0):  # DSLASH_OPT_MARCH_UNITS: smaller blocks, more slots per warp; same bits
+            B.dslash_set_option(lat.ctx, B.DSLASH_OPT_MARCH_UNITS, units)
+            assert B.dslash_get_option(lat.ctx, B.DSLASH_OPT_MARCH_UNITS) == units
+            for policy in (4 | 8 | 16, 4 | 8, 0):  # late / early ring fill (bit 16)
+                B.dslash_set_option(lat.ctx, B.DSLASH_OPT_L2_POLICY, policy)
+                o.fill_(0x7f)
+                lat.apply(o, pi, gi)
+                assert np.array_equal(lat.download_spinor(o), direct), (units, policy)
+        B.dslash_set_option(lat.ctx, B.DSLASH_OPT_L2_POLICY, -1)
+        # dslash_tune() picks by measurement among direct (+ march / wpipe when L_X == 32); gmarch lost everywhere it was
+        # measured and is not a candidate
+        chosen, ms = B.dslash_tune(lat.ctx, o.data_ptr(), pi.data_ptr(), gi.data_ptr(), lat.stream())
+        assert ms > 0 and chosen == B.DSLASH_KERNEL_DIRECT
         assert env.checks.parity_error(lat.download_spinor(o), ref) <= TOL["f32"]
