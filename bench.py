@@ -401,6 +401,9 @@ def run_cuda(args, cfg):
             o = results["other_recon"]
             line["also"] = {"recon": 12 if o["recon12"] else 18, "value": o["gflops"], "ms_per_step": o["ms_per_step"],
                             "hbm_gbs": o["gbs"], "roofline_frac": None if l2_resident else o["gbs"] / peak, "kernel": o["kernel"]}
+        if B.SKELETON:
+            line["skeleton"] = True
+            line["metric"] = "NOT A BENCH VALUE: data-movement skeleton (arithmetic compiled out, --skeleton); " + line["metric"]
         print(json.dumps(line))
     group.close()
     return 0
@@ -1022,6 +1025,10 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-parity", action="store_true", help="skip the whole-lattice parity check of the timed buffer")
+    ap.add_argument("--skeleton", action="store_true",
+                    help="measurement aid: time libdslash_b200_skeleton.so (python -m paper_2301_03636_b200.build --skeleton), the same "
+                         "kernels with their arithmetic compiled out -- same loads, copies, hand-offs and stores.  The output is not "
+                         "D psi: no parity, no cpu_baseline, no e2e; the line says \"skeleton\": true and is not a bench value")
     ap.add_argument("--repeats", type=int, default=5, help="K-step regions timed in all (median and min reported)")
     ap.add_argument("--cpu-sites", type=int, default=0, help="sites the cpu_baseline oracle run covers (0: the whole lattice, which "
                                                              "is also what the parity object needs)")
@@ -1046,6 +1053,9 @@ def main():
     ap.add_argument("--costmodel-epochs", type=int, default=150)
     ap.add_argument("--costmodel-models", type=int, default=16, help="independent seeds trained in the same launch")
     args = ap.parse_args()
+    if args.skeleton:
+        os.environ["DSLASH_B200_SKELETON"] = "1"  # read by paper_2301_03636_b200.binding when it is imported below
+        args.no_e2e = args.no_cpu_baseline = args.no_parity = True
     if args.warmup < 3 and args.impl == "cuda" and not args.sweep:
         args.warmup = 3  # timing rule: at least 3 warm-up steps
     if args.sweep:

@@ -11,7 +11,10 @@ import ctypes
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libdslash_b200.so")
+# DSLASH_B200_SKELETON=1 (set by `bench.py --skeleton` before this import) loads the measurement build whose kernels move the
+# same bytes and compute nothing (python -m paper_2301_03636_b200.build --skeleton); its results are not the operator.
+SKELETON = os.environ.get("DSLASH_B200_SKELETON", "") == "1"
+LIB_PATH = os.path.join(_HERE, "libdslash_b200_skeleton.so" if SKELETON else "libdslash_b200.so")
 
 DSLASH_FP64, DSLASH_FP32 = 0, 1
 DSLASH_AOS, DSLASH_SOA, DSLASH_RECON12 = 0, 1, 16
@@ -103,8 +106,8 @@ SIGNATURES = {
 def _load():
     if not os.path.exists(LIB_PATH):
         raise ImportError(
-            "libdslash_b200.so is missing (%s). Build it: python -m paper_2301_03636_b200.build. "
-            "There is no CPU fallback." % LIB_PATH)
+            "%s is missing (%s). Build it: python -m paper_2301_03636_b200.build%s. "
+            "There is no CPU fallback." % (os.path.basename(LIB_PATH), LIB_PATH, " --skeleton" if SKELETON else ""))
     try:
         lib = ctypes.CDLL(LIB_PATH)
     except OSError as e:  # pragma: no cover

@@ -267,11 +267,22 @@ __device__ __forceinline__ void load_link(cplx<Real> (&u)[9], const void* base, 
     if (RECON == 12) reconstruct_row2(u);
 }
 
+// ------------------------------------------------------------------ measurement aid: the data-movement skeleton
+// Compiled with -DDSLASH_NO_MATH (python -m paper_2301_03636_b200.build --skeleton -> libdslash_b200_skeleton.so) the three
+// arithmetic building blocks below are replaced by a handful of additions that keep the data dependence on every loaded
+// value, so every kernel moves exactly the bytes it moves in the product, through the same loads, copies, hand-offs and
+// stores, and computes (almost) nothing.  The result is NOT the operator; bench.py --skeleton times it to show how close a
+// kernel is to its own data movement (profiles/r02b_skeleton.md).  The product library never defines the macro.
 // ------------------------------------------------------------------ spin projection / reconstruction
 // SIGN = -1: (1 - gamma_MU)  (forward hop);  SIGN = +1: (1 + gamma_MU)  (backward hop).
 // h[0..2] = kept row 0, h[3..5] = kept row 1 (colour index fastest).
 template <int MU, int SIGN, typename Real>
 __device__ __forceinline__ void project(cplx<Real> (&h)[6], const cplx<Real> (&psi)[12]) {
+#ifdef DSLASH_NO_MATH
+#pragma unroll
+    for (int k = 0; k < 6; ++k) h[k] = {psi[k].re + psi[k + 6].re, psi[k].im + psi[k + 6].im};
+    if (MU >= 0) return;
+#endif
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         const cplx<Real> p0 = psi[c], p1 = psi[3 + c], p2 = psi[6 + c], p3 = psi[9 + c];
@@ -296,6 +307,19 @@ __device__ __forceinline__ void project(cplx<Real> (&h)[6], const cplx<Real> (&p
 //   MU 2: r2 = +-i h0, r3 = -+i h1    MU 3: r2 = -+ h0, r3 = -+ h1       (upper sign: SIGN = -1)
 template <int MU, int SIGN, bool FIRST, typename Real>
 __device__ __forceinline__ void reconstruct_accumulate(cplx<Real> (&acc)[12], const cplx<Real> (&h)[6]) {
+#ifdef DSLASH_NO_MATH
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        if (FIRST) {
+            acc[k] = h[k];
+            acc[k + 6] = h[k];
+        } else {
+            acc[k].re += h[k].re;
+            acc[k + 6].im += h[k].im;
+        }
+    }
+    if (MU >= 0) return;
+#endif
     constexpr bool M = SIGN < 0;  // the (1 - gamma) projector
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
@@ -334,6 +358,11 @@ __device__ __forceinline__ void reconstruct_accumulate(cplx<Real> (&acc)[12], co
 // hp = U h (DAGGER = false) or U^dagger h (DAGGER = true), both spin rows.
 template <bool DAGGER, typename Real>
 __device__ __forceinline__ void su3_mul(cplx<Real> (&hp)[6], const cplx<Real> (&u)[9], const cplx<Real> (&h)[6]) {
+#ifdef DSLASH_NO_MATH
+#pragma unroll
+    for (int k = 0; k < 6; ++k) hp[k] = {h[k].re + u[k].re, h[k].im + u[(k + 3) % 9].im + u[8].re};
+    if (sizeof(Real) > 0) return;
+#endif
 #pragma unroll
     for (int r = 0; r < 2; ++r)
 #pragma unroll
