@@ -56,6 +56,9 @@ NCU_FIGURES = {
     "32x32x32x64_f64_soa_r18_direct": dict(traffic=2032698000, fp64_pipe_pct=31.0, source="profiles/r01_ncu_tuned_kernel.txt"),
     "32x32x32x64_f64_soa_r18_wpipe": dict(traffic=2051962000, fp64_pipe_pct=None, source="profiles/r01f_wpipe.md"),
     "32x32x32x64_f64_soa_r18_march": dict(traffic=1995707392, fp64_pipe_pct=30.4, source="profiles/r02_march.md"),
+    "32x32x32x64_f64_soa_r12_march": dict(traffic=1593540816, fp64_pipe_pct=37.9, source="profiles/r02b_skeleton.md"),
+    "48x48x48x96_f32_soa_r18_direct": dict(traffic=5293000000, fp64_pipe_pct=None, source="profiles/r02_cfg4_r12.md"),
+    "48x48x48x96_f32_soa_r18_gmarch": dict(traffic=5990817000, fp64_pipe_pct=None, source="profiles/r02b_gmarch.md"),
 }
 KERNEL_NAMES = {"direct": "dslash_tuned_kernel", "wpipe": "dslash_wpipe_kernel", "march": "dslash_march_kernel",
                 "gmarch": "dslash_gmarch_kernel"}
