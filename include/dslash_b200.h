@@ -328,7 +328,8 @@ DSLASH_API int dslash_march_stats(dslash_ctx *ctx, unsigned *stats, size_t capac
  * three slot/warp configurations; not DSLASH_KERNEL_GMARCH, which loses to _DIRECT on every lattice measured) is timed on the caller's buffers
  * (2 warm-up + 8 timed applications each, CUDA events on `stream`; about 15 ms in all, so that every candidate is
  * timed inside the board's boost window -- call it on an idle device; with DSLASH_OPT_TUNE_MODE = DSLASH_TUNE_SUSTAINED:
- * every candidate runs 300 applications to reach its own power-capped steady state, then 100 timed ones, ~0.8 s in all) and the fastest becomes the
+ * every candidate runs 300 applications to reach its own power-capped steady state, then 100 timed ones, ~0.8 s in all) and the fastest
+ * (DSLASH_KERNEL_MARCH if it is within 1 % of the fastest: it moves the fewest on-chip bytes and keeps its time under load) becomes the
  * context's kernel, as if set by dslash_set_kernel() (and DSLASH_OPT_PIPE_SLOTS / _WARPS).  out, in, gauge: device pointers as for dslash_apply(); out is left
  * holding D in.  *chosen (may be NULL) receives the kernel, *ms_per_apply (may be NULL) its time.  This call SYNCHRONISES
  * with `stream`.  Errors: those of dslash_apply(); DSLASH_ERR_UNSUPPORTED when a sweep variant is selected.
