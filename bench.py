@@ -714,7 +714,10 @@ def run_costmodel_profile_one(args):
     from paper_2301_03636_b200 import costmodel as C
     from paper_2301_03636_b200 import inputs
     dev = torch.device("cuda:0")
-    f, n, epochs, batch = 33, 400, 4, 16
+    f, n, epochs, batch = args.costmodel_f, 400, 4, 16
+    cluster = args.costmodel_cluster
+    if args.costmodel_threads:
+        C.costmodel_set_option(C.COSTMODEL_OPT_THREADS, args.costmodel_threads)
     rng = np.random.default_rng([SEED, 33])
     xs = torch.from_numpy(rng.standard_normal((n, f))).to(dev)
     ys = torch.from_numpy(rng.standard_normal(n)).to(dev)
@@ -726,11 +729,12 @@ def run_costmodel_profile_one(args):
     for _ in range(3):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
-        model.train(xs, ys, uni, perms, epochs=epochs, batch=batch, cluster_size=8)
+        model.train(xs, ys, uni, perms, epochs=epochs, batch=batch, cluster_size=cluster)
         e1.record()
         torch.cuda.synchronize()
         ms.append(e0.elapsed_time(e1))
-    print(json.dumps({"costmodel_profile_one": True, "f": f, "rows": n, "epochs": epochs, "batch": batch, "cluster": 8,
+    print(json.dumps({"costmodel_profile_one": True, "f": f, "rows": n, "epochs": epochs, "batch": batch,
+                      "cluster": cluster if cluster else "library default", "threads": args.costmodel_threads or "library default",
                       "updates": updates, "ms_per_launch": ms, "us_per_update": min(ms) * 1e3 / updates}))
     return 0
 
@@ -1052,6 +1056,9 @@ def main():
     ap.add_argument("--probe", action="store_true", help="read/write/copy/4:1-mix bandwidth and FP64 FMA rate of this board")
     ap.add_argument("--costmodel", action="store_true", help="fit the Advisor's cost model on the variants' measured runtimes")
     ap.add_argument("--profile-one", action="store_true", help="with --costmodel: one training launch of the paper's network size")
+    ap.add_argument("--costmodel-f", type=int, default=33, help="--profile-one: number of features (33 = the paper's network)")
+    ap.add_argument("--costmodel-cluster", type=int, default=8, help="--profile-one: thread blocks per model (0: library default)")
+    ap.add_argument("--costmodel-threads", type=int, default=0, help="--profile-one: COSTMODEL_OPT_THREADS (0: library default)")
     ap.add_argument("--costmodel-lattices", type=int, default=len(COSTMODEL_LATTICES))
     ap.add_argument("--costmodel-epochs", type=int, default=150)
     ap.add_argument("--costmodel-models", type=int, default=16, help="independent seeds trained in the same launch")

@@ -58,7 +58,10 @@ DSLASH_API size_t costmodel_train_smem_bytes(int f, int batch, int cluster_size)
  *   learning rate of epoch e = lr0 * lr_gamma^(e / lr_step) (integer division; lr_step <= 0: constant lr0; at most 32 steps)
  *   weight_decay                     L2 coefficient added to every gradient (weights and biases)
  *   max_steps                        < 0: no limit; otherwise stop after that many updates in total (step-by-step comparisons)
- *   cluster_size                     1, 2, 4 or 8 thread blocks per model; 0 = the library chooses
+ *   cluster_size                     1, 2, 4 or 8 thread blocks per model; 0 = the library chooses (8 while n_models <= 16, for
+ *                                    latency: every phase of an update gets shorter with more blocks; else the fewest blocks that
+ *                                    hold the model, for throughput).  The partial sums are added in block order, so the low bits
+ *                                    of the result depend on the cluster size
  *   params_out     [n_models][costmodel_param_count(F)]
  *   epoch_loss_out [n_models][epochs]   mean mini-batch RMSE of each epoch (NaN for an epoch without updates); may be NULL
  *

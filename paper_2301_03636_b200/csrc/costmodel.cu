@@ -515,14 +515,25 @@ int costmodel_train(int f, int n, const double* x, const double* y, const double
         return DSLASH_ERR_UNSUPPORTED;
     const int nlr = (lr_step > 0 && epochs > 0) ? (epochs - 1) / lr_step + 1 : 1;
     if (nlr > kMaxLrSteps) return DSLASH_ERR_UNSUPPORTED;
-    const int threads = g_train_threads.load() > 0 ? g_train_threads.load() : 512;
-    if (threads < batch) return DSLASH_ERR_UNSUPPORTED;  // the training kernel loads one mini-batch index per thread
+    // Defaults by measurement (profiles/r02b_costmodel.md, one model, batch 16, us per update):
+    //   F = 33: cluster 4 / 8 at 256 threads 44.8 / 34.6, at 512 threads 36.3 / 29.3, at 1024 threads 43.3 / 35.5
+    //   F = 12: cluster 1 / 2 / 4 / 8 at 256 threads 27.6 / 23.5 / 19.1 / 17.5, at 512 threads 23.9 / 22.1 / 19.9 / 19.4
+    // The update is a chain of ~25 short dependent phases, so more blocks per model shorten every phase even when a single
+    // block could hold the model: a cluster of 8 whenever the launch's models still fit the device side by side.
+    int threads = g_train_threads.load() > 0 ? g_train_threads.load() : 512;
     int C = cluster_size;
     if (C == 0) {
-        // one block while the widest layer gives every thread at most one work item, more blocks as the layers grow
-        C = 1;
-        while (C < 8 && (costmodel_train_smem_bytes(f, batch, C) > kMaxSmem || 4 * f * ((batch + 3) / 4) > threads * C)) C *= 2;
+        if (n_models <= 16 && costmodel_train_smem_bytes(f, batch, 8) <= kMaxSmem) {
+            C = 8;  // latency: 16 clusters of 8 are resident together on 148 SMs
+        } else {
+            // throughput (many models per launch): one block while the widest layer gives every thread at most one work
+            // item, more blocks as the layers grow
+            C = 1;
+            while (C < 8 && (costmodel_train_smem_bytes(f, batch, C) > kMaxSmem || 4 * f * ((batch + 3) / 4) > threads * C)) C *= 2;
+        }
     }
+    if (g_train_threads.load() <= 0 && C == 8 && f <= 16 && batch <= 256) threads = 256;  // small layers spread over 8 blocks
+    if (threads < batch) return DSLASH_ERR_UNSUPPORTED;  // the training kernel loads one mini-batch index per thread
     const size_t smem = costmodel_train_smem_bytes(f, batch, C);
     if (smem == 0 || smem > kMaxSmem) return DSLASH_ERR_UNSUPPORTED;
 
