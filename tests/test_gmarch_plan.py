@@ -159,3 +159,25 @@ def test_ineligible_lattices_are_refused(B):
             B.dslash_gmarch_plan(dims, FP32, 18, 0, dims[3], 148)
     with pytest.raises(Exception):
         B.dslash_gmarch_plan((48, 48, 48, 96), FP32, 18, 3, 3, 148)
+
+
+def test_seeded_random_geometries(B):
+    """Forty seeded random lattices (every x extent from 1 to 96 that the kernel accepts has a chance): whatever the unit shape,
+    the plan resolves every neighbour.  Lattices the library refuses must be exactly the ineligible ones."""
+    import math
+    import random
+    rnd = random.Random(230103636)
+    checked = 0
+    while checked < 40:
+        lx = rnd.choice([1, 2, 3, 4, 6, 8, 12, 16, 20, 24, 32, 40, 48, 64, 80, 96])
+        ly, lz, lt = rnd.randint(1, 12), rnd.randint(1, 5), rnd.randint(1, 5)
+        precision, recon = rnd.choice([FP64, FP32]), rnd.choice([18, 12])
+        unit_vectors = lx // math.gcd(lx, 32)  # lcm(L_X, 32) / 32
+        eligible = (lx * ly) % 32 == 0 and unit_vectors <= (8 if precision == FP64 else 12)
+        try:
+            check_plan(B, (lx, ly, lz, lt), precision, recon, 0, lt, rnd.choice([1, 7, 148]))
+            assert eligible, (lx, ly, lz, lt)
+            checked += 1
+        except B.DslashError:
+            # refused: ineligible, or eligible in principle but no decomposition fits the shared memory of a block
+            assert not eligible or (precision == FP64 and unit_vectors >= 5), (lx, ly, lz, lt, precision)

@@ -151,3 +151,33 @@ def test_units_option_rebuilds_the_plan_and_tune_leaves_gmarch_alone(env):
         chosen, ms = B.dslash_tune(lat.ctx, o.data_ptr(), pi.data_ptr(), gi.data_ptr(), lat.stream())
         assert ms > 0 and chosen == B.DSLASH_KERNEL_DIRECT
         assert env.checks.parity_error(lat.download_spinor(o), ref) <= TOL["f32"]
+
+
+def test_gmarch_seeded_random_geometries(env):
+    """Ten seeded random eligible lattices (x extents 2 ... 96), fp64 or fp32, 18- or 12-real: oracle parity and bits."""
+    import random
+    B = env.B
+    rnd = random.Random(230103636 + 7)
+    done = 0
+    while done < 10:
+        lx = rnd.choice([2, 4, 8, 16, 24, 32, 40, 48, 64, 96])
+        ly = rnd.choice([k for k in range(1, 13) if (lx * k) % 32 == 0] or [0])
+        if ly == 0:
+            continue
+        dims = (lx, ly, rnd.randint(1, 4), rnd.randint(1, 4))
+        precision, recon12 = rnd.choice(["f64", "f32"]), rnd.choice([False, True])
+        g, p, ref = fields_and_ref(env, dims, SEED + 100 + done, precision)
+        with env.device.Lattice(dims, precision, "soa", recon12) as lat:
+            gi, pi, o = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
+            lat.apply(o, pi, gi)
+            direct = lat.download_spinor(o)
+            try:
+                lat.set_kernel("gmarch")
+            except B.DslashError:
+                continue  # no decomposition fits a block (fp64 units of many vectors)
+            o.fill_(0x7f)
+            lat.apply(o, pi, gi)
+            got = lat.download_spinor(o)
+            assert env.checks.parity_error(got, ref) <= TOL[precision], (dims, precision, recon12)
+            assert np.array_equal(got, direct), (dims, precision, recon12)
+        done += 1
