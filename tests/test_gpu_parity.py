@@ -621,6 +621,33 @@ def test_config3_full_size_properties(env):
         assert np.abs(out - 8.0 * psi).max() <= 1e-13
 
 
+def test_config3_staged_kernels_are_bit_stable_under_back_to_back_launches(env):
+    """At the bench size, in the bench's launch pattern (back-to-back applications, no host synchronisation in between), every
+    tenth result of 200 launches of each staged kernel equals the direct kernel's bit for bit: the hand-offs of the marching
+    and warp-pipelined kernels (mbarriers, async-proxy refills, row counters) leave no window in which a slot is overwritten
+    early -- the class of fault round 1 found only on a small lattice (one wrong row in 9 % of the launches)."""
+    torch = env.torch
+    dims = (32, 32, 32, 64)
+    with env.device.Lattice(dims, "f64", "soa", False) as lat:
+        g, p, ref = lat.new_gauge(), lat.new_spinor(), lat.new_spinor()
+        gen = torch.Generator(device=g.device).manual_seed(SEED + 77)
+        g.view(torch.float64).normal_(generator=gen)   # bit-stability does not need SU(3) links
+        p.view(torch.float64).normal_(generator=gen)
+        lat.apply(ref, p, g)
+        torch.cuda.synchronize()
+        for kernel in ("march", "wpipe", "gmarch"):
+            lat.set_kernel(kernel)
+            o = lat.new_spinor()
+            bad = 0
+            for i in range(200 if kernel != "gmarch" else 50):
+                lat.apply(o, p, g)
+                if i % 10 == 9:
+                    torch.cuda.synchronize()
+                    bad += 0 if torch.equal(o, ref) else 1
+                    o.fill_(0x7f)
+            assert bad == 0, kernel
+
+
 # ---------------------------------------------------------------- config 4: 48^3 x 96 FP32 vs the FP64 oracle
 def test_config4_48x48x48x96_fp32(env):
     """WHOLE lattice (10.6 M sites) against the fp64 oracle; dslash_tune() first, so the kernel checked is the one bench.py times."""
