@@ -648,6 +648,81 @@ def test_config3_staged_kernels_are_bit_stable_under_back_to_back_launches(env):
             assert bad == 0, kernel
 
 
+# ---------------------------------------------------------------- the largest lattice the 32-bit site index allows
+def test_maximum_lattice_size(env):
+    """32 x 128 x 112 x 128 = 58 720 256 sites, FP32: 36 V = 2 113 929 216 < 2^31 is the limit dslash_create enforces
+    (dims one step larger are refused).  No oracle run fits this size, so the check is a property that holds at any size and is
+    sensitive to every neighbour index: with unit links and psi(x) = s(x) chi (s a random real field, chi one spinor), Eq. 1
+     gives  D psi(x) = [sum_mu s(x+mu) + s(x-mu)] chi - sum_mu [s(x+mu) - s(x-mu)] gamma_mu chi,  evaluated here
+    with torch.roll and the oracle's gamma matrices.  Then, on random links and spinors, the marching and warp-pipelined
+    kernels (plan- and row-based addressing) must give the direct kernel's bits."""
+    torch, B = env.torch, env.B
+    dims = (32, 128, 112, 128)
+    lx, ly, lz, lt = dims
+    v = lx * ly * lz * lt
+    with pytest.raises(B.DslashError):
+        B.dslash_create((32, 128, 114, 128), B.DSLASH_FP32, B.DSLASH_SOA)
+    dev = torch.device("cuda:0")
+    gen = torch.Generator(device=dev).manual_seed(SEED + 58)
+    rng = np.random.default_rng(SEED + 58)
+    chi = rng.standard_normal(12) + 1j * rng.standard_normal(12)          # index = spin * 3 + colour
+    gchi = [np.einsum("ab,bc->ac", env.oracle.gamma(mu), chi.reshape(4, 3)).reshape(12) for mu in range(4)]
+    to_ri = lambda z: torch.from_numpy(np.stack([z.real, z.imag], -1)).to(dev)   # [12, 2] float64
+    chi_t, gchi_t = to_ri(chi), [to_ri(z) for z in gchi]
+    s = torch.randn((lt, lz, ly, lx), generator=gen, device=dev, dtype=torch.float64)
+    with env.device.Lattice(dims, "f32", "soa", False) as lat:
+        st = lat.stream()
+        # inputs in the canonical layout on the device, packed by the library
+        can = (s[..., None, None] * chi_t).to(torch.float32).contiguous()                      # [T,Z,Y,X,12,2]
+        p = lat.new_spinor()
+        B.dslash_pack_spinor(lat.ctx, p.data_ptr(), can.data_ptr(), st)
+        del can
+        u = torch.zeros((v, 4, 3, 3, 2), device=dev, dtype=torch.float32)
+        u[:, :, range(3), range(3), 0] = 1.0
+        g = lat.new_gauge()
+        B.dslash_pack_gauge(lat.ctx, g.data_ptr(), u.data_ptr(), st)
+        torch.cuda.synchronize()
+        del u
+        o = lat.new_spinor()
+        o.fill_(0x7f)
+        lat.apply(o, p, g)
+        out = torch.empty((lt, lz, ly, lx, 12, 2), device=dev, dtype=torch.float32)
+        B.dslash_unpack_spinor(lat.ctx, out.data_ptr(), o.data_ptr(), st)
+        torch.cuda.synchronize()
+        # expected, slab by slab in t (fp64)
+        shift = {0: 3, 1: 2, 2: 1, 3: 0}   # axis of direction mu in [T,Z,Y,X]
+        fwd = [torch.roll(s, -1, shift[mu]) for mu in range(4)]
+        bwd = [torch.roll(s, +1, shift[mu]) for mu in range(4)]
+        a = sum(fwd) + sum(bwd)
+        err2 = 0.0
+        ref2 = 0.0
+        worst = 0.0
+        for t0 in range(0, lt, 8):
+            sl = slice(t0, t0 + 8)
+            exp = a[sl][..., None, None] * chi_t
+            for mu in range(4):
+                exp = exp - (fwd[mu][sl] - bwd[mu][sl])[..., None, None] * gchi_t[mu]
+            d = out[sl].to(torch.float64) - exp
+            worst = max(worst, float(d.abs().max()))
+            ref2 += float((exp * exp).sum())
+        rms = (ref2 / (v * 12)) ** 0.5          # rms magnitude of a complex component
+        assert worst / rms <= TOL["f32"], (worst, rms)
+        del out, fwd, bwd, a, s
+        # random links and spinors: three independent addressing schemes, the same bits
+        g.view(torch.float32).normal_(generator=gen)
+        p.view(torch.float32).normal_(generator=gen)
+        lat.apply(o, p, g)
+        torch.cuda.synchronize()
+        for kernel in ("march", "wpipe"):
+            lat.set_kernel(kernel)
+            o2 = lat.new_spinor()
+            o2.fill_(0x7f)
+            lat.apply(o2, p, g)
+            torch.cuda.synchronize()
+            assert torch.equal(o2, o), kernel
+            del o2
+
+
 # ---------------------------------------------------------------- config 4: 48^3 x 96 FP32 vs the FP64 oracle
 def test_config4_48x48x48x96_fp32(env):
     """WHOLE lattice (10.6 M sites) against the fp64 oracle; dslash_tune() first, so the kernel checked is the one bench.py times."""
