@@ -21,6 +21,8 @@ LIB = os.path.join(HERE, "libdslash_b200.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
+# extra compiler flags for measurement builds (e.g. -DDSLASH_F32X2 / -DDSLASH_SCALAR_F32, csrc/dslash_site.cuh); use with --force
+FLAGS += os.environ.get("DSLASH_NVCC_EXTRA", "").split()
 
 
 def _sources():

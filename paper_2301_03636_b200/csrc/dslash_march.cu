@@ -40,6 +40,7 @@
 #include <algorithm>
 #include <vector>
 
+#define DSLASH_F32X2  // packed FP32 arithmetic (FFMA2 / FADD2), see dslash_site.cuh
 #include "../../include/dslash_b200.h"
 #include "dslash_async.cuh"
 #include "dslash_kernels.cuh"

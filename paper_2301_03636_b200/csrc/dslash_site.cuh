@@ -164,6 +164,77 @@ __device__ __forceinline__ cplx<Real> c_mul_conj(cplx<Real> a, cplx<Real> b) {
     return r;
 }
 
+// ------------------------------------------------------------------ FP32: two lanes per instruction (sm_100a f32x2)
+// Blackwell's FP32 pipe executes add / mul / fma on PAIRS of floats held in a 64-bit register (PTX add/mul/fma.rn.f32x2,
+// SASS FADD2 / FMUL2 / FFMA2), and ptxas folds a scalar broadcast (R.F32), a lane swap (.LO_HI) and a one-lane negation (.NP)
+// into the operand, so a complex number IS a pair: c_madd is two FFMA2 instead of four FFMA, c_add_i one FADD2 instead of two
+// FADD, with no packing instructions (the mov.b64 below disappear when (re, im) sit in an aligned register pair, which is how
+// the float4 / float2 loads deliver them).  Every component sees the same operations in the same order as in the scalar
+// templates above (one IEEE fma / add / mul per lane), so results are bit-identical to them -- and to one another across
+// kernels, whichever form a translation unit uses.  A translation unit opts in with #define DSLASH_F32X2 before including
+// this header.  Measured in one call, scalar vs packed (profiles/r02b_f32x2.md): the marching kernels gain 10-12 % in FP32
+// (fewer instructions in the compute warps' serial timeline: 32^3x64 0.244 -> 0.221 ms, 48^3x96 gmarch 2.36 -> 2.09 ms); the
+// direct kernel gains nothing at 48^3x96 (0.915 vs 0.916 ms) and LOSES 4.5 % at 32^3x64 (0.184 vs 0.1765 ms: with 128
+// registers and aligned pairs the compiler keeps fewer loads in flight), so dslash_tuned.cu and the other one-thread-per-site
+// units stay scalar.  For A/B measurements the whole library can be built one way or the other:
+//   DSLASH_NVCC_EXTRA=-DDSLASH_F32X2 (packed everywhere) / -DDSLASH_SCALAR_F32 (scalar everywhere), see build.py.
+#if defined(DSLASH_F32X2) && !defined(DSLASH_SCALAR_F32)
+__device__ __forceinline__ uint64_t f2_pack(float lo, float hi) {
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ cplx<float> f2_unpack(uint64_t v) {
+    cplx<float> c;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(c.re), "=f"(c.im) : "l"(v));
+    return c;
+}
+__device__ __forceinline__ uint64_t f2_add(uint64_t a, uint64_t b) {
+    uint64_t d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ uint64_t f2_sub(uint64_t a, uint64_t b) {
+    uint64_t d;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ uint64_t f2_mul(uint64_t a, uint64_t b) {
+    uint64_t d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ uint64_t f2_fma(uint64_t a, uint64_t b, uint64_t c) {
+    uint64_t d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+// non-template overloads: preferred over the templates above for cplx<float>
+__device__ __forceinline__ cplx<float> c_add(cplx<float> a, cplx<float> b) { return f2_unpack(f2_add(f2_pack(a.re, a.im), f2_pack(b.re, b.im))); }
+__device__ __forceinline__ cplx<float> c_sub(cplx<float> a, cplx<float> b) { return f2_unpack(f2_sub(f2_pack(a.re, a.im), f2_pack(b.re, b.im))); }
+// a + i*b = (a.re - b.im, a.im + b.re);  a - i*b = (a.re + b.im, a.im - b.re)
+__device__ __forceinline__ cplx<float> c_add_i(cplx<float> a, cplx<float> b) { return f2_unpack(f2_add(f2_pack(a.re, a.im), f2_pack(-b.im, b.re))); }
+__device__ __forceinline__ cplx<float> c_sub_i(cplx<float> a, cplx<float> b) { return f2_unpack(f2_add(f2_pack(a.re, a.im), f2_pack(b.im, -b.re))); }
+// acc += a * b:        re: fma(a.re, b.re, .) then fma(-a.im, b.im, .);   im: fma(a.re, b.im, .) then fma(a.im, b.re, .)
+__device__ __forceinline__ void c_madd(cplx<float>& acc, cplx<float> a, cplx<float> b) {
+    uint64_t r = f2_fma(f2_pack(a.re, a.re), f2_pack(b.re, b.im), f2_pack(acc.re, acc.im));
+    acc = f2_unpack(f2_fma(f2_pack(-a.im, a.im), f2_pack(b.im, b.re), r));
+}
+// acc += conj(a) * b:  re: fma(a.re, b.re, .) then fma(a.im, b.im, .);    im: fma(a.re, b.im, .) then fma(-a.im, b.re, .)
+__device__ __forceinline__ void c_madd_conj(cplx<float>& acc, cplx<float> a, cplx<float> b) {
+    uint64_t r = f2_fma(f2_pack(a.re, a.re), f2_pack(b.re, b.im), f2_pack(acc.re, acc.im));
+    acc = f2_unpack(f2_fma(f2_pack(a.im, -a.im), f2_pack(b.im, b.re), r));
+}
+__device__ __forceinline__ cplx<float> c_mul(cplx<float> a, cplx<float> b) {
+    uint64_t r = f2_mul(f2_pack(a.re, a.re), f2_pack(b.re, b.im));
+    return f2_unpack(f2_fma(f2_pack(-a.im, a.im), f2_pack(b.im, b.re), r));
+}
+__device__ __forceinline__ cplx<float> c_mul_conj(cplx<float> a, cplx<float> b) {
+    uint64_t r = f2_mul(f2_pack(a.re, a.re), f2_pack(b.re, b.im));
+    return f2_unpack(f2_fma(f2_pack(a.im, -a.im), f2_pack(b.im, b.re), r));
+}
+#endif
+
 // ------------------------------------------------------------------ field access (read-only path, 128-bit where the layout allows)
 // Spinor, 12 complex components of site s.
 template <typename Real, int LAYOUT>
