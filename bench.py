@@ -17,6 +17,8 @@ region the library picks its kernel by measurement (dslash_tune), then the devic
 launching stream) of the K timed steps; `repeats` = the same region four more times (median, min); `sustained` = the same
 after ~0.6 s of continuous load, when the board runs against its power cap (what a solver sees); `parity` = the buffer the
 timed region wrote, compared with the oracle on the whole lattice (outside the timed region).
+For lattices whose working set fits L2 (configs[0], [1]: an application takes 3-11 us) the K applications of a timed region
+are captured once in a CUDA graph and replayed (--graph auto): the eager loop measured the host's launch rate there.
 `e2e` = the same metric through dslash_apply_host with pinned HOST buffers (H2D copy of gauge and spinor, pack, apply, unpack,
 D2H copy of the result inside the timed region).
 Multi-GPU: default = replicas (every rank its own lattice, weak scaling, no collective: north_star keeps the path on one
@@ -189,17 +191,41 @@ def run_reference(args, cfg):
 
 
 # ------------------------------------------------------------------ the CUDA arm
+USE_GRAPH = False  # set by run_cuda: the K applications of a timed region are captured in one CUDA graph and replayed
+
+
 def time_applies(torch, lat, out, inp, gauge, steps, warmup, group, sampler_index):
-    for _ in range(warmup):
-        lat.apply(out, inp, gauge)
+    graph = None
+    if USE_GRAPH:
+        # A lattice whose application takes ~10 us is bound by the HOST's launch rate when every step is a ctypes call
+        # (measured: 12.4 us per step on 16^4 whatever the tile).  The same K launches captured once and replayed by the
+        # device measure the kernels.  Still K launches of the library's kernel per timed region, each through dslash_apply.
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            for _ in range(warmup):
+                lat.apply(out, inp, gauge)
+            side.synchronize()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=side):
+                for _ in range(steps):
+                    lat.apply(out, inp, gauge)
+        torch.cuda.current_stream().wait_stream(side)
+        graph.replay()  # one untimed replay (uploads the graph)
+    else:
+        for _ in range(warmup):
+            lat.apply(out, inp, gauge)
     torch.cuda.synchronize()
     group.barrier()
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with ClockSampler(sampler_index) as cs:
         e0.record()
-        for _ in range(steps):
-            lat.apply(out, inp, gauge)
+        if graph is not None:
+            graph.replay()
+        else:
+            for _ in range(steps):
+                lat.apply(out, inp, gauge)
         e1.record()
         torch.cuda.synchronize()
     group.barrier()
@@ -240,6 +266,8 @@ def run_cuda(args, cfg):
     group = replicas.Group("nccl", torch.device("cuda", local))
     dims, prec = cfg["dims"], cfg["precision"]
     v = inputs.volume(dims)
+    global USE_GRAPH
+    USE_GRAPH = args.graph == "on" or (args.graph == "auto" and bytes_per_site(prec, cfg["recon12"]) * v < 126e6)
     g, p = inputs.fields(dims, SEED + 3 + 1000 * rank, prec, check=False)  # every rank its own replica
 
     results = {}
@@ -385,6 +413,8 @@ def run_cuda(args, cfg):
                        "tile": main["tile"], "kernel": main["kernel"],
                        "kernel_chosen_by": "dslash_tune (measured before the timed region)" if main["tuned_ms"] is not None else "option", "occupancy_option": main["occupancy"],
                        "x_shuffle_option": main["x_shuffle"], "l2_policy_option": main["l2_policy"], "pipe_slots": main["pipe_slots"], "pipe_warps": main["pipe_warps"], "sites": v, "parallelism": "replicas x%d" % world,
+                       "launch": "the K applications of a timed region are one CUDA graph replay (K dslash_apply launches captured once)" if USE_GRAPH
+                                 else "K dslash_apply calls from the host",
                        "l2": ("working set %.1f MB fits L2: L2-resident by design of this config" % (working_set / 1e6)) if l2_resident else
                              ("inputs larger than L2: %.2f GB working set per apply vs 126 MB L2, no flush needed" % (working_set / 1e9))},
             "hbm_gbs": None if l2_resident else main["gbs"], "roofline": roofline, "parity": parity,
@@ -1032,6 +1062,9 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-parity", action="store_true", help="skip the whole-lattice parity check of the timed buffer")
+    ap.add_argument("--graph", choices=["auto", "on", "off"], default="auto",
+                    help="time the K applications of a region as one CUDA graph replay (auto: when the working set is L2-resident, "
+                         "i.e. an application is too short for the host's launch rate)")
     ap.add_argument("--skeleton", action="store_true",
                     help="measurement aid: time libdslash_b200_skeleton.so (python -m paper_2301_03636_b200.build --skeleton), the same "
                          "kernels with their arithmetic compiled out -- same loads, copies, hand-offs and stores.  The output is not "
