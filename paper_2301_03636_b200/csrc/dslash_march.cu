@@ -45,6 +45,13 @@
 #include "dslash_async.cuh"
 #include "dslash_kernels.cuh"
 
+// A producer warp with nothing to issue sleeps this long.  Measured in one call (DSLASH_NVCC_EXTRA=-DMARCH_IDLE_NS=..., burst /
+// sustained ms on 32^3x64 fp64): 32 ns 0.3397 / 0.3760, 128 ns 0.3421 / 0.3792, 512 ns 0.3774 / 0.3896, 2000 ns 0.4262 / 0.4345:
+// a late refill costs more than the polling instructions do, also under the power cap.
+#ifndef MARCH_IDLE_NS
+#define MARCH_IDLE_NS 32
+#endif
+
 namespace dslash {
 
 namespace {
@@ -294,7 +301,7 @@ __device__ __forceinline__ void march_producer(unsigned char* smem, const unsign
                 ++round;
             }
         }
-        if (!__any_sync(0xffffffffu, ready)) __nanosleep(32);  // (sleeping up to 512 ns changes neither time nor power measurably)
+        if (!__any_sync(0xffffffffu, ready)) __nanosleep(MARCH_IDLE_NS);
     }
 }
 
