@@ -83,6 +83,7 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
 #define DSLASH_ERR_UNSUPPORTED (-7) /* variant / tuning parameters outside the supported set */
 #define DSLASH_ERR_CUDA (-8)        /* a CUDA runtime call failed; see dslash_last_cuda_error() */
 #define DSLASH_ERR_NOMEM (-9)       /* host or device allocation failed */
+#define DSLASH_ERR_TOO_LARGE (-10)  /* the field does not fit the library's built-in scratch array (dslash_eo_apply_schur_static) */
 
 /* variant selection: collapse_depth DSLASH_VARIANT_TUNED selects the library's tuned kernel */
 #define DSLASH_VARIANT_TUNED 0
@@ -419,6 +420,48 @@ DSLASH_API int dslash_eo_cg_solve(dslash_ctx *ctx, void *x_even, const void *b_e
                                   int max_iter, int *iterations, double *rel_residual, dslash_stream_t stream);
 DSLASH_API int dslash_eo_solve(dslash_ctx *ctx, void *x_even, void *x_odd, const void *b_even, const void *b_odd, const void *gauge_eo,
                                double mass, double tol, int max_iter, int *iterations, double *rel_residual, dslash_stream_t stream);
+
+/*
+ * The Schur operator for callers that must not allocate device memory.
+ *
+ * dslash_eo_apply_schur() needs a half-lattice scratch field from its caller, and the solvers above cudaMalloc their work
+ * fields on first use.  Some users of this library can do neither once they are running:
+ *   - a program that handed all of the GPU's memory to its own pool at start-up (a framework's caching allocator, a job
+ *     whose lattice fields were sized to fill HBM): a cudaMalloc made on its behalf fails, or takes memory the pool counts on;
+ *   - a solver loop with a latency budget: cudaMalloc and cudaFree take driver-wide locks and can wait for all work on
+ *     the device, which stalls the streams the loop is trying to keep busy;
+ *   - a component that is only given pointers (a plug-in under a host application's memory policy) and has no way to
+ *     obtain or to own a device buffer of its own.
+ * For them dslash_eo_apply_schur_static() computes the same thing,
+ *     out_even = Mhat in_even,   Mhat = (4+mass) - D_eo D_oe / (4 (4+mass))      (dagger = 1: Mhat^dagger),
+ * with the odd-parity intermediate D_oe in_even held in an array that is part of the library image itself
+ * (`static __device__`, csrc/dslash_eo.cu).  The caller passes only the input, the output and the gauge field.  The call
+ * makes no cudaMalloc / cudaFree and uses no allocating library routine; results are bit-identical to
+ * dslash_eo_apply_schur() (the same two kernels run on the same data).
+ *
+ * Limit.  The array is DSLASH_STATIC_SCRATCH_BYTES = 8 MiB (dslash_static_scratch_bytes() returns the same number).  A
+ * ctx whose half-lattice spinor, dslash_eo_spinor_bytes(), is larger is refused with DSLASH_ERR_TOO_LARGE before anything
+ * is launched: in FP64 that admits 43 690 sites per parity (16^4 fits: 6.3 MB; 24^4 does not), in FP32 twice as many.  Every GPU
+ * on which the library's code is loaded holds these 8 MiB from then until the process exits, used or not.
+ *
+ * Set-up.  The first call on each device looks the array's device address up (cudaGetSymbolAddress, with that device
+ * current) and remembers it; later calls on that device only launch.  Make that first call during initialisation, before
+ * any stream capture is begun.  The ctx must belong to the current device (DSLASH_ERR_UNSUPPORTED otherwise).
+ *
+ * Sharing.  There is ONE array per device, shared by every ctx, stream and host thread in the process, and it keeps
+ * whatever the last call left in it.  Nothing in it has to start at zero -- the first kernel writes every element the
+ * second one reads -- so no clearing is done.  But two calls whose kernels can run at the same time on one GPU (different
+ * streams without an ordering between them, two host threads) overwrite each other's intermediate and both results are
+ * garbage: order such calls yourself (one stream, or events), or use dslash_eo_apply_schur() with separate scratch fields.
+ *
+ * Arguments as for dslash_eo_apply_schur() without tmp_odd: device pointers, 16-byte aligned, out_even must not overlap
+ * in_even; asynchronous on `stream`; two launches.  Errors: NULL, DIMS (an extent is odd), UNSUPPORTED (dagger not 0/1,
+ * 4+mass == 0, ctx of another device), TOO_LARGE, ALIGN, ALIAS, CUDA (including a failed address look-up).
+ */
+#define DSLASH_STATIC_SCRATCH_BYTES (8u << 20)
+DSLASH_API size_t dslash_static_scratch_bytes(void);
+DSLASH_API int dslash_eo_apply_schur_static(dslash_ctx *ctx, int dagger, double mass, void *out_even, const void *in_even,
+                                            const void *gauge_eo, dslash_stream_t stream);
 
 /*
  * Multi-GPU form of Eq. 1 by T-slab decomposition (the paper's future work).

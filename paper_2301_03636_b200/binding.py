@@ -21,6 +21,8 @@ DSLASH_AOS, DSLASH_SOA, DSLASH_RECON12 = 0, 1, 16
 DSLASH_OK = 0
 DSLASH_ERR_NULL, DSLASH_ERR_DIMS, DSLASH_ERR_PRECISION, DSLASH_ERR_LAYOUT = -1, -2, -3, -4
 DSLASH_ERR_ALIGN, DSLASH_ERR_ALIAS, DSLASH_ERR_UNSUPPORTED, DSLASH_ERR_CUDA, DSLASH_ERR_NOMEM = -5, -6, -7, -8, -9
+DSLASH_ERR_TOO_LARGE = -10
+DSLASH_STATIC_SCRATCH_BYTES = 8 << 20
 DSLASH_VARIANT_TUNED = 0
 DSLASH_MAP_MINIMAL, DSLASH_MAP_TOFROM = 0, 1
 DSLASH_KERNEL_AUTO, DSLASH_KERNEL_DIRECT = 0, 1
@@ -58,6 +60,8 @@ SIGNATURES = {
     "dslash_eo_apply_xpay": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int, _vp, _vp, _vp, _vp, ctypes.c_double, ctypes.c_double,
                                              _vp]),
     "dslash_eo_apply_schur": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_double, _vp, _vp, _vp, _vp, _vp]),
+    "dslash_static_scratch_bytes": (ctypes.c_size_t, []),
+    "dslash_eo_apply_schur_static": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_double, _vp, _vp, _vp, _vp]),
     "dslash_eo_cg_solve": (ctypes.c_int, [_vp, _vp, _vp, _vp, ctypes.c_double, ctypes.c_double, ctypes.c_int, _c_int_p,
                                            ctypes.POINTER(ctypes.c_double), _vp]),
     "dslash_eo_solve": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, ctypes.c_double, ctypes.c_double, ctypes.c_int, _c_int_p,
@@ -222,6 +226,22 @@ def dslash_eo_apply_xpay(ctx, out_parity: int, dagger: int, out, inp, gauge_eo, 
 def dslash_eo_apply_schur(ctx, dagger: int, mass: float, out_even, in_even, tmp_odd, gauge_eo, stream=0) -> None:
     _check(_lib.dslash_eo_apply_schur(_ptr(ctx), int(dagger), float(mass), _ptr(out_even), _ptr(in_even), _ptr(tmp_odd),
                                       _ptr(gauge_eo), _ptr(stream)), "dslash_eo_apply_schur")
+
+
+def dslash_static_scratch_bytes() -> int:
+    return int(_lib.dslash_static_scratch_bytes())
+
+
+def dslash_eo_apply_schur_static(ctx, dagger: int, mass: float, out_even, in_even, gauge_eo, stream=0) -> None:
+    """dslash_eo_apply_schur without a scratch argument, for callers that cannot allocate device memory: the intermediate
+    lives in an 8 MiB array inside the library (one per GPU, shared by all calls; see include/dslash_b200.h)."""
+    _check(_lib.dslash_eo_apply_schur_static(_ptr(ctx), int(dagger), float(mass), _ptr(out_even), _ptr(in_even), _ptr(gauge_eo),
+                                             _ptr(stream)), "dslash_eo_apply_schur_static")
+
+
+def dslash_eo_apply_schur_static_status(ctx, dagger: int, mass: float, out_even, in_even, gauge_eo, stream=0) -> int:
+    return int(_lib.dslash_eo_apply_schur_static(_ptr(ctx), int(dagger), float(mass), _ptr(out_even), _ptr(in_even), _ptr(gauge_eo),
+                                                 _ptr(stream)))
 
 
 def dslash_eo_cg_solve(ctx, x_even, b_even, gauge_eo, mass: float, tol: float, max_iter: int, stream=0):

@@ -563,6 +563,29 @@ int dslash_eo_apply_schur(dslash_ctx* c, int dagger, double mass, void* out_even
     return eo_apply_checked(c, 0, dagger, out_even, tmp_odd, gauge_eo, 1, in_even, a, -1.0 / (4.0 * a), stream);  // a in - D_eo(.)/(4a)
 }
 
+size_t dslash_static_scratch_bytes(void) { return eo_static_scratch_bytes(); }
+
+// The Schur operator for callers that cannot allocate: same checks and the same two kernels as dslash_eo_apply_schur, the
+// intermediate in the library's static device array (dslash_eo.cu).  No cudaMalloc / cudaFree on this path.
+int dslash_eo_apply_schur_static(dslash_ctx* c, int dagger, double mass, void* out_even, const void* in_even, const void* gauge_eo,
+                                 dslash_stream_t stream) {
+    if (!c || !out_even || !in_even || !gauge_eo) return DSLASH_ERR_NULL;
+    if (!c->eo_ok) return DSLASH_ERR_DIMS;
+    const double a = 4.0 + mass;
+    if ((dagger != 0 && dagger != 1) || !(a != 0.0)) return DSLASH_ERR_UNSUPPORTED;
+    const size_t sb = dslash_eo_spinor_bytes(c);
+    if (sb > eo_static_scratch_bytes()) return DSLASH_ERR_TOO_LARGE;
+    if (misaligned(out_even) || misaligned(in_even) || misaligned(gauge_eo)) return DSLASH_ERR_ALIGN;
+    if (overlap(out_even, sb, in_even, sb)) return DSLASH_ERR_ALIAS;
+    int cur_dev = -1;
+    if (cudaGetDevice(&cur_dev) != cudaSuccess || cur_dev != c->device) return DSLASH_ERR_UNSUPPORTED;  // the array is per device
+    cudaError_t e = launch_eo_schur_static(c->precision, c->layout_base, c->recon, out_even, in_even, gauge_eo, eo_gauge_half_bytes(c),
+                                           sb, c->gh, c->tg_eo, dagger, a, static_cast<cudaStream_t>(stream));
+    if (e != cudaSuccess) return cuda_fail(c, e);
+    c->launches += 2;
+    return DSLASH_OK;
+}
+
 int dslash_eo_cg_solve(dslash_ctx* c, void* x_even, const void* b_even, const void* gauge_eo, double mass, double tol, int max_iter,
                        int* iterations, double* rel_residual, dslash_stream_t stream_) {
     if (!c || !x_even || !b_even || !gauge_eo) return DSLASH_ERR_NULL;
@@ -1183,6 +1206,9 @@ const char* dslash_error_string(int status) {
         case DSLASH_ERR_UNSUPPORTED: return "DSLASH_ERR_UNSUPPORTED: parameter outside the supported set";
         case DSLASH_ERR_CUDA: return "DSLASH_ERR_CUDA: a CUDA runtime call failed (see dslash_last_cuda_error)";
         case DSLASH_ERR_NOMEM: return "DSLASH_ERR_NOMEM: allocation failed";
+        case DSLASH_ERR_TOO_LARGE:
+            return "DSLASH_ERR_TOO_LARGE: the half-lattice field exceeds the library's built-in scratch array "
+                   "(DSLASH_STATIC_SCRATCH_BYTES); use dslash_eo_apply_schur with your own scratch field";
         default: return "DSLASH_ERR_?: unknown status code";
     }
 }

@@ -16,8 +16,17 @@
 //     x-1: o == 1 -> h         o == 0 -> h - 1 (wrap to the end of the row)
 // so all eight gathers of a warp stay contiguous.  The forward link U_mu(x) comes from the output parity's half of the
 // gauge field at h, the backward link U_mu(x - mu^) from the other half at the neighbour's half-index.
+#include <mutex>
+
+#include "../../include/dslash_b200.h"
 #include "dslash_hop_rt.cuh"
 #include "dslash_kernels.cuh"
+
+// Scratch field of dslash_eo_apply_schur_static() (see "Schur operator with the library's own scratch field" below).
+// g_schur_scratch is a DEVICE symbol.  In host code its name only stands for it -- taking its address on the host gives
+// a host address that a kernel cannot use -- so the device address is asked for with cudaGetSymbolAddress(), once per
+// device, while that device is current, and that pointer is what the kernels get.
+static __device__ __align__(256) unsigned char g_schur_scratch[DSLASH_STATIC_SCRATCH_BYTES];
 
 namespace dslash {
 
@@ -114,6 +123,54 @@ cudaError_t launch_eo(int precision, int layout_base, int recon, void* out, cons
                                               : launch_eo_t<REAL, LAYOUT_SOA, 18>(out, in, g_out, g_in, gh, tg, p, st)))
     return precision == 0 ? DSLASH_EO(double) : DSLASH_EO(float);
 #undef DSLASH_EO
+}
+
+// ------------------------------------------------------------------ Schur operator with the library's own scratch field
+// dslash_eo_apply_schur_static() (include/dslash_b200.h) serves callers that cannot allocate device memory -- their
+// application owns all of it, or an allocation's device-wide stall is not affordable where they run -- so the odd-parity
+// intermediate of Mhat lives here, in the library image: one array per GPU the library is loaded on, there until exit.
+//
+// (the array itself, g_schur_scratch, is defined at file scope at the top of this file)
+static constexpr int kMaxDevices = 64;
+static std::mutex g_schur_scratch_mutex;
+static void* g_schur_scratch_addr[kMaxDevices];  // per device, filled by the first call made with that device current
+
+size_t eo_static_scratch_bytes() { return sizeof(g_schur_scratch); }
+
+// Device address of the scratch array on the CURRENT device.  The first call per device does the look-up (set-up: do it
+// before any stream capture); later calls read the cached pointer.  Never allocates.
+static cudaError_t schur_scratch_address(void** ptr) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_schur_scratch_mutex);
+    if (!g_schur_scratch_addr[dev]) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_schur_scratch);
+        if (e != cudaSuccess) return e;
+        if (!p) return cudaErrorInvalidSymbol;
+        g_schur_scratch_addr[dev] = p;
+    }
+    *ptr = g_schur_scratch_addr[dev];
+    return cudaSuccess;
+}
+
+// out_even = a * in_even - D_eo (D_oe in_even) / (4a), a = 4 + mass, with D_oe in_even in g_schur_scratch.  half_bytes =
+// size of a half-lattice spinor; the caller has checked that it fits.  The array keeps the previous call's contents: the
+// first launch overwrites every site the second one reads (padding lanes of a blocked-SoA field are never read), so
+// nothing is cleared.  Calls that overlap on the GPU share the array and race.
+cudaError_t launch_eo_schur_static(int precision, int layout_base, int recon, void* out_even, const void* in_even, const void* gauge_eo,
+                                   size_t gauge_half_bytes, size_t half_bytes, const Geom& gh, const TileGeom& tg, int dagger, double a,
+                                   cudaStream_t st) {
+    if (half_bytes > sizeof(g_schur_scratch)) return cudaErrorInvalidValue;
+    void* tmp_odd = nullptr;
+    cudaError_t e = schur_scratch_address(&tmp_odd);
+    if (e != cudaSuccess) return e;
+    e = launch_eo(precision, layout_base, recon, tmp_odd, in_even, gauge_eo, gauge_half_bytes, gh, tg, 1, dagger, 0, 0.0, 1.0, nullptr, st);
+    if (e != cudaSuccess) return e;
+    return launch_eo(precision, layout_base, recon, out_even, tmp_odd, gauge_eo, gauge_half_bytes, gh, tg, 0, dagger, 1, a,
+                     -1.0 / (4.0 * a), in_even, st);
 }
 
 // ------------------------------------------------------------------ layout: canonical full lattice <-> checkerboard halves

@@ -163,6 +163,11 @@ int reduction_scratch_doubles();
 cudaError_t launch_eo(int precision, int layout_base, int recon, void* out, const void* in, const void* gauge_eo,
                       size_t gauge_half_bytes, const Geom& gh, const TileGeom& tg, int parity, int dagger, int xpay, double a,
                       double b, const void* c, cudaStream_t st);
+// the same Schur operator as two launch_eo calls with the intermediate in the library's static device array (no allocation)
+size_t eo_static_scratch_bytes();
+cudaError_t launch_eo_schur_static(int precision, int layout_base, int recon, void* out_even, const void* in_even, const void* gauge_eo,
+                                   size_t gauge_half_bytes, size_t half_bytes, const Geom& gh, const TileGeom& tg, int dagger, double a,
+                                   cudaStream_t st);
 cudaError_t launch_eo_convert_spinor(int precision, int layout_base, void* dst, const void* src, const Geom& gh, int parity, int dir,
                                      cudaStream_t st);
 cudaError_t launch_eo_pack_gauge(int precision, int layout_base, int recon, void* dst_eo, const void* src, size_t gauge_half_bytes,

@@ -137,6 +137,12 @@ class Lattice:
         B.dslash_eo_apply_schur(self.ctx, dagger, mass, out_even.data_ptr(), in_even.data_ptr(), tmp_odd.data_ptr(),
                                 gauge_eo.data_ptr(), self.stream())
 
+    def eo_apply_schur_static(self, dagger, mass, out_even, in_even, gauge_eo):
+        """The same operator with the intermediate in the library's built-in array: nothing is allocated (half-lattice
+        fields up to B.DSLASH_STATIC_SCRATCH_BYTES; calls that overlap on the GPU share that array)."""
+        B.dslash_eo_apply_schur_static(self.ctx, dagger, mass, out_even.data_ptr(), in_even.data_ptr(), gauge_eo.data_ptr(),
+                                       self.stream())
+
     def eo_cg_solve(self, x_even, b_even, gauge_eo, mass, tol, max_iter):
         """x_even <- solution of Mhat^dagger Mhat x = b_even; returns (iterations, rel_residual)."""
         return B.dslash_eo_cg_solve(self.ctx, x_even.data_ptr(), b_even.data_ptr(), gauge_eo.data_ptr(), mass, tol, max_iter,

@@ -68,7 +68,7 @@ def test_costmodel_header_symbols_are_exported_and_bound(B):
 
 def test_error_strings(B):
     assert B.dslash_error_string(0) == "DSLASH_OK"
-    for code in range(-9, 0):
+    for code in range(-10, 0):
         s = B.dslash_error_string(code)
         assert s.startswith("DSLASH_ERR_") and "?" not in s
     assert "?" in B.dslash_error_string(-99)
