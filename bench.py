@@ -1097,7 +1097,8 @@ def main():
     ap.add_argument("--costmodel-models", type=int, default=16, help="independent seeds trained in the same launch")
     args = ap.parse_args()
     if args.skeleton:
-        os.environ["DSLASH_B200_SKELETON"] = "1"  # read by paper_2301_03636_b200.binding when it is imported below
+        from paper_2301_03636_b200 import binding
+        binding.load_skeleton()  # explicit switch: every later use of the binding in this process calls the skeleton library
         args.no_e2e = args.no_cpu_baseline = args.no_parity = True
     if args.warmup < 3 and args.impl == "cuda" and not args.sweep:
         args.warmup = 3  # timing rule: at least 3 warm-up steps

@@ -11,10 +11,12 @@ import ctypes
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-# DSLASH_B200_SKELETON=1 (set by `bench.py --skeleton` before this import) loads the measurement build whose kernels move the
-# same bytes and compute nothing (python -m paper_2301_03636_b200.build --skeleton); its results are not the operator.
-SKELETON = os.environ.get("DSLASH_B200_SKELETON", "") == "1"
-LIB_PATH = os.path.join(_HERE, "libdslash_b200_skeleton.so" if SKELETON else "libdslash_b200.so")
+# Importing this module always loads the operator library, whatever the environment says.  The measurement build whose kernels
+# move the same bytes and compute nothing (python -m paper_2301_03636_b200.build --skeleton) is only ever loaded by an explicit
+# load_skeleton() call (bench.py --skeleton makes it); SKELETON is True from then on and results are not the operator.
+SKELETON = False
+LIB_PATH = os.path.join(_HERE, "libdslash_b200.so")
+SKELETON_LIB_PATH = os.path.join(_HERE, "libdslash_b200_skeleton.so")
 
 DSLASH_FP64, DSLASH_FP32 = 0, 1
 DSLASH_AOS, DSLASH_SOA, DSLASH_RECON12 = 0, 1, 16
@@ -107,26 +109,38 @@ SIGNATURES = {
 }
 
 
-def _load():
-    if not os.path.exists(LIB_PATH):
+def _load(path=LIB_PATH, build_hint=""):
+    if not os.path.exists(path):
         raise ImportError(
             "%s is missing (%s). Build it: python -m paper_2301_03636_b200.build%s. "
-            "There is no CPU fallback." % (os.path.basename(LIB_PATH), LIB_PATH, " --skeleton" if SKELETON else ""))
+            "There is no CPU fallback." % (os.path.basename(path), path, build_hint))
     try:
-        lib = ctypes.CDLL(LIB_PATH)
+        lib = ctypes.CDLL(path)
     except OSError as e:  # pragma: no cover
-        raise ImportError("cannot load %s: %s" % (LIB_PATH, e))
+        raise ImportError("cannot load %s: %s" % (path, e))
     for name, (res, args) in SIGNATURES.items():
         try:
             fn = getattr(lib, name)
         except AttributeError:
-            raise ImportError("%s does not export %s" % (LIB_PATH, name))
+            raise ImportError("%s does not export %s" % (path, name))
         fn.restype = res
         fn.argtypes = args
     return lib
 
 
 _lib = _load()
+
+
+def load_skeleton() -> None:
+    """Measurement aid, for bench.py --skeleton only: route every call of this module to libdslash_b200_skeleton.so, whose
+    kernels have their arithmetic compiled out.  From here on nothing this process computes is D psi; SKELETON says so and a
+    warning is printed.  Contexts created before the switch belong to the operator library and must not be used after it."""
+    global _lib, SKELETON
+    import warnings
+    _lib = _load(SKELETON_LIB_PATH, " --skeleton")
+    SKELETON = True
+    warnings.warn("paper_2301_03636_b200.binding now calls the data-movement skeleton: results are NOT the Dslash operator",
+                  RuntimeWarning, stacklevel=2)
 
 
 class DslashError(RuntimeError):

@@ -149,6 +149,20 @@ def test_omp_variant_space_reproduces_table_1(B):
     assert [B.dslash_omp_variant_count(n) // 6 for n in (1, 2, 3, 4)] == [1, 3, 7, 14]
 
 
+def test_environment_cannot_swap_the_operator_library_for_the_skeleton(B):
+    """The measurement build (arithmetic compiled out) is reachable through binding.load_skeleton() only: an ambient
+    DSLASH_B200_SKELETON=1, which older revisions obeyed at import, must not change what `import binding` loads."""
+    import subprocess
+    import sys
+    env = dict(os.environ, DSLASH_B200_SKELETON="1")
+    code = ("from paper_2301_03636_b200 import binding as B; import os; "
+            "assert os.path.basename(B.LIB_PATH) == 'libdslash_b200.so' and B.SKELETON is False; "
+            "assert B._lib._name == B.LIB_PATH; print('ok')")
+    r = subprocess.run([sys.executable, "-c", code], cwd=ROOT, env=env, capture_output=True, text=True)
+    assert r.returncode == 0 and r.stdout.strip() == "ok", r.stderr
+    assert callable(B.load_skeleton) and B.SKELETON is False
+
+
 def test_no_cuda_device_is_an_error_not_a_fallback(B):
     import torch
     if torch.cuda.is_available():
