@@ -244,6 +244,8 @@ def lattice_options(B, lat, args):
         B.dslash_set_option(lat.ctx, B.DSLASH_OPT_X_SHUFFLE, args.x_shuffle)
     if args.l2_policy is not None:
         B.dslash_set_option(lat.ctx, B.DSLASH_OPT_L2_POLICY, args.l2_policy)
+    if args.march_policy is not None:
+        B.dslash_set_option(lat.ctx, B.DSLASH_OPT_MARCH_POLICY, args.march_policy)
     if args.march_lead is not None:
         B.dslash_set_option(lat.ctx, B.DSLASH_OPT_MARCH_LEAD, args.march_lead)
     if args.march_units is not None:
@@ -1049,7 +1051,8 @@ def main():
     ap.add_argument("--tile", type=int, nargs=4, default=None, help="tile of the tuned kernel (x y z t)")
     ap.add_argument("--occupancy", type=int, default=None, help="DSLASH_OPT_OCCUPANCY override")
     ap.add_argument("--kernel", choices=["auto", "direct", "wpipe", "march", "gmarch"], default=None)
-    ap.add_argument("--l2-policy", type=int, default=None, help="DSLASH_OPT_L2_POLICY bits")
+    ap.add_argument("--l2-policy", type=int, default=None, help="DSLASH_OPT_L2_POLICY bits (direct kernel)")
+    ap.add_argument("--march-policy", type=int, default=None, help="DSLASH_OPT_MARCH_POLICY bits (marching kernels)")
     ap.add_argument("--march-lead", type=int, default=None, help="DSLASH_OPT_MARCH_LEAD")
     ap.add_argument("--march-units", type=int, default=None, help="DSLASH_OPT_MARCH_UNITS (gmarch kernel: cap on the units per block)")
     ap.add_argument("--no-tune", action="store_true", help="skip dslash_tune (keep the library's static default kernel)")

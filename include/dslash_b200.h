@@ -125,13 +125,11 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
 /* options of the tuned kernels, dslash_set_option() */
 #define DSLASH_OPT_OCCUPANCY 2        /* blocks of <= 128 threads: 0 = 168 registers/thread (12 warps/SM), 1 = 128 (16 warps),
                                          2 = 255 (8 warps, deeper load hoisting) */
-#define DSLASH_OPT_L2_POLICY 3        /* bit mask of L2 hints, -1 (default) = each kernel's own default.
-                                         Direct kernel (default 0): 1 spinor loads evict_last, 2 U_t loads evict_last,
-                                         4 U_x/U_y/U_z loads evict_first, 8 stores of `out` evict_first, 16 t-direction loads
-                                         bypass L1 allocation.
-                                         Marching kernel (default 4|8|16): 1 data other blocks read too evict_last, 4 links
-                                         read once per application evict_first, 8 stores evict_first, 16 a ring row is
-                                         fetched late, about one step before its first use instead of two */
+#define DSLASH_OPT_L2_POLICY 3        /* direct kernel: bit mask of L2 hints, -1 or 0 (default) = none: 1 spinor loads evict_last,
+                                         2 U_t loads evict_last, 4 U_x/U_y/U_z loads evict_first, 8 stores of `out` evict_first,
+                                         16 t-direction loads bypass L1 allocation.  The marching kernels do not read it (their
+                                         bits mean other things: DSLASH_OPT_MARCH_POLICY), so a value tuned for one kernel never
+                                         leaks into another and dslash_tune() compares every candidate under its own setting */
 #define DSLASH_OPT_L1_CARVEOUT 4      /* direct kernel: preferred shared-memory carve-out in percent, -1 = driver default */
 #define DSLASH_OPT_X_SHUFFLE 5        /* direct kernel: 1 (default for FP64; FP32 defaults to 0) = when a whole x row sits inside one warp
                                          (tile x-extent == L_X, a power of two <= 32) the two x hops are exchanged between
@@ -152,7 +150,12 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
                                          many as fit; fewer units leave shared memory for more link / halo slots per warp.  The block
                                          plan is rebuilt by the call (synchronous) when DSLASH_KERNEL_GMARCH is selected */
 #define DSLASH_OPT_MARCH_LEAD 11      /* marching kernel: steps a block may run ahead of the slowest block of its chunk, 0..16
-                                         (0 = unbounded).  Blocks that stay close share their halo rows through L2 */
+                                         (0 = unbounded, the default: measured slower than unbounded on 32^3x64).  Blocks that
+                                         stay close share their halo rows through L2.  Only single-wave plans honour it */
+#define DSLASH_OPT_MARCH_POLICY 13    /* marching kernels (DSLASH_KERNEL_MARCH / _GMARCH): bit mask, -1 (default) = 4|8|16: 1 data other
+                                         blocks read too evict_last (measured harmful), 4 links read once per application
+                                         evict_first, 8 stores evict_first, 16 a ring row is fetched late, about one step before
+                                         its first use instead of two.  0..31 */
 #define DSLASH_TUNE_BURST 0
 #define DSLASH_TUNE_SUSTAINED 1
 
@@ -505,6 +508,9 @@ DSLASH_API int dslash_get_option(const dslash_ctx *ctx, int option, int *value);
  *   kernel on the slab's time range) and unpacked and slab k-1 of `out` travels back, so both directions of the host link
  *   are busy.  Every byte crosses the link exactly once.  (A blocked-SoA lattice whose time slice is not a whole number of
  *   32-site vectors, or a ctx with a partial time range, runs as one slab.)
+ *   The kernel is always the direct kernel with the ctx's tile and options: a kernel chosen by dslash_set_kernel() / dslash_tune()
+ *   and a sweep variant chosen by dslash_set_variant() / dslash_set_omp_variant() are NOT used here (the call is bound by the host
+ *   link, 50x slower than any of them).
  *   With DSLASH_MAP_TOFROM all three fields travel both ways (what an offload without
  *   data analysis does); with DSLASH_MAP_MINIMAL only gauge,in go to the device and only out comes back.
  *   out_host, in_host, gauge_host   host pointers (pinned memory makes the copies asynchronous and
@@ -512,7 +518,8 @@ DSLASH_API int dslash_get_option(const dslash_ctx *ctx, int option, int *value);
  *   with the identical values.
  * The ctx owns the device staging buffers, streams and events (created on first use, freed by dslash_destroy).
  * h2d_bytes / d2h_bytes (optional, may be NULL) receive the bytes copied in each direction.
- * Errors: NULL, UNSUPPORTED (map_mode), NOMEM, CUDA.
+ * Errors: NULL, UNSUPPORTED (map_mode; the current device is not the ctx's), NOMEM, CUDA.  After a CUDA error in mid-pipeline the
+ * call waits for the copies it has already queued before it returns, so the host buffers are the caller's again on return.
  */
 DSLASH_API int dslash_apply_host(dslash_ctx *ctx, void *out_host, const void *in_host, const void *gauge_host, int map_mode,
                       dslash_stream_t stream, size_t *h2d_bytes, size_t *d2h_bytes);

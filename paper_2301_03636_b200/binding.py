@@ -35,7 +35,7 @@ GM_NW_MAX, GM_SRC_MAX, GM_NWB_MAX = 12, 3, 36
 GM_WARP_INTS = 12 + 2 * 3 * GM_SRC_MAX * 2
 GM_BLOCK_INTS = 4 + GM_NW_MAX + GM_NWB_MAX + GM_NW_MAX * GM_WARP_INTS  # block plan of dslash_gmarch_plan()
 DSLASH_OPT_PIPE_SLOTS, DSLASH_OPT_PIPE_WARPS, DSLASH_OPT_PIPE_ZBLOCK, DSLASH_OPT_TUNE_MODE, DSLASH_OPT_MARCH_LEAD = 7, 8, 9, 10, 11
-DSLASH_OPT_MARCH_UNITS = 12
+DSLASH_OPT_MARCH_UNITS, DSLASH_OPT_MARCH_POLICY = 12, 13
 DSLASH_TUNE_BURST, DSLASH_TUNE_SUSTAINED = 0, 1
 DSLASH_OPT_OCCUPANCY, DSLASH_OPT_L2_POLICY, DSLASH_OPT_L1_CARVEOUT, DSLASH_OPT_X_SHUFFLE = 2, 3, 4, 5
 DSLASH_SCHED_STATIC, DSLASH_SCHED_DYNAMIC, DSLASH_SCHED_GUIDED = 0, 1, 2

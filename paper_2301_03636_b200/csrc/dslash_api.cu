@@ -48,7 +48,8 @@ struct dslash_ctx {
     // ensure_kernel_resources(), never by dslash_apply)
     void* march_plan;
     int march_blocks, march_t0, march_t1;
-    unsigned march_epoch;  // launches on the current plan (its progress counters accumulate)
+    unsigned march_epoch;  // throttled (lead > 0) launches on the current plan: its progress counters accumulate over those
+    int march_sms;         // SM count of the ctx's device, from march_prepare() (0: not prepared yet)
     // the same for the generalised marching kernel (any L_X): plan, its shape (warps, slots, shared-memory size), time range
     void* gm_plan;
     int gm_blocks, gm_t0, gm_t1;
@@ -211,6 +212,20 @@ static int cg_normal_equations(dslash_ctx* c, unsigned V, size_t sb, void** vec,
 // plan of the marching kernel.  Called where a kernel is SELECTED (dslash_set_kernel, dslash_tune, dslash_set_time_range,
 // dslash_create), so that dslash_apply itself never allocates, copies or synchronises.
 static int ensure_kernel_resources(dslash_ctx* c, int kernel) {
+    if (kernel == DSLASH_KERNEL_WARP_PIPE || kernel == DSLASH_KERNEL_MARCH || kernel == DSLASH_KERNEL_GMARCH) {
+        // everything below allocates on, and asks about, the CURRENT device: it has to be the ctx's
+        int cur_dev = -1;
+        if (cudaGetDevice(&cur_dev) != cudaSuccess || cur_dev != c->device) return DSLASH_ERR_UNSUPPORTED;
+    }
+    if (kernel == DSLASH_KERNEL_MARCH && march_eligible(c->layout_base, c->geom) && c->march_sms == 0) {
+        int sms = 0;
+        cudaError_t e = march_prepare(c->precision, c->recon, c->device, &sms);
+        if (e != cudaSuccess || sms < 1) {
+            (void)cudaGetLastError();
+            return cuda_fail(c, e != cudaSuccess ? e : cudaErrorInvalidDevice);
+        }
+        c->march_sms = sms;
+    }
     if (kernel == DSLASH_KERNEL_WARP_PIPE && !c->pipe_ctr && wpipe_eligible(c->layout_base, c->geom)) {
         cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&c->pipe_ctr), 32 * sizeof(unsigned));
         if (e != cudaSuccess) {
@@ -318,6 +333,8 @@ int dslash_create(dslash_ctx** ctx, const int dims[4], int precision, int layout
     c->march_blocks = 0;
     c->march_t0 = c->march_t1 = -1;
     c->march_epoch = 0;
+    c->march_sms = 0;
+    c->cfg.march_policy = -1;
     c->gm_plan = nullptr;
     c->gm_blocks = 0;
     c->gm_t0 = c->gm_t1 = -1;
@@ -389,6 +406,11 @@ static int resolve_kernel(const dslash_ctx* c) {
     return DSLASH_KERNEL_DIRECT;  // AUTO
 }
 
+// the ctx belongs to the device that was current when it was created: kernels launched through it must run there
+static bool on_ctx_device(const dslash_ctx* c) {
+    int cur_dev = -1;
+    return cudaGetDevice(&cur_dev) == cudaSuccess && cur_dev == c->device;
+}
 static bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
 static bool overlap(const void* a, size_t na, const void* b, size_t nb) {
     const uintptr_t A = reinterpret_cast<uintptr_t>(a), B = reinterpret_cast<uintptr_t>(b);
@@ -415,11 +437,11 @@ int dslash_apply(dslash_ctx* c, void* out, const void* in, const void* gauge, ds
             cudaError_t ez = cudaMemsetAsync(c->cfg.pipe_counters, 0, 2 * sizeof(unsigned), a.stream);
             if (ez != cudaSuccess) return cuda_fail(c, ez);
         }
-        if (k == DSLASH_KERNEL_MARCH && (!c->march_plan || c->march_t0 != c->tg.t_begin || c->march_t1 != c->tg.t_end))
+        if (k == DSLASH_KERNEL_MARCH && (!c->march_plan || c->march_sms < 1 || c->march_t0 != c->tg.t_begin || c->march_t1 != c->tg.t_end))
             return DSLASH_ERR_UNSUPPORTED;
         if (k == DSLASH_KERNEL_GMARCH && (!c->gm_plan || c->gm_t0 != c->tg.t_begin || c->gm_t1 != c->tg.t_end)) return DSLASH_ERR_UNSUPPORTED;
         e = (k == DSLASH_KERNEL_WARP_PIPE) ? launch_wpipe(c->precision, c->layout_base, c->recon, a, c->tg, c->cfg)
-            : (k == DSLASH_KERNEL_MARCH)   ? launch_march(c->precision, c->layout_base, c->recon, a, c->march_plan, c->march_blocks, c->cfg, ++c->march_epoch)
+            : (k == DSLASH_KERNEL_MARCH)   ? launch_march(c->precision, c->layout_base, c->recon, a, c->march_plan, c->march_blocks, c->cfg, c->march_sms, &c->march_epoch)
             : (k == DSLASH_KERNEL_GMARCH)  ? launch_gmarch(c->precision, c->layout_base, c->recon, a, c->gm_plan, c->gm_blocks, c->gm_shape, c->cfg)
                                            : launch_tuned(c->precision, c->layout_base, c->recon, a, c->tg, c->cfg);
     } else if (!full_time_range(c)) {
@@ -429,10 +451,7 @@ int dslash_apply(dslash_ctx* c, void* out, const void* in, const void* gauge, ds
                                c->omp_team_size);
     } else
         e = launch_variant(c->precision, c->layout_base, c->recon, a, c->var_depth, c->var_tpb, c->var_spt);
-    if (e != cudaSuccess) {
-        if (c->var_depth == DSLASH_VARIANT_TUNED && resolve_kernel(c) == DSLASH_KERNEL_MARCH) --c->march_epoch;  // nothing was counted
-        return cuda_fail(c, e);
-    }
+    if (e != cudaSuccess) return cuda_fail(c, e);
     c->launches += 1;
     return DSLASH_OK;
 }
@@ -783,10 +802,20 @@ int dslash_set_tile(dslash_ctx* c, const int tile[4]) {
 int dslash_set_time_range(dslash_ctx* c, int t_begin, int t_end) {
     if (!c) return DSLASH_ERR_NULL;
     if (t_begin < 0 || t_end > c->geom.L[3] || t_begin >= t_end) return DSLASH_ERR_UNSUPPORTED;
+    const int old_begin = c->tg.t_begin, old_end = c->tg.t_end;
     c->tg.t_begin = t_begin;
     c->tg.t_end = t_end;
     set_tile_geom(c, c->tile);
-    return ensure_kernel_resources(c, c->kernel);
+    const int rc = ensure_kernel_resources(c, c->kernel);
+    if (rc != DSLASH_OK) {
+        // the new range has no plan: go back to the old one, and rebuild its plan if the failed attempt freed it (best effort;
+        // if that fails too, dslash_apply of the marching kernels reports UNSUPPORTED until a range or kernel is set again)
+        c->tg.t_begin = old_begin;
+        c->tg.t_end = old_end;
+        set_tile_geom(c, c->tile);
+        (void)ensure_kernel_resources(c, c->kernel);
+    }
+    return rc;
 }
 
 int dslash_get_time_range(const dslash_ctx* c, int* t_begin, int* t_end) {
@@ -850,6 +879,10 @@ int dslash_set_option(dslash_ctx* c, int option, int value) {
             if (value < 0 || value > 16) return DSLASH_ERR_UNSUPPORTED;
             c->cfg.march_lead = value;
             return DSLASH_OK;
+        case DSLASH_OPT_MARCH_POLICY:
+            if (value < -1 || value > 31) return DSLASH_ERR_UNSUPPORTED;
+            c->cfg.march_policy = value;
+            return DSLASH_OK;
         default:
             return DSLASH_ERR_UNSUPPORTED;
     }
@@ -865,6 +898,7 @@ int dslash_get_option(const dslash_ctx* c, int option, int* value) {
         case DSLASH_OPT_PIPE_SLOTS: *value = c->cfg.pipe_slots; return DSLASH_OK;
         case DSLASH_OPT_PIPE_WARPS: *value = c->cfg.pipe_warps; return DSLASH_OK;
         case DSLASH_OPT_MARCH_LEAD: *value = c->cfg.march_lead; return DSLASH_OK;
+        case DSLASH_OPT_MARCH_POLICY: *value = c->cfg.march_policy; return DSLASH_OK;
         case DSLASH_OPT_MARCH_UNITS: *value = c->cfg.march_units; return DSLASH_OK;
         case DSLASH_OPT_PIPE_ZBLOCK: *value = c->cfg.pipe_zblock; return DSLASH_OK;
         case DSLASH_OPT_TUNE_MODE: *value = c->tune_mode; return DSLASH_OK;
@@ -982,6 +1016,7 @@ int dslash_apply_host(dslash_ctx* c, void* out_host, const void* in_host, const 
                       dslash_stream_t stream_, size_t* h2d_bytes, size_t* d2h_bytes) {
     if (!c || !out_host || !in_host || !gauge_host) return DSLASH_ERR_NULL;
     if (map_mode != DSLASH_MAP_MINIMAL && map_mode != DSLASH_MAP_TOFROM) return DSLASH_ERR_UNSUPPORTED;
+    if (!on_ctx_device(c)) return DSLASH_ERR_UNSUPPORTED;  // staging buffers, streams and events live on the ctx's device
     cudaStream_t stream = static_cast<cudaStream_t>(stream_);
     const size_t can_bytes[3] = {dslash_canonical_gauge_bytes(c), dslash_canonical_spinor_bytes(c),
                                  dslash_canonical_spinor_bytes(c)};
@@ -1037,9 +1072,16 @@ int dslash_apply_host(dslash_ctx* c, void* out_host, const void* in_host, const 
     auto slab_t0 = [&](int k) { return (int)((long long)k * LT / NS); };
     cudaStream_t s_up = c->host_stream[0], s_run = c->host_stream[1], s_down = c->host_stream[2];
     cudaEvent_t ev_entry = c->host_event[64], ev_exit = c->host_event[65];
-#define HOST_TRY(call)                                           \
-    do {                                                         \
-        if ((e = (call)) != cudaSuccess) return cuda_fail(c, e); \
+    // On an error in mid-pipeline, copies already queued on the three streams still read and write the CALLER's host buffers:
+    // wait for them before handing the buffers back with the error.
+    auto fail_drained = [&](cudaError_t err) {
+        for (int i = 0; i < 3; ++i) (void)cudaStreamSynchronize(c->host_stream[i]);
+        (void)cudaGetLastError();
+        return cuda_fail(c, err);
+    };
+#define HOST_TRY(call)                                             \
+    do {                                                           \
+        if ((e = (call)) != cudaSuccess) return fail_drained(e);   \
     } while (0)
     HOST_TRY(cudaEventRecord(ev_entry, stream));  // everything here is ordered after the caller's earlier work on `stream`
     HOST_TRY(cudaStreamWaitEvent(s_up, ev_entry, 0));
@@ -1136,6 +1178,7 @@ size_t dslash_slab_face_bytes(const dslash_ctx* c) {
 int dslash_slab_pack_faces(dslash_ctx* c, void* face_down, void* face_up, const void* in, const void* gauge, dslash_stream_t stream) {
     if (!c || !face_down || !face_up || !in || !gauge) return DSLASH_ERR_NULL;
     if (misaligned(face_down) || misaligned(face_up) || misaligned(in) || misaligned(gauge)) return DSLASH_ERR_ALIGN;
+    if (!on_ctx_device(c)) return DSLASH_ERR_UNSUPPORTED;
     if (!full_time_range(c)) return DSLASH_ERR_UNSUPPORTED;
     const size_t fb = dslash_slab_face_bytes(c);
     if (overlap(face_down, fb, face_up, fb)) return DSLASH_ERR_ALIAS;
@@ -1151,6 +1194,7 @@ int dslash_slab_interior(dslash_ctx* c, void* out, const void* in, const void* g
     if (misaligned(out) || misaligned(in) || misaligned(gauge)) return DSLASH_ERR_ALIGN;
     const size_t sb = dslash_spinor_bytes(c);
     if (overlap(out, sb, in, sb)) return DSLASH_ERR_ALIAS;
+    if (!on_ctx_device(c)) return DSLASH_ERR_UNSUPPORTED;
     if (!full_time_range(c)) return DSLASH_ERR_UNSUPPORTED;
     if (c->geom.L[3] <= 2) return DSLASH_OK;  // every slice is a boundary slice
     TileGeom tg = c->tg;  // the direct kernel on slices 1 .. lt-2: none of their hops leaves the slab
@@ -1171,6 +1215,7 @@ int dslash_slab_boundary(dslash_ctx* c, void* out, const void* in, const void* g
         return DSLASH_ERR_ALIGN;
     const size_t sb = dslash_spinor_bytes(c), fb = dslash_slab_face_bytes(c);
     if (overlap(out, sb, in, sb) || overlap(out, sb, face_from_below, fb) || overlap(out, sb, face_from_above, fb)) return DSLASH_ERR_ALIAS;
+    if (!on_ctx_device(c)) return DSLASH_ERR_UNSUPPORTED;
     if (!full_time_range(c)) return DSLASH_ERR_UNSUPPORTED;
     cudaError_t e = launch_slab_boundary(c->precision, c->layout_base, c->recon, out, in, gauge, face_from_below, face_from_above, c->geom,
                                          static_cast<cudaStream_t>(stream));

@@ -769,7 +769,7 @@ cudaError_t launch_gmarch(int precision, int layout_base, int recon, const Launc
     const GmLayout L = gm_layout(precision, recon, shape.NW, shape.NLS, shape.NHS, shape.NWB);
     if (L.total > GM_SMEM_MAX || shape.NW > (int)(4u * gm_cwg(precision))) return cudaErrorInvalidConfiguration;
     const GmBlockPlan* p = static_cast<const GmBlockPlan*>(d_plan);
-    const int h = cfg.l2_policy >= 0 ? cfg.l2_policy : (4 | 8 | 16);  // the defaults dslash_march.cu measured
+    const int h = cfg.march_policy >= 0 ? cfg.march_policy : (4 | 8 | 16);  // the defaults dslash_march.cu measured
     if (precision == 0)
         return recon == 12 ? launch_gmarch_k<double, 12, 2>(a, p, nblocks, L, h) : launch_gmarch_k<double, 18, 2>(a, p, nblocks, L, h);
     return recon == 12 ? launch_gmarch_k<float, 12, 3>(a, p, nblocks, L, h) : launch_gmarch_k<float, 18, 3>(a, p, nblocks, L, h);

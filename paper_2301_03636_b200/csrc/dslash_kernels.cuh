@@ -52,7 +52,8 @@ cudaError_t launch_omp_variant(int precision, int layout_base, int recon, const 
 // Options of the tuned kernels (dslash_set_option).
 struct TunedConfig {
     int occupancy;         // 0: default register budget, 1: 128-register variant
-    int l2_policy;         // DSLASH_OPT_L2_POLICY bits (0: no cache hints)
+    int l2_policy;         // DSLASH_OPT_L2_POLICY bits (0: no cache hints); direct kernel only
+    int march_policy;      // DSLASH_OPT_MARCH_POLICY bits (-1: the marching kernels' default 4|8|16)
     int l1_carveout;       // preferred shared-memory carve-out of the direct kernel in percent (-1: driver default)
     int pipe_slots;        // warp-pipelined kernel: stages in flight per warp (2..4; 0: default 2)
     int pipe_warps;        // warp-pipelined kernel: warps per block (1, 2 or 4; 0: default 4)
@@ -94,9 +95,12 @@ struct MarchBlockPlan {
 constexpr int MARCH_MAX_CHUNKS = 64;
 bool march_eligible(int layout_base, const Geom& g);
 cudaError_t march_plan_create(const Geom& g, int t_begin, int t_end, int device, void** d_plan, int* nblocks);
-// epoch = number of this launch on this plan (1, 2, ...): the progress counters behind the plan accumulate across launches
+// once per (ctx, device) where the kernel is selected: shared-memory attribute of the instantiation, SM count
+cudaError_t march_prepare(int precision, int recon, int device, int* sms);
+// sms from march_prepare(); *epoch = throttled launches on this plan so far (the progress counters behind the plan accumulate
+// across exactly those launches); no CUDA runtime query on this path
 cudaError_t launch_march(int precision, int layout_base, int recon, const LaunchArgs& a, const void* d_plan, int nblocks,
-                         const TunedConfig& cfg, unsigned epoch);
+                         const TunedConfig& cfg, int sms, unsigned* epoch);
 
 // generalised marching kernel (dslash_gmarch.cu): the same block-cooperative t-march for any L_X whose x rows tile whole
 // 32-site vectors together (L_X * L_Y a multiple of 32).  A compute warp owns one storage VECTOR (32 consecutive sites,

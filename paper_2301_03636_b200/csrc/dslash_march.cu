@@ -532,37 +532,55 @@ template <typename Real, int RECON, int NLS>
 cudaError_t launch_march_k(const LaunchArgs& a, const MarchBlockPlan* d_plan, int nblocks, int hints, unsigned* stats, unsigned* progress,
                            unsigned target, int lead) {
     using S = MarchSmem<Real, RECON, NLS>;
-    auto kernel = dslash_march_kernel<Real, RECON, NLS>;
-    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::TOTAL);
-    if (e != cudaSuccess) return e;
-    kernel<<<(unsigned)nblocks, MARCH_THREADS, S::TOTAL, a.stream>>>(a.out, a.in, a.gauge, a.geom.V, a.geom.L[1] * a.geom.L[2], a.geom.L[3],
-                                                                      d_plan, hints, stats, progress, target, lead);
+    dslash_march_kernel<Real, RECON, NLS><<<(unsigned)nblocks, MARCH_THREADS, S::TOTAL, a.stream>>>(
+        a.out, a.in, a.gauge, a.geom.V, a.geom.L[1] * a.geom.L[2], a.geom.L[3], d_plan, hints, stats, progress, target, lead);
     return cudaGetLastError();
+}
+
+template <typename Real, int RECON, int NLS>
+cudaError_t prepare_march_k() {
+    return cudaFuncSetAttribute(dslash_march_kernel<Real, RECON, NLS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)MarchSmem<Real, RECON, NLS>::TOTAL);
 }
 
 }  // namespace
 
+// What a launch needs from the runtime besides the plan, done once where the kernel is selected (the current device must be
+// `device`): the dynamic shared-memory limit of this precision/recon's instantiation and the SM count.  launch_march() then
+// makes no CUDA runtime query.
+cudaError_t march_prepare(int precision, int recon, int device, int* sms) {
+    cudaError_t e = cudaDeviceGetAttribute(sms, cudaDevAttrMultiProcessorCount, device);
+    if (e != cudaSuccess) return e;
+    if (precision == 0) return recon == 12 ? prepare_march_k<double, 12, 3>() : prepare_march_k<double, 18, 2>();
+    return recon == 12 ? prepare_march_k<float, 12, 4>() : prepare_march_k<float, 18, 4>();
+}
+
 // The plan is followed in device memory by 3 * nblocks unsigned: {SM id, cycles, globaltimer (ns, low word) at mid-march} of
 // every block of the last launch, then by MARCH_MAX_CHUNKS * L_T progress counters (zero when the plan is made).
+// sms: SM count from march_prepare().  *epoch counts the launches on this plan that ran WITH the throttle (lead > 0): only those
+// add to the progress counters, so only those may move the target the counters are compared with.
 cudaError_t launch_march(int precision, int layout_base, int recon, const LaunchArgs& a, const void* d_plan, int nblocks, const TunedConfig& cfg,
-                         unsigned epoch) {
-    if (!march_eligible(layout_base, a.geom) || !d_plan || nblocks < 1) return cudaErrorInvalidConfiguration;
+                         int sms, unsigned* epoch) {
+    if (!march_eligible(layout_base, a.geom) || !d_plan || nblocks < 1 || !epoch) return cudaErrorInvalidConfiguration;
     const MarchBlockPlan* p = static_cast<const MarchBlockPlan*>(d_plan);
     unsigned* st = reinterpret_cast<unsigned*>(const_cast<MarchBlockPlan*>(p + nblocks));
     unsigned* pr = st + 3u * (unsigned)nblocks;
     // default policy of this kernel (measured, profiles/r02_march.md): 4 read-once links evict_first, 8 stores evict_first,
     // 16 late ring fill; 1 (shared data evict_last) is harmful
-    const int h = cfg.l2_policy >= 0 ? cfg.l2_policy : (4 | 8 | 16);
+    const int h = cfg.march_policy >= 0 ? cfg.march_policy : (4 | 8 | 16);
     // the throttle needs every block of a chunk resident at the same time: single-wave plans only
-    int dev = 0, sms = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) sms = 0;
     const int lead = nblocks <= sms ? cfg.march_lead : 0;
-    const unsigned target = epoch * (unsigned)(a.geom.L[1] * a.geom.L[2]);  // rows of a chunk x launches so far (mod 2^32)
+    if (lead > 0) ++*epoch;
+    const unsigned target = *epoch * (unsigned)(a.geom.L[1] * a.geom.L[2]);  // rows of a chunk x throttled launches so far (mod 2^32)
+    cudaError_t e;
     if (precision == 0)
-        return recon == 12 ? launch_march_k<double, 12, 3>(a, p, nblocks, h, st, pr, target, lead)
-                           : launch_march_k<double, 18, 2>(a, p, nblocks, h, st, pr, target, lead);
-    return recon == 12 ? launch_march_k<float, 12, 4>(a, p, nblocks, h, st, pr, target, lead)
-                       : launch_march_k<float, 18, 4>(a, p, nblocks, h, st, pr, target, lead);
+        e = recon == 12 ? launch_march_k<double, 12, 3>(a, p, nblocks, h, st, pr, target, lead)
+                        : launch_march_k<double, 18, 2>(a, p, nblocks, h, st, pr, target, lead);
+    else
+        e = recon == 12 ? launch_march_k<float, 12, 4>(a, p, nblocks, h, st, pr, target, lead)
+                        : launch_march_k<float, 18, 4>(a, p, nblocks, h, st, pr, target, lead);
+    if (e != cudaSuccess && lead > 0) --*epoch;  // nothing ran, nothing was counted
+    return e;
 }
 
 // Builds the plan for the time range and uploads it (synchronous: cudaMalloc + cudaMemcpy).  *d_plan must be NULL or a plan

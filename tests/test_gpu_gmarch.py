@@ -141,11 +141,11 @@ def test_units_option_rebuilds_the_plan_and_tune_leaves_gmarch_alone(env):
             B.dslash_set_option(lat.ctx, B.DSLASH_OPT_MARCH_UNITS, units)
             assert B.dslash_get_option(lat.ctx, B.DSLASH_OPT_MARCH_UNITS) == units
             for policy in (4 | 8 | 16, 4 | 8, 0):  # late / early ring fill (bit 16)
-                B.dslash_set_option(lat.ctx, B.DSLASH_OPT_L2_POLICY, policy)
+                B.dslash_set_option(lat.ctx, B.DSLASH_OPT_MARCH_POLICY, policy)
                 o.fill_(0x7f)
                 lat.apply(o, pi, gi)
                 assert np.array_equal(lat.download_spinor(o), direct), (units, policy)
-        B.dslash_set_option(lat.ctx, B.DSLASH_OPT_L2_POLICY, -1)
+        B.dslash_set_option(lat.ctx, B.DSLASH_OPT_MARCH_POLICY, -1)
         # dslash_tune() picks by measurement among direct (+ march / wpipe when L_X == 32); gmarch lost everywhere it was
         # measured and is not a candidate
         chosen, ms = B.dslash_tune(lat.ctx, o.data_ptr(), pi.data_ptr(), gi.data_ptr(), lat.stream())

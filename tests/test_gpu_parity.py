@@ -206,6 +206,100 @@ def test_marching_kernel_matches_the_oracle_and_the_direct_kernel_bit_for_bit(en
             assert not part[:t0].any() and not part[t1:].any(), (t0, t1)
 
 
+@pytest.mark.parametrize("dims", [(32, 16, 12, 9), (32, 32, 32, 4), (32, 40, 30, 3)])  # the last one: more than one wave
+@pytest.mark.parametrize("precision", ["f64", "f32"])
+def test_marching_kernel_options_keep_the_bits(env, dims, precision):
+    """DSLASH_OPT_MARCH_POLICY changes the producers' gating (bit 16: late ring fill) and the copies' L2 hints;
+    DSLASH_OPT_MARCH_LEAD > 0 adds cross-block progress counters that accumulate over launches (the plan's epoch).  Every
+    combination, 20 back-to-back launches each on a non-blocking stream of ONE context (so the counters run through many
+    epochs, lead-0 launches in between included -- a round-2 advisor finding: those must not move the throttle's target), has
+    to give the direct kernel's bits.  A multi-wave plan switches the throttle off by itself; a new time range resets the epoch."""
+    B, torch = env.B, env.torch
+    g, p, ref, _ = fields_and_ref(env, dims, SEED + 41, precision)
+    with env.device.Lattice(dims, precision, "soa", False) as lat:
+        gi, pi, o = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
+        lat.apply(o, pi, gi)
+        direct_dev = o.clone()
+        assert env.checks.parity_error(lat.download_spinor(o), ref) <= TOL[precision]
+        lat.set_kernel("march")
+        torch.cuda.synchronize()
+        st = torch.cuda.Stream()
+
+        def run(n=20):
+            o.fill_(0x7f)
+            torch.cuda.synchronize()
+            for _ in range(n):
+                B.dslash_apply(lat.ctx, o.data_ptr(), pi.data_ptr(), gi.data_ptr(), st.cuda_stream)
+            st.synchronize()
+            return bool(torch.equal(o, direct_dev))
+
+        for policy in (0, 4, 12, 16, 28, 29, -1):
+            B.dslash_set_option(lat.ctx, B.DSLASH_OPT_MARCH_POLICY, policy)
+            assert B.dslash_get_option(lat.ctx, B.DSLASH_OPT_MARCH_POLICY) == policy
+            for lead in (0, 1, 4, 0, 2):
+                B.dslash_set_option(lat.ctx, B.DSLASH_OPT_MARCH_LEAD, lead)
+                assert run(), (policy, lead)
+        # the direct kernel's option no longer reaches the marching kernel: 16 there means "t loads bypass L1"
+        B.dslash_set_option(lat.ctx, B.DSLASH_OPT_L2_POLICY, 16)
+        assert run(3) and B.dslash_get_option(lat.ctx, B.DSLASH_OPT_MARCH_POLICY) == -1
+        B.dslash_set_option(lat.ctx, B.DSLASH_OPT_L2_POLICY, -1)
+        # a new time range rebuilds the plan (fresh counters, epoch 0) with the throttle still on
+        B.dslash_set_option(lat.ctx, B.DSLASH_OPT_MARCH_LEAD, 1)
+        lt = dims[3]
+        B.dslash_set_time_range(lat.ctx, 1, lt)
+        o.zero_()
+        torch.cuda.synchronize()
+        for _ in range(5):
+            B.dslash_apply(lat.ctx, o.data_ptr(), pi.data_ptr(), gi.data_ptr(), st.cuda_stream)
+        st.synchronize()
+        nat = B.dslash_spinor_bytes(lat.ctx) // lt  # a time slice of a blocked-SoA field with L_X = 32 is a whole number of vectors
+        assert torch.equal(o[nat:], direct_dev[nat:]) and not o[:nat].any()
+        B.dslash_set_time_range(lat.ctx, 0, lt)
+        assert run()
+
+
+def test_marching_kernel_throttle_is_not_left_behind_by_unthrottled_launches(env):
+    """Round-2 advisor finding: launches with DSLASH_OPT_MARCH_LEAD = 0 used to advance the epoch the throttle's target is
+    derived from, while only throttled launches advance the counters; once the option was switched on, every ring queue then
+    waited out its patience (~50 us) in every launch.  Timed: throttled launches after 50 unthrottled ones must not be slower
+    than throttled launches on a fresh context (best of three, 10 % margin; the defect costs 15 % and more)."""
+    B, torch = env.B, env.torch
+    dims = (32, 32, 32, 16)
+    g, p = env.inputs.fields(dims, SEED + 43, "f64")
+
+    def timed(lat, gi, pi, o, n=20):
+        best = None
+        for _ in range(3):
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            for _ in range(n):
+                lat.apply(o, pi, gi)
+            b.record()
+            torch.cuda.synchronize()
+            ms = a.elapsed_time(b) / n
+            best = ms if best is None else min(best, ms)
+        return best
+
+    with env.device.Lattice(dims, "f64", "soa", False) as lat:
+        gi, pi, o = lat.upload_gauge(g), lat.upload_spinor(p), lat.new_spinor()
+        lat.apply(o, pi, gi)
+        direct_dev = o.clone()
+        lat.set_kernel("march")
+        B.dslash_set_option(lat.ctx, B.DSLASH_OPT_MARCH_LEAD, 2)
+        for _ in range(10):
+            lat.apply(o, pi, gi)
+        fresh = timed(lat, gi, pi, o)
+        B.dslash_set_option(lat.ctx, B.DSLASH_OPT_MARCH_LEAD, 0)
+        for _ in range(50):
+            lat.apply(o, pi, gi)
+        B.dslash_set_option(lat.ctx, B.DSLASH_OPT_MARCH_LEAD, 2)
+        o.fill_(0x7f)
+        after = timed(lat, gi, pi, o)
+        assert torch.equal(o, direct_dev)
+        assert after <= 1.10 * fresh, (fresh, after)
+
+
 def test_marching_kernel_refuses_what_it_cannot_run(env):
     B = env.B
     for dims, layout in [((32, 4, 4, 4), "aos"),   # AoS rows are not contiguous vectors
