@@ -8,7 +8,7 @@
     python bench.py --costmodel                                     # the Advisor's cost model fitted on measured variant runtimes
     python bench.py --probe                                         # read/write/copy/4:1-mix bandwidth, FP64 FMA rate of this board
     python bench.py --cg | --eo | --decomposition slab              # solver, even-odd operator, multi-GPU slab form
-    python bench.py --kernel direct|wpipe|march|gmarch ...                 # force a kernel instead of letting dslash_tune pick
+    python bench.py --kernel direct|wpipe|march ...                        # force a kernel instead of letting dslash_tune pick
 
 A "step" is one application of D (one dslash_apply = one kernel launch covering SURVEY.md section 8(a)
 steps a1-a7) to one seeded synthetic lattice that is already resident in HBM in the native layout.  Before the timed
@@ -60,13 +60,11 @@ NCU_FIGURES = {
     "32x32x32x64_f64_soa_r18_march": dict(traffic=2000138688, fp64_pipe_pct=30.3, source="profiles/r03_ncu_march_raw.csv"),
     "32x32x32x64_f64_soa_r12_march": dict(traffic=1593540816, fp64_pipe_pct=37.9, source="profiles/r02b_skeleton.md"),
     "48x48x48x96_f32_soa_r18_direct": dict(traffic=5294248000, fp64_pipe_pct=None, source="profiles/r03_ncu_direct_cfg4_raw.csv"),
-    "48x48x48x96_f32_soa_r18_gmarch": dict(traffic=5990817000, fp64_pipe_pct=None, source="profiles/r02b_gmarch.md"),
 }
-KERNEL_NAMES = {"direct": "dslash_tuned_kernel", "wpipe": "dslash_wpipe_kernel", "march": "dslash_march_kernel",
-                "gmarch": "dslash_gmarch_kernel"}
+KERNEL_NAMES = {"direct": "dslash_tuned_kernel", "wpipe": "dslash_wpipe_kernel", "march": "dslash_march_kernel"}
 
 
-KERNEL_IDS = {1: "direct", 5: "wpipe", 6: "march", 7: "gmarch"}  # DSLASH_KERNEL_*
+KERNEL_IDS = {1: "direct", 5: "wpipe", 6: "march"}  # DSLASH_KERNEL_*
 
 
 def bytes_per_site(precision, recon12):
@@ -248,8 +246,6 @@ def lattice_options(B, lat, args):
         B.dslash_set_option(lat.ctx, B.DSLASH_OPT_MARCH_POLICY, args.march_policy)
     if args.march_lead is not None:
         B.dslash_set_option(lat.ctx, B.DSLASH_OPT_MARCH_LEAD, args.march_lead)
-    if args.march_units is not None:
-        B.dslash_set_option(lat.ctx, B.DSLASH_OPT_MARCH_UNITS, args.march_units)
     if args.pipe_slots is not None:
         B.dslash_set_option(lat.ctx, B.DSLASH_OPT_PIPE_SLOTS, args.pipe_slots)
     if args.pipe_warps is not None:
@@ -1120,11 +1116,10 @@ def main():
     ap.add_argument("--layout", choices=["soa", "aos"], default="soa")
     ap.add_argument("--tile", type=int, nargs=4, default=None, help="tile of the tuned kernel (x y z t)")
     ap.add_argument("--occupancy", type=int, default=None, help="DSLASH_OPT_OCCUPANCY override")
-    ap.add_argument("--kernel", choices=["auto", "direct", "wpipe", "march", "gmarch"], default=None)
+    ap.add_argument("--kernel", choices=["auto", "direct", "wpipe", "march"], default=None)
     ap.add_argument("--l2-policy", type=int, default=None, help="DSLASH_OPT_L2_POLICY bits (direct kernel)")
     ap.add_argument("--march-policy", type=int, default=None, help="DSLASH_OPT_MARCH_POLICY bits (marching kernels)")
     ap.add_argument("--march-lead", type=int, default=None, help="DSLASH_OPT_MARCH_LEAD")
-    ap.add_argument("--march-units", type=int, default=None, help="DSLASH_OPT_MARCH_UNITS (gmarch kernel: cap on the units per block)")
     ap.add_argument("--no-tune", action="store_true", help="skip dslash_tune (keep the library's static default kernel)")
     ap.add_argument("--pipe-slots", type=int, default=None, help="DSLASH_OPT_PIPE_SLOTS override (wpipe kernel)")
     ap.add_argument("--pipe-warps", type=int, default=None, help="DSLASH_OPT_PIPE_WARPS override (wpipe kernel)")

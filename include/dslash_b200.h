@@ -113,21 +113,15 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
                                   L2 -> SM once (links used for the own forward hop AND the neighbour's backward contribution,
                                   spinor rows kept in a shared-memory ring), all operands by bulk async copies
                                   (blocked SoA, L_X == 32); bit-identical to DSLASH_KERNEL_DIRECT */
-#define DSLASH_KERNEL_GMARCH 7 /* the same t-marching design for ANY x extent (48^3x96, 24^4, 16^4 ...): a compute warp owns one
-                                  32-site storage vector, a block owns whole units of lcm(L_X, 32) sites (whole rows = whole
-                                  vectors) that are neighbours in the (y,z) plane; x and y neighbours are lane-shifted and spread
-                                  over up to three vectors, so every hop is resolved through a host-built plan (source vectors
-                                  + lane masks) and x hops go through shared memory like y and z hops
-                                  (blocked SoA, L_X * L_Y a multiple of 32, a unit of <= 12 (FP32) / <= 8 (FP64) vectors);
-                                  bit-identical to DSLASH_KERNEL_DIRECT.  Opt-in only: measured 2.4-2.9 x slower than _DIRECT
-                                  (profiles/r02b_gmarch.md), dslash_tune() does not consider it */
+/* (7 was DSLASH_KERNEL_GMARCH, the marching design for any L_X: built in round 2, 2.4-2.9 x slower than _DIRECT on every lattice,
+   removed in round 3 -- profiles/r02b_gmarch.md, profiles/r03_fp32_path.md; dslash_set_kernel(ctx, 7) returns UNSUPPORTED) */
 
 /* options of the tuned kernels, dslash_set_option() */
 #define DSLASH_OPT_OCCUPANCY 2        /* blocks of <= 128 threads: 0 = 168 registers/thread (12 warps/SM), 1 = 128 (16 warps),
                                          2 = 255 (8 warps, deeper load hoisting) */
 #define DSLASH_OPT_L2_POLICY 3        /* direct kernel: bit mask of L2 hints, -1 or 0 (default) = none: 1 spinor loads evict_last,
                                          2 U_t loads evict_last, 4 U_x/U_y/U_z loads evict_first, 8 stores of `out` evict_first,
-                                         16 t-direction loads bypass L1 allocation.  The marching kernels do not read it (their
+                                         16 t-direction loads bypass L1 allocation.  The marching kernel does not read it (its
                                          bits mean other things: DSLASH_OPT_MARCH_POLICY), so a value tuned for one kernel never
                                          leaks into another and dslash_tune() compares every candidate under its own setting */
 #define DSLASH_OPT_L1_CARVEOUT 4      /* direct kernel: preferred shared-memory carve-out in percent, -1 = driver default */
@@ -146,13 +140,10 @@ typedef void *dslash_stream_t; /* a cudaStream_t */
                                          the L2 reuse distance of the t hops (48^3x96 fp32: HBM reads 1.26 x -> see profiles/) */
 #define DSLASH_OPT_TUNE_MODE 10       /* what dslash_tune() optimises: DSLASH_TUNE_BURST (default; the first ~35 ms after idle, board at its
                                          boost clock) or DSLASH_TUNE_SUSTAINED (continuous load, board at its power-capped clock) */
-#define DSLASH_OPT_MARCH_UNITS 12     /* generalised marching kernel: most units (of lcm(L_X, 32) sites) a block may own, 0 (default) = as
-                                         many as fit; fewer units leave shared memory for more link / halo slots per warp.  The block
-                                         plan is rebuilt by the call (synchronous) when DSLASH_KERNEL_GMARCH is selected */
 #define DSLASH_OPT_MARCH_LEAD 11      /* marching kernel: steps a block may run ahead of the slowest block of its chunk, 0..16
                                          (0 = unbounded, the default: measured slower than unbounded on 32^3x64).  Blocks that
                                          stay close share their halo rows through L2.  Only single-wave plans honour it */
-#define DSLASH_OPT_MARCH_POLICY 13    /* marching kernels (DSLASH_KERNEL_MARCH / _GMARCH): bit mask, -1 (default) = 4|8|16: 1 data other
+#define DSLASH_OPT_MARCH_POLICY 13    /* marching kernel (DSLASH_KERNEL_MARCH): bit mask           , -1 (default) = 4|8|16: 1 data other
                                          blocks read too evict_last (measured harmful), 4 links read once per application
                                          evict_first, 8 stores evict_first, 16 a ring row is fetched late, about one step before
                                          its first use instead of two.  0..31 */
@@ -270,12 +261,12 @@ DSLASH_API int dslash_get_time_range(const dslash_ctx *ctx, int *t_begin, int *t
 
 /*
  * Choose the implementation behind DSLASH_VARIANT_TUNED: DSLASH_KERNEL_AUTO (default: _DIRECT until dslash_tune() has
- * picked one), _DIRECT, _WARP_PIPE, _MARCH or _GMARCH (eligibility: see their definitions above).  The call also creates the
- * device-side resources the kernel needs besides the caller's fields (row counters of _WARP_PIPE, block plan of _MARCH / _GMARCH:
+ * picked one), _DIRECT, _WARP_PIPE or _MARCH (eligibility: see their definitions above).  The call also creates the
+ * device-side resources the kernel needs besides the caller's fields (row counters of _WARP_PIPE, block plan of _MARCH:
  * one small cudaMalloc + cudaMemcpy, synchronous), so that dslash_apply itself never allocates, copies or synchronises.
  * If a kernel is selected explicitly and the lattice/layout do not allow it, dslash_apply returns DSLASH_ERR_UNSUPPORTED.
  * dslash_get_kernel reports the kernel the next dslash_apply would launch.  All kernels give bit-identical results.
- * Errors: NULL, UNSUPPORTED (unknown value; _GMARCH: no decomposition of this lattice fits a block's shared memory), NOMEM, CUDA.
+ * Errors: NULL, UNSUPPORTED (unknown value; the ctx's device is not the current one), NOMEM, CUDA.
  */
 DSLASH_API int dslash_set_kernel(dslash_ctx *ctx, int kernel);
 DSLASH_API int dslash_get_kernel(const dslash_ctx *ctx, int *kernel);
@@ -293,31 +284,6 @@ DSLASH_API int dslash_get_kernel(const dslash_ctx *ctx, int *kernel);
 DSLASH_API int dslash_march_plan(const int dims[4], int t_begin, int t_end, int wave, int *ints, size_t capacity_ints, int *nblocks);
 
 /*
- * Host-side view of the work decomposition of DSLASH_KERNEL_GMARCH (no device needed; what dslash_set_kernel uploads).
- * A time slice is cut into units of lcm(L_X, 32) consecutive sites (whole x rows AND whole 32-site vectors); the units of
- * the (y,z) plane are ordered along the same snake as the rows of DSLASH_KERNEL_MARCH and cut into S segments, the time
- * range into G chunks; block c*S + s marches segment s through chunk c, one compute warp per vector.  Every neighbour
- * relation of Eq. 1 (periodic wrap = the Kronecker deltas of a periodic lattice) inside a time slice is in
- * the plan: per warp and direction d = x, y, z up to 3 forward and 3 backward sources {id, lane mask}.
- *   forward  id >= 0: ring row (id & 0xff) of the block (bit 8: the warp's last read of that row in a step);
- *            id <  0: vector -(id+1) of the slice, fetched from global memory (halo)
- *   backward id >= 0: exchange buffer filled by the warp that owns the source vector; id < 0: halo vector -(id+1)
- * The lane inside the source vector follows from the geometry (x+1: next lane, or L_X-1 lanes back at the end of a row;
- * y+1: L_X lanes on, mod 32; z+1: same lane).
- *   dims, precision (DSLASH_FP64 / DSLASH_FP32), recon (18 / 12): decide how many vectors a block can hold;
- *   shape (may be NULL) receives {NW compute warps, link slots per warp, halo spinor slots per warp, exchange buffers,
- *         units per block, vectors per unit, S, G, shared-memory bytes per block};
- *   ints  (may be NULL to query *nblocks and shape only) receives, per block, 4 + 12 + 36 + 12*48 ints:
- *         {t0, nt, active warps, chunk}, ring_readers[12], wbuf_readers[36], then per warp
- *         {vec, own_done, wr[3], nf[3], nb[3], link_shared, f[3][3]{id, mask}, b[3][3]{id, mask}}
- *         (GmBlockPlan / GmWarpPlan in csrc/dslash_kernels.cuh); capacity_ints = its size in ints.
- * Errors: NULL, DIMS, PRECISION, LAYOUT (recon), UNSUPPORTED (lattice not eligible, nothing fits, bad range, wave < 1,
- * capacity too small).
- */
-DSLASH_API int dslash_gmarch_plan(const int dims[4], int precision, int recon, int t_begin, int t_end, int wave, int shape[9], int *ints,
-                                  size_t capacity_ints, int *nblocks);
-
-/*
  * Where and how fast the blocks of the LAST DSLASH_KERNEL_MARCH launch of this ctx ran (a measurement aid: the kernel's work is
  * split statically, one block per SM, so the slowest SM sets the time).  stats (host, may be NULL to query *nblocks)
  * receives per block {SM id, SM clock cycles from block start to the last store of its first compute warp, low word of
@@ -329,7 +295,7 @@ DSLASH_API int dslash_march_stats(dslash_ctx *ctx, unsigned *stats, size_t capac
 /*
  * Pick the kernel by measurement (the Advisor's own method, applied to the library's kernels): every kernel
  * that can run this context (DSLASH_KERNEL_DIRECT; where eligible DSLASH_KERNEL_MARCH and DSLASH_KERNEL_WARP_PIPE in
- * three slot/warp configurations; not DSLASH_KERNEL_GMARCH, which loses to _DIRECT on every lattice measured) is timed on the caller's buffers
+ * three slot/warp configurations) is timed on the caller's buffers
  * (2 warm-up + 8 timed applications each, CUDA events on `stream`; about 15 ms in all, so that every candidate is
  * timed inside the board's boost window -- call it on an idle device; with DSLASH_OPT_TUNE_MODE = DSLASH_TUNE_SUSTAINED:
  * every candidate runs 300 applications to reach its own power-capped steady state, then 100 timed ones, ~0.8 s in all) and the fastest

@@ -28,14 +28,11 @@ DSLASH_STATIC_SCRATCH_BYTES = 8 << 20
 DSLASH_VARIANT_TUNED = 0
 DSLASH_MAP_MINIMAL, DSLASH_MAP_TOFROM = 0, 1
 DSLASH_KERNEL_AUTO, DSLASH_KERNEL_DIRECT = 0, 1
-DSLASH_KERNEL_WARP_PIPE, DSLASH_KERNEL_MARCH, DSLASH_KERNEL_GMARCH = 5, 6, 7
+DSLASH_KERNEL_WARP_PIPE, DSLASH_KERNEL_MARCH = 5, 6
 MARCH_NW, MARCH_NWS, MARCH_WARP_INTS = 7, 9, 9
 MARCH_BLOCK_INTS = 4 + MARCH_NW * MARCH_WARP_INTS  # block plan of dslash_march_plan()
-GM_NW_MAX, GM_SRC_MAX, GM_NWB_MAX = 12, 3, 36
-GM_WARP_INTS = 12 + 2 * 3 * GM_SRC_MAX * 2
-GM_BLOCK_INTS = 4 + GM_NW_MAX + GM_NWB_MAX + GM_NW_MAX * GM_WARP_INTS  # block plan of dslash_gmarch_plan()
 DSLASH_OPT_PIPE_SLOTS, DSLASH_OPT_PIPE_WARPS, DSLASH_OPT_PIPE_ZBLOCK, DSLASH_OPT_TUNE_MODE, DSLASH_OPT_MARCH_LEAD = 7, 8, 9, 10, 11
-DSLASH_OPT_MARCH_UNITS, DSLASH_OPT_MARCH_POLICY = 12, 13
+DSLASH_OPT_MARCH_POLICY = 13
 DSLASH_TUNE_BURST, DSLASH_TUNE_SUSTAINED = 0, 1
 DSLASH_OPT_OCCUPANCY, DSLASH_OPT_L2_POLICY, DSLASH_OPT_L1_CARVEOUT, DSLASH_OPT_X_SHUFFLE = 2, 3, 4, 5
 DSLASH_SCHED_STATIC, DSLASH_SCHED_DYNAMIC, DSLASH_SCHED_GUIDED = 0, 1, 2
@@ -95,8 +92,6 @@ SIGNATURES = {
     "dslash_slab_boundary": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "dslash_march_stats": (ctypes.c_int, [_vp, ctypes.POINTER(ctypes.c_uint), ctypes.c_size_t, _c_int_p]),
     "dslash_march_plan": (ctypes.c_int, [_c_int_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, _c_int_p, ctypes.c_size_t, _c_int_p]),
-    "dslash_gmarch_plan": (ctypes.c_int, [_c_int_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, _c_int_p, _c_int_p,
-                                          ctypes.c_size_t, _c_int_p]),
     "dslash_probe_launch": (ctypes.c_int, [ctypes.c_int, _vp, _vp, ctypes.c_size_t, ctypes.c_int, _vp]),
     "dslash_tune": (ctypes.c_int, [_vp, _vp, _vp, _vp, _vp, _c_int_p, ctypes.POINTER(ctypes.c_float)]),
     "dslash_set_option": (ctypes.c_int, [_vp, ctypes.c_int, ctypes.c_int]),
@@ -430,43 +425,6 @@ def dslash_slab_interior(ctx, out, inp, gauge, stream=0) -> None:
 def dslash_slab_boundary(ctx, out, inp, gauge, face_from_below, face_from_above, stream=0) -> None:
     _check(_lib.dslash_slab_boundary(_ptr(ctx), _ptr(out), _ptr(inp), _ptr(gauge), _ptr(face_from_below), _ptr(face_from_above),
                                      _ptr(stream)), "dslash_slab_boundary")
-
-
-def dslash_gmarch_plan(dims, precision: int, recon: int, t_begin: int, t_end: int, wave: int, shape_only: bool = False):
-    """Host-side block plan of DSLASH_KERNEL_GMARCH (no device needed): (shape, blocks) with
-    shape = {NW, NLS, NHS, NWB, units_per_block, vecs_per_unit, S, G, smem_bytes} and blocks a list of
-    {t0, nt, nact, chunk, ring_readers, wbuf_readers, warps: [{vec, own_done, wr, link_shared, f, b}]},
-    f[d] / b[d] = the forward / backward sources [(id, mask)] of direction d = x, y, z."""
-    arr = (ctypes.c_int * 4)(*[int(d) for d in dims])
-    nb = ctypes.c_int()
-    sh = (ctypes.c_int * 9)()
-    args = (arr, int(precision), int(recon), int(t_begin), int(t_end), int(wave), sh)
-    _check(_lib.dslash_gmarch_plan(*args, None, 0, ctypes.byref(nb)), "dslash_gmarch_plan")
-    shape = dict(zip(("NW", "NLS", "NHS", "NWB", "units_per_block", "vecs_per_unit", "S", "G", "smem_bytes"), list(sh)))
-    shape["nblocks"] = nb.value
-    if shape_only:
-        return shape, None
-    n = nb.value * GM_BLOCK_INTS
-    buf = (ctypes.c_int * n)()
-    _check(_lib.dslash_gmarch_plan(*args, buf, n, ctypes.byref(nb)), "dslash_gmarch_plan")
-    blocks = []
-    for b in range(nb.value):
-        v = buf[b * GM_BLOCK_INTS:(b + 1) * GM_BLOCK_INTS]
-        o = 4 + GM_NW_MAX + GM_NWB_MAX
-        warps = []
-        for w in range(GM_NW_MAX):
-            q = v[o + GM_WARP_INTS * w:o + GM_WARP_INTS * (w + 1)]
-            nf, nbk = q[5:8], q[8:11]
-            src = q[12:]
-
-            def entries(base, cnt):
-                return [[(src[base + (d * GM_SRC_MAX + e) * 2], src[base + (d * GM_SRC_MAX + e) * 2 + 1] & 0xFFFFFFFF) for e in range(cnt[d])]
-                        for d in range(3)]
-            warps.append(dict(vec=q[0], own_done=q[1], wr=tuple(q[2:5]), link_shared=q[11] & 0xFFFFFFFF, f=entries(0, nf),
-                              b=entries(3 * GM_SRC_MAX * 2, nbk)))
-        blocks.append(dict(t0=v[0], nt=v[1], nact=v[2], chunk=v[3], ring_readers=list(v[4:4 + GM_NW_MAX]),
-                           wbuf_readers=list(v[4 + GM_NW_MAX:o]), warps=warps))
-    return shape, blocks
 
 
 def dslash_march_stats(ctx):

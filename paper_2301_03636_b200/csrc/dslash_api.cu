@@ -50,10 +50,6 @@ struct dslash_ctx {
     int march_blocks, march_t0, march_t1;
     unsigned march_epoch;  // throttled (lead > 0) launches on the current plan: its progress counters accumulate over those
     int march_sms;         // SM count of the ctx's device, from march_prepare() (0: not prepared yet)
-    // the same for the generalised marching kernel (any L_X): plan, its shape (warps, slots, shared-memory size), time range
-    void* gm_plan;
-    int gm_blocks, gm_t0, gm_t1;
-    GmShape gm_shape;
 };
 
 static int cuda_fail(dslash_ctx* c, cudaError_t e) {
@@ -212,7 +208,7 @@ static int cg_normal_equations(dslash_ctx* c, unsigned V, size_t sb, void** vec,
 // plan of the marching kernel.  Called where a kernel is SELECTED (dslash_set_kernel, dslash_tune, dslash_set_time_range,
 // dslash_create), so that dslash_apply itself never allocates, copies or synchronises.
 static int ensure_kernel_resources(dslash_ctx* c, int kernel) {
-    if (kernel == DSLASH_KERNEL_WARP_PIPE || kernel == DSLASH_KERNEL_MARCH || kernel == DSLASH_KERNEL_GMARCH) {
+    if (kernel == DSLASH_KERNEL_WARP_PIPE || kernel == DSLASH_KERNEL_MARCH) {
         // everything below allocates on, and asks about, the CURRENT device: it has to be the ctx's
         int cur_dev = -1;
         if (cudaGetDevice(&cur_dev) != cudaSuccess || cur_dev != c->device) return DSLASH_ERR_UNSUPPORTED;
@@ -246,23 +242,6 @@ static int ensure_kernel_resources(dslash_ctx* c, int kernel) {
         c->march_t0 = c->tg.t_begin;
         c->march_t1 = c->tg.t_end;
         c->march_epoch = 0;
-    }
-    if (kernel == DSLASH_KERNEL_GMARCH && gmarch_eligible(c->precision, c->layout_base, c->recon, c->geom) &&
-        (!c->gm_plan || c->gm_t0 != c->tg.t_begin || c->gm_t1 != c->tg.t_end)) {
-        if (c->gm_plan && cudaDeviceSynchronize() != cudaSuccess) return cuda_fail(c, cudaGetLastError());  // a launch may still read it
-        cudaError_t e = gmarch_plan_create(c->precision, c->recon, c->geom, c->tg.t_begin, c->tg.t_end, c->device, c->cfg.march_units,
-                                           &c->gm_plan, &c->gm_blocks, &c->gm_shape);
-        if (e == cudaErrorInvalidValue) {  // no decomposition fits the shared memory of a block: the kernel cannot run this lattice
-            (void)cudaGetLastError();
-            c->gm_t0 = c->gm_t1 = -1;
-            return DSLASH_ERR_UNSUPPORTED;
-        }
-        if (e != cudaSuccess) {
-            (void)cudaGetLastError();
-            return cuda_fail(c, e);
-        }
-        c->gm_t0 = c->tg.t_begin;
-        c->gm_t1 = c->tg.t_end;
     }
     return DSLASH_OK;
 }
@@ -335,12 +314,7 @@ int dslash_create(dslash_ctx** ctx, const int dims[4], int precision, int layout
     c->march_epoch = 0;
     c->march_sms = 0;
     c->cfg.march_policy = -1;
-    c->gm_plan = nullptr;
-    c->gm_blocks = 0;
-    c->gm_t0 = c->gm_t1 = -1;
-    c->gm_shape = GmShape{};
     c->cfg.march_lead = 0;
-    c->cfg.march_units = 0;
     c->tune_mode = DSLASH_TUNE_BURST;
     c->cfg.x_shuffle = precision == DSLASH_FP64 ? 1 : 0;  // measured: -1.3 % (burst) / -2 % (sustained) in fp64, +0.8 % in fp32
     c->launches = 0;
@@ -357,7 +331,7 @@ int dslash_create(dslash_ctx** ctx, const int dims[4], int precision, int layout
 int dslash_destroy(dslash_ctx* c) {
     if (!c) return DSLASH_OK;
     int rc = DSLASH_OK;
-    bool any = c->cg_scratch != nullptr || c->pipe_ctr != nullptr || c->march_plan != nullptr || c->gm_plan != nullptr;
+    bool any = c->cg_scratch != nullptr || c->pipe_ctr != nullptr || c->march_plan != nullptr;
     for (int i = 0; i < 3; ++i) any = any || c->d_can[i] || c->d_nat[i];
     for (int i = 0; i < 4; ++i) any = any || c->cg_vec[i];
     for (int i = 0; i < 6; ++i) any = any || c->eo_vec[i];
@@ -370,7 +344,6 @@ int dslash_destroy(dslash_ctx* c) {
         if (c->cg_scratch) cudaFree(c->cg_scratch);
         if (c->pipe_ctr) cudaFree(c->pipe_ctr);
         if (c->march_plan) cudaFree(c->march_plan);
-        if (c->gm_plan) cudaFree(c->gm_plan);
         for (int i = 0; i < 66; ++i)
             if (c->host_event[i]) cudaEventDestroy(c->host_event[i]);
         for (int i = 0; i < 3; ++i)
@@ -401,8 +374,6 @@ static int resolve_kernel(const dslash_ctx* c) {
     if (c->kernel == DSLASH_KERNEL_DIRECT) return DSLASH_KERNEL_DIRECT;
     if (c->kernel == DSLASH_KERNEL_WARP_PIPE) return wpipe_eligible(c->layout_base, c->geom) ? DSLASH_KERNEL_WARP_PIPE : -1;
     if (c->kernel == DSLASH_KERNEL_MARCH) return march_eligible(c->layout_base, c->geom) ? DSLASH_KERNEL_MARCH : -1;
-    if (c->kernel == DSLASH_KERNEL_GMARCH)
-        return gmarch_eligible(c->precision, c->layout_base, c->recon, c->geom) ? DSLASH_KERNEL_GMARCH : -1;
     return DSLASH_KERNEL_DIRECT;  // AUTO
 }
 
@@ -439,10 +410,8 @@ int dslash_apply(dslash_ctx* c, void* out, const void* in, const void* gauge, ds
         }
         if (k == DSLASH_KERNEL_MARCH && (!c->march_plan || c->march_sms < 1 || c->march_t0 != c->tg.t_begin || c->march_t1 != c->tg.t_end))
             return DSLASH_ERR_UNSUPPORTED;
-        if (k == DSLASH_KERNEL_GMARCH && (!c->gm_plan || c->gm_t0 != c->tg.t_begin || c->gm_t1 != c->tg.t_end)) return DSLASH_ERR_UNSUPPORTED;
         e = (k == DSLASH_KERNEL_WARP_PIPE) ? launch_wpipe(c->precision, c->layout_base, c->recon, a, c->tg, c->cfg)
             : (k == DSLASH_KERNEL_MARCH)   ? launch_march(c->precision, c->layout_base, c->recon, a, c->march_plan, c->march_blocks, c->cfg, c->march_sms, &c->march_epoch)
-            : (k == DSLASH_KERNEL_GMARCH)  ? launch_gmarch(c->precision, c->layout_base, c->recon, a, c->gm_plan, c->gm_blocks, c->gm_shape, c->cfg)
                                            : launch_tuned(c->precision, c->layout_base, c->recon, a, c->tg, c->cfg);
     } else if (!full_time_range(c)) {
         return DSLASH_ERR_UNSUPPORTED;  // the variant kernels always sweep the whole lattice
@@ -867,14 +836,6 @@ int dslash_set_option(dslash_ctx* c, int option, int value) {
             if (value != 0 && value != 1 && value != 2 && value != 4) return DSLASH_ERR_UNSUPPORTED;
             c->cfg.pipe_warps = value;
             return DSLASH_OK;
-        case DSLASH_OPT_MARCH_UNITS:
-            if (value < 0 || value > GM_NW_MAX) return DSLASH_ERR_UNSUPPORTED;
-            if (value != c->cfg.march_units) {
-                c->cfg.march_units = value;
-                c->gm_t0 = c->gm_t1 = -1;  // the plan no longer matches: rebuilt now if the kernel is selected, else when it is
-                if (c->kernel == DSLASH_KERNEL_GMARCH) return ensure_kernel_resources(c, c->kernel);
-            }
-            return DSLASH_OK;
         case DSLASH_OPT_MARCH_LEAD:
             if (value < 0 || value > 16) return DSLASH_ERR_UNSUPPORTED;
             c->cfg.march_lead = value;
@@ -899,7 +860,6 @@ int dslash_get_option(const dslash_ctx* c, int option, int* value) {
         case DSLASH_OPT_PIPE_WARPS: *value = c->cfg.pipe_warps; return DSLASH_OK;
         case DSLASH_OPT_MARCH_LEAD: *value = c->cfg.march_lead; return DSLASH_OK;
         case DSLASH_OPT_MARCH_POLICY: *value = c->cfg.march_policy; return DSLASH_OK;
-        case DSLASH_OPT_MARCH_UNITS: *value = c->cfg.march_units; return DSLASH_OK;
         case DSLASH_OPT_PIPE_ZBLOCK: *value = c->cfg.pipe_zblock; return DSLASH_OK;
         case DSLASH_OPT_TUNE_MODE: *value = c->tune_mode; return DSLASH_OK;
         default: return DSLASH_ERR_UNSUPPORTED;
@@ -909,7 +869,7 @@ int dslash_get_option(const dslash_ctx* c, int option, int* value) {
 int dslash_set_kernel(dslash_ctx* c, int kernel) {
     if (!c) return DSLASH_ERR_NULL;
     if (kernel != DSLASH_KERNEL_AUTO && kernel != DSLASH_KERNEL_DIRECT && kernel != DSLASH_KERNEL_WARP_PIPE &&
-        kernel != DSLASH_KERNEL_MARCH && kernel != DSLASH_KERNEL_GMARCH)
+        kernel != DSLASH_KERNEL_MARCH)
         return DSLASH_ERR_UNSUPPORTED;
     const int rc = ensure_kernel_resources(c, kernel);
     if (rc != DSLASH_OK) return rc;
@@ -941,9 +901,8 @@ int dslash_tune(dslash_ctx* c, void* out, const void* in, const void* gauge, dsl
         const int rcr = ensure_kernel_resources(c, cand[k].kernel);
         if (rcr != DSLASH_OK) return rcr;
     }
-    // DSLASH_KERNEL_GMARCH is NOT a candidate: measured on every lattice it can run (profiles/r02b_gmarch.md: 48^3x96 fp32
-    // 2.36 ms against 0.91 ms, 24^4 fp64 0.148 against 0.062 ms) it is 2.4-2.9 x slower than the direct kernel, and timing it
-    // here would only heat the board before the caller's own measurement.  It stays selectable with dslash_set_kernel().
+    // (A marching design for any L_X was built in round 2 and removed in round 3: 2.4-2.9 x slower than the direct kernel on
+    // every lattice it ran, profiles/r02b_gmarch.md, profiles/r03_fp32_path.md.)
     if (wpipe_eligible(c->layout_base, c->geom) && ensure_kernel_resources(c, DSLASH_KERNEL_WARP_PIPE) == DSLASH_OK) {
         cand[ncand++] = {DSLASH_KERNEL_WARP_PIPE, 2, 4};  // 8 warps x 2 stages in flight per SM (fp64, 18-real)
         cand[ncand++] = {DSLASH_KERNEL_WARP_PIPE, 3, 1};  // 6 warps x 3 stages

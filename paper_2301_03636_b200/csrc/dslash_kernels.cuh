@@ -59,7 +59,6 @@ struct TunedConfig {
     int pipe_warps;        // warp-pipelined kernel: warps per block (1, 2 or 4; 0: default 4)
     unsigned* pipe_counters;  // warp-pipelined kernel: {next row, finished warps} of this launch (device memory, zero between launches)
     int pipe_zblock;       // warp-pipelined kernel: z planes per block of the row order (0: L_Z, i.e. plain lexicographic)
-    int march_units;       // generalised marching kernel: cap on the units per block (0: none)
     int march_lead;        // marching kernel: steps a block may run ahead of the slowest block of its chunk (0: unbounded)
     int x_shuffle;         // 1: exchange the x hops inside the warp when the tile allows it (fp64 default), 0: always load them
 };
@@ -101,52 +100,6 @@ cudaError_t march_prepare(int precision, int recon, int device, int* sms);
 // across exactly those launches); no CUDA runtime query on this path
 cudaError_t launch_march(int precision, int layout_base, int recon, const LaunchArgs& a, const void* d_plan, int nblocks,
                          const TunedConfig& cfg, int sms, unsigned* epoch);
-
-// generalised marching kernel (dslash_gmarch.cu): the same block-cooperative t-march for any L_X whose x rows tile whole
-// 32-site vectors together (L_X * L_Y a multiple of 32).  A compute warp owns one storage VECTOR (32 consecutive sites,
-// which is an x row only when L_X == 32); a block owns whole UNITS (lcm(L_X, 32) sites = whole rows = whole vectors), so
-// x neighbours never leave the block.  Every hop of a lane is resolved through the plan: up to GM_SRC_MAX source vectors
-// per (warp, direction), each with the mask of lanes it serves; the lane inside the source follows from the geometry.
-constexpr int GM_NW_MAX = 12;   // compute warps (= vectors) per block
-constexpr int GM_SRC_MAX = 3;   // distinct source vectors of one hop direction of one warp
-constexpr int GM_NWB_MAX = 36;  // exchange buffers per block
-struct GmSrc {
-    int id;         // forward hop: >= 0 ring row (id & 0xff) of this block, bit 8 = the warp's last read of that row in the step;
-                    //              < 0 halo: vector -(id + 1) of the slice, fetched from global memory
-                    // backward hop: >= 0 exchange buffer holding U^dagger P+ psi of the source vector; < 0 halo: spinor AND link
-                    //              of vector -(id + 1) are fetched and the product is formed here
-    unsigned mask;  // lanes of this warp whose neighbour lies in that vector
-};
-struct GmWarpPlan {
-    int vec;               // the warp's vector inside a time slice (site = 32 * vec + lane); -1: idle warp
-    int own_done;          // 1: reading its own spinors is the warp's last read of its ring row in a step
-    int wr[3];             // exchange buffer this warp fills with U_d^dagger P+_d psi, d = x, y, z (-1: no reader in the block)
-    int nf[3], nb[3];      // number of forward / backward sources per direction
-    unsigned link_shared;  // bit d: U_d of this vector is fetched by another block too (its backward halo hop)
-    GmSrc f[3][GM_SRC_MAX], b[3][GM_SRC_MAX];
-};
-struct GmBlockPlan {
-    int t0, nt;  // first time slice and number of steps
-    int nact;    // active warps
-    int chunk;
-    int ring_readers[GM_NW_MAX];   // warps that read ring row r in a step (the owner included)
-    int wbuf_readers[GM_NWB_MAX];  // warps that read exchange buffer b in a step
-    GmWarpPlan w[GM_NW_MAX];
-};
-struct GmShape {
-    int NW, NLS, NHS, NWB;  // compute warps, link slots per warp, halo spinor slots per warp, exchange buffers
-    int units_per_block, vecs_per_unit, S, G;
-    unsigned smem_bytes;
-};
-bool gmarch_eligible(int precision, int layout_base, int recon, const Geom& g);
-// host only: decomposition and plan for [t_begin, t_end) with `wave` co-resident blocks; returns the number of blocks (0: none)
-// max_units > 0 caps the units per block
-int gmarch_plan_build(int precision, int recon, const Geom& g, int t_begin, int t_end, int wave, int max_units, GmShape* shape,
-                      GmBlockPlan* plan_out, size_t capacity_blocks);
-cudaError_t gmarch_plan_create(int precision, int recon, const Geom& g, int t_begin, int t_end, int device, int max_units, void** d_plan,
-                               int* nblocks, GmShape* shape);
-cudaError_t launch_gmarch(int precision, int layout_base, int recon, const LaunchArgs& a, const void* d_plan, int nblocks,
-                          const GmShape& shape, const TunedConfig& cfg);
 
 // Multi-GPU T-slab form (dslash_slab.cu): half-spinor faces and the boundary slices that consume them.
 cudaError_t launch_slab_pack_faces(int precision, int layout_base, int recon, void* face_down, void* face_up, const void* in,

@@ -173,7 +173,7 @@ __device__ __forceinline__ cplx<Real> c_mul_conj(cplx<Real> a, cplx<Real> b) {
 // templates above (one IEEE fma / add / mul per lane), so results are bit-identical to them -- and to one another across
 // kernels, whichever form a translation unit uses.  A translation unit opts in with #define DSLASH_F32X2 before including
 // this header.  Measured in one call, scalar vs packed (profiles/r02b_f32x2.md): the marching kernels gain 10-12 % in FP32
-// (fewer instructions in the compute warps' serial timeline: 32^3x64 0.244 -> 0.221 ms, 48^3x96 gmarch 2.36 -> 2.09 ms); the
+// (fewer instructions in the compute warps' serial timeline: 32^3x64 0.244 -> 0.221 ms, 48^3x96 (generalised march, since removed) gmarch 2.36 -> 2.09 ms); the
 // direct kernel gains nothing at 48^3x96 (0.915 vs 0.916 ms) and LOSES 4.5 % at 32^3x64 (0.184 vs 0.1765 ms: with 128
 // registers and aligned pairs the compiler keeps fewer loads in flight), so dslash_tuned.cu and the other one-thread-per-site
 // units stay scalar.  For A/B measurements the whole library can be built one way or the other:

@@ -161,7 +161,7 @@ class Lattice:
 
     def set_kernel(self, kernel):
         B.dslash_set_kernel(self.ctx, {"auto": B.DSLASH_KERNEL_AUTO, "direct": B.DSLASH_KERNEL_DIRECT,
-                                       "wpipe": B.DSLASH_KERNEL_WARP_PIPE, "march": B.DSLASH_KERNEL_MARCH, "gmarch": B.DSLASH_KERNEL_GMARCH}.get(kernel, kernel))
+                                       "wpipe": B.DSLASH_KERNEL_WARP_PIPE, "march": B.DSLASH_KERNEL_MARCH}.get(kernel, kernel))
 
     def dslash(self, gauge_canonical, spinor_canonical):
         """Convenience: canonical NumPy in -> canonical NumPy out (one application on the device)."""

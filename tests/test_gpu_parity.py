@@ -313,6 +313,8 @@ def test_marching_kernel_refuses_what_it_cannot_run(env):
             assert B.dslash_apply_status(lat.ctx, o.data_ptr(), p.data_ptr(), g.data_ptr()) == B.DSLASH_OK
             with pytest.raises(B.DslashError):
                 B.dslash_set_kernel(lat.ctx, 2)  # a kernel of round 1 that no longer exists
+            with pytest.raises(B.DslashError):
+                B.dslash_set_kernel(lat.ctx, 7)  # the generalised marching kernel of round 2, removed in round 3
 
 
 @pytest.mark.parametrize("kernel", ["march", "wpipe"])
@@ -729,11 +731,11 @@ def test_config3_staged_kernels_are_bit_stable_under_back_to_back_launches(env):
         p.view(torch.float64).normal_(generator=gen)
         lat.apply(ref, p, g)
         torch.cuda.synchronize()
-        for kernel in ("march", "wpipe", "gmarch"):
+        for kernel in ("march", "wpipe"):
             lat.set_kernel(kernel)
             o = lat.new_spinor()
             bad = 0
-            for i in range(200 if kernel != "gmarch" else 50):
+            for i in range(200):
                 lat.apply(o, p, g)
                 if i % 10 == 9:
                     torch.cuda.synchronize()
