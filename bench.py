@@ -432,6 +432,14 @@ def run_cuda(args, cfg):
             o = results["other_recon"]
             line["also"] = {"recon": 12 if o["recon12"] else 18, "value": o["gflops"], "ms_per_step": o["ms_per_step"],
                             "hbm_gbs": o["gbs"], "roofline_frac": None if l2_resident else o["gbs"] / peak, "kernel": o["kernel"]}
+        if args.all_configs and not l2_resident and "sustained" in results:
+            # the honest ceiling of the sustained leg: the board's own 4:1 read/write rate after the same kind of heat
+            sp = probe_sustained(local)
+            roofline["sustained_peak"] = {"value": sp["read4_write1"]["GB/s"], "unit": "GB/s", "kind": "dslash_probe READ4_WRITE1 after 0.5 s of "
+                                          "back-to-back launches (csrc/dslash_probe.cu)", "sm_mhz": sp["read4_write1"]["sm_mhz"],
+                                          "reasons": sp["read4_write1"]["reasons"], "copy_gbs": sp["copy"]["GB/s"],
+                                          "copy_sm_mhz": sp["copy"]["sm_mhz"]}
+            roofline["sustained_frac_of_sustained_peak"] = results["sustained"]["gbs"] / sp["read4_write1"]["GB/s"]
         if args.all_configs:
             # north_star: "throughput on the synthetic lattices below ... with the variant sweep's top-10 ranking reported":
             # BASELINE.json configs[0], [1], [3], [4] after the headline (configs[2]), then the 120-variant sweep on configs[4]
@@ -955,6 +963,49 @@ def run_costmodel(args):
 
 
 # ------------------------------------------------------------------ ceilings of the board at hand
+def probe_sustained(index, heat_s=0.5, timed_s=0.12):
+    """What the board's memory system holds under CONTINUOUS load: the library's 4:1 read/write probe (the Dslash's own mix)
+    and its copy probe, each launched back to back for heat_s seconds (about the duration of the headline's 1500-apply heat),
+    then timed over timed_s seconds with the SM clock and throttle reasons sampled.  MEASURED_PEAKS.json's hbm_gbs is a burst
+    figure (best of a few copies from idle); the sustained Dslash number has this one as its honest ceiling."""
+    import torch
+    from paper_2301_03636_b200 import binding as B
+    dev = torch.device("cuda", index)
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    n = 1 << 26  # 16-byte units: 1 GiB per stream, far beyond L2
+    src = torch.empty(4 * n * 2, dtype=torch.float64, device=dev).normal_()
+    dst = torch.empty(n * 2, dtype=torch.float64, device=dev)
+    st = torch.cuda.current_stream().cuda_stream
+    out = {}
+    for name, kind, nbytes in (("read4_write1", B.DSLASH_PROBE_READ4_WRITE1, 80 * n), ("copy", B.DSLASH_PROBE_COPY, 32 * n)):
+        def launch(k):
+            for _ in range(k):
+                B.dslash_probe_launch(kind, dst.data_ptr(), src.data_ptr(), n, sms * 8, st)
+        launch(3)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        launch(5)
+        e1.record()
+        torch.cuda.synchronize()
+        per = e0.elapsed_time(e1) / 5 / 1e3  # seconds per launch, to size the two regions
+        heat, timed = max(10, int(heat_s / per)), max(10, int(timed_s / per))
+        time.sleep(1.0)
+        launch(heat)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        with ClockSampler(index) as cs:
+            e0.record()
+            launch(timed)
+            e1.record()
+            torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / timed
+        ck = cs.summary()
+        out[name] = {"GB/s": nbytes / ms / 1e6, "ms_per_launch": ms, "bytes_per_launch": nbytes, "heat_launches": heat,
+                     "timed_launches": timed, "sm_mhz": ck.get("sm_mhz"), "reasons": ck.get("reasons"), "power_w": ck.get("power_w")}
+    del src, dst
+    return out
+
+
 def run_probe(args):
     """Read / write / copy / 4:1-mix bandwidth over 4 GiB working sets and the FP64 FMA rate, each the best of 5 launches after
     1 s idle (boost window), with the library's own probe kernels (csrc/dslash_probe.cu)."""
@@ -993,6 +1044,8 @@ def run_probe(args):
            "read4_write1": best(B.DSLASH_PROBE_READ4_WRITE1, n, blocks, bytes_moved=80 * n),
            "dfma": best(B.DSLASH_PROBE_DFMA, iters, blocks, flops=2.0 * 8 * iters * blocks * 256),
            "measured_peaks_hbm_gbs": peak, "peak_source": peak_src}
+    del src, dst
+    out["sustained"] = probe_sustained(0)
     print(json.dumps(out))
     return 0
 
