@@ -42,7 +42,8 @@ _c_int_p = ctypes.POINTER(ctypes.c_int)
 _c_size_p = ctypes.POINTER(ctypes.c_size_t)
 _vp = ctypes.c_void_p
 
-# name -> (restype, argtypes); mirrors include/dslash_b200.h one to one
+# name -> (restype, argtypes); mirrors include/dslash_b200.h (the operator) and include/dslash_b200_diag.h (dslash_probe_launch,
+# dslash_march_stats: measurement aids) one to one
 SIGNATURES = {
     "dslash_create": (ctypes.c_int, [ctypes.POINTER(_vp), _c_int_p, ctypes.c_int, ctypes.c_int]),
     "dslash_destroy": (ctypes.c_int, [_vp]),

@@ -6,6 +6,7 @@
 #include <new>
 
 #include "../../include/dslash_b200.h"
+#include "../../include/dslash_b200_diag.h"
 #include "dslash_kernels.cuh"
 
 using namespace dslash;

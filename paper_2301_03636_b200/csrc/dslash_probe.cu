@@ -6,6 +6,7 @@
 #include <stdint.h>
 
 #include "../../include/dslash_b200.h"
+#include "../../include/dslash_b200_diag.h"
 
 namespace {
 

@@ -8,6 +8,7 @@ import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 HEADER = os.path.join(ROOT, "include", "dslash_b200.h")
+DIAG_HEADER = os.path.join(ROOT, "include", "dslash_b200_diag.h")  # measurement aids, kept out of the operator's header
 
 
 @pytest.fixture(scope="module")
@@ -18,14 +19,22 @@ def B():
     return binding
 
 
-def declared_symbols():
-    text = open(HEADER).read()
+def declared_symbols(header=None):
+    if header is None:  # everything the library exports under the dslash_ prefix: operator header + diagnostics header
+        return sorted(set(declared_symbols(HEADER)) | set(declared_symbols(DIAG_HEADER)))
+    text = open(header).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(dslash_[a-z0-9_]+)\s*\(", text)))
 
 
+def test_measurement_aids_live_in_their_own_header():
+    assert declared_symbols(DIAG_HEADER) == ["dslash_march_stats", "dslash_probe_launch"]
+    assert not set(declared_symbols(DIAG_HEADER)) & set(declared_symbols(HEADER))
+    assert "DSLASH_PROBE_" not in open(HEADER).read().replace("dslash_b200_diag.h", "")
+
+
 def test_header_declares_the_north_star_calls():
-    names = declared_symbols()
+    names = declared_symbols(HEADER)
     for must in ("dslash_create", "dslash_apply", "dslash_destroy", "dslash_pack_spinor", "dslash_unpack_spinor",
                  "dslash_pack_gauge", "dslash_set_variant", "dslash_apply_host"):
         assert must in names
